@@ -1,0 +1,22 @@
+"""CPU oracle for H|psi> -- TEST INFRASTRUCTURE, not the product.
+
+Plain, slow, obviously-correct implementation of what the hot path computes,
+written from /root/reference/PAPER.md (cited per function as PAPER.md:<line>).
+Only ``tests/``, ``__graft_entry__.smoke()`` and the ``cpu_baseline`` /
+``--impl reference`` legs of ``bench.py`` may import this package.  It shares
+no code with ``paper_2308_07277_b200`` and neither imports the other.
+
+Parts:
+  O1  gsphere.py      G-sphere enumeration, sphere->box index map, |k+G|^2
+  O2  hpsi.py         H apply by direct O(N_G^2) G-space summation
+                      (dense-matrix numpy form for small N_G; the same triple
+                      sum as explicit C loops in hpsi_direct.c for large N_G)
+  O3  dft.py          naive DFT straight from the definition (8^3-size checks)
+
+Pins (tests/test_oracle_*.py, ``-m "not gpu"``): the paper's printed bcc
+example, closed-form plane-wave
+eigenvalues, single-Fourier-component shift, rank-1 projector, Hermiticity,
+naive-DFT brute force on 8^3, numpy fftn identity.
+Parity unpinned: none of the functions here; absolute physical energies of
+real Si are out of scope (no pseudopotential data).
+"""
