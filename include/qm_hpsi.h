@@ -1,0 +1,128 @@
+/*
+ * qm_hpsi.h -- C ABI of the B200-native plane-wave Kohn-Sham Hamiltonian apply.
+ *
+ *   H|psi_nk>(G) = 1/2 |k+G|^2 psi(G)                                   PAPER.md:146 (eq. 12), 668-674 (eqs. 49-51)
+ *                + [ FFT( V_loc(r) * IFFT(psi) ) ](G)                    PAPER.md:652-666 (eqs. 46-48), 725-730
+ *                + sum_ij beta_i(G) D_ij <beta_j|psi>                    PAPER.md:153-161 (eq. 14), 1019-1024
+ *
+ * The operator is the paper's KSHam.h_psi(): a black-box
+ * Hermitian apply on a block of trial vectors in complex128.
+ *
+ * Conventions (readings A1-A8 of DESIGN.md section 3):
+ *  - Hartree / bohr inside; ecutwfc given in Ry; sphere = { m : |k+G_m|^2 [bohr^-2] <= ecutwfc [Ry] }.
+ *  - lattice rows are a_i; b_i = rows of 2 pi (A^-1)^T; k in fractions of b_i.
+ *  - sphere order = ascending C-order flat box index
+ *        idx = ((m1 mod n1)*n2 + (m2 mod n2))*n3 + (m3 mod n3)
+ *  - V_r is flat C order over (n1,n2,n3), r_j = sum_i (j_i/n_i) a_i.
+ *  - wavefunction blocks are [nbands][ng(k)] row-major complex128 (last axis = G,
+ *    PAPER.md:783-784), interleaved (re,im), 16-byte aligned.
+ *
+ * Pointer kinds are stated per argument: HOST or DEVICE.  No torch types, no
+ * exceptions, no printing.  Every function returns QM_OK (0) or a negative
+ * qm_status; qm_last_error() gives thread-local text for the last failure.
+ * Hot-path calls (qm_apply_h) only enqueue work on `stream` (a cudaStream_t
+ * passed as void*): no device synchronisation, no host<->device copy, no
+ * allocation after the first call with a given nbands.
+ * There is no CPU fallback: without a CUDA device every compute call fails
+ * with QM_ECUDA.
+ */
+#ifndef QM_HPSI_H
+#define QM_HPSI_H
+
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define QM_API __attribute__((visibility("default")))
+#else
+#define QM_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qm_gspace qm_gspace;                 /* opaque, owned by the library */
+typedef struct { double re, im; } qm_c128;          /* interleaved complex128 */
+
+typedef enum {
+    QM_OK = 0,
+    QM_EINVAL = -1,      /* bad argument (null pointer, k out of range, nbands <= 0, overlap ...) */
+    QM_ENOTSET = -2,     /* qm_apply_h before qm_set_vloc / qm_set_nonlocal for that k */
+    QM_EGRID = -3,       /* sphere does not fit the FFT grid (2|m_i|+1 > n_i) or grid size unsupported */
+    QM_ECUDA = -4,       /* CUDA runtime error (text in qm_last_error) */
+    QM_ENOMEM = -5       /* host or device allocation failed */
+} qm_status;
+
+/* Build the G-sphere, its sphere->box index map and the stick tables for nk k-points.
+ * (GSpace(recilat, ecut) and the per-k gkspc.)
+ *  lattice_bohr  HOST  9 doubles, rows a1,a2,a3
+ *  ecutwfc_ry          cut-off in Rydberg
+ *  fft_grid      HOST  3 ints n1,n2,n3; each must be a supported FFT length (see qm_fft_size_supported)
+ *  kpts_cryst    HOST  nk*3 doubles (may be NULL iff nk==1 => Gamma)
+ *  out                 receives the handle; destroy with qm_gspace_destroy.
+ * Uploads the tables to the current CUDA device (synchronously; this is set-up, not hot path). */
+QM_API int qm_gspace_create(const double *lattice_bohr, double ecutwfc_ry, const int *fft_grid,
+                     const double *kpts_cryst, int nk, qm_gspace **out);
+QM_API int qm_gspace_destroy(qm_gspace *g);
+
+/* Queries (HOST outputs). */
+QM_API int qm_gspace_num_k(const qm_gspace *g, int *nk);
+QM_API int qm_gspace_num_g(const qm_gspace *g, int k, int *ng);
+QM_API int qm_gspace_num_sticks(const qm_gspace *g, int k, int *nsticks, int *nxcols);
+QM_API int qm_gspace_get_index_map(const qm_gspace *g, int k, int32_t *idx_host);   /* ng */
+QM_API int qm_gspace_get_miller(const qm_gspace *g, int k, int32_t *miller_host);   /* ng*3 */
+QM_API int qm_gspace_get_g2(const qm_gspace *g, int k, double *g2_host);            /* |k+G|^2, bohr^-2 */
+/* *flag = 1 if n_i >= 4 max|m_i| + 1 on every axis (the product V*psi is alias free) */
+QM_API int qm_gspace_alias_free(const qm_gspace *g, int k, int *flag);
+/* 1 if `n` is a supported FFT length, else 0. */
+QM_API int qm_fft_size_supported(int n);
+
+/* Set the local potential (eq. 47).
+ *  V_r_dev  DEVICE  n1*n2*n3 doubles, C order, Hartree.
+ * The library copies (and re-lays-out) V on `stream`; the caller may free its buffer once the
+ * stream reaches that point. */
+QM_API int qm_set_vloc(qm_gspace *g, const double *V_r_dev, void *stream);
+
+/* Set the non-local projectors for k-point k.
+ *  beta_kG_dev  DEVICE  [nproj][ng(k)] row-major complex128
+ *  D_dev        DEVICE  (nproj/d_block) real symmetric blocks [d_block][d_block], Hartree;
+ *                       d_block == nproj => one dense matrix.  nproj % d_block == 0.
+ *  nproj == 0 (pointers may be NULL) selects a local-only Hamiltonian.
+ * The library copies both on `stream`. */
+QM_API int qm_set_nonlocal(qm_gspace *g, int k, const qm_c128 *beta_kG_dev, int nproj,
+                    const double *D_dev, int d_block, void *stream);
+
+/* psi_out = H psi_in for a block of nbands wavefunctions at k-point k.
+ *  psi_in_dev, psi_out_dev  DEVICE  [nbands][ng(k)] row-major complex128; must not overlap;
+ *                           psi_out is overwritten. */
+QM_API int qm_apply_h(qm_gspace *g, const qm_c128 *psi_in_dev, qm_c128 *psi_out_dev,
+               int nbands, int k, void *stream);
+
+/* Same operation with HOST buffers (pinned memory recommended): the library copies psi_in to
+ * a library-owned device buffer, applies H, copies the result back, all on `stream`, then
+ * synchronises the stream.  This is the end-to-end entry bench.py times. */
+QM_API int qm_apply_h_host(qm_gspace *g, const qm_c128 *psi_in_host, qm_c128 *psi_out_host,
+                    int nbands, int k, void *stream);
+
+/* Test hooks (not hot path) exercising the same kernels (A5):
+ *  qm_debug_g2r : box_r[b][n1*n2*n3] = (1/N) sum_G psi_g[b][G] e^{+iG.r}   (scatter + backward FFT)
+ *  qm_debug_r2g : psi_g[b][ng]       = sum_r box_r[b][r] e^{-iG.r}, taken on the sphere (unnormalised)
+ * all buffers DEVICE. */
+QM_API int qm_debug_g2r(qm_gspace *g, const qm_c128 *psi_g_dev, qm_c128 *box_r_dev, int nbands, int k, void *stream);
+QM_API int qm_debug_r2g(qm_gspace *g, const qm_c128 *box_r_dev, qm_c128 *psi_g_dev, int nbands, int k, void *stream);
+
+/* Number of CUDA kernels this handle has launched so far (for bench.py's gpu_launches). */
+QM_API int qm_get_launch_count(const qm_gspace *g, unsigned long long *count);
+
+/* FP64 tensor-core (DMMA m8n8k4) peak probe: runs a register-resident DMMA loop on every SM
+ * and returns the measured TFLOP/s (HOST output).  Used as the roofline denominator for the
+ * projector GEMMs (MEASURED_PEAKS.json has no FP64 entry). Synchronous. */
+QM_API int qm_probe_fp64_tensor_peak(double *tflops_dmma, double *tflops_dfma);
+
+QM_API const char *qm_last_error(void);                    /* thread-local text */
+QM_API const char *qm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QM_HPSI_H */

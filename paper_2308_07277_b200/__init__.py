@@ -1,0 +1,14 @@
+"""B200-native batched H|psi> for plane-wave Kohn-Sham DFT (the hot path of arxiv 2308.07277).
+
+The product is the C-ABI library ``libqm_hpsi.so`` (include/qm_hpsi.h, csrc/); this package is
+its thin ctypes binding.  Importing the package does not load the library; the first call does,
+and fails loudly if it has not been built (``python __graft_entry__.py``).
+"""
+from .binding import (  # noqa: F401
+    GSpace, QmError, EXPORTS, LIB_PATH, load_library,
+    qm_version, qm_fft_size_supported,
+    qm_gspace_create, qm_gspace_destroy, qm_gspace_num_k, qm_gspace_num_g, qm_gspace_num_sticks,
+    qm_gspace_get_index_map, qm_gspace_get_miller, qm_gspace_get_g2, qm_gspace_alias_free,
+    qm_set_vloc, qm_set_nonlocal, qm_apply_h, qm_apply_h_host, qm_debug_g2r, qm_debug_r2g,
+    qm_get_launch_count, qm_probe_fp64_tensor_peak,
+)

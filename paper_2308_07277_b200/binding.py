@@ -1,0 +1,288 @@
+"""Thin ctypes binding of include/qm_hpsi.h -- argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of libqm_hpsi.so; PyTorch is used for device
+memory and streams.  The functions carry the C names (qm_gspace_create, qm_set_vloc,
+qm_set_nonlocal, qm_apply_h, ...).  There is no fallback: a missing library or a failing call
+raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libqm_hpsi.so")
+
+QM_OK, QM_EINVAL, QM_ENOTSET, QM_EGRID, QM_ECUDA, QM_ENOMEM = 0, -1, -2, -3, -4, -5
+_CODES = {QM_EINVAL: "QM_EINVAL", QM_ENOTSET: "QM_ENOTSET", QM_EGRID: "QM_EGRID", QM_ECUDA: "QM_ECUDA",
+          QM_ENOMEM: "QM_ENOMEM"}
+
+
+class QmError(RuntimeError):
+    def __init__(self, code: int, text: str):
+        super().__init__(f"{_CODES.get(code, code)}: {text}")
+        self.code = code
+
+
+_lib = None
+_vp, _i, _d = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+_SIGS = {
+    "qm_gspace_create": [_vp, _d, _vp, _vp, _i, ctypes.POINTER(_vp)],
+    "qm_gspace_destroy": [_vp],
+    "qm_gspace_num_k": [_vp, ctypes.POINTER(_i)],
+    "qm_gspace_num_g": [_vp, _i, ctypes.POINTER(_i)],
+    "qm_gspace_num_sticks": [_vp, _i, ctypes.POINTER(_i), ctypes.POINTER(_i)],
+    "qm_gspace_get_index_map": [_vp, _i, _vp],
+    "qm_gspace_get_miller": [_vp, _i, _vp],
+    "qm_gspace_get_g2": [_vp, _i, _vp],
+    "qm_gspace_alias_free": [_vp, _i, ctypes.POINTER(_i)],
+    "qm_fft_size_supported": [_i],
+    "qm_set_vloc": [_vp, _vp, _vp],
+    "qm_set_nonlocal": [_vp, _i, _vp, _i, _vp, _i, _vp],
+    "qm_apply_h": [_vp, _vp, _vp, _i, _i, _vp],
+    "qm_apply_h_host": [_vp, _vp, _vp, _i, _i, _vp],
+    "qm_debug_g2r": [_vp, _vp, _vp, _i, _i, _vp],
+    "qm_debug_r2g": [_vp, _vp, _vp, _i, _i, _vp],
+    "qm_get_launch_count": [_vp, ctypes.POINTER(ctypes.c_ulonglong)],
+    "qm_probe_fp64_tensor_peak": [ctypes.POINTER(_d), ctypes.POINTER(_d)],
+}
+EXPORTS = sorted(list(_SIGS) + ["qm_last_error", "qm_version"])
+
+
+def load_library():
+    """dlopen libqm_hpsi.so (built in-tree by paper_2308_07277_b200/build.py).  Fails loudly."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python __graft_entry__.py` (build()) first; "
+                              "there is no CPU fallback")
+        lib = ctypes.CDLL(LIB_PATH)
+        for name, args in _SIGS.items():
+            fn = getattr(lib, name)
+            fn.restype = _i
+            fn.argtypes = args
+        lib.qm_last_error.restype = ctypes.c_char_p
+        lib.qm_version.restype = ctypes.c_char_p
+        _lib = lib
+    return _lib
+
+
+def _check(rc: int):
+    if rc != QM_OK:
+        raise QmError(rc, load_library().qm_last_error().decode())
+
+
+def _stream_ptr(stream):
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+def _dev_ptr(t, dtype, what):
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{what}: expected a CUDA torch.Tensor")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{what}: expected contiguous {dtype}, got {t.dtype}")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+# ---- C-named functions ---------------------------------------------------------------------------
+def qm_version() -> str:
+    return load_library().qm_version().decode()
+
+
+def qm_fft_size_supported(n: int) -> bool:
+    return bool(load_library().qm_fft_size_supported(int(n)))
+
+
+def qm_gspace_create(lattice_bohr, ecutwfc_ry, fft_grid, kpts_cryst=None):
+    lib = load_library()
+    lat = np.ascontiguousarray(lattice_bohr, dtype=np.float64).reshape(9)
+    grid = np.ascontiguousarray(fft_grid, dtype=np.int32).reshape(3)
+    if kpts_cryst is None:
+        kp, nk, kptr = None, 1, None
+    else:
+        kp = np.ascontiguousarray(kpts_cryst, dtype=np.float64).reshape(-1, 3)
+        nk, kptr = kp.shape[0], kp.ctypes.data
+    h = _vp()
+    _check(lib.qm_gspace_create(lat.ctypes.data, float(ecutwfc_ry), grid.ctypes.data, kptr, nk, ctypes.byref(h)))
+    return h
+
+
+def qm_gspace_destroy(h):
+    _check(load_library().qm_gspace_destroy(h))
+
+
+def qm_gspace_num_k(h) -> int:
+    n = _i()
+    _check(load_library().qm_gspace_num_k(h, ctypes.byref(n)))
+    return n.value
+
+
+def qm_gspace_num_g(h, k=0) -> int:
+    n = _i()
+    _check(load_library().qm_gspace_num_g(h, k, ctypes.byref(n)))
+    return n.value
+
+
+def qm_gspace_num_sticks(h, k=0):
+    s, x = _i(), _i()
+    _check(load_library().qm_gspace_num_sticks(h, k, ctypes.byref(s), ctypes.byref(x)))
+    return s.value, x.value
+
+
+def qm_gspace_get_index_map(h, k=0) -> np.ndarray:
+    out = np.empty(qm_gspace_num_g(h, k), dtype=np.int32)
+    _check(load_library().qm_gspace_get_index_map(h, k, out.ctypes.data))
+    return out
+
+
+def qm_gspace_get_miller(h, k=0) -> np.ndarray:
+    out = np.empty((qm_gspace_num_g(h, k), 3), dtype=np.int32)
+    _check(load_library().qm_gspace_get_miller(h, k, out.ctypes.data))
+    return out
+
+
+def qm_gspace_get_g2(h, k=0) -> np.ndarray:
+    out = np.empty(qm_gspace_num_g(h, k), dtype=np.float64)
+    _check(load_library().qm_gspace_get_g2(h, k, out.ctypes.data))
+    return out
+
+
+def qm_gspace_alias_free(h, k=0) -> bool:
+    f = _i()
+    _check(load_library().qm_gspace_alias_free(h, k, ctypes.byref(f)))
+    return bool(f.value)
+
+
+def qm_set_vloc(h, v_r_dev, stream=None):
+    import torch
+    _check(load_library().qm_set_vloc(h, _dev_ptr(v_r_dev, torch.float64, "V_r"), _stream_ptr(stream)))
+
+
+def qm_set_nonlocal(h, k, beta_dev, d_dev, stream=None):
+    """beta_dev [nproj][ng] complex128 CUDA tensor (or None); d_dev [nblk][db][db] float64 CUDA tensor."""
+    import torch
+    lib = load_library()
+    if beta_dev is None or beta_dev.shape[0] == 0:
+        _check(lib.qm_set_nonlocal(h, k, None, 0, None, 0, _stream_ptr(stream)))
+        return
+    nproj = beta_dev.shape[0]
+    if beta_dev.dim() != 2 or beta_dev.shape[1] != qm_gspace_num_g(h, k):
+        raise TypeError("beta: expected shape [nproj][ng(k)]")   # wrong basis => error
+    if d_dev.dim() != 3 or d_dev.shape[1] != d_dev.shape[2] or d_dev.shape[0] * d_dev.shape[1] != nproj:
+        raise TypeError("D: expected shape [nproj/d_block][d_block][d_block]")
+    _check(lib.qm_set_nonlocal(h, k, _dev_ptr(beta_dev, torch.complex128, "beta"), nproj,
+                               _dev_ptr(d_dev, torch.float64, "D"), int(d_dev.shape[1]), _stream_ptr(stream)))
+
+
+def _check_block(h, k, t, what):
+    ng = qm_gspace_num_g(h, k)
+    if t.dim() != 2 or t.shape[1] != ng:
+        raise TypeError(f"{what}: expected shape [nbands][{ng}]")     # check_array_type
+    return int(t.shape[0])
+
+
+def qm_apply_h(h, psi_in_dev, psi_out_dev, k=0, stream=None):
+    import torch
+    nb = _check_block(h, k, psi_in_dev, "psi_in")
+    if tuple(psi_out_dev.shape) != tuple(psi_in_dev.shape):
+        raise TypeError("psi_out: shape differs from psi_in")
+    _check(load_library().qm_apply_h(h, _dev_ptr(psi_in_dev, torch.complex128, "psi_in"),
+                                     _dev_ptr(psi_out_dev, torch.complex128, "psi_out"), nb, k,
+                                     _stream_ptr(stream)))
+    return psi_out_dev
+
+
+def qm_apply_h_host(h, psi_in_host, psi_out_host, k=0, stream=None):
+    """Host (ideally pinned) torch tensors [nb][ng] complex128; copies are done inside the C call."""
+    import torch
+    nb = _check_block(h, k, psi_in_host, "psi_in")
+    for t in (psi_in_host, psi_out_host):
+        if t.is_cuda or t.dtype != torch.complex128 or not t.is_contiguous():
+            raise TypeError("qm_apply_h_host: expected contiguous complex128 host tensors")
+    _check(load_library().qm_apply_h_host(h, ctypes.c_void_p(psi_in_host.data_ptr()),
+                                          ctypes.c_void_p(psi_out_host.data_ptr()), nb, k, _stream_ptr(stream)))
+    return psi_out_host
+
+
+def qm_debug_g2r(h, psi_g_dev, box_r_dev, k=0, stream=None):
+    import torch
+    nb = _check_block(h, k, psi_g_dev, "psi_g")
+    _check(load_library().qm_debug_g2r(h, _dev_ptr(psi_g_dev, torch.complex128, "psi_g"),
+                                       _dev_ptr(box_r_dev, torch.complex128, "box_r"), nb, k, _stream_ptr(stream)))
+    return box_r_dev
+
+
+def qm_debug_r2g(h, box_r_dev, psi_g_dev, k=0, stream=None):
+    import torch
+    nb = _check_block(h, k, psi_g_dev, "psi_g")
+    _check(load_library().qm_debug_r2g(h, _dev_ptr(box_r_dev, torch.complex128, "box_r"),
+                                       _dev_ptr(psi_g_dev, torch.complex128, "psi_g"), nb, k, _stream_ptr(stream)))
+    return psi_g_dev
+
+
+def qm_get_launch_count(h) -> int:
+    c = ctypes.c_ulonglong()
+    _check(load_library().qm_get_launch_count(h, ctypes.byref(c)))
+    return c.value
+
+
+def qm_probe_fp64_tensor_peak():
+    a, b = _d(), _d()
+    _check(load_library().qm_probe_fp64_tensor_peak(ctypes.byref(a), ctypes.byref(b)))
+    return a.value, b.value
+
+
+class GSpace:
+    """Owning wrapper of a qm_gspace handle (the paper's GSpace + KSHam.h_psi)."""
+
+    def __init__(self, lattice_bohr, ecutwfc_ry, fft_grid, kpts_cryst=None):
+        self.grid = tuple(int(x) for x in fft_grid)
+        self._h = qm_gspace_create(lattice_bohr, ecutwfc_ry, fft_grid, kpts_cryst)
+        self.nk = qm_gspace_num_k(self._h)
+
+    def close(self):
+        if getattr(self, "_h", None) is not None:
+            qm_gspace_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    @property
+    def handle(self):
+        return self._h
+
+    def num_g(self, k=0): return qm_gspace_num_g(self._h, k)
+    def num_sticks(self, k=0): return qm_gspace_num_sticks(self._h, k)
+    def index_map(self, k=0): return qm_gspace_get_index_map(self._h, k)
+    def miller(self, k=0): return qm_gspace_get_miller(self._h, k)
+    def g2(self, k=0): return qm_gspace_get_g2(self._h, k)
+    def alias_free(self, k=0): return qm_gspace_alias_free(self._h, k)
+    def set_vloc(self, v, stream=None): qm_set_vloc(self._h, v, stream)
+    def set_nonlocal(self, k, beta, d, stream=None): qm_set_nonlocal(self._h, k, beta, d, stream)
+
+    def apply_h(self, psi_in, psi_out=None, k=0, stream=None):
+        import torch
+        if psi_out is None:
+            psi_out = torch.empty_like(psi_in)
+        return qm_apply_h(self._h, psi_in, psi_out, k, stream)
+
+    def apply_h_host(self, psi_in, psi_out, k=0, stream=None):
+        return qm_apply_h_host(self._h, psi_in, psi_out, k, stream)
+
+    def g2r(self, psi_g, k=0, stream=None):
+        import torch
+        box = torch.empty((psi_g.shape[0], int(np.prod(self.grid))), dtype=torch.complex128, device=psi_g.device)
+        return qm_debug_g2r(self._h, psi_g, box, k, stream)
+
+    def r2g(self, box_r, k=0, stream=None):
+        import torch
+        out = torch.empty((box_r.shape[0], self.num_g(k)), dtype=torch.complex128, device=box_r.device)
+        return qm_debug_r2g(self._h, box_r, out, k, stream)
+
+    def launch_count(self): return qm_get_launch_count(self._h)

@@ -1,0 +1,118 @@
+// Phase functions of the pruned 3-D FFT pipeline ("sticks").
+//
+// A length-N line (N = R1*R2) lives in shared memory as a padded 2-D array [R1][R2P], R2P = R2|1
+// (odd pitch => the strided accesses of the second four-step pass are bank-conflict free).
+//   natural index i      <-> pos(i) = (i / R2) * R2P + i % R2
+//   transposed label p   <-> same pos(p); label p = k1*R2 + k2 stands for index k1 + R1*k2
+// Backward transform "A": natural in  -> transposed out, in place, one barrier between its two steps.
+// Forward  transform "B": transposed in -> natural out,  in place, one barrier between its two steps.
+// So G -> r -> G never needs a transpose or a digit-reversal pass: the r-space data simply lives in
+// transposed order and V_loc is re-laid-out once (qm_set_vloc) to match.
+//
+// Every function here is one "phase": it is executed by all threads of a CTA between two barriers.
+// They are __host__ __device__ so tests/test_host_emulation.py can run the identical index logic
+// on the CPU with a loop over thread ids.
+#pragma once
+#include "fft_reg.cuh"
+
+template <int R1_, int R2_> struct LineCfg {
+    static constexpr int R1 = R1_, R2 = R2_;
+    static constexpr int N = R1 * R2;
+    static constexpr int R2P = R2 | 1;
+    static constexpr int L = R1 * R2P;                  // padded line length
+    static constexpr int TT = R1 > R2 ? R1 : R2;        // team size (threads per line)
+    static QM_HD int pos(int i) { return (i / R2) * R2P + (i % R2); }
+};
+
+// tw[j] = exp(-2 pi i j / N)
+template <class C> QM_HD void lineA_step1(c128 *line, int u, const c128 *tw) {
+    if (u >= C::R2) return;
+    c128 t[C::R1];
+    static_for<C::R1>([&](auto I) { constexpr int n1 = decltype(I)::value; t[n1] = line[n1 * C::R2P + u]; });
+    Dft<C::R1, +1>::run(t);
+    static_for<C::R1>([&](auto I) {
+        constexpr int k1 = decltype(I)::value;
+        line[k1 * C::R2P + u] = (k1 == 0) ? t[k1] : cmul_conj(t[k1], tw[u * k1]);
+    });
+}
+template <class C> QM_HD void lineA_step2(c128 *line, int u) {
+    if (u >= C::R1) return;
+    c128 t[C::R2];
+    static_for<C::R2>([&](auto I) { constexpr int n2 = decltype(I)::value; t[n2] = line[u * C::R2P + n2]; });
+    Dft<C::R2, +1>::run(t);
+    static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; line[u * C::R2P + k2] = t[k2]; });
+}
+template <class C> QM_HD void lineB_step1(c128 *line, int u, const c128 *tw) {
+    if (u >= C::R1) return;
+    c128 t[C::R2];
+    static_for<C::R2>([&](auto I) { constexpr int b = decltype(I)::value; t[b] = line[u * C::R2P + b]; });
+    Dft<C::R2, -1>::run(t);
+    static_for<C::R2>([&](auto I) {
+        constexpr int d = decltype(I)::value;
+        line[u * C::R2P + d] = (d == 0) ? t[d] : cmul(t[d], tw[u * d]);
+    });
+}
+template <class C> QM_HD void lineB_step2(c128 *line, int u) {
+    if (u >= C::R2) return;
+    c128 t[C::R1];
+    static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = line[a * C::R2P + u]; });
+    Dft<C::R1, -1>::run(t);
+    static_for<C::R1>([&](auto I) { constexpr int c = decltype(I)::value; line[c * C::R2P + u] = t[c]; });
+}
+
+// ---- x direction of the plane kernel: X compact rows <-> full length-N1 line in scratch -------------
+// A: plane array [X][rowpitch]; xrow[i1] = compact row of box index i1, or -1.
+template <class C> QM_HD void xcol_step1(const c128 *A, int rowpitch, int colpos, const short *xrow,
+                                         c128 *scr, int u, const c128 *tw) {
+    if (u >= C::R2) return;
+    c128 t[C::R1];
+    static_for<C::R1>([&](auto I) {
+        constexpr int n1 = decltype(I)::value;
+        const int r = xrow[n1 * C::R2 + u];
+        t[n1] = (r >= 0) ? A[r * rowpitch + colpos] : c128{0.0, 0.0};
+    });
+    Dft<C::R1, +1>::run(t);
+    static_for<C::R1>([&](auto I) {
+        constexpr int k1 = decltype(I)::value;
+        scr[k1 * C::R2P + u] = (k1 == 0) ? t[k1] : cmul_conj(t[k1], tw[u * k1]);
+    });
+}
+// MODE 0: apply  (backward step 2, multiply by v[x], forward step 1)      PAPER.md:659-662 (eq. 47)
+// MODE 1: g2r    (backward step 2, write psi(r)*scale to box, stop)
+// MODE 2: r2g    (read box, forward step 1)
+// v: pointer to the N1 potential values of this (plane, column), natural x order.
+// box: pointer to element x=0 of this column in a natural-order box, xstride = n2*n3.
+template <class C, int MODE> QM_HD void xcol_step2(c128 *scr, int u, const c128 *tw, const double *v,
+                                                   c128 *box, long xstride, double scale) {
+    if (u >= C::R1) return;
+    c128 t[C::R2];
+    if constexpr (MODE == 2) {
+        static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; t[k2] = box[(long)(u + C::R1 * k2) * xstride]; });
+    } else {
+        static_for<C::R2>([&](auto I) { constexpr int n2 = decltype(I)::value; t[n2] = scr[u * C::R2P + n2]; });
+        Dft<C::R2, +1>::run(t);                      // t[k2] = psi(x = u + R1*k2)
+        if constexpr (MODE == 1) {
+            static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; box[(long)(u + C::R1 * k2) * xstride] = cscale(t[k2], scale); });
+            return;
+        } else {
+            static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; t[k2] = cscale(t[k2], v[u + C::R1 * k2]); });
+        }
+    }
+    Dft<C::R2, -1>::run(t);
+    static_for<C::R2>([&](auto I) {
+        constexpr int d = decltype(I)::value;
+        scr[u * C::R2P + d] = (d == 0) ? t[d] : cmul(t[d], tw[u * d]);
+    });
+}
+template <class C> QM_HD void xcol_step3(c128 *A, int rowpitch, int colpos, const short *xrow,
+                                         const c128 *scr, int u) {
+    if (u >= C::R2) return;
+    c128 t[C::R1];
+    static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = scr[a * C::R2P + u]; });
+    Dft<C::R1, -1>::run(t);
+    static_for<C::R1>([&](auto I) {
+        constexpr int c = decltype(I)::value;
+        const int r = xrow[u + C::R2 * c];
+        if (r >= 0) A[r * rowpitch + colpos] = t[c];
+    });
+}

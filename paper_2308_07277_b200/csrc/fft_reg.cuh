@@ -1,0 +1,131 @@
+// In-register complex128 DFT codelets (radix 2,3,4,5 and their composites) for sm_100a.
+// Sign convention: DIR = -1 forward  e^{-2 pi i jk/R}  (r -> G),
+//                  DIR = +1 backward e^{+2 pi i jk/R}  (G -> r, eq. 9).
+// Everything is resolved at compile time (static indices only) so the arrays live in registers.
+#pragma once
+#include <utility>
+#include "roots_gen.cuh"
+
+#ifndef QM_HD
+#define QM_HD __host__ __device__ __forceinline__
+#endif
+
+struct __align__(16) c128 { double x, y; };
+
+QM_HD c128 operator+(c128 a, c128 b) { return {a.x + b.x, a.y + b.y}; }
+QM_HD c128 operator-(c128 a, c128 b) { return {a.x - b.x, a.y - b.y}; }
+QM_HD c128 cmul(c128 a, c128 b) {
+    return {a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x};
+}
+QM_HD c128 cmul_conj(c128 a, c128 b) {   // a * conj(b)
+    return {a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y};
+}
+QM_HD c128 cscale(c128 a, double s) { return {a.x * s, a.y * s}; }
+
+// multiply by (DIR * i)
+template <int DIR> QM_HD c128 mul_i(c128 a) {
+    if constexpr (DIR > 0) return {-a.y, a.x};
+    else return {a.y, -a.x};
+}
+
+template <class F, int... I>
+QM_HD void static_for_impl(F &&f, std::integer_sequence<int, I...>) {
+    (f(std::integral_constant<int, I>{}), ...);
+}
+template <int N, class F> QM_HD void static_for(F &&f) {
+    static_for_impl(f, std::make_integer_sequence<int, N>{});
+}
+
+// a * exp(DIR * 2 pi i J / R), J and R compile-time
+template <int R, int J, int DIR> QM_HD c128 mul_root(c128 a) {
+    constexpr int j = ((J % R) + R) % R;
+    if constexpr (j == 0) return a;
+    else if constexpr (2 * j == R) return {-a.x, -a.y};
+    else if constexpr (4 * j == R) return mul_i<DIR>(a);
+    else if constexpr (4 * j == 3 * R) return mul_i<-DIR>(a);
+    else {
+        constexpr double c = qm_cos2pi(j, R);
+        constexpr double s = (DIR > 0 ? 1.0 : -1.0) * qm_sin2pi(j, R);
+        return {a.x * c - a.y * s, a.x * s + a.y * c};
+    }
+}
+
+template <int R, int DIR> struct Dft;
+
+template <int DIR> struct Dft<1, DIR> {
+    static QM_HD void run(c128 (&)[1]) {}
+};
+template <int DIR> struct Dft<2, DIR> {
+    static QM_HD void run(c128 (&x)[2]) {
+        c128 a = x[0], b = x[1];
+        x[0] = a + b; x[1] = a - b;
+    }
+};
+template <int DIR> struct Dft<3, DIR> {
+    static QM_HD void run(c128 (&x)[3]) {
+        constexpr double s3 = 0.8660254037844386;   // sqrt(3)/2
+        c128 t1 = x[1] + x[2];
+        c128 t2 = {x[0].x - 0.5 * t1.x, x[0].y - 0.5 * t1.y};
+        c128 d = x[1] - x[2];
+        c128 t3 = mul_i<DIR>(c128{s3 * d.x, s3 * d.y});
+        x[0] = x[0] + t1;
+        x[1] = t2 + t3;
+        x[2] = t2 - t3;
+    }
+};
+template <int DIR> struct Dft<4, DIR> {
+    static QM_HD void run(c128 (&x)[4]) {
+        c128 s02 = x[0] + x[2], d02 = x[0] - x[2];
+        c128 s13 = x[1] + x[3], d13 = mul_i<DIR>(x[1] - x[3]);
+        x[0] = s02 + s13; x[2] = s02 - s13;
+        x[1] = d02 + d13; x[3] = d02 - d13;
+    }
+};
+template <int DIR> struct Dft<5, DIR> {
+    static QM_HD void run(c128 (&x)[5]) {
+        constexpr double c1 = qm_cos2pi(1, 5), c2 = qm_cos2pi(2, 5);
+        constexpr double s1 = qm_sin2pi(1, 5), s2 = qm_sin2pi(2, 5);
+        c128 a14 = x[1] + x[4], d14 = x[1] - x[4];
+        c128 a23 = x[2] + x[3], d23 = x[2] - x[3];
+        c128 p1 = {x[0].x + c1 * a14.x + c2 * a23.x, x[0].y + c1 * a14.y + c2 * a23.y};
+        c128 p2 = {x[0].x + c2 * a14.x + c1 * a23.x, x[0].y + c2 * a14.y + c1 * a23.y};
+        c128 q1 = mul_i<DIR>(c128{s1 * d14.x + s2 * d23.x, s1 * d14.y + s2 * d23.y});
+        c128 q2 = mul_i<DIR>(c128{s2 * d14.x - s1 * d23.x, s2 * d14.y - s1 * d23.y});
+        x[0] = x[0] + a14 + a23;
+        x[1] = p1 + q1; x[4] = p1 - q1;
+        x[2] = p2 + q2; x[3] = p2 - q2;
+    }
+};
+
+// R = RA * RB, input index n = n1*RB + n2, output index k = k1 + RA*k2 (natural order in place).
+template <int RA, int RB, int DIR> struct DftComposite {
+    static constexpr int R = RA * RB;
+    static QM_HD void run(c128 (&x)[R]) {
+        c128 y[R];
+        static_for<RB>([&](auto N2) {
+            constexpr int n2 = decltype(N2)::value;
+            c128 t[RA];
+            static_for<RA>([&](auto N1) { constexpr int n1 = decltype(N1)::value; t[n1] = x[n1 * RB + n2]; });
+            Dft<RA, DIR>::run(t);
+            static_for<RA>([&](auto K1) {
+                constexpr int k1 = decltype(K1)::value;
+                y[k1 * RB + n2] = mul_root<R, n2 * k1, DIR>(t[k1]);
+            });
+        });
+        static_for<RA>([&](auto K1) {
+            constexpr int k1 = decltype(K1)::value;
+            c128 t[RB];
+            static_for<RB>([&](auto N2) { constexpr int n2 = decltype(N2)::value; t[n2] = y[k1 * RB + n2]; });
+            Dft<RB, DIR>::run(t);
+            static_for<RB>([&](auto K2) { constexpr int k2 = decltype(K2)::value; x[k1 + RA * k2] = t[k2]; });
+        });
+    }
+};
+
+template <int DIR> struct Dft<6, DIR> { static QM_HD void run(c128 (&x)[6]) { DftComposite<2, 3, DIR>::run(x); } };
+template <int DIR> struct Dft<8, DIR> { static QM_HD void run(c128 (&x)[8]) { DftComposite<2, 4, DIR>::run(x); } };
+template <int DIR> struct Dft<9, DIR> { static QM_HD void run(c128 (&x)[9]) { DftComposite<3, 3, DIR>::run(x); } };
+template <int DIR> struct Dft<10, DIR> { static QM_HD void run(c128 (&x)[10]) { DftComposite<2, 5, DIR>::run(x); } };
+template <int DIR> struct Dft<12, DIR> { static QM_HD void run(c128 (&x)[12]) { DftComposite<3, 4, DIR>::run(x); } };
+template <int DIR> struct Dft<15, DIR> { static QM_HD void run(c128 (&x)[15]) { DftComposite<3, 5, DIR>::run(x); } };
+template <int DIR> struct Dft<16, DIR> { static QM_HD void run(c128 (&x)[16]) { DftComposite<4, 4, DIR>::run(x); } };

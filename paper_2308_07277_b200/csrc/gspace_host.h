@@ -1,0 +1,124 @@
+// Host-side set-up of one k-point: G-sphere enumeration, sphere->box index map, stick tables.
+// Pure C++ (no CUDA): used by qm_api.cu and by the CPU thread-emulation test (tests/host_emu).
+//   sphere:  all integer m with |k + G_m|^2 [bohr^-2] <= ecutwfc [Ry]
+//   order:   ascending idx = ((m1 mod n1)*n2 + (m2 mod n2))*n3 + (m3 mod n3)
+//   sticks:  the (i1,i2) lines of the box that hold at least one G
+#pragma once
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <string>
+#include <vector>
+#include "qm_plan.h"
+
+struct FftSize { int n, r1, r2; };
+// supported FFT lengths and their two-pass factorisation n = r1 * r2
+static const FftSize kQmSizes[] = {
+    {8, 2, 4},   {12, 3, 4},  {16, 4, 4},  {18, 3, 6},  {20, 4, 5},   {24, 4, 6},   {30, 5, 6},
+    {32, 4, 8},  {36, 6, 6},  {40, 5, 8},  {48, 6, 8},  {60, 6, 10},  {64, 8, 8},   {72, 8, 9},
+    {80, 8, 10}, {96, 8, 12}, {100, 10, 10}, {108, 9, 12}, {120, 10, 12}, {128, 8, 16}, {144, 12, 12},
+};
+static inline const FftSize *qm_find_size(int n) {
+    for (const auto &s : kQmSizes) if (s.n == n) return &s;
+    return nullptr;
+}
+static inline QmAxis qm_make_axis(const FftSize &s) {
+    QmAxis a; a.n = s.n; a.r1 = s.r1; a.r2 = s.r2; a.r2p = s.r2 | 1; a.len = s.r1 * a.r2p; return a;
+}
+
+static inline void qm_reciprocal(const double *a, double *b) {
+    // b_i = rows of 2 pi (A^-1)^T; (A^-1)^T = cofactor matrix / det
+    const double c00 = a[4] * a[8] - a[5] * a[7], c01 = a[5] * a[6] - a[3] * a[8], c02 = a[3] * a[7] - a[4] * a[6];
+    const double c10 = a[2] * a[7] - a[1] * a[8], c11 = a[0] * a[8] - a[2] * a[6], c12 = a[1] * a[6] - a[0] * a[7];
+    const double c20 = a[1] * a[5] - a[2] * a[4], c21 = a[2] * a[3] - a[0] * a[5], c22 = a[0] * a[4] - a[1] * a[3];
+    const double det = a[0] * c00 + a[1] * c01 + a[2] * c02;
+    const double f = 2.0 * M_PI / det;
+    b[0] = f * c00; b[1] = f * c01; b[2] = f * c02;
+    b[3] = f * c10; b[4] = f * c11; b[5] = f * c12;
+    b[6] = f * c20; b[7] = f * c21; b[8] = f * c22;
+}
+
+struct QmKTables {
+    double k[3] = {0, 0, 0};
+    int ng = 0, nsticks = 0, nx = 0, rowpitch = 0;
+    int mmax[3] = {0, 0, 0};
+    std::vector<int32_t> idx, miller;          // miller: ng*3
+    std::vector<double> g2;
+    std::vector<int32_t> gstick, stickoff, stickapos;
+    std::vector<uint16_t> gzpos;
+    std::vector<int16_t> xrow;
+};
+
+// returns 0, or -1 (sphere does not fit the grid) / -2 (empty sphere); msg gets the reason
+static inline int qm_build_tables(const double *lattice, const double *recip, double ecut, const int *grid,
+                                  const QmAxis *ax, QmKTables *kp, std::string *msg)
+{
+    const double *b = recip, *a = lattice;
+    const int n1 = grid[0], n2 = grid[1], n3 = grid[2];
+    const double qmax = std::sqrt(ecut);
+    int bound[3];
+    for (int i = 0; i < 3; ++i) {
+        const double an = std::sqrt(a[3 * i] * a[3 * i] + a[3 * i + 1] * a[3 * i + 1] + a[3 * i + 2] * a[3 * i + 2]);
+        bound[i] = (int)std::floor(qmax * an / (2.0 * M_PI) + std::fabs(kp->k[i])) + 1;
+    }
+    struct Ent { int64_t idx; int m[3]; double g2; };
+    std::vector<Ent> ents;
+    for (int m1 = -bound[0]; m1 <= bound[0]; ++m1)
+        for (int m2 = -bound[1]; m2 <= bound[1]; ++m2)
+            for (int m3 = -bound[2]; m3 <= bound[2]; ++m3) {
+                const double f1 = m1 + kp->k[0], f2 = m2 + kp->k[1], f3 = m3 + kp->k[2];
+                const double qx = f1 * b[0] + f2 * b[3] + f3 * b[6];
+                const double qy = f1 * b[1] + f2 * b[4] + f3 * b[7];
+                const double qz = f1 * b[2] + f2 * b[5] + f3 * b[8];
+                const double q2 = qx * qx + qy * qy + qz * qz;
+                if (q2 <= ecut) {
+                    Ent e; e.m[0] = m1; e.m[1] = m2; e.m[2] = m3; e.g2 = q2; e.idx = 0;
+                    ents.push_back(e);
+                    kp->mmax[0] = std::max(kp->mmax[0], std::abs(m1));
+                    kp->mmax[1] = std::max(kp->mmax[1], std::abs(m2));
+                    kp->mmax[2] = std::max(kp->mmax[2], std::abs(m3));
+                }
+            }
+    for (int i = 0; i < 3; ++i)
+        if (2 * kp->mmax[i] + 1 > grid[i]) { *msg = "G-sphere does not fit the FFT grid (2|m|+1 > n)"; return -1; }
+    if (ents.empty()) { *msg = "empty G-sphere"; return -2; }
+    auto wrapi = [](int m, int n) { int r = m % n; return r < 0 ? r + n : r; };
+    for (auto &e : ents)
+        e.idx = ((int64_t)wrapi(e.m[0], n1) * n2 + wrapi(e.m[1], n2)) * n3 + wrapi(e.m[2], n3);
+    std::sort(ents.begin(), ents.end(), [](const Ent &x, const Ent &y) { return x.idx < y.idx; });
+    const int ng = (int)ents.size();
+    kp->ng = ng;
+    kp->idx.resize(ng); kp->miller.resize((size_t)ng * 3); kp->g2.resize(ng);
+    kp->gstick.resize(ng); kp->gzpos.resize(ng);
+    kp->stickoff.clear();
+    std::vector<int32_t> stick_i1, stick_i2;
+    int64_t cur = -1;
+    for (int i = 0; i < ng; ++i) {
+        const Ent &e = ents[i];
+        kp->idx[i] = (int32_t)e.idx;
+        kp->miller[3 * i] = e.m[0]; kp->miller[3 * i + 1] = e.m[1]; kp->miller[3 * i + 2] = e.m[2];
+        kp->g2[i] = e.g2;
+        const int64_t line = e.idx / n3;
+        if (line != cur) {
+            cur = line;
+            kp->stickoff.push_back(i);
+            stick_i1.push_back((int)(line / n2));
+            stick_i2.push_back((int)(line % n2));
+        }
+        kp->gstick[i] = (int32_t)kp->stickoff.size() - 1;
+        kp->gzpos[i] = (uint16_t)qm_pos(ax[2], (int)(e.idx % n3));
+    }
+    const int S = (int)kp->stickoff.size();
+    kp->stickoff.push_back(ng);
+    kp->nsticks = S;
+    kp->xrow.assign(n1, -1);
+    int nx = 0;
+    for (int s = 0; s < S; ++s)
+        if (kp->xrow[stick_i1[s]] < 0) kp->xrow[stick_i1[s]] = (int16_t)nx++;   // sticks ascend in i1
+    kp->nx = nx;
+    kp->rowpitch = ax[1].len | 1;
+    kp->stickapos.resize(S);
+    for (int s = 0; s < S; ++s)
+        kp->stickapos[s] = kp->xrow[stick_i1[s]] * kp->rowpitch + qm_pos(ax[1], stick_i2[s]);
+    return 0;
+}

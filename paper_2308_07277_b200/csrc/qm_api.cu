@@ -1,0 +1,503 @@
+// C ABI of libqm_hpsi (see include/qm_hpsi.h).  Host-side set-up (G-sphere, stick tables) and
+// kernel launches.  No CPU fallback: compute entry points fail with QM_ECUDA without a device.
+#include <cuda_runtime.h>
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/qm_hpsi.h"
+#include "fft_kernels.cuh"
+#include "proj_kernels.cuh"
+#include "qm_plan.h"
+#include "gspace_host.h"
+
+namespace {
+
+thread_local std::string g_err;
+int fail(int code, const std::string &msg) { g_err = msg; return code; }
+
+#define CU_TRY(expr)                                                                        \
+    do {                                                                                    \
+        cudaError_t _e = (expr);                                                            \
+        if (_e != cudaSuccess)                                                              \
+            return fail(_e == cudaErrorMemoryAllocation ? QM_ENOMEM : QM_ECUDA,             \
+                        std::string(#expr) + ": " + cudaGetErrorString(_e));                \
+    } while (0)
+
+template <class T> struct DevBuf {
+    T *p = nullptr; size_t n = 0;
+    ~DevBuf() { if (p) cudaFree(p); }
+    cudaError_t resize(size_t m) {
+        if (m <= n) return cudaSuccess;
+        if (p) { cudaFree(p); p = nullptr; n = 0; }
+        cudaError_t e = cudaMalloc(&p, m * sizeof(T));
+        if (e == cudaSuccess) n = m;
+        return e;
+    }
+    cudaError_t upload(const std::vector<T> &h) {
+        cudaError_t e = resize(h.size() ? h.size() : 1);
+        if (e != cudaSuccess) return e;
+        if (h.empty()) return cudaSuccess;
+        return cudaMemcpy(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice);
+    }
+};
+
+struct KPoint : QmKTables {
+    DevBuf<int32_t> d_gstick, d_stickoff, d_stickapos;
+    DevBuf<uint16_t> d_gzpos;
+    DevBuf<int16_t> d_xrow;
+    DevBuf<double> d_g2;
+    // non-local
+    bool nl_set = false;
+    int nproj = 0, nproj_pad = 0, ldb = 0, dblock = 0;
+    DevBuf<c128> d_beta;
+    DevBuf<double> d_D;
+    QmKPlanDev plan() const {
+        QmKPlanDev p;
+        p.ng = ng; p.nsticks = nsticks; p.nx = nx; p.rowpitch = rowpitch;
+        p.g_stick = d_gstick.p; p.g_zpos = d_gzpos.p; p.stick_off = d_stickoff.p;
+        p.stick_apos = d_stickapos.p; p.xrow = d_xrow.p; p.g2 = d_g2.p;
+        return p;
+    }
+};
+
+}  // namespace
+
+struct qm_gspace {
+    double lattice[9], recip[9];
+    double ecut;
+    int grid[3];
+    QmAxis ax[3];
+    std::vector<KPoint *> kpts;
+    DevBuf<c128> d_tw[3];
+    DevBuf<double> d_vt;
+    bool v_set = false;
+    DevBuf<c128> d_W, d_Ppart, d_P, d_Q, d_stage_in, d_stage_out;
+    unsigned long long launches = 0;
+    int sm_count = 148;
+    int max_smem = 0;
+    ~qm_gspace() { for (auto *k : kpts) delete k; }
+};
+
+namespace {
+
+constexpr int PROJ_MT = 4, PROJ_NT = 2, PROJ_WARPS = 4;
+constexpr int PROJ_MBLK = 8 * PROJ_MT * PROJ_WARPS;   // 128 rows (GEMM1) / 128 G (GEMM2) per CTA
+constexpr int PROJ_NB = 8 * PROJ_NT;                  // bands per projector pass
+constexpr int ZT_STICKS = 16;                         // sticks per CTA in the z kernels
+
+int build_kpoint(qm_gspace *g, KPoint *kp) {
+    std::string msg;
+    const int rc = qm_build_tables(g->lattice, g->recip, g->ecut, g->grid, g->ax, kp, &msg);
+    if (rc == -1) return fail(QM_EGRID, msg);
+    if (rc != 0) return fail(QM_EINVAL, msg);
+    CU_TRY(kp->d_gstick.upload(kp->gstick));
+    CU_TRY(kp->d_gzpos.upload(kp->gzpos));
+    CU_TRY(kp->d_stickoff.upload(kp->stickoff));
+    CU_TRY(kp->d_stickapos.upload(kp->stickapos));
+    CU_TRY(kp->d_xrow.upload(kp->xrow));
+    CU_TRY(kp->d_g2.upload(kp->g2));
+    return QM_OK;
+}
+
+size_t plane_smem(const qm_gspace *g, const KPoint *kp, int ncol) {
+    const QmAxis &ax = g->ax[0];
+    const size_t sl = (size_t)(ax.len | 1);
+    return ((size_t)ax.n + (size_t)kp->nx * kp->rowpitch + (size_t)ncol * sl) * sizeof(c128)
+           + (size_t)ax.n * sizeof(short) + 16;
+}
+
+// choose the number of columns processed concurrently by the plane kernel
+int plane_ncol(const qm_gspace *g, const KPoint *kp) {
+    const QmAxis &ax = g->ax[0];
+    const int tt = std::max(ax.r1, ax.r2);
+    int ncol = std::min(ax.n, 512 / tt);
+    while (ncol > 1 && plane_smem(g, kp, ncol) > (size_t)g->max_smem) --ncol;
+    // prefer a divisor-friendly count so the last pass is not mostly idle
+    int best = ncol;
+    for (int c = ncol; c >= std::max(1, ncol - ncol / 4); --c)
+        if (ax.n % c == 0) { best = c; break; }
+    return best;
+}
+
+template <class C> int launch_zinv(qm_gspace *g, KPoint *kp, const c128 *psi, int nb, cudaStream_t st) {
+    const int TS = ZT_STICKS;
+    const size_t smem = ((size_t)C::N + (size_t)TS * (C::L | 1)) * sizeof(c128);
+    static bool attr = false;
+    if (!attr) { CU_TRY(cudaFuncSetAttribute(k_zinv<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
+    dim3 grid((kp->nsticks + TS - 1) / TS, nb);
+    k_zinv<C><<<grid, TS * C::TT, smem, st>>>(kp->plan(), g->d_tw[2].p, psi, g->d_W.p, TS);
+    g->launches++;
+    CU_TRY(cudaGetLastError());
+    return QM_OK;
+}
+template <class C> int launch_zfwd(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb, int kinetic,
+                                   cudaStream_t st) {
+    const int TS = ZT_STICKS;
+    const size_t smem = ((size_t)C::N + (size_t)TS * (C::L | 1)) * sizeof(c128);
+    static bool attr = false;
+    if (!attr) { CU_TRY(cudaFuncSetAttribute(k_zfwd<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
+    dim3 grid((kp->nsticks + TS - 1) / TS, nb);
+    k_zfwd<C><<<grid, TS * C::TT, smem, st>>>(kp->plan(), g->d_tw[2].p, g->d_W.p, psi_in, out, TS, kinetic);
+    g->launches++;
+    CU_TRY(cudaGetLastError());
+    return QM_OK;
+}
+template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *box, int nb, double scale,
+                                              cudaStream_t st) {
+    const int ncol = plane_ncol(g, kp);
+    const size_t smem = plane_smem(g, kp, ncol);
+    if (smem > (size_t)g->max_smem)
+        return fail(QM_EGRID, "plane kernel does not fit shared memory for this grid / sphere");
+    CU_TRY(cudaFuncSetAttribute(k_plane<C, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    QmGridDev gd;
+    for (int i = 0; i < 3; ++i) { gd.ax[i] = g->ax[i]; gd.tw[i] = g->d_tw[i].p; }
+    gd.vt = g->d_vt.p;
+    dim3 grid(g->grid[2], nb);
+    k_plane<C, MODE><<<grid, ncol * C::TT, smem, st>>>(kp->plan(), gd, g->d_W.p, box, ncol, scale);
+    g->launches++;
+    CU_TRY(cudaGetLastError());
+    return QM_OK;
+}
+
+// dispatch on FFT length ---------------------------------------------------------------------
+#define QM_FOR_SIZES(X)                                                                              \
+    X(8, 2, 4) X(12, 3, 4) X(16, 4, 4) X(18, 3, 6) X(20, 4, 5) X(24, 4, 6) X(30, 5, 6) X(32, 4, 8)   \
+    X(36, 6, 6) X(40, 5, 8) X(48, 6, 8) X(60, 6, 10) X(64, 8, 8) X(72, 8, 9) X(80, 8, 10)            \
+    X(96, 8, 12) X(100, 10, 10) X(108, 9, 12) X(120, 10, 12) X(128, 8, 16) X(144, 12, 12)
+
+int dispatch_zinv(qm_gspace *g, KPoint *kp, const c128 *psi, int nb, cudaStream_t st) {
+    switch (g->grid[2]) {
+#define X(N, A, B) case N: return launch_zinv<LineCfg<A, B>>(g, kp, psi, nb, st);
+        QM_FOR_SIZES(X)
+#undef X
+    }
+    return fail(QM_EGRID, "unsupported FFT length (axis 3)");
+}
+int dispatch_zfwd(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb, int kinetic, cudaStream_t st) {
+    switch (g->grid[2]) {
+#define X(N, A, B) case N: return launch_zfwd<LineCfg<A, B>>(g, kp, psi_in, out, nb, kinetic, st);
+        QM_FOR_SIZES(X)
+#undef X
+    }
+    return fail(QM_EGRID, "unsupported FFT length (axis 3)");
+}
+template <int MODE> int dispatch_plane(qm_gspace *g, KPoint *kp, c128 *box, int nb, double scale, cudaStream_t st) {
+    switch (g->grid[0]) {
+#define X(N, A, B) case N: return launch_plane<LineCfg<A, B>, MODE>(g, kp, box, nb, scale, st);
+        QM_FOR_SIZES(X)
+#undef X
+    }
+    return fail(QM_EGRID, "unsupported FFT length (axes 1,2)");
+}
+
+__global__ void k_relayout_v(const double *__restrict__ v, double *__restrict__ vt, QmAxis a1, QmAxis a2, QmAxis a3,
+                             double scale)
+{
+    // vt[p][col][x] = scale * v[x][y(col)][z(p)]
+    const size_t total = (size_t)a1.n * a2.n * a3.n;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int x = (int)(i % a1.n);
+        const int col = (int)((i / a1.n) % a2.n);
+        const int p = (int)(i / ((size_t)a1.n * a2.n));
+        const int y = (col / a2.r2) + a2.r1 * (col % a2.r2);
+        const int z = (p / a3.r2) + a3.r1 * (p % a3.r2);
+        vt[i] = scale * v[((size_t)x * a2.n + y) * a3.n + z];
+    }
+}
+
+__global__ void k_pad_beta(const c128 *__restrict__ src, int ng, int nproj, c128 *__restrict__ dst, int ldb,
+                           int nproj_pad)
+{
+    const size_t total = (size_t)nproj_pad * ldb;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int row = (int)(i / ldb), col = (int)(i % ldb);
+        dst[i] = (row < nproj && col < ng) ? src[(size_t)row * ng + col] : c128{0.0, 0.0};
+    }
+}
+
+int check_handle(const qm_gspace *g, int k) {
+    if (!g) return fail(QM_EINVAL, "null handle");
+    if (k < 0 || k >= (int)g->kpts.size()) return fail(QM_EINVAL, "k-point index out of range");
+    return QM_OK;
+}
+
+int ensure_workspace(qm_gspace *g, const KPoint *kp, int nb) {
+    CU_TRY(g->d_W.resize((size_t)nb * g->grid[2] * kp->nsticks));
+    return QM_OK;
+}
+
+int run_nonlocal(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb, cudaStream_t st) {
+    if (kp->nproj == 0) return QM_OK;
+    const int nbp = PROJ_NB;
+    const int mblocks = kp->nproj_pad / PROJ_MBLK;
+    int nsplit = std::max(1, (g->sm_count * 4) / std::max(1, mblocks));
+    int kchunk = (kp->ng + nsplit - 1) / nsplit;
+    kchunk = std::max(64, ((kchunk + 3) / 4) * 4);
+    nsplit = (kp->ng + kchunk - 1) / kchunk;
+    const size_t pcount = (size_t)kp->nproj_pad * nbp;
+    CU_TRY(g->d_Ppart.resize(pcount * nsplit));
+    CU_TRY(g->d_P.resize(pcount));
+    CU_TRY(g->d_Q.resize(pcount));
+    for (int band0 = 0; band0 < nb; band0 += PROJ_NB) {
+        dim3 g1(mblocks, nsplit);
+        k_proj1_direct<PROJ_MT, PROJ_NT, PROJ_WARPS><<<g1, PROJ_WARPS * 32, 0, st>>>(
+            kp->d_beta.p, kp->ldb, psi_in, kp->ng, nb, band0, nbp, kp->nproj_pad, g->d_Ppart.p, kchunk);
+        k_reduce_p<<<(unsigned)((pcount + 255) / 256), 256, 0, st>>>(g->d_Ppart.p, nsplit, (int)pcount, g->d_P.p);
+        k_dmul<<<(unsigned)((pcount + 255) / 256), 256, 0, st>>>(kp->d_D.p, kp->dblock, kp->nproj, kp->nproj_pad, nbp,
+                                                                 g->d_P.p, g->d_Q.p);
+        const int gblocks = (kp->ng + PROJ_MBLK - 1) / PROJ_MBLK;
+        k_proj2_direct<PROJ_MT, PROJ_NT, PROJ_WARPS><<<gblocks, PROJ_WARPS * 32, 0, st>>>(
+            kp->d_beta.p, kp->ldb, g->d_Q.p, nbp, kp->nproj_pad, kp->ng, nb, band0, out);
+        g->launches += 4;
+    }
+    CU_TRY(cudaGetLastError());
+    return QM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+QM_API const char *qm_last_error(void) { return g_err.c_str(); }
+QM_API const char *qm_version(void) { return "qm_hpsi 0.1 (sm_100a)"; }
+
+QM_API int qm_fft_size_supported(int n) { return qm_find_size(n) ? 1 : 0; }
+
+QM_API int qm_gspace_create(const double *lattice_bohr, double ecutwfc_ry, const int *fft_grid,
+                     const double *kpts_cryst, int nk, qm_gspace **out)
+{
+    if (!lattice_bohr || !fft_grid || !out || nk < 1 || !(ecutwfc_ry > 0.0))
+        return fail(QM_EINVAL, "qm_gspace_create: bad argument");
+    if (!kpts_cryst && nk != 1) return fail(QM_EINVAL, "qm_gspace_create: kpts_cryst is NULL with nk > 1");
+    *out = nullptr;
+    for (int i = 0; i < 3; ++i)
+        if (!qm_find_size(fft_grid[i])) return fail(QM_EGRID, "unsupported FFT length " + std::to_string(fft_grid[i]));
+    if (fft_grid[0] != fft_grid[1]) return fail(QM_EGRID, "this version needs n1 == n2");
+    int dev = 0, count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || count == 0)
+        return fail(QM_ECUDA, "no CUDA device (there is no CPU fallback)");
+    qm_gspace *g = new (std::nothrow) qm_gspace();
+    if (!g) return fail(QM_ENOMEM, "host allocation failed");
+    std::memcpy(g->lattice, lattice_bohr, sizeof(g->lattice));
+    qm_reciprocal(g->lattice, g->recip);
+    g->ecut = ecutwfc_ry;
+    for (int i = 0; i < 3; ++i) { g->grid[i] = fft_grid[i]; g->ax[i] = qm_make_axis(*qm_find_size(fft_grid[i])); }
+    int rc = QM_OK;
+    auto bail = [&](int code) { delete g; return code; };
+    {
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&g->sm_count, cudaDevAttrMultiProcessorCount, dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&g->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+        if (e != cudaSuccess) { fail(QM_ECUDA, cudaGetErrorString(e)); return bail(QM_ECUDA); }
+    }
+    for (int a = 0; a < 3; ++a) {
+        const int n = g->grid[a];
+        std::vector<c128> tw(n);
+        for (int j = 0; j < n; ++j) {
+            // exact octant symmetries first, long double elsewhere
+            const long double ang = -2.0L * 3.14159265358979323846264338327950288L * (long double)j / (long double)n;
+            double c = (double)cosl(ang), s = (double)sinl(ang);
+            if ((4 * j) % n == 0) {
+                const int q = (4 * j) / n;
+                const double cc[4] = {1, 0, -1, 0}, ss[4] = {0, -1, 0, 1};
+                c = cc[q]; s = ss[q];
+            }
+            tw[j] = c128{c, s};
+        }
+        cudaError_t e = g->d_tw[a].upload(tw);
+        if (e != cudaSuccess) { fail(QM_ECUDA, cudaGetErrorString(e)); return bail(QM_ECUDA); }
+    }
+    for (int ik = 0; ik < nk; ++ik) {
+        KPoint *kp = new (std::nothrow) KPoint();
+        if (!kp) { fail(QM_ENOMEM, "host allocation failed"); return bail(QM_ENOMEM); }
+        g->kpts.push_back(kp);
+        for (int i = 0; i < 3; ++i) kp->k[i] = kpts_cryst ? kpts_cryst[3 * ik + i] : 0.0;
+        rc = build_kpoint(g, kp);
+        if (rc != QM_OK) return bail(rc);
+        if (plane_smem(g, kp, 1) > (size_t)g->max_smem) {
+            fail(QM_EGRID, "plane working set exceeds shared memory for this grid / sphere");
+            return bail(QM_EGRID);
+        }
+    }
+    *out = g;
+    return QM_OK;
+}
+
+QM_API int qm_gspace_destroy(qm_gspace *g) { delete g; return QM_OK; }
+
+QM_API int qm_gspace_num_k(const qm_gspace *g, int *nk) {
+    if (!g || !nk) return fail(QM_EINVAL, "null argument");
+    *nk = (int)g->kpts.size(); return QM_OK;
+}
+QM_API int qm_gspace_num_g(const qm_gspace *g, int k, int *ng) {
+    int rc = check_handle(g, k); if (rc) return rc;
+    if (!ng) return fail(QM_EINVAL, "null argument");
+    *ng = g->kpts[k]->ng; return QM_OK;
+}
+QM_API int qm_gspace_num_sticks(const qm_gspace *g, int k, int *nsticks, int *nxcols) {
+    int rc = check_handle(g, k); if (rc) return rc;
+    if (nsticks) *nsticks = g->kpts[k]->nsticks;
+    if (nxcols) *nxcols = g->kpts[k]->nx;
+    return QM_OK;
+}
+QM_API int qm_gspace_get_index_map(const qm_gspace *g, int k, int32_t *idx_host) {
+    int rc = check_handle(g, k); if (rc) return rc;
+    if (!idx_host) return fail(QM_EINVAL, "null argument");
+    std::memcpy(idx_host, g->kpts[k]->idx.data(), g->kpts[k]->idx.size() * sizeof(int32_t)); return QM_OK;
+}
+QM_API int qm_gspace_get_miller(const qm_gspace *g, int k, int32_t *m_host) {
+    int rc = check_handle(g, k); if (rc) return rc;
+    if (!m_host) return fail(QM_EINVAL, "null argument");
+    std::memcpy(m_host, g->kpts[k]->miller.data(), g->kpts[k]->miller.size() * sizeof(int32_t)); return QM_OK;
+}
+QM_API int qm_gspace_get_g2(const qm_gspace *g, int k, double *g2_host) {
+    int rc = check_handle(g, k); if (rc) return rc;
+    if (!g2_host) return fail(QM_EINVAL, "null argument");
+    std::memcpy(g2_host, g->kpts[k]->g2.data(), g->kpts[k]->g2.size() * sizeof(double)); return QM_OK;
+}
+QM_API int qm_gspace_alias_free(const qm_gspace *g, int k, int *flag) {
+    int rc = check_handle(g, k); if (rc) return rc;
+    if (!flag) return fail(QM_EINVAL, "null argument");
+    *flag = 1;
+    for (int i = 0; i < 3; ++i) if (4 * g->kpts[k]->mmax[i] + 1 > g->grid[i]) *flag = 0;
+    return QM_OK;
+}
+
+QM_API int qm_set_vloc(qm_gspace *g, const double *V_r_dev, void *stream) {
+    if (!g || !V_r_dev) return fail(QM_EINVAL, "qm_set_vloc: null argument");
+    const size_t n = (size_t)g->grid[0] * g->grid[1] * g->grid[2];
+    CU_TRY(g->d_vt.resize(n));
+    k_relayout_v<<<g->sm_count * 4, 256, 0, (cudaStream_t)stream>>>(V_r_dev, g->d_vt.p, g->ax[0], g->ax[1], g->ax[2],
+                                                                   1.0 / (double)n);
+    g->launches++;
+    CU_TRY(cudaGetLastError());
+    g->v_set = true;
+    return QM_OK;
+}
+
+QM_API int qm_set_nonlocal(qm_gspace *g, int k, const qm_c128 *beta_kG_dev, int nproj, const double *D_dev, int d_block,
+                    void *stream) {
+    int rc = check_handle(g, k); if (rc) return rc;
+    KPoint *kp = g->kpts[k];
+    if (nproj < 0) return fail(QM_EINVAL, "qm_set_nonlocal: nproj < 0");
+    if (nproj == 0) { kp->nproj = 0; kp->nproj_pad = 0; kp->nl_set = true; return QM_OK; }
+    if (!beta_kG_dev || !D_dev || d_block <= 0 || nproj % d_block != 0)
+        return fail(QM_EINVAL, "qm_set_nonlocal: bad beta / D / d_block");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int nproj_pad = ((nproj + PROJ_MBLK - 1) / PROJ_MBLK) * PROJ_MBLK;
+    const int ldb = ((kp->ng + PROJ_MBLK - 1) / PROJ_MBLK) * PROJ_MBLK;
+    CU_TRY(kp->d_beta.resize((size_t)nproj_pad * ldb));
+    const size_t dcount = (size_t)nproj * d_block;
+    CU_TRY(kp->d_D.resize(dcount));
+    k_pad_beta<<<g->sm_count * 8, 256, 0, st>>>(reinterpret_cast<const c128 *>(beta_kG_dev), kp->ng, nproj,
+                                                kp->d_beta.p, ldb, nproj_pad);
+    g->launches++;
+    CU_TRY(cudaGetLastError());
+    CU_TRY(cudaMemcpyAsync(kp->d_D.p, D_dev, dcount * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    kp->nproj = nproj; kp->nproj_pad = nproj_pad; kp->ldb = ldb; kp->dblock = d_block; kp->nl_set = true;
+    return QM_OK;
+}
+
+QM_API int qm_apply_h(qm_gspace *g, const qm_c128 *psi_in_dev, qm_c128 *psi_out_dev, int nbands, int k, void *stream) {
+    int rc = check_handle(g, k); if (rc) return rc;
+    if (!psi_in_dev || !psi_out_dev || nbands <= 0) return fail(QM_EINVAL, "qm_apply_h: bad argument");
+    KPoint *kp = g->kpts[k];
+    if (!g->v_set) return fail(QM_ENOTSET, "qm_apply_h before qm_set_vloc");
+    if (!kp->nl_set) return fail(QM_ENOTSET, "qm_apply_h before qm_set_nonlocal for this k");
+    const c128 *in = reinterpret_cast<const c128 *>(psi_in_dev);
+    c128 *out = reinterpret_cast<c128 *>(psi_out_dev);
+    const size_t bytes = (size_t)nbands * kp->ng * sizeof(c128);
+    const char *a = (const char *)in, *b = (const char *)out;
+    if (a < b + bytes && b < a + bytes) return fail(QM_EINVAL, "qm_apply_h: psi_in and psi_out overlap");
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = ensure_workspace(g, kp, nbands); if (rc) return rc;
+    rc = dispatch_zinv(g, kp, in, nbands, st); if (rc) return rc;
+    rc = dispatch_plane<0>(g, kp, nullptr, nbands, 1.0, st); if (rc) return rc;
+    rc = dispatch_zfwd(g, kp, in, out, nbands, 1, st); if (rc) return rc;
+    return run_nonlocal(g, kp, in, out, nbands, st);
+}
+
+QM_API int qm_apply_h_host(qm_gspace *g, const qm_c128 *psi_in_host, qm_c128 *psi_out_host, int nbands, int k,
+                    void *stream) {
+    int rc = check_handle(g, k); if (rc) return rc;
+    if (!psi_in_host || !psi_out_host || nbands <= 0) return fail(QM_EINVAL, "qm_apply_h_host: bad argument");
+    KPoint *kp = g->kpts[k];
+    const size_t count = (size_t)nbands * kp->ng;
+    CU_TRY(g->d_stage_in.resize(count));
+    CU_TRY(g->d_stage_out.resize(count));
+    cudaStream_t st = (cudaStream_t)stream;
+    CU_TRY(cudaMemcpyAsync(g->d_stage_in.p, psi_in_host, count * sizeof(c128), cudaMemcpyHostToDevice, st));
+    rc = qm_apply_h(g, reinterpret_cast<const qm_c128 *>(g->d_stage_in.p),
+                    reinterpret_cast<qm_c128 *>(g->d_stage_out.p), nbands, k, stream);
+    if (rc) return rc;
+    CU_TRY(cudaMemcpyAsync(psi_out_host, g->d_stage_out.p, count * sizeof(c128), cudaMemcpyDeviceToHost, st));
+    CU_TRY(cudaStreamSynchronize(st));
+    return QM_OK;
+}
+
+QM_API int qm_debug_g2r(qm_gspace *g, const qm_c128 *psi_g_dev, qm_c128 *box_r_dev, int nbands, int k, void *stream) {
+    int rc = check_handle(g, k); if (rc) return rc;
+    if (!psi_g_dev || !box_r_dev || nbands <= 0) return fail(QM_EINVAL, "qm_debug_g2r: bad argument");
+    KPoint *kp = g->kpts[k];
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = ensure_workspace(g, kp, nbands); if (rc) return rc;
+    rc = dispatch_zinv(g, kp, reinterpret_cast<const c128 *>(psi_g_dev), nbands, st); if (rc) return rc;
+    const double scale = 1.0 / ((double)g->grid[0] * g->grid[1] * g->grid[2]);
+    return dispatch_plane<1>(g, kp, reinterpret_cast<c128 *>(box_r_dev), nbands, scale, st);
+}
+
+QM_API int qm_debug_r2g(qm_gspace *g, const qm_c128 *box_r_dev, qm_c128 *psi_g_dev, int nbands, int k, void *stream) {
+    int rc = check_handle(g, k); if (rc) return rc;
+    if (!psi_g_dev || !box_r_dev || nbands <= 0) return fail(QM_EINVAL, "qm_debug_r2g: bad argument");
+    KPoint *kp = g->kpts[k];
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = ensure_workspace(g, kp, nbands); if (rc) return rc;
+    rc = dispatch_plane<2>(g, kp, const_cast<c128 *>(reinterpret_cast<const c128 *>(box_r_dev)), nbands, 1.0, st);
+    if (rc) return rc;
+    return dispatch_zfwd(g, kp, nullptr, reinterpret_cast<c128 *>(psi_g_dev), nbands, 0, st);
+}
+
+QM_API int qm_get_launch_count(const qm_gspace *g, unsigned long long *count) {
+    if (!g || !count) return fail(QM_EINVAL, "null argument");
+    *count = g->launches; return QM_OK;
+}
+
+QM_API int qm_probe_fp64_tensor_peak(double *tflops_dmma, double *tflops_dfma) {
+    int dev = 0, sms = 0, count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || count == 0) return fail(QM_ECUDA, "no CUDA device");
+    CU_TRY(cudaGetDevice(&dev));
+    CU_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    double *sink = nullptr;
+    CU_TRY(cudaMalloc(&sink, sizeof(double)));
+    cudaEvent_t e0, e1;
+    CU_TRY(cudaEventCreate(&e0)); CU_TRY(cudaEventCreate(&e1));
+    const int iters = 1 << 15, threads = 512, blocks = sms * 4;
+    float ms = 0.f;
+    double best_mma = 0.0, best_fma = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {
+        CU_TRY(cudaEventRecord(e0));
+        k_probe_dmma<<<blocks, threads>>>(sink, iters);
+        CU_TRY(cudaEventRecord(e1)); CU_TRY(cudaEventSynchronize(e1));
+        CU_TRY(cudaEventElapsedTime(&ms, e0, e1));
+        // one DMMA m8n8k4 = 8*8*4 FMA = 512 flop per warp instruction
+        const double fl = (double)blocks * (threads / 32) * (double)iters * 8.0 * 512.0;
+        best_mma = std::max(best_mma, fl / (ms * 1e-3) * 1e-12);
+        CU_TRY(cudaEventRecord(e0));
+        k_probe_dfma<<<blocks, threads>>>(sink, iters);
+        CU_TRY(cudaEventRecord(e1)); CU_TRY(cudaEventSynchronize(e1));
+        CU_TRY(cudaEventElapsedTime(&ms, e0, e1));
+        const double fl2 = (double)blocks * threads * (double)iters * 16.0 * 2.0;
+        best_fma = std::max(best_fma, fl2 / (ms * 1e-3) * 1e-12);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    if (tflops_dmma) *tflops_dmma = best_mma;
+    if (tflops_dfma) *tflops_dfma = best_fma;
+    return QM_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,32 @@
+// Plain-old-data plans handed to the kernels (device pointers inside).
+#pragma once
+#include <stdint.h>
+
+struct c128;
+
+struct QmAxis {            // one FFT axis: n = r1 * r2
+    int n, r1, r2, r2p, len;   // len = r1 * r2p (padded line length)
+};
+
+struct QmKPlanDev {        // per k-point tables on the device
+    int ng;                // plane waves in the sphere
+    int nsticks;           // S: (i1,i2) lines that intersect the sphere
+    int nx;                // X: distinct i1 among the sticks
+    int rowpitch;          // pitch of one plane row (odd, >= axis2.len)
+    const int32_t *g_stick;      // [ng]   stick of each G
+    const uint16_t *g_zpos;      // [ng]   padded position of its z index (LineCfg::pos(i3))
+    const int32_t *stick_off;    // [S+1]  first G of each stick
+    const int32_t *stick_apos;   // [S]    position in the plane array: row*rowpitch + pos(i2)
+    const int16_t *xrow;         // [n1]   compact row of box index i1, or -1
+    const double *g2;            // [ng]   |k+G|^2
+};
+
+struct QmGridDev {
+    QmAxis ax[3];
+    const c128 *tw[3];     // tw[a][j] = exp(-2 pi i j / n_a)
+    const double *vt;      // re-laid-out potential [p(z)][pcol(y)][x] * 1/(n1 n2 n3), or nullptr
+};
+
+// transposed label p -> natural index (p / r2) + r1 * (p % r2)
+static inline int qm_label_to_index(const QmAxis &a, int p) { return (p / a.r2) + a.r1 * (p % a.r2); }
+static inline int qm_pos(const QmAxis &a, int i) { return (i / a.r2) * a.r2p + (i % a.r2); }

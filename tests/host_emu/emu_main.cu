@@ -1,0 +1,155 @@
+// CPU thread-emulation of the FFT-path kernels (TEST ONLY; never linked into libqm_hpsi.so).
+// Runs the very same __host__ __device__ phase functions and host-built stick tables that the CUDA
+// kernels use, with "for (tid ...)" loops standing in for the threads between two barriers, so the
+// index logic of the pipeline can be checked against numpy on a machine without a GPU.
+//
+// usage: emu_main <n> <lat9.bin> <ecut> <k1> <k2> <k3> <nb> <psi.bin> <v.bin> <out_prefix>
+// writes <out_prefix>.idx (int32), .hloc (T+L apply, c128 [nb][ng]), .g2r (c128 [nb][n^3]), .r2g
+#include <cstdio>
+#include <cstdlib>
+#include <string>
+#include <vector>
+#include "../../paper_2308_07277_b200/csrc/fft_phases.cuh"
+#include "../../paper_2308_07277_b200/csrc/gspace_host.h"
+
+template <class T> std::vector<T> slurp(const char *path) {
+    FILE *f = fopen(path, "rb"); if (!f) { perror(path); exit(2); }
+    fseek(f, 0, SEEK_END); long n = ftell(f); fseek(f, 0, SEEK_SET);
+    std::vector<T> v(n / sizeof(T));
+    if (fread(v.data(), 1, n, f) != (size_t)n) exit(2);
+    fclose(f); return v;
+}
+template <class T> void dump(const std::string &path, const std::vector<T> &v) {
+    FILE *f = fopen(path.c_str(), "wb"); fwrite(v.data(), sizeof(T), v.size(), f); fclose(f);
+}
+
+template <class C> struct Emu {
+    static constexpr int LP = C::L | 1, SL = C::L | 1, TS = 16;
+    const QmKTables &kp; QmAxis ax; std::vector<c128> tw;
+    Emu(const QmKTables &k, QmAxis a) : kp(k), ax(a), tw(C::N) {
+        for (int j = 0; j < C::N; ++j) {
+            long double ang = -2.0L * 3.14159265358979323846264338327950288L * j / C::N;
+            tw[j] = c128{(double)cosl(ang), (double)sinl(ang)};
+        }
+    }
+    // k_zinv for one band: psi[ng] -> W[N][S]
+    void zinv(const c128 *psi, c128 *W) {
+        const int S = kp.nsticks, nthr = TS * C::TT;
+        for (int s0 = 0; s0 < S; s0 += TS) {
+            const int ns = std::min(TS, S - s0);
+            std::vector<c128> lines(TS * LP, c128{0, 0});
+            for (int g = kp.stickoff[s0]; g < kp.stickoff[s0 + ns]; ++g)
+                lines[(kp.gstick[g] - s0) * LP + kp.gzpos[g]] = psi[g];
+            for (int tid = 0; tid < nthr; ++tid) { int t = tid / C::TT, u = tid % C::TT; if (t < ns) lineA_step1<C>(&lines[t * LP], u, tw.data()); }
+            for (int tid = 0; tid < nthr; ++tid) { int t = tid / C::TT, u = tid % C::TT; if (t < ns) lineA_step2<C>(&lines[t * LP], u); }
+            for (int i = 0; i < C::N * TS; ++i) { int p = i / TS, tt = i % TS; if (tt < ns) W[(size_t)p * S + s0 + tt] = lines[tt * LP + C::pos(p)]; }
+        }
+    }
+    void zfwd(const c128 *W, const c128 *psi_in, c128 *out, bool kinetic) {
+        const int S = kp.nsticks, nthr = TS * C::TT;
+        for (int s0 = 0; s0 < S; s0 += TS) {
+            const int ns = std::min(TS, S - s0);
+            std::vector<c128> lines(TS * LP, c128{0, 0});
+            for (int i = 0; i < C::N * TS; ++i) { int p = i / TS, tt = i % TS; if (tt < ns) lines[tt * LP + C::pos(p)] = W[(size_t)p * S + s0 + tt]; }
+            for (int tid = 0; tid < nthr; ++tid) { int t = tid / C::TT, u = tid % C::TT; if (t < ns) lineB_step1<C>(&lines[t * LP], u, tw.data()); }
+            for (int tid = 0; tid < nthr; ++tid) { int t = tid / C::TT, u = tid % C::TT; if (t < ns) lineB_step2<C>(&lines[t * LP], u); }
+            for (int g = kp.stickoff[s0]; g < kp.stickoff[s0 + ns]; ++g) {
+                c128 v = lines[(kp.gstick[g] - s0) * LP + kp.gzpos[g]];
+                if (kinetic) { double h = 0.5 * kp.g2[g]; v.x += h * psi_in[g].x; v.y += h * psi_in[g].y; }
+                out[g] = v;
+            }
+        }
+    }
+    // k_plane for one (band, p).  vt: relaid potential; box: natural-order box of this band
+    template <int MODE> void plane(int p, c128 *W, const double *vt, c128 *box, double scale, int ncol) {
+        const int X = kp.nx, rp = kp.rowpitch, S = kp.nsticks, n3 = ax.n, nthr = ncol * C::TT;
+        std::vector<c128> A((size_t)X * rp, c128{0, 0}), scr((size_t)ncol * SL);
+        c128 *Wp = W + (size_t)p * S;
+        if (MODE != 2) {
+            for (int s = 0; s < S; ++s) A[kp.stickapos[s]] = Wp[s];
+            for (int task = 0; task < X * C::TT; ++task) lineA_step1<C>(&A[(task / C::TT) * rp], task % C::TT, tw.data());
+            for (int task = 0; task < X * C::TT; ++task) lineA_step2<C>(&A[(task / C::TT) * rp], task % C::TT);
+        }
+        const int z = (p / ax.r2) + ax.r1 * (p % ax.r2);
+        for (int cbase = 0; cbase < C::N; cbase += ncol) {
+            if (MODE != 2)
+                for (int tid = 0; tid < nthr; ++tid) {
+                    int c = tid / C::TT, u = tid % C::TT, col = cbase + c;
+                    if (col < C::N) xcol_step1<C>(A.data(), rp, C::pos(col), kp.xrow.data(), &scr[(size_t)c * SL], u, tw.data());
+                }
+            for (int tid = 0; tid < nthr; ++tid) {
+                int c = tid / C::TT, u = tid % C::TT, col = cbase + c;
+                if (col >= C::N) continue;
+                int y = (col / C::R2) + C::R1 * (col % C::R2);
+                const double *v = MODE == 0 ? vt + ((size_t)p * C::N + col) * C::N : nullptr;
+                c128 *bx = MODE == 0 ? nullptr : box + (size_t)y * n3 + z;
+                xcol_step2<C, MODE>(&scr[(size_t)c * SL], u, tw.data(), v, bx, (long)C::N * n3, scale);
+            }
+            if (MODE != 1)
+                for (int tid = 0; tid < nthr; ++tid) {
+                    int c = tid / C::TT, u = tid % C::TT, col = cbase + c;
+                    if (col < C::N) xcol_step3<C>(A.data(), rp, C::pos(col), kp.xrow.data(), &scr[(size_t)c * SL], u);
+                }
+        }
+        if (MODE != 1) {
+            for (int task = 0; task < X * C::TT; ++task) lineB_step1<C>(&A[(task / C::TT) * rp], task % C::TT, tw.data());
+            for (int task = 0; task < X * C::TT; ++task) lineB_step2<C>(&A[(task / C::TT) * rp], task % C::TT);
+            for (int s = 0; s < S; ++s) Wp[s] = A[kp.stickapos[s]];
+        }
+    }
+};
+
+template <class C> int run(int n, const double *lat, double ecut, const double *k, int nb, const char *psi_path,
+                           const char *v_path, const std::string &prefix)
+{
+    int grid[3] = {n, n, n};
+    QmAxis ax[3];
+    for (int i = 0; i < 3; ++i) ax[i] = qm_make_axis(*qm_find_size(n));
+    double recip[9]; qm_reciprocal(lat, recip);
+    QmKTables kp; for (int i = 0; i < 3; ++i) kp.k[i] = k[i];
+    std::string msg;
+    if (qm_build_tables(lat, recip, ecut, grid, ax, &kp, &msg)) { fprintf(stderr, "%s\n", msg.c_str()); return 3; }
+    auto psi = slurp<c128>(psi_path);
+    auto v = slurp<double>(v_path);
+    if ((int)psi.size() != nb * kp.ng || (int)v.size() != n * n * n) { fprintf(stderr, "size mismatch ng=%d\n", kp.ng); return 4; }
+    const size_t n3 = (size_t)n * n * n;
+    std::vector<double> vt(n3);
+    for (size_t i = 0; i < n3; ++i) {
+        int x = i % n, col = (i / n) % n, p = i / ((size_t)n * n);
+        int y = (col / ax[1].r2) + ax[1].r1 * (col % ax[1].r2), z = (p / ax[2].r2) + ax[2].r1 * (p % ax[2].r2);
+        vt[i] = v[((size_t)x * n + y) * n + z] / (double)n3;
+    }
+    Emu<C> emu(kp, ax[2]);
+    const int S = kp.nsticks, ncol = 5;     // odd column count on purpose: exercises the ragged last pass
+    std::vector<c128> hloc((size_t)nb * kp.ng), g2r(nb * n3), r2g((size_t)nb * kp.ng), W((size_t)n * S);
+    for (int b = 0; b < nb; ++b) {
+        emu.zinv(&psi[(size_t)b * kp.ng], W.data());
+        for (int p = 0; p < n; ++p) emu.template plane<0>(p, W.data(), vt.data(), nullptr, 1.0, ncol);
+        emu.zfwd(W.data(), &psi[(size_t)b * kp.ng], &hloc[(size_t)b * kp.ng], true);
+        emu.zinv(&psi[(size_t)b * kp.ng], W.data());
+        for (int p = 0; p < n; ++p) emu.template plane<1>(p, W.data(), nullptr, &g2r[b * n3], 1.0 / (double)n3, ncol);
+        for (int p = 0; p < n; ++p) emu.template plane<2>(p, W.data(), nullptr, &g2r[b * n3], 1.0, ncol);
+        emu.zfwd(W.data(), nullptr, &r2g[(size_t)b * kp.ng], false);
+    }
+    dump(prefix + ".idx", kp.idx); dump(prefix + ".hloc", hloc); dump(prefix + ".g2r", g2r); dump(prefix + ".r2g", r2g);
+    printf("ng %d sticks %d nx %d\n", kp.ng, kp.nsticks, kp.nx);
+    return 0;
+}
+
+int main(int argc, char **argv) {
+    if (argc != 11) { fprintf(stderr, "usage\n"); return 1; }
+    const int n = atoi(argv[1]);
+    auto lat = slurp<double>(argv[2]);
+    const double ecut = atof(argv[3]);
+    const double k[3] = {atof(argv[4]), atof(argv[5]), atof(argv[6])};
+    const int nb = atoi(argv[7]);
+    switch (n) {
+#define X(N, A, B) case N: return run<LineCfg<A, B>>(n, lat.data(), ecut, k, nb, argv[8], argv[9], argv[10]);
+        X(8, 2, 4) X(12, 3, 4) X(16, 4, 4) X(18, 3, 6) X(20, 4, 5) X(24, 4, 6) X(30, 5, 6) X(32, 4, 8)
+        X(36, 6, 6) X(40, 5, 8) X(48, 6, 8) X(60, 6, 10) X(64, 8, 8) X(72, 8, 9) X(80, 8, 10)
+        X(96, 8, 12) X(100, 10, 10) X(108, 9, 12) X(120, 10, 12) X(128, 8, 16) X(144, 12, 12)
+#undef X
+    }
+    fprintf(stderr, "unsupported n\n");
+    return 1;
+}

@@ -1,0 +1,195 @@
+"""GPU parity: qm_apply_h (through the C ABI) vs the CPU oracle, element by element (-m gpu).
+
+Tolerance 1e-11 max relative error per band (north_star; A13); index maps bit exact; g2 <= 2 ulp (A14).
+Each config is run three times (A19): full H, D = 0 (no projectors), V = 0.
+"""
+import numpy as np
+import pytest
+
+from tests.common import TOL, band_errors, problem
+from oracle import hpsi as oh
+from oracle import hpsi_fft as of
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def qm():
+    import __graft_entry__ as ge
+    ge.build()
+    import paper_2308_07277_b200 as q
+    return q
+
+
+def _torch():
+    import torch
+    return torch, torch.device("cuda:0")
+
+
+def _gspace(qm, p, all_k=False):
+    cfg = p["cfg"]
+    return qm.GSpace(p["lat"], cfg.ecutwfc_ry, cfg.grid, p["kpts"] if all_k else p["k"][None, :])
+
+
+def _apply(qm, gs, p, psi, variant, k=0):
+    torch, dev = _torch()
+    cfg = p["cfg"]
+    v = p["v"] if variant != "v0" else np.zeros_like(p["v"])
+    gs.set_vloc(torch.from_numpy(v).to(dev))
+    if variant == "d0":
+        gs.set_nonlocal(k, None, None)
+    else:
+        gs.set_nonlocal(k, torch.from_numpy(p["beta"]).to(dev), torch.from_numpy(p["dblk"]).to(dev))
+    out = gs.apply_h(torch.from_numpy(psi).to(dev), k=k)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def _oracle(p, psi, variant, rows=None):
+    vhat = p["vhat"] if variant != "v0" else np.zeros_like(p["vhat"])
+    beta = None if variant == "d0" else p["beta"]
+    d = None if variant == "d0" else oh.expand_d(p["dblk"])
+    return oh.apply_h_rows(psi, p["miller"], p["g2"], vhat, p["cfg"].grid, beta, d, rows=rows)
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+def test_index_map_bit_exact(qm, name):
+    p = problem(name, 0, nbands=1, orthonormalise=False)
+    gs = _gspace(qm, p, all_k=True)
+    for ik in range(p["cfg"].nk):
+        pk = problem(name, ik, nbands=1, orthonormalise=False)
+        assert gs.num_g(ik) == pk["idx"].size
+        np.testing.assert_array_equal(gs.index_map(ik), pk["idx"])
+        np.testing.assert_array_equal(gs.miller(ik), pk["miller"])
+        g2 = gs.g2(ik)
+        assert np.max(np.abs(g2 - pk["g2"]) / np.maximum(np.spacing(pk["g2"]), 1e-300)) <= 2.0
+        assert gs.alias_free(ik)
+    gs.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg3"])
+def test_debug_g2r_r2g_match_library_fft(qm, name):
+    torch, dev = _torch()
+    p = problem(name)
+    gs = _gspace(qm, p)
+    psi = p["psi"][:4]
+    grid = p["cfg"].grid
+    box = gs.g2r(torch.from_numpy(psi).to(dev)).cpu().numpy()
+    ref = of.g2r(psi, p["idx"], grid).reshape(4, -1)
+    assert np.max(np.abs(box - ref)) <= 1e-13 * np.max(np.abs(ref)) * 10
+    # Parseval on the box (A5): sum_r |f|^2 = (1/N) sum_G |F|^2
+    n = box.shape[1]
+    np.testing.assert_allclose(np.sum(np.abs(box) ** 2, axis=1) * n, np.sum(np.abs(psi) ** 2, axis=1), rtol=1e-12)
+    rng = np.random.default_rng(0)
+    r = rng.standard_normal((2, n)) + 1j * rng.standard_normal((2, n))
+    got = gs.r2g(torch.from_numpy(r).to(dev)).cpu().numpy()
+    want = np.fft.fftn(r.reshape((2,) + grid), axes=(1, 2, 3)).reshape(2, -1)[:, p["idx"]]
+    assert np.max(np.abs(got - want)) <= 1e-12 * np.max(np.abs(want))
+    # round trip sphere -> box -> sphere
+    back = gs.r2g(gs.g2r(torch.from_numpy(psi).to(dev))).cpu().numpy()
+    assert np.max(np.abs(back - psi)) <= 1e-12 * np.max(np.abs(psi))
+    gs.close()
+
+
+@pytest.mark.parametrize("variant", ["full", "d0", "v0"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg3"])
+def test_parity_all_elements_small_configs(qm, name, variant):
+    p = problem(name)
+    gs = _gspace(qm, p)
+    got = _apply(qm, gs, p, p["psi"], variant)
+    ref = _oracle(p, p["psi"], variant)
+    e_inf, e_2 = band_errors(got, ref)
+    assert e_inf <= TOL and e_2 <= TOL, (e_inf, e_2)
+    gs.close()
+
+
+def test_parity_cfg2_all_kpoints_batched(qm):
+    torch, dev = _torch()
+    p0 = problem("cfg2", 0)
+    gs = _gspace(qm, p0, all_k=True)
+    gs.set_vloc(torch.from_numpy(p0["v"]).to(dev))
+    outs = []
+    for ik in range(p0["cfg"].nk):
+        p = problem("cfg2", ik)
+        gs.set_nonlocal(ik, torch.from_numpy(p["beta"]).to(dev), torch.from_numpy(p["dblk"]).to(dev))
+        outs.append(gs.apply_h(torch.from_numpy(p["psi"]).to(dev), k=ik))
+    torch.cuda.synchronize()
+    for ik in range(p0["cfg"].nk):
+        p = problem("cfg2", ik)
+        ref = _oracle(p, p["psi"], "full")
+        e_inf, e_2 = band_errors(outs[ik].cpu().numpy(), ref)
+        assert e_inf <= TOL and e_2 <= TOL, (ik, e_inf, e_2)
+    gs.close()
+
+
+@pytest.mark.parametrize("name,nb", [("cfg4", 32), ("cfg5", 16)])
+def test_parity_sampled_rows_full_size(qm, name, nb):
+    """Full-size configs in bench.py's launch configuration (call batch), on sampled output rows."""
+    p = problem(name, 0, nbands=nb, orthonormalise=False)
+    gs = _gspace(qm, p)
+    ng = p["idx"].size
+    rng = np.random.default_rng(123)
+    rows = np.unique(np.concatenate([[0, 1, ng - 2, ng - 1], rng.integers(0, ng, size=60)])).astype(np.int32)
+    for variant in ("full", "d0", "v0"):
+        got = _apply(qm, gs, p, p["psi"], variant)
+        ref = _oracle(p, p["psi"], variant, rows=rows)
+        e_inf, _ = band_errors(got[:, rows], ref)
+        assert e_inf <= TOL, (variant, e_inf)
+        if variant == "full":
+            # properties that hold at any size: Hermiticity of the GPU operator on these vectors
+            h = np.conj(p["psi"]) @ got.T
+            assert np.max(np.abs(h - np.conj(h.T))) <= 1e-11 * np.max(np.abs(h))
+            # and agreement of every element with the paper's FFT route (second opinion)
+            alt = of.apply_h_fft(p["psi"], p["idx"], p["g2"], p["v"], p["cfg"].grid, p["beta"],
+                                 oh.expand_d(p["dblk"]))
+            e_inf, e_2 = band_errors(got, alt)
+            assert e_inf <= TOL and e_2 <= TOL, (e_inf, e_2)
+    gs.close()
+
+
+@pytest.mark.parametrize("nb", [1, 3, 17])
+def test_ragged_band_counts(qm, nb):
+    p = problem("cfg3")
+    gs = _gspace(qm, p)
+    psi = np.ascontiguousarray(p["psi"][:nb])
+    got = _apply(qm, gs, p, psi, "full")
+    ref = _oracle(p, psi, "full")
+    e_inf, e_2 = band_errors(got, ref)
+    assert e_inf <= TOL and e_2 <= TOL
+    gs.close()
+
+
+def test_host_entry_matches_device_entry(qm):
+    torch, dev = _torch()
+    p = problem("cfg1")
+    gs = _gspace(qm, p)
+    a = _apply(qm, gs, p, p["psi"], "full")
+    hin = torch.from_numpy(p["psi"]).pin_memory()
+    hout = torch.empty_like(hin).pin_memory()
+    gs.apply_h_host(hin, hout)
+    np.testing.assert_array_equal(hout.numpy(), a)
+    gs.close()
+
+
+def test_error_codes(qm):
+    torch, dev = _torch()
+    p = problem("cfg1")
+    gs = _gspace(qm, p)
+    psi = torch.from_numpy(p["psi"]).to(dev)
+    with pytest.raises(qm.QmError) as e:
+        gs.apply_h(psi)
+    assert e.value.code == -2                                    # QM_ENOTSET
+    gs.set_vloc(torch.from_numpy(p["v"]).to(dev))
+    gs.set_nonlocal(0, None, None)
+    with pytest.raises(qm.QmError) as e:
+        qm.qm_apply_h(gs.handle, psi, psi)
+    assert e.value.code == -1                                    # overlap
+    with pytest.raises(qm.QmError) as e:
+        qm.qm_gspace_num_g(gs.handle, 5)
+    assert e.value.code == -1
+    with pytest.raises(TypeError):
+        gs.apply_h(psi[:, :-1].contiguous())                     # wrong basis size
+    with pytest.raises(qm.QmError) as e:
+        qm.GSpace(p["lat"], 25.0, (8, 8, 8))
+    assert e.value.code == -3                                    # sphere does not fit
+    gs.close()
