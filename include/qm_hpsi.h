@@ -114,6 +114,25 @@ QM_API int qm_debug_r2g(qm_gspace *g, const qm_c128 *box_r_dev, qm_c128 *psi_g_d
 /* Number of CUDA kernels this handle has launched so far (for bench.py's gpu_launches). */
 QM_API int qm_get_launch_count(const qm_gspace *g, unsigned long long *count);
 
+/* Per-kernel device timing (measurement aid for bench.py's roofline block; off by default).
+ * When enabled every hot-path kernel launch is bracketed by CUDA events on its own stream.
+ * qm_profile_read synchronises those events and returns the accumulated device time (ms) and
+ * the number of launches of one kernel kind since the last reset. */
+typedef enum {
+    QM_K_ZINV = 0,      /* scatter + backward z-FFT on sticks           (a1, a2) */
+    QM_K_PLANE = 1,     /* fused xy-plane kernel incl. V_loc multiply   (a2, a3, a4) */
+    QM_K_ZFWD = 2,      /* forward z-FFT + gather + kinetic             (a4, a5) */
+    QM_K_PROJ1 = 3,     /* P = beta^H psi   (DMMA)                      (a6) */
+    QM_K_PREDUCE = 4,   /* split-K reduction of P */
+    QM_K_DMUL = 5,      /* Q = D P                                      (a7) */
+    QM_K_PROJ2 = 6,     /* out += beta Q    (DMMA)                      (a8) */
+    QM_K_COUNT = 7
+} qm_kernel_kind;
+QM_API int qm_profile_enable(qm_gspace *g, int on);
+QM_API int qm_profile_reset(qm_gspace *g);
+QM_API int qm_profile_read(qm_gspace *g, int kind, double *total_ms, unsigned long long *launches);
+QM_API const char *qm_kernel_name(int kind);
+
 /* FP64 tensor-core (DMMA m8n8k4) peak probe: runs a register-resident DMMA loop on every SM
  * and returns the measured TFLOP/s (HOST output).  Used as the roofline denominator for the
  * projector GEMMs (MEASURED_PEAKS.json has no FP64 entry). Synchronous. */

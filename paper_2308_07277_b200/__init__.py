@@ -11,4 +11,5 @@ from .binding import (  # noqa: F401
     qm_gspace_get_index_map, qm_gspace_get_miller, qm_gspace_get_g2, qm_gspace_alias_free,
     qm_set_vloc, qm_set_nonlocal, qm_apply_h, qm_apply_h_host, qm_debug_g2r, qm_debug_r2g,
     qm_get_launch_count, qm_probe_fp64_tensor_peak,
+    qm_profile_enable, qm_profile_reset, qm_profile_read, qm_kernel_name,
 )

@@ -47,8 +47,12 @@ _SIGS = {
     "qm_debug_r2g": [_vp, _vp, _vp, _i, _i, _vp],
     "qm_get_launch_count": [_vp, ctypes.POINTER(ctypes.c_ulonglong)],
     "qm_probe_fp64_tensor_peak": [ctypes.POINTER(_d), ctypes.POINTER(_d)],
+    "qm_profile_enable": [_vp, _i],
+    "qm_profile_reset": [_vp],
+    "qm_profile_read": [_vp, _i, ctypes.POINTER(_d), ctypes.POINTER(ctypes.c_ulonglong)],
 }
-EXPORTS = sorted(list(_SIGS) + ["qm_last_error", "qm_version"])
+EXPORTS = sorted(list(_SIGS) + ["qm_last_error", "qm_version", "qm_kernel_name"])
+QM_K_COUNT = 7
 
 
 def load_library():
@@ -65,6 +69,8 @@ def load_library():
             fn.argtypes = args
         lib.qm_last_error.restype = ctypes.c_char_p
         lib.qm_version.restype = ctypes.c_char_p
+        lib.qm_kernel_name.restype = ctypes.c_char_p
+        lib.qm_kernel_name.argtypes = [_i]
         _lib = lib
     return _lib
 
@@ -236,6 +242,28 @@ def qm_probe_fp64_tensor_peak():
     a, b = _d(), _d()
     _check(load_library().qm_probe_fp64_tensor_peak(ctypes.byref(a), ctypes.byref(b)))
     return a.value, b.value
+
+
+def qm_profile_enable(h, on: bool):
+    _check(load_library().qm_profile_enable(h, int(bool(on))))
+
+
+def qm_profile_reset(h):
+    _check(load_library().qm_profile_reset(h))
+
+
+def qm_kernel_name(kind: int) -> str:
+    return load_library().qm_kernel_name(int(kind)).decode()
+
+
+def qm_profile_read(h):
+    """{kernel name: (total device ms, launches)} since the last reset."""
+    out = {}
+    for kind in range(QM_K_COUNT):
+        ms, n = _d(), ctypes.c_ulonglong()
+        _check(load_library().qm_profile_read(h, kind, ctypes.byref(ms), ctypes.byref(n)))
+        out[qm_kernel_name(kind)] = (ms.value, n.value)
+    return out
 
 
 class GSpace:

@@ -67,7 +67,41 @@ struct KPoint : QmKTables {
 
 }  // namespace
 
+struct Profiler {
+    bool on = false;
+    std::vector<cudaEvent_t> pool;
+    size_t used = 0;
+    struct Rec { int kind; size_t e0, e1; };
+    std::vector<Rec> recs;
+    double total_ms[QM_K_COUNT] = {0};
+    unsigned long long count[QM_K_COUNT] = {0};
+    ~Profiler() { for (auto e : pool) cudaEventDestroy(e); }
+    size_t next() {
+        if (used == pool.size()) { cudaEvent_t e; cudaEventCreate(&e); pool.push_back(e); }
+        return used++;
+    }
+    void begin(int kind, cudaStream_t st) {
+        if (!on) return;
+        Rec r; r.kind = kind; r.e0 = next(); r.e1 = next();
+        cudaEventRecord(pool[r.e0], st);
+        recs.push_back(r);
+    }
+    void end(cudaStream_t st) { if (on) cudaEventRecord(pool[recs.back().e1], st); }
+    void collect() {
+        for (const Rec &r : recs) {
+            cudaEventSynchronize(pool[r.e1]);
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, pool[r.e0], pool[r.e1]) == cudaSuccess) {
+                total_ms[r.kind] += ms; count[r.kind]++;
+            }
+        }
+        recs.clear(); used = 0;
+    }
+    void reset() { collect(); for (int i = 0; i < QM_K_COUNT; ++i) { total_ms[i] = 0; count[i] = 0; } }
+};
+
 struct qm_gspace {
+    Profiler prof;
     double lattice[9], recip[9];
     double ecut;
     int grid[3];
@@ -130,7 +164,9 @@ template <class C> int launch_zinv(qm_gspace *g, KPoint *kp, const c128 *psi, in
     static bool attr = false;
     if (!attr) { CU_TRY(cudaFuncSetAttribute(k_zinv<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
     dim3 grid((kp->nsticks + TS - 1) / TS, nb);
+    g->prof.begin(QM_K_ZINV, st);
     k_zinv<C><<<grid, TS * C::TT, smem, st>>>(kp->plan(), g->d_tw[2].p, psi, g->d_W.p, TS);
+    g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
     return QM_OK;
@@ -142,7 +178,9 @@ template <class C> int launch_zfwd(qm_gspace *g, KPoint *kp, const c128 *psi_in,
     static bool attr = false;
     if (!attr) { CU_TRY(cudaFuncSetAttribute(k_zfwd<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
     dim3 grid((kp->nsticks + TS - 1) / TS, nb);
+    g->prof.begin(QM_K_ZFWD, st);
     k_zfwd<C><<<grid, TS * C::TT, smem, st>>>(kp->plan(), g->d_tw[2].p, g->d_W.p, psi_in, out, TS, kinetic);
+    g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
     return QM_OK;
@@ -158,7 +196,9 @@ template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *bo
     for (int i = 0; i < 3; ++i) { gd.ax[i] = g->ax[i]; gd.tw[i] = g->d_tw[i].p; }
     gd.vt = g->d_vt.p;
     dim3 grid(g->grid[2], nb);
+    g->prof.begin(QM_K_PLANE, st);
     k_plane<C, MODE><<<grid, ncol * C::TT, smem, st>>>(kp->plan(), gd, g->d_W.p, box, ncol, scale);
+    g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
     return QM_OK;
@@ -245,14 +285,22 @@ int run_nonlocal(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb
     CU_TRY(g->d_Q.resize(pcount));
     for (int band0 = 0; band0 < nb; band0 += PROJ_NB) {
         dim3 g1(mblocks, nsplit);
+        g->prof.begin(QM_K_PROJ1, st);
         k_proj1_direct<PROJ_MT, PROJ_NT, PROJ_WARPS><<<g1, PROJ_WARPS * 32, 0, st>>>(
             kp->d_beta.p, kp->ldb, psi_in, kp->ng, nb, band0, nbp, kp->nproj_pad, g->d_Ppart.p, kchunk);
+        g->prof.end(st);
+        g->prof.begin(QM_K_PREDUCE, st);
         k_reduce_p<<<(unsigned)((pcount + 255) / 256), 256, 0, st>>>(g->d_Ppart.p, nsplit, (int)pcount, g->d_P.p);
+        g->prof.end(st);
+        g->prof.begin(QM_K_DMUL, st);
         k_dmul<<<(unsigned)((pcount + 255) / 256), 256, 0, st>>>(kp->d_D.p, kp->dblock, kp->nproj, kp->nproj_pad, nbp,
                                                                  g->d_P.p, g->d_Q.p);
+        g->prof.end(st);
         const int gblocks = (kp->ng + PROJ_MBLK - 1) / PROJ_MBLK;
+        g->prof.begin(QM_K_PROJ2, st);
         k_proj2_direct<PROJ_MT, PROJ_NT, PROJ_WARPS><<<gblocks, PROJ_WARPS * 32, 0, st>>>(
             kp->d_beta.p, kp->ldb, g->d_Q.p, nbp, kp->nproj_pad, kp->ng, nb, band0, out);
+        g->prof.end(st);
         g->launches += 4;
     }
     CU_TRY(cudaGetLastError());
@@ -465,6 +513,30 @@ QM_API int qm_debug_r2g(qm_gspace *g, const qm_c128 *box_r_dev, qm_c128 *psi_g_d
 QM_API int qm_get_launch_count(const qm_gspace *g, unsigned long long *count) {
     if (!g || !count) return fail(QM_EINVAL, "null argument");
     *count = g->launches; return QM_OK;
+}
+
+QM_API int qm_profile_enable(qm_gspace *g, int on) {
+    if (!g) return fail(QM_EINVAL, "null handle");
+    g->prof.collect();
+    g->prof.on = on != 0;
+    return QM_OK;
+}
+QM_API int qm_profile_reset(qm_gspace *g) {
+    if (!g) return fail(QM_EINVAL, "null handle");
+    g->prof.reset();
+    return QM_OK;
+}
+QM_API int qm_profile_read(qm_gspace *g, int kind, double *total_ms, unsigned long long *launches) {
+    if (!g || kind < 0 || kind >= QM_K_COUNT) return fail(QM_EINVAL, "qm_profile_read: bad argument");
+    g->prof.collect();
+    if (total_ms) *total_ms = g->prof.total_ms[kind];
+    if (launches) *launches = g->prof.count[kind];
+    return QM_OK;
+}
+QM_API const char *qm_kernel_name(int kind) {
+    static const char *names[QM_K_COUNT] = {"k_zinv", "k_plane", "k_zfwd", "k_proj1", "k_reduce_p", "k_dmul",
+                                            "k_proj2"};
+    return (kind >= 0 && kind < QM_K_COUNT) ? names[kind] : "?";
 }
 
 QM_API int qm_probe_fp64_tensor_peak(double *tflops_dmma, double *tflops_dfma) {
