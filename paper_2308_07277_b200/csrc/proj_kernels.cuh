@@ -159,6 +159,310 @@ k_proj2_direct(const c128 *__restrict__ beta, int ldb, const c128 *__restrict__ 
 }
 
 // ---------------------------------------------------------------------------------------------
+// v2 kernels: shared-memory ring fed by cp.async.bulk (TMA engine, mbarrier complete_tx), one producer
+// warp + consumer warps issuing DMMA; complex products by the 3M scheme (three real products:
+//   T1 = ar*br, T2 = ai*bi, T3 = (ar -/+ ai)*(br + bi)), which cuts the DMMA count by a quarter.
+// beta is kept in two library-owned tiled copies (qm_set_nonlocal "may re-lay-out"):
+//   beta1[mblk][kc][128 rows][16 k]  element (r,k) at r*16 + (k ^ ((r&1)<<2))      (GEMM 1, one 32 KB copy/stage)
+//   beta2[gt][ic][16 i][64 G]        element (i,g) at i*64 + (g ^ ((i&3)<<1))      (GEMM 2, one 16 KB copy/stage)
+// The XOR swizzles make every DMMA fragment load (one 16-byte LDS per thread) bank-conflict free.
+constexpr int P1_ROWS = 128, P1_KS = 16, P1_CW = 8, P1_ST = 4, P1_PSI_PITCH = 20, P_NB = 16;
+constexpr int P1_BETA_BYTES = P1_ROWS * P1_KS * 16;                 // 32768
+constexpr int P1_PSI_BYTES = P_NB * P1_PSI_PITCH * 16;              // 5120
+constexpr int P1_STAGE_BYTES = P1_BETA_BYTES + P1_PSI_BYTES;
+constexpr int P1_SMEM = P1_ST * P1_STAGE_BYTES + 2 * P1_ST * 8 + 16;
+constexpr int P2_G = 64, P2_KS = 16, P2_CW = 4, P2_ST = 4, P2_Q_PITCH = 20;
+constexpr int P2_BETA_BYTES = P2_KS * P2_G * 16;                    // 16384
+constexpr int P2_Q_DOUBLES = 3 * P2_KS * P2_Q_PITCH;                // 960
+constexpr int P2_Q_BYTES = P2_Q_DOUBLES * 8;                        // 7680
+constexpr int P2_STAGE_BYTES = P2_BETA_BYTES + P2_Q_BYTES;
+constexpr int P2_SMEM = P2_ST * P2_STAGE_BYTES + 2 * P2_ST * 8 + 16;
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ double2 lds_c128(const unsigned char *base, int byte_off) {
+    return *reinterpret_cast<const double2 *>(base + byte_off);
+}
+
+// re-layout kernels (set-up time) ------------------------------------------------------------
+__global__ void k_tile_beta1(const c128 *__restrict__ src, int ng, int nproj, c128 *__restrict__ dst, int nmblk, int nkc)
+{
+    const size_t total = (size_t)nmblk * nkc * (P1_ROWS * P1_KS);
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int e = (int)(i % (P1_ROWS * P1_KS));
+        const size_t tile = i / (P1_ROWS * P1_KS);
+        const int kc = (int)(tile % nkc), mb = (int)(tile / nkc);
+        const int r = e / P1_KS, ks = e % P1_KS;
+        const int k = ks ^ ((r & 1) << 2);                 // the element stored at slot (r, ks)
+        const int row = mb * P1_ROWS + r, col = kc * P1_KS + k;
+        dst[i] = (row < nproj && col < ng) ? src[(size_t)row * ng + col] : c128{0.0, 0.0};
+    }
+}
+__global__ void k_tile_beta2(const c128 *__restrict__ src, int ng, int nproj, c128 *__restrict__ dst, int ngt, int nic)
+{
+    const size_t total = (size_t)ngt * nic * (P2_KS * P2_G);
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int e = (int)(i % (P2_KS * P2_G));
+        const size_t tile = i / (P2_KS * P2_G);
+        const int ic = (int)(tile % nic), gt = (int)(tile / nic);
+        const int ii = e / P2_G, gs = e % P2_G;
+        const int gg = gs ^ ((ii & 3) << 1);
+        const int row = ic * P2_KS + ii, col = gt * P2_G + gg;
+        dst[i] = (row < nproj && col < ng) ? src[(size_t)row * ng + col] : c128{0.0, 0.0};
+    }
+}
+
+// GEMM 1:  Ppart[split][row][n] = sum_{k in split} conj(beta[row][k]) psi[band0+n][k]
+__global__ void __launch_bounds__((P1_CW + 1) * 32, 1)
+k_proj1_pipe(const c128 *__restrict__ beta1, int nkc, const c128 *__restrict__ psi, int ng, int nb, int band0,
+             c128 *__restrict__ Ppart, int nrows_pad, int nsplit)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + P1_ST * P1_STAGE_BYTES);
+    uint64_t *empty = full + P1_ST;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int mb = blockIdx.x, split = blockIdx.y;
+    const int kc0 = (int)((long long)split * nkc / nsplit), kc1 = (int)((long long)(split + 1) * nkc / nsplit);
+    const int nit = kc1 - kc0;
+    const int nvalid = min(P_NB, nb - band0);
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < P1_ST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], P1_CW); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int s = 0; s < P1_ST; ++s) {       // rows of bands that do not exist stay zero for the whole kernel
+        double2 *pz = reinterpret_cast<double2 *>(smem + s * P1_STAGE_BYTES + P1_BETA_BYTES);
+        for (int i = threadIdx.x; i < P1_PSI_BYTES / 16; i += blockDim.x) pz[i] = make_double2(0.0, 0.0);
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncthreads();
+
+    if (warp == P1_CW) {
+        // ---- producer warp: one 32 KB bulk copy of the beta tile + one row copy per band ----
+        for (int it = 0; it < nit; ++it) {
+            const int s = it % P1_ST;
+            if (it >= P1_ST) mbar_wait(&empty[s], ((it / P1_ST) - 1) & 1);
+            unsigned char *stage = smem + s * P1_STAGE_BYTES;
+            const int kc = kc0 + it;
+            const int nk = min(P1_KS, ng - kc * P1_KS);
+            if (nk < P1_KS && lane < nvalid) {          // ragged K tail: clear what the short copy will not write
+                double2 *row = reinterpret_cast<double2 *>(stage + P1_BETA_BYTES) + lane * P1_PSI_PITCH;
+                for (int k = nk; k < P1_KS; ++k) row[k] = make_double2(0.0, 0.0);
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            }
+            __syncwarp();
+            if (lane == 0) {
+                mbar_expect_tx(&full[s], (uint32_t)(P1_BETA_BYTES + nvalid * nk * 16));
+                bulk_g2s(stage, beta1 + ((size_t)mb * nkc + kc) * (P1_ROWS * P1_KS), P1_BETA_BYTES, &full[s]);
+            }
+            __syncwarp();
+            if (lane < nvalid)
+                bulk_g2s(stage + P1_BETA_BYTES + lane * P1_PSI_PITCH * 16,
+                         psi + (size_t)(band0 + lane) * ng + (size_t)kc * P1_KS, (uint32_t)(nk * 16), &full[s]);
+        }
+    } else {
+        // ---- consumer warps: rows 16*warp .. 16*warp+15, all 16 bands ----
+        const int r8 = lane >> 2, c = lane & 3;
+        double t1[2][2][2], t2[2][2][2], t3[2][2][2];
+#pragma unroll
+        for (int i = 0; i < 2; ++i)
+#pragma unroll
+            for (int j = 0; j < 2; ++j)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) { t1[i][j][e] = 0.0; t2[i][j][e] = 0.0; t3[i][j][e] = 0.0; }
+        int aoff[2], boff[2];
+#pragma unroll
+        for (int i = 0; i < 2; ++i) aoff[i] = ((warp * 16 + i * 8 + r8) * P1_KS) * 16;
+#pragma unroll
+        for (int j = 0; j < 2; ++j) boff[j] = P1_BETA_BYTES + ((j * 8 + r8) * P1_PSI_PITCH + c) * 16;
+        const int sw = (r8 & 1) << 2;
+        for (int it = 0; it < nit; ++it) {
+            const int s = it % P1_ST;
+            mbar_wait(&full[s], (it / P1_ST) & 1);
+            const unsigned char *stage = smem + s * P1_STAGE_BYTES;
+#pragma unroll
+            for (int kk = 0; kk < P1_KS / 4; ++kk) {
+                double2 a[2], b[2];
+#pragma unroll
+                for (int i = 0; i < 2; ++i) a[i] = lds_c128(stage, aoff[i] + (((4 * kk) ^ sw) + c) * 16);
+#pragma unroll
+                for (int j = 0; j < 2; ++j) b[j] = lds_c128(stage, boff[j] + 4 * kk * 16);
+#pragma unroll
+                for (int i = 0; i < 2; ++i) {
+                    const double as = a[i].x - a[i].y;
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) {
+                        const double bs = b[j].x + b[j].y;
+                        dmma884(t1[i][j][0], t1[i][j][1], a[i].x, b[j].x);
+                        dmma884(t2[i][j][0], t2[i][j][1], a[i].y, b[j].y);
+                        dmma884(t3[i][j][0], t3[i][j][1], as, bs);
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[s]);
+        }
+        // conj(a) b:  re = T1 + T2,  im = T3 - T1 + T2
+        c128 *P = Ppart + (size_t)split * nrows_pad * P_NB;
+#pragma unroll
+        for (int i = 0; i < 2; ++i)
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const int row = mb * P1_ROWS + warp * 16 + i * 8 + r8, col = j * 8 + 2 * c;
+#pragma unroll
+                for (int e = 0; e < 2; ++e)
+                    P[(size_t)row * P_NB + col + e] =
+                        c128{t1[i][j][e] + t2[i][j][e], t3[i][j][e] - t1[i][j][e] + t2[i][j][e]};
+            }
+    }
+}
+
+// Q tiles for GEMM 2: qt[ic][plane][16][20], planes (Qr, Qi, Qr+Qi);  Q = D * (sum of the split partials)
+__global__ void k_reduce_p2(const c128 *__restrict__ Ppart, int nsplit, int count, c128 *__restrict__ P)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    double sr = 0.0, si = 0.0;
+    for (int s = 0; s < nsplit; ++s) {
+        const double2 v = ldg_c128(Ppart + (size_t)s * count + i);
+        sr += v.x; si += v.y;
+    }
+    P[i] = c128{sr, si};
+}
+__global__ void k_dmul_tiles(const double *__restrict__ D, int db, int nproj, int nic, const c128 *__restrict__ P,
+                             double *__restrict__ qt)
+{
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= nic * P2_KS * P_NB) return;
+    const int i = idx / P_NB, n = idx % P_NB;
+    double sr = 0.0, si = 0.0;
+    if (i < nproj) {
+        const int blk = i / db, ii = i % db;
+        const double *d = D + ((size_t)blk * db + ii) * db;
+        for (int j = 0; j < db; ++j) {
+            const double2 v = ldg_c128(P + (size_t)(blk * db + j) * P_NB + n);
+            sr += d[j] * v.x; si += d[j] * v.y;
+        }
+    }
+    double *t = qt + (size_t)(i / P2_KS) * P2_Q_DOUBLES + (i % P2_KS) * P2_Q_PITCH + n;
+    t[0] = sr; t[P2_KS * P2_Q_PITCH] = si; t[2 * P2_KS * P2_Q_PITCH] = sr + si;
+}
+
+// GEMM 2:  out[band0+n][g] += sum_i beta[i][g] Q[i][n]
+__global__ void __launch_bounds__((P2_CW + 1) * 32, 2)
+k_proj2_pipe(const c128 *__restrict__ beta2, int nic, const double *__restrict__ qt, int ng, int nb, int band0,
+             c128 *__restrict__ out)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + P2_ST * P2_STAGE_BYTES);
+    uint64_t *empty = full + P2_ST;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int gt = blockIdx.x;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < P2_ST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], P2_CW); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (warp == P2_CW) {
+        if (lane == 0) {
+            for (int it = 0; it < nic; ++it) {
+                const int s = it % P2_ST;
+                if (it >= P2_ST) mbar_wait(&empty[s], ((it / P2_ST) - 1) & 1);
+                unsigned char *stage = smem + s * P2_STAGE_BYTES;
+                mbar_expect_tx(&full[s], P2_STAGE_BYTES);
+                bulk_g2s(stage, beta2 + ((size_t)gt * nic + it) * (P2_KS * P2_G), P2_BETA_BYTES, &full[s]);
+                bulk_g2s(stage + P2_BETA_BYTES, qt + (size_t)it * P2_Q_DOUBLES, P2_Q_BYTES, &full[s]);
+            }
+        }
+    } else {
+        const int r8 = lane >> 2, c = lane & 3;
+        double t1[2][2][2], t2[2][2][2], t3[2][2][2];
+#pragma unroll
+        for (int i = 0; i < 2; ++i)
+#pragma unroll
+            for (int j = 0; j < 2; ++j)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) { t1[i][j][e] = 0.0; t2[i][j][e] = 0.0; t3[i][j][e] = 0.0; }
+        int aoff[2], qoff[2];
+#pragma unroll
+        for (int i = 0; i < 2; ++i) aoff[i] = (c * P2_G + 8 * (2 * warp + i) + (r8 ^ (2 * c))) * 16;
+#pragma unroll
+        for (int j = 0; j < 2; ++j) qoff[j] = P2_BETA_BYTES + (c * P2_Q_PITCH + 8 * j + r8) * 8;
+        for (int it = 0; it < nic; ++it) {
+            const int s = it % P2_ST;
+            mbar_wait(&full[s], (it / P2_ST) & 1);
+            const unsigned char *stage = smem + s * P2_STAGE_BYTES;
+#pragma unroll
+            for (int kk = 0; kk < P2_KS / 4; ++kk) {
+                double2 a[2];
+                double qr[2], qi[2], qs[2];
+#pragma unroll
+                for (int i = 0; i < 2; ++i) a[i] = lds_c128(stage, aoff[i] + 4 * kk * P2_G * 16);
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    const double *q = reinterpret_cast<const double *>(stage + qoff[j] + 4 * kk * P2_Q_PITCH * 8);
+                    qr[j] = q[0]; qi[j] = q[P2_KS * P2_Q_PITCH]; qs[j] = q[2 * P2_KS * P2_Q_PITCH];
+                }
+#pragma unroll
+                for (int i = 0; i < 2; ++i) {
+                    const double as = a[i].x + a[i].y;
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) {
+                        dmma884(t1[i][j][0], t1[i][j][1], a[i].x, qr[j]);
+                        dmma884(t2[i][j][0], t2[i][j][1], a[i].y, qi[j]);
+                        dmma884(t3[i][j][0], t3[i][j][1], as, qs[j]);
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[s]);
+        }
+        // a q:  re = T1 - T2,  im = T3 - T1 - T2
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const int g = gt * P2_G + 8 * (2 * warp + i) + r8;
+            if (g >= ng) continue;
+#pragma unroll
+            for (int j = 0; j < 2; ++j)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int n = band0 + j * 8 + 2 * c + e;
+                    if (n < nb) {
+                        c128 *o = out + (size_t)n * ng + g;
+                        c128 v = *o;
+                        v.x += t1[i][j][e] - t2[i][j][e];
+                        v.y += t3[i][j][e] - t1[i][j][e] - t2[i][j][e];
+                        *o = v;
+                    }
+                }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // Peak probes: register-resident DMMA / DFMA loops (roofline denominators for the projector GEMMs).
 __global__ void k_probe_dmma(double *sink, int iters)
 {

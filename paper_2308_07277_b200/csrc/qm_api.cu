@@ -53,8 +53,9 @@ struct KPoint : QmKTables {
     DevBuf<double> d_g2;
     // non-local
     bool nl_set = false;
-    int nproj = 0, nproj_pad = 0, ldb = 0, dblock = 0;
-    DevBuf<c128> d_beta;
+    int nproj = 0, dblock = 0;
+    int nmblk = 0, nkc = 0, ngt = 0, nic = 0;          // tile counts of the two beta copies
+    DevBuf<c128> d_beta1, d_beta2;
     DevBuf<double> d_D;
     QmKPlanDev plan() const {
         QmKPlanDev p;
@@ -110,7 +111,8 @@ struct qm_gspace {
     DevBuf<c128> d_tw[3];
     DevBuf<double> d_vt;
     bool v_set = false;
-    DevBuf<c128> d_W, d_Ppart, d_P, d_Q, d_stage_in, d_stage_out;
+    DevBuf<c128> d_W, d_Ppart, d_P, d_stage_in, d_stage_out;
+    DevBuf<double> d_qt;
     unsigned long long launches = 0;
     int sm_count = 148;
     int max_smem = 0;
@@ -119,9 +121,6 @@ struct qm_gspace {
 
 namespace {
 
-constexpr int PROJ_MT = 4, PROJ_NT = 2, PROJ_WARPS = 4;
-constexpr int PROJ_MBLK = 8 * PROJ_MT * PROJ_WARPS;   // 128 rows (GEMM1) / 128 G (GEMM2) per CTA
-constexpr int PROJ_NB = 8 * PROJ_NT;                  // bands per projector pass
 constexpr int ZT_STICKS = 16;                         // sticks per CTA in the z kernels
 
 int build_kpoint(qm_gspace *g, KPoint *kp) {
@@ -250,16 +249,6 @@ __global__ void k_relayout_v(const double *__restrict__ v, double *__restrict__ 
     }
 }
 
-__global__ void k_pad_beta(const c128 *__restrict__ src, int ng, int nproj, c128 *__restrict__ dst, int ldb,
-                           int nproj_pad)
-{
-    const size_t total = (size_t)nproj_pad * ldb;
-    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
-        const int row = (int)(i / ldb), col = (int)(i % ldb);
-        dst[i] = (row < nproj && col < ng) ? src[(size_t)row * ng + col] : c128{0.0, 0.0};
-    }
-}
-
 int check_handle(const qm_gspace *g, int k) {
     if (!g) return fail(QM_EINVAL, "null handle");
     if (k < 0 || k >= (int)g->kpts.size()) return fail(QM_EINVAL, "k-point index out of range");
@@ -273,33 +262,34 @@ int ensure_workspace(qm_gspace *g, const KPoint *kp, int nb) {
 
 int run_nonlocal(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb, cudaStream_t st) {
     if (kp->nproj == 0) return QM_OK;
-    const int nbp = PROJ_NB;
-    const int mblocks = kp->nproj_pad / PROJ_MBLK;
-    int nsplit = std::max(1, (g->sm_count * 4) / std::max(1, mblocks));
-    int kchunk = (kp->ng + nsplit - 1) / nsplit;
-    kchunk = std::max(64, ((kchunk + 3) / 4) * 4);
-    nsplit = (kp->ng + kchunk - 1) / kchunk;
-    const size_t pcount = (size_t)kp->nproj_pad * nbp;
+    static bool attr = false;
+    if (!attr) {
+        CU_TRY(cudaFuncSetAttribute(k_proj1_pipe, cudaFuncAttributeMaxDynamicSharedMemorySize, P1_SMEM));
+        CU_TRY(cudaFuncSetAttribute(k_proj2_pipe, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM));
+        attr = true;
+    }
+    const int nsplit = std::max(1, std::min(kp->nkc, g->sm_count / kp->nmblk));
+    const int nrows_pad = kp->nmblk * P1_ROWS;
+    const size_t pcount = (size_t)nrows_pad * P_NB;
     CU_TRY(g->d_Ppart.resize(pcount * nsplit));
     CU_TRY(g->d_P.resize(pcount));
-    CU_TRY(g->d_Q.resize(pcount));
-    for (int band0 = 0; band0 < nb; band0 += PROJ_NB) {
-        dim3 g1(mblocks, nsplit);
+    CU_TRY(g->d_qt.resize((size_t)kp->nic * P2_Q_DOUBLES));
+    for (int band0 = 0; band0 < nb; band0 += P_NB) {
         g->prof.begin(QM_K_PROJ1, st);
-        k_proj1_direct<PROJ_MT, PROJ_NT, PROJ_WARPS><<<g1, PROJ_WARPS * 32, 0, st>>>(
-            kp->d_beta.p, kp->ldb, psi_in, kp->ng, nb, band0, nbp, kp->nproj_pad, g->d_Ppart.p, kchunk);
+        k_proj1_pipe<<<dim3(kp->nmblk, nsplit), (P1_CW + 1) * 32, P1_SMEM, st>>>(
+            kp->d_beta1.p, kp->nkc, psi_in, kp->ng, nb, band0, g->d_Ppart.p, nrows_pad, nsplit);
         g->prof.end(st);
         g->prof.begin(QM_K_PREDUCE, st);
-        k_reduce_p<<<(unsigned)((pcount + 255) / 256), 256, 0, st>>>(g->d_Ppart.p, nsplit, (int)pcount, g->d_P.p);
+        k_reduce_p2<<<(unsigned)((pcount + 255) / 256), 256, 0, st>>>(g->d_Ppart.p, nsplit, (int)pcount, g->d_P.p);
         g->prof.end(st);
         g->prof.begin(QM_K_DMUL, st);
-        k_dmul<<<(unsigned)((pcount + 255) / 256), 256, 0, st>>>(kp->d_D.p, kp->dblock, kp->nproj, kp->nproj_pad, nbp,
-                                                                 g->d_P.p, g->d_Q.p);
+        const int qcount = kp->nic * P2_KS * P_NB;
+        k_dmul_tiles<<<(qcount + 255) / 256, 256, 0, st>>>(kp->d_D.p, kp->dblock, kp->nproj, kp->nic, g->d_P.p,
+                                                          g->d_qt.p);
         g->prof.end(st);
-        const int gblocks = (kp->ng + PROJ_MBLK - 1) / PROJ_MBLK;
         g->prof.begin(QM_K_PROJ2, st);
-        k_proj2_direct<PROJ_MT, PROJ_NT, PROJ_WARPS><<<gblocks, PROJ_WARPS * 32, 0, st>>>(
-            kp->d_beta.p, kp->ldb, g->d_Q.p, nbp, kp->nproj_pad, kp->ng, nb, band0, out);
+        k_proj2_pipe<<<kp->ngt, (P2_CW + 1) * 32, P2_SMEM, st>>>(kp->d_beta2.p, kp->nic, g->d_qt.p, kp->ng, nb, band0,
+                                                                 out);
         g->prof.end(st);
         g->launches += 4;
     }
@@ -433,21 +423,24 @@ QM_API int qm_set_nonlocal(qm_gspace *g, int k, const qm_c128 *beta_kG_dev, int 
     int rc = check_handle(g, k); if (rc) return rc;
     KPoint *kp = g->kpts[k];
     if (nproj < 0) return fail(QM_EINVAL, "qm_set_nonlocal: nproj < 0");
-    if (nproj == 0) { kp->nproj = 0; kp->nproj_pad = 0; kp->nl_set = true; return QM_OK; }
+    if (nproj == 0) { kp->nproj = 0; kp->nl_set = true; return QM_OK; }
     if (!beta_kG_dev || !D_dev || d_block <= 0 || nproj % d_block != 0)
         return fail(QM_EINVAL, "qm_set_nonlocal: bad beta / D / d_block");
     cudaStream_t st = (cudaStream_t)stream;
-    const int nproj_pad = ((nproj + PROJ_MBLK - 1) / PROJ_MBLK) * PROJ_MBLK;
-    const int ldb = ((kp->ng + PROJ_MBLK - 1) / PROJ_MBLK) * PROJ_MBLK;
-    CU_TRY(kp->d_beta.resize((size_t)nproj_pad * ldb));
+    const int nmblk = (nproj + P1_ROWS - 1) / P1_ROWS, nkc = (kp->ng + P1_KS - 1) / P1_KS;
+    const int ngt = (kp->ng + P2_G - 1) / P2_G, nic = (nproj + P2_KS - 1) / P2_KS;
+    CU_TRY(kp->d_beta1.resize((size_t)nmblk * nkc * P1_ROWS * P1_KS));
+    CU_TRY(kp->d_beta2.resize((size_t)ngt * nic * P2_KS * P2_G));
     const size_t dcount = (size_t)nproj * d_block;
     CU_TRY(kp->d_D.resize(dcount));
-    k_pad_beta<<<g->sm_count * 8, 256, 0, st>>>(reinterpret_cast<const c128 *>(beta_kG_dev), kp->ng, nproj,
-                                                kp->d_beta.p, ldb, nproj_pad);
-    g->launches++;
+    const c128 *src = reinterpret_cast<const c128 *>(beta_kG_dev);
+    k_tile_beta1<<<g->sm_count * 8, 256, 0, st>>>(src, kp->ng, nproj, kp->d_beta1.p, nmblk, nkc);
+    k_tile_beta2<<<g->sm_count * 8, 256, 0, st>>>(src, kp->ng, nproj, kp->d_beta2.p, ngt, nic);
+    g->launches += 2;
     CU_TRY(cudaGetLastError());
     CU_TRY(cudaMemcpyAsync(kp->d_D.p, D_dev, dcount * sizeof(double), cudaMemcpyDeviceToDevice, st));
-    kp->nproj = nproj; kp->nproj_pad = nproj_pad; kp->ldb = ldb; kp->dblock = d_block; kp->nl_set = true;
+    kp->nproj = nproj; kp->dblock = d_block; kp->nl_set = true;
+    kp->nmblk = nmblk; kp->nkc = nkc; kp->ngt = ngt; kp->nic = nic;
     return QM_OK;
 }
 
