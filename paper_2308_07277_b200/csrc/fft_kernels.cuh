@@ -15,13 +15,15 @@ k_zinv(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ psi,
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int LP = C::L | 1;
-    c128 *tw_s = reinterpret_cast<c128 *>(smem_raw);
-    c128 *lines = tw_s + C::N;
+    c128 *lines = reinterpret_cast<c128 *>(smem_raw);
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int s0 = blockIdx.x * TS;
     const int ns = min(TS, kp.nsticks - s0);
     const int band = blockIdx.y;
     const int S = kp.nsticks;
+    const int t = tid / C::TT, u = tid % C::TT;
+    c128 *tw_s = lines + TS * LP;
+    const TwTable twa{tw_s, u};
 
     for (int i = tid; i < C::N; i += nthr) tw_s[i] = tw[i];
     for (int i = tid; i < TS * LP; i += nthr) lines[i] = c128{0.0, 0.0};
@@ -31,8 +33,7 @@ k_zinv(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ psi,
     for (int g = g0 + tid; g < g1; g += nthr)
         lines[(kp.g_stick[g] - s0) * LP + kp.g_zpos[g]] = psib[g];
     __syncthreads();
-    const int t = tid / C::TT, u = tid % C::TT;
-    if (t < ns) lineA_step1<C>(lines + t * LP, u, tw_s);
+    if (t < ns) lineA_step1<C>(lines + t * LP, u, twa);
     __syncthreads();
     if (t < ns) lineA_step2<C>(lines + t * LP, u);
     __syncthreads();
@@ -50,23 +51,24 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int LP = C::L | 1;
-    c128 *tw_s = reinterpret_cast<c128 *>(smem_raw);
-    c128 *lines = tw_s + C::N;
+    c128 *lines = reinterpret_cast<c128 *>(smem_raw);
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int s0 = blockIdx.x * TS;
     const int ns = min(TS, kp.nsticks - s0);
     const int band = blockIdx.y;
     const int S = kp.nsticks;
-
+    const int t = tid / C::TT, u = tid % C::TT;
+    c128 *tw_s = lines + TS * LP;
+    const TwTable twb{tw_s, u};
     for (int i = tid; i < C::N; i += nthr) tw_s[i] = tw[i];
+
     const c128 *Wb = W + (size_t)band * C::N * S;
     for (int i = tid; i < C::N * TS; i += nthr) {
         const int p = i / TS, tt = i % TS;
         if (tt < ns) lines[tt * LP + C::pos(p)] = Wb[(size_t)p * S + s0 + tt];
     }
     __syncthreads();
-    const int t = tid / C::TT, u = tid % C::TT;
-    if (t < ns) lineB_step1<C>(lines + t * LP, u, tw_s);
+    if (t < ns) lineB_step1<C>(lines + t * LP, u, twb);
     __syncthreads();
     if (t < ns) lineB_step2<C>(lines + t * LP, u);
     __syncthreads();
@@ -84,75 +86,104 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
 }
 
 // MODE 0 apply, 1 g2r (write natural-order box), 2 r2g (read natural-order box)
+//
+// One CTA per (band, z-plane).  The CTA is split into independent groups of 64 threads (two warps =
+// 64/TT teams of TT threads, one team per line); a group walks its own rows / columns and only
+// synchronises with itself (named barrier), so the groups hide each other's latencies.  CTA-wide
+// barriers remain only between the four phases (load | y backward | x round trip | y forward | store).
+constexpr int QM_GROUP = 64;
+__device__ __forceinline__ void group_barrier(int grp) {
+    asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "r"(QM_GROUP) : "memory");
+}
+
 template <class C, int MODE>
-__global__ void __launch_bounds__(512)
-k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ box, int ncol, double scale)
+__global__ void __launch_bounds__(384)
+k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ box, int ngroups, double scale)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int SL = C::L | 1;                         // scratch line pitch
+    constexpr int TPG = QM_GROUP / C::TT;                // teams (lines) per group
     const int X = kp.nx, rowpitch = kp.rowpitch, S = kp.nsticks;
-    c128 *tw_s = reinterpret_cast<c128 *>(smem_raw);
-    c128 *A = tw_s + C::N;
+    c128 *A = reinterpret_cast<c128 *>(smem_raw);
     c128 *scr = A + (size_t)X * rowpitch;
-    short *xrow_s = reinterpret_cast<short *>(scr + (size_t)ncol * SL);
+    short4 *rowiv_s = reinterpret_cast<short4 *>(scr + (size_t)ngroups * TPG * SL);
+    const XRows xr{kp.x_iv.x, kp.x_iv.y, kp.x_iv.z, kp.x_iv.w};
     const int tid = threadIdx.x, nthr = blockDim.x;
+    const int grp = tid / QM_GROUP, gl = tid % QM_GROUP;
+    const int team = gl / C::TT, u = gl % C::TT;
+    const bool team_ok = team < TPG;
     const int p = blockIdx.x, band = blockIdx.y;
     const int n3 = gd.ax[2].n;
     c128 *Wp = W + ((size_t)band * n3 + p) * S;
 
-    for (int i = tid; i < C::N; i += nthr) { tw_s[i] = gd.tw[0][i]; xrow_s[i] = kp.xrow[i]; }
+    // per-thread twiddle rows (u is fixed for the whole kernel)
+    TwRow<C::R1> twa;
+    load_twrow(twa, gd.tw[0], u, C::R2);
+    TwRow<C::R2> twb_store;
+    if constexpr (C::R1 != C::R2) load_twrow(twb_store, gd.tw[0], u, C::R1);
+    const auto &twb = [&]() -> const TwRow<C::R2> & {
+        if constexpr (C::R1 == C::R2) return twa; else return twb_store;
+    }();
+
+    for (int i = tid; i < X; i += nthr) rowiv_s[i] = kp.row_iv[i];
     if constexpr (MODE != 2) {
-        for (int i = tid; i < X * rowpitch; i += nthr) A[i] = c128{0.0, 0.0};
-        __syncthreads();
+        if (kp.zero_fill) {
+            for (int i = tid; i < X * rowpitch; i += nthr) A[i] = c128{0.0, 0.0};
+            __syncthreads();
+        }
         for (int s = tid; s < S; s += nthr) A[kp.stick_apos[s]] = Wp[s];
         __syncthreads();
-        for (int base = 0; base < X * C::TT; base += nthr) {
-            const int task = base + tid;
-            if (task < X * C::TT) lineA_step1<C>(A + (task / C::TT) * rowpitch, task % C::TT, tw_s);
-        }
-        __syncthreads();
-        for (int base = 0; base < X * C::TT; base += nthr) {
-            const int task = base + tid;
-            if (task < X * C::TT) lineA_step2<C>(A + (task / C::TT) * rowpitch, task % C::TT);
+        for (int rc = grp; rc * TPG < X; rc += ngroups) {
+            const int r = rc * TPG + team;
+            const bool ok = team_ok && r < X;
+            if (ok) lineA_step1_pruned<C>(A + r * rowpitch, u, twa, rowiv_s[r]);
+            group_barrier(grp);
+            if (ok) lineA_step2<C>(A + r * rowpitch, u);
         }
     }
     __syncthreads();
     {
-        const int c = tid / C::TT, u = tid % C::TT;
         const int z = (p / gd.ax[2].r2) + gd.ax[2].r1 * (p % gd.ax[2].r2);
-        c128 *myscr = scr + (size_t)c * SL;
-        for (int cbase = 0; cbase < C::N; cbase += ncol) {
-            const int col = cbase + c;
-            const bool active = (c < ncol) && (col < C::N);
+        c128 *myscr = scr + (size_t)(grp * TPG + team) * SL;
+        const double *vplane = gd.vt + (size_t)p * C::N * C::N;
+        VRow<C::R2> vr;
+        if constexpr (MODE == 0) {       // V of the first column: in flight while step 1 runs
+            const int col0 = grp * TPG + team;
+            if (team_ok && col0 < C::N) load_vrow<C>(vr, vplane + (size_t)col0 * C::N, u);
+        }
+        for (int cc = grp; cc * TPG < C::N; cc += ngroups) {
+            const int col = cc * TPG + team;
+            const bool ok = team_ok && col < C::N;
             const int colpos = C::pos(col);
             if constexpr (MODE != 2) {
-                if (active) xcol_step1<C>(A, rowpitch, colpos, xrow_s, myscr, u, tw_s);
-                __syncthreads();
+                if (ok) xcol_step1<C>(A, rowpitch, colpos, xr, myscr, u, twa);
+                group_barrier(grp);
             }
-            if (active) {
+            if (ok) {
                 const int y = (col / C::R2) + C::R1 * (col % C::R2);
-                const double *v = nullptr;
                 c128 *bx = nullptr;
-                if constexpr (MODE == 0) v = gd.vt + ((size_t)p * C::N + col) * C::N;
-                else bx = box + (size_t)band * C::N * C::N * n3 + (size_t)y * n3 + z;
-                xcol_step2<C, MODE>(myscr, u, tw_s, v, bx, (long)C::N * n3, scale);
+                if constexpr (MODE != 0) bx = box + (size_t)band * C::N * C::N * n3 + (size_t)y * n3 + z;
+                xcol_step2<C, MODE>(myscr, u, twb, vr, bx, (long)C::N * n3, scale);
             }
-            __syncthreads();
+            if constexpr (MODE == 0) {   // prefetch V of this team's next column behind steps 3 and 1
+                const int ncol = col + ngroups * TPG;
+                if (team_ok && ncol < C::N) load_vrow<C>(vr, vplane + (size_t)ncol * C::N, u);
+            }
+            group_barrier(grp);
             if constexpr (MODE != 1) {
-                if (active) xcol_step3<C>(A, rowpitch, colpos, xrow_s, myscr, u);
-                __syncthreads();
+                if (ok) xcol_step3<C>(A, rowpitch, colpos, xr, myscr, u);
+                group_barrier(grp);
             }
         }
     }
+    __syncthreads();
     if constexpr (MODE != 1) {
-        for (int base = 0; base < X * C::TT; base += nthr) {
-            const int task = base + tid;
-            if (task < X * C::TT) lineB_step1<C>(A + (task / C::TT) * rowpitch, task % C::TT, tw_s);
-        }
-        __syncthreads();
-        for (int base = 0; base < X * C::TT; base += nthr) {
-            const int task = base + tid;
-            if (task < X * C::TT) lineB_step2<C>(A + (task / C::TT) * rowpitch, task % C::TT);
+        for (int rc = grp; rc * TPG < X; rc += ngroups) {
+            const int r = rc * TPG + team;
+            const bool ok = team_ok && r < X;
+            if (ok) lineB_step1<C>(A + r * rowpitch, u, twb);
+            group_barrier(grp);
+            if (ok) lineB_step2<C>(A + r * rowpitch, u);
         }
         __syncthreads();
         for (int s = tid; s < S; s += nthr) Wp[s] = A[kp.stick_apos[s]];

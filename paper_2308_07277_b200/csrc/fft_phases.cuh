@@ -24,15 +24,47 @@ template <int R1_, int R2_> struct LineCfg {
     static QM_HD int pos(int i) { return (i / R2) * R2P + (i % R2); }
 };
 
-// tw[j] = exp(-2 pi i j / N)
-template <class C> QM_HD void lineA_step1(c128 *line, int u, const c128 *tw) {
+// Per-thread twiddle rows held in registers: TW[j] = exp(-2 pi i u j / N) for the thread's fixed u.
+// (Looking them up in shared memory at stride j costs up to 8-way bank conflicts; every thread keeps
+//  the same u for the whole kernel, so the row is loaded once.)
+template <int R> struct TwRow {
+    c128 w[R];
+    template <int J> QM_HD c128 get() const { return w[J]; }
+};
+// Same interface, but looked up in a table on every use (kernels that use each twiddle only once).
+struct TwTable {
+    const c128 *tw; int u;
+    template <int J> QM_HD c128 get() const { return tw[u * J]; }
+};
+template <int R> QM_HD void load_twrow(TwRow<R> &t, const c128 *tw, int u, int limit) {
+    static_for<R>([&](auto I) { constexpr int j = decltype(I)::value; t.w[j] = (u < limit) ? tw[u * j] : c128{1.0, 0.0}; });
+}
+
+// iv: the line holds data only at natural indices [iv.x, iv.y] and [iv.z, iv.w]; everything else reads as zero
+// (so the plane array never needs a zero-fill pass)
+template <class C, class TW> QM_HD void lineA_step1_pruned(c128 *line, int u, const TW &tw, short4 iv) {
+    if (u >= C::R2) return;
+    c128 t[C::R1];
+    static_for<C::R1>([&](auto I) {
+        constexpr int n1 = decltype(I)::value;
+        const int i = n1 * C::R2 + u;
+        t[n1] = ((i >= iv.x && i <= iv.y) || (i >= iv.z && i <= iv.w)) ? line[n1 * C::R2P + u] : c128{0.0, 0.0};
+    });
+    Dft<C::R1, +1>::run(t);
+    static_for<C::R1>([&](auto I) {
+        constexpr int k1 = decltype(I)::value;
+        line[k1 * C::R2P + u] = (k1 == 0) ? t[k1] : cmul_conj(t[k1], tw.template get<k1>());
+    });
+}
+
+template <class C, class TW> QM_HD void lineA_step1(c128 *line, int u, const TW &tw) {
     if (u >= C::R2) return;
     c128 t[C::R1];
     static_for<C::R1>([&](auto I) { constexpr int n1 = decltype(I)::value; t[n1] = line[n1 * C::R2P + u]; });
     Dft<C::R1, +1>::run(t);
     static_for<C::R1>([&](auto I) {
         constexpr int k1 = decltype(I)::value;
-        line[k1 * C::R2P + u] = (k1 == 0) ? t[k1] : cmul_conj(t[k1], tw[u * k1]);
+        line[k1 * C::R2P + u] = (k1 == 0) ? t[k1] : cmul_conj(t[k1], tw.template get<k1>());
     });
 }
 template <class C> QM_HD void lineA_step2(c128 *line, int u) {
@@ -42,14 +74,14 @@ template <class C> QM_HD void lineA_step2(c128 *line, int u) {
     Dft<C::R2, +1>::run(t);
     static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; line[u * C::R2P + k2] = t[k2]; });
 }
-template <class C> QM_HD void lineB_step1(c128 *line, int u, const c128 *tw) {
+template <class C, class TW> QM_HD void lineB_step1(c128 *line, int u, const TW &tw) {
     if (u >= C::R1) return;
     c128 t[C::R2];
     static_for<C::R2>([&](auto I) { constexpr int b = decltype(I)::value; t[b] = line[u * C::R2P + b]; });
     Dft<C::R2, -1>::run(t);
     static_for<C::R2>([&](auto I) {
         constexpr int d = decltype(I)::value;
-        line[u * C::R2P + d] = (d == 0) ? t[d] : cmul(t[d], tw[u * d]);
+        line[u * C::R2P + d] = (d == 0) ? t[d] : cmul(t[d], tw.template get<d>());
     });
 }
 template <class C> QM_HD void lineB_step2(c128 *line, int u) {
@@ -61,29 +93,41 @@ template <class C> QM_HD void lineB_step2(c128 *line, int u) {
 }
 
 // ---- x direction of the plane kernel: X compact rows <-> full length-N1 line in scratch -------------
-// A: plane array [X][rowpitch]; xrow[i1] = compact row of box index i1, or -1.
-template <class C> QM_HD void xcol_step1(const c128 *A, int rowpitch, int colpos, const short *xrow,
-                                         c128 *scr, int u, const c128 *tw) {
+// A: plane array [X][rowpitch].  The occupied box indices i1 form two intervals (the sphere is convex):
+// [a1,b1] -> rows 0.., [a2,b2] -> rows (b1-a1+1)..; everything else is not stored (zero).
+struct XRows {
+    int a1, b1, a2, b2;
+    QM_HD int row(int i1) const {
+        return (i1 >= a1 && i1 <= b1) ? i1 - a1 : ((i1 >= a2 && i1 <= b2) ? i1 - a2 + (b1 - a1 + 1) : -1);
+    }
+};
+template <class C, class TW> QM_HD void xcol_step1(const c128 *A, int rowpitch, int colpos, const XRows xr,
+                                                   c128 *scr, int u, const TW &tw) {
     if (u >= C::R2) return;
     c128 t[C::R1];
     static_for<C::R1>([&](auto I) {
         constexpr int n1 = decltype(I)::value;
-        const int r = xrow[n1 * C::R2 + u];
+        const int r = xr.row(n1 * C::R2 + u);
         t[n1] = (r >= 0) ? A[r * rowpitch + colpos] : c128{0.0, 0.0};
     });
     Dft<C::R1, +1>::run(t);
     static_for<C::R1>([&](auto I) {
         constexpr int k1 = decltype(I)::value;
-        scr[k1 * C::R2P + u] = (k1 == 0) ? t[k1] : cmul_conj(t[k1], tw[u * k1]);
+        scr[k1 * C::R2P + u] = (k1 == 0) ? t[k1] : cmul_conj(t[k1], tw.template get<k1>());
     });
 }
 // MODE 0: apply  (backward step 2, multiply by v[x], forward step 1)      PAPER.md:659-662 (eq. 47)
 // MODE 1: g2r    (backward step 2, write psi(r)*scale to box, stop)
 // MODE 2: r2g    (read box, forward step 1)
-// v: pointer to the N1 potential values of this (plane, column), natural x order.
+// v: this thread's R2 potential values V(x = u + R1*k2), already in registers (prefetched by the caller).
 // box: pointer to element x=0 of this column in a natural-order box, xstride = n2*n3.
-template <class C, int MODE> QM_HD void xcol_step2(c128 *scr, int u, const c128 *tw, const double *v,
-                                                   c128 *box, long xstride, double scale) {
+template <int R> struct VRow { double v[R]; };
+template <class C> QM_HD void load_vrow(VRow<C::R2> &vr, const double *v, int u) {
+    if (u >= C::R1) return;
+    static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; vr.v[k2] = v[u + C::R1 * k2]; });
+}
+template <class C, int MODE, class TW> QM_HD void xcol_step2(c128 *scr, int u, const TW &tw, const VRow<C::R2> &vr,
+                                                             c128 *box, long xstride, double scale) {
     if (u >= C::R1) return;
     c128 t[C::R2];
     if constexpr (MODE == 2) {
@@ -95,16 +139,16 @@ template <class C, int MODE> QM_HD void xcol_step2(c128 *scr, int u, const c128 
             static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; box[(long)(u + C::R1 * k2) * xstride] = cscale(t[k2], scale); });
             return;
         } else {
-            static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; t[k2] = cscale(t[k2], v[u + C::R1 * k2]); });
+            static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; t[k2] = cscale(t[k2], vr.v[k2]); });
         }
     }
     Dft<C::R2, -1>::run(t);
     static_for<C::R2>([&](auto I) {
         constexpr int d = decltype(I)::value;
-        scr[u * C::R2P + d] = (d == 0) ? t[d] : cmul(t[d], tw[u * d]);
+        scr[u * C::R2P + d] = (d == 0) ? t[d] : cmul(t[d], tw.template get<d>());
     });
 }
-template <class C> QM_HD void xcol_step3(c128 *A, int rowpitch, int colpos, const short *xrow,
+template <class C> QM_HD void xcol_step3(c128 *A, int rowpitch, int colpos, const XRows xr,
                                          const c128 *scr, int u) {
     if (u >= C::R2) return;
     c128 t[C::R1];
@@ -112,7 +156,7 @@ template <class C> QM_HD void xcol_step3(c128 *A, int rowpitch, int colpos, cons
     Dft<C::R1, -1>::run(t);
     static_for<C::R1>([&](auto I) {
         constexpr int c = decltype(I)::value;
-        const int r = xrow[u + C::R2 * c];
+        const int r = xr.row(u + C::R2 * c);
         if (r >= 0) A[r * rowpitch + colpos] = t[c];
     });
 }

@@ -47,6 +47,10 @@ struct QmKTables {
     std::vector<int32_t> gstick, stickoff, stickapos;
     std::vector<uint16_t> gzpos;
     std::vector<int16_t> xrow;
+    std::vector<short4> rowiv;                 // per plane row: occupied i2 intervals
+    short4 xiv = {1, 0, 1, 0};                 // occupied i1 intervals (rows 0.. and following)
+    bool x_contiguous = true;
+    int zero_fill = 0;
 };
 
 // returns 0, or -1 (sphere does not fit the grid) / -2 (empty sphere); msg gets the reason
@@ -116,7 +120,46 @@ static inline int qm_build_tables(const double *lattice, const double *recip, do
     for (int s = 0; s < S; ++s)
         if (kp->xrow[stick_i1[s]] < 0) kp->xrow[stick_i1[s]] = (int16_t)nx++;   // sticks ascend in i1
     kp->nx = nx;
+    {   // occupied i1 intervals; rows must follow them in order (true for a convex sphere)
+        short4 iv = {1, 0, 1, 0};
+        for (int i1 = 0; i1 < n1; ++i1) {
+            if (kp->xrow[i1] < 0) continue;
+            if (2 * i1 < n1) { if (iv.x > iv.y) iv.x = (short)i1; iv.y = (short)i1; }
+            else { if (iv.z > iv.w) iv.z = (short)i1; iv.w = (short)i1; }
+        }
+        kp->xiv = iv;
+        kp->x_contiguous = true;
+        const int c1 = iv.x <= iv.y ? iv.y - iv.x + 1 : 0;
+        for (int i1 = 0; i1 < n1; ++i1) {
+            const int want = (i1 >= iv.x && i1 <= iv.y) ? i1 - iv.x
+                             : ((i1 >= iv.z && i1 <= iv.w) ? i1 - iv.z + c1 : -1);
+            if (want != kp->xrow[i1]) kp->x_contiguous = false;
+        }
+        if (!kp->x_contiguous) { *msg = "occupied x columns are not two contiguous intervals"; return -1; }
+    }
     kp->rowpitch = ax[1].len | 1;
+    // occupied i2 intervals of every plane row: [0..m2max] and [n2+m2min..n2-1] (the sphere is convex, so
+    // the sticks of a row are contiguous in m2); verified below, else the plane kernel zero-fills.
+    kp->rowiv.assign(nx, short4{1, 0, 1, 0});
+    std::vector<int> rowcount(nx, 0);
+    for (int s = 0; s < S; ++s) {
+        short4 &iv = kp->rowiv[kp->xrow[stick_i1[s]]];
+        const int i2 = stick_i2[s];
+        rowcount[kp->xrow[stick_i1[s]]]++;
+        if (2 * i2 < n2) {        // non-negative m2
+            if (iv.x > iv.y) { iv.x = (short)i2; iv.y = (short)i2; }
+            else { iv.x = std::min<short>(iv.x, (short)i2); iv.y = std::max<short>(iv.y, (short)i2); }
+        } else {
+            if (iv.z > iv.w) { iv.z = (short)i2; iv.w = (short)i2; }
+            else { iv.z = std::min<short>(iv.z, (short)i2); iv.w = std::max<short>(iv.w, (short)i2); }
+        }
+    }
+    kp->zero_fill = 0;
+    for (int r = 0; r < nx; ++r) {
+        const short4 iv = kp->rowiv[r];
+        const int span = (iv.x <= iv.y ? iv.y - iv.x + 1 : 0) + (iv.z <= iv.w ? iv.w - iv.z + 1 : 0);
+        if (span != rowcount[r]) kp->zero_fill = 1;
+    }
     kp->stickapos.resize(S);
     for (int s = 0; s < S; ++s)
         kp->stickapos[s] = kp->xrow[stick_i1[s]] * kp->rowpitch + qm_pos(ax[1], stick_i2[s]);

@@ -50,6 +50,7 @@ struct KPoint : QmKTables {
     DevBuf<int32_t> d_gstick, d_stickoff, d_stickapos;
     DevBuf<uint16_t> d_gzpos;
     DevBuf<int16_t> d_xrow;
+    DevBuf<short4> d_rowiv;
     DevBuf<double> d_g2;
     // non-local
     bool nl_set = false;
@@ -62,6 +63,7 @@ struct KPoint : QmKTables {
         p.ng = ng; p.nsticks = nsticks; p.nx = nx; p.rowpitch = rowpitch;
         p.g_stick = d_gstick.p; p.g_zpos = d_gzpos.p; p.stick_off = d_stickoff.p;
         p.stick_apos = d_stickapos.p; p.xrow = d_xrow.p; p.g2 = d_g2.p;
+        p.row_iv = d_rowiv.p; p.zero_fill = zero_fill; p.x_iv = xiv;
         return p;
     }
 };
@@ -133,27 +135,32 @@ int build_kpoint(qm_gspace *g, KPoint *kp) {
     CU_TRY(kp->d_stickoff.upload(kp->stickoff));
     CU_TRY(kp->d_stickapos.upload(kp->stickapos));
     CU_TRY(kp->d_xrow.upload(kp->xrow));
+    CU_TRY(kp->d_rowiv.upload(kp->rowiv));
     CU_TRY(kp->d_g2.upload(kp->g2));
     return QM_OK;
 }
 
-size_t plane_smem(const qm_gspace *g, const KPoint *kp, int ncol) {
+constexpr int PLANE_GROUP = 64;
+size_t plane_smem(const qm_gspace *g, const KPoint *kp, int ngroups) {
     const QmAxis &ax = g->ax[0];
     const size_t sl = (size_t)(ax.len | 1);
-    return ((size_t)ax.n + (size_t)kp->nx * kp->rowpitch + (size_t)ncol * sl) * sizeof(c128)
-           + (size_t)ax.n * sizeof(short) + 16;
+    const int tpg = PLANE_GROUP / std::max(ax.r1, ax.r2);
+    return ((size_t)kp->nx * kp->rowpitch + (size_t)ngroups * tpg * sl) * sizeof(c128)
+           + (size_t)kp->nx * sizeof(short4) + 16;
 }
 
-// choose the number of columns processed concurrently by the plane kernel
-int plane_ncol(const qm_gspace *g, const KPoint *kp) {
+// number of independent 64-thread groups of the plane kernel: the fewest groups that reach the
+// minimum number of column rounds within the shared-memory and thread limits
+int plane_groups(const qm_gspace *g, const KPoint *kp) {
     const QmAxis &ax = g->ax[0];
-    const int tt = std::max(ax.r1, ax.r2);
-    int ncol = std::min(ax.n, 512 / tt);
-    while (ncol > 1 && plane_smem(g, kp, ncol) > (size_t)g->max_smem) --ncol;
-    // prefer a divisor-friendly count so the last pass is not mostly idle
-    int best = ncol;
-    for (int c = ncol; c >= std::max(1, ncol - ncol / 4); --c)
-        if (ax.n % c == 0) { best = c; break; }
+    const int tpg = PLANE_GROUP / std::max(ax.r1, ax.r2);
+    const int nchunks = (ax.n + tpg - 1) / tpg;
+    int gmax = std::min(384 / PLANE_GROUP, nchunks);
+    while (gmax > 1 && plane_smem(g, kp, gmax) > (size_t)g->max_smem) --gmax;
+    const int rounds = (nchunks + gmax - 1) / gmax;
+    int best = gmax;
+    for (int c = gmax; c >= 1; --c)
+        if ((nchunks + c - 1) / c == rounds) best = c;
     return best;
 }
 
@@ -186,8 +193,8 @@ template <class C> int launch_zfwd(qm_gspace *g, KPoint *kp, const c128 *psi_in,
 }
 template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *box, int nb, double scale,
                                               cudaStream_t st) {
-    const int ncol = plane_ncol(g, kp);
-    const size_t smem = plane_smem(g, kp, ncol);
+    const int ngroups = plane_groups(g, kp);
+    const size_t smem = plane_smem(g, kp, ngroups);
     if (smem > (size_t)g->max_smem)
         return fail(QM_EGRID, "plane kernel does not fit shared memory for this grid / sphere");
     CU_TRY(cudaFuncSetAttribute(k_plane<C, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -196,7 +203,7 @@ template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *bo
     gd.vt = g->d_vt.p;
     dim3 grid(g->grid[2], nb);
     g->prof.begin(QM_K_PLANE, st);
-    k_plane<C, MODE><<<grid, ncol * C::TT, smem, st>>>(kp->plan(), gd, g->d_W.p, box, ncol, scale);
+    k_plane<C, MODE><<<grid, ngroups * PLANE_GROUP, smem, st>>>(kp->plan(), gd, g->d_W.p, box, ngroups, scale);
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());

@@ -1,6 +1,7 @@
 // Plain-old-data plans handed to the kernels (device pointers inside).
 #pragma once
 #include <stdint.h>
+#include <vector_types.h>
 
 struct c128;
 
@@ -18,6 +19,9 @@ struct QmKPlanDev {        // per k-point tables on the device
     const int32_t *stick_off;    // [S+1]  first G of each stick
     const int32_t *stick_apos;   // [S]    position in the plane array: row*rowpitch + pos(i2)
     const int16_t *xrow;         // [n1]   compact row of box index i1, or -1
+    short4 x_iv;                 //        occupied i1 intervals [x,y] -> rows 0.., [z,w] -> following rows
+    const short4 *row_iv;        // [X]    per plane row: occupied i2 intervals [x,y] and [z,w]
+    int zero_fill;               // 1 if some row's sticks do not fill its intervals (plane must be zeroed)
     const double *g2;            // [ng]   |k+G|^2
 };
 

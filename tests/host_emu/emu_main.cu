@@ -32,6 +32,8 @@ template <class C> struct Emu {
             tw[j] = c128{(double)cosl(ang), (double)sinl(ang)};
         }
     }
+    TwRow<C::R1> rowA(int u) { TwRow<C::R1> t; load_twrow(t, tw.data(), u, C::R2); return t; }
+    TwRow<C::R2> rowB(int u) { TwRow<C::R2> t; load_twrow(t, tw.data(), u, C::R1); return t; }
     // k_zinv for one band: psi[ng] -> W[N][S]
     void zinv(const c128 *psi, c128 *W) {
         const int S = kp.nsticks, nthr = TS * C::TT;
@@ -40,7 +42,7 @@ template <class C> struct Emu {
             std::vector<c128> lines(TS * LP, c128{0, 0});
             for (int g = kp.stickoff[s0]; g < kp.stickoff[s0 + ns]; ++g)
                 lines[(kp.gstick[g] - s0) * LP + kp.gzpos[g]] = psi[g];
-            for (int tid = 0; tid < nthr; ++tid) { int t = tid / C::TT, u = tid % C::TT; if (t < ns) lineA_step1<C>(&lines[t * LP], u, tw.data()); }
+            for (int tid = 0; tid < nthr; ++tid) { int t = tid / C::TT, u = tid % C::TT; if (t < ns) lineA_step1<C>(&lines[t * LP], u, rowA(u)); }
             for (int tid = 0; tid < nthr; ++tid) { int t = tid / C::TT, u = tid % C::TT; if (t < ns) lineA_step2<C>(&lines[t * LP], u); }
             for (int i = 0; i < C::N * TS; ++i) { int p = i / TS, tt = i % TS; if (tt < ns) W[(size_t)p * S + s0 + tt] = lines[tt * LP + C::pos(p)]; }
         }
@@ -51,7 +53,7 @@ template <class C> struct Emu {
             const int ns = std::min(TS, S - s0);
             std::vector<c128> lines(TS * LP, c128{0, 0});
             for (int i = 0; i < C::N * TS; ++i) { int p = i / TS, tt = i % TS; if (tt < ns) lines[tt * LP + C::pos(p)] = W[(size_t)p * S + s0 + tt]; }
-            for (int tid = 0; tid < nthr; ++tid) { int t = tid / C::TT, u = tid % C::TT; if (t < ns) lineB_step1<C>(&lines[t * LP], u, tw.data()); }
+            for (int tid = 0; tid < nthr; ++tid) { int t = tid / C::TT, u = tid % C::TT; if (t < ns) lineB_step1<C>(&lines[t * LP], u, rowB(u)); }
             for (int tid = 0; tid < nthr; ++tid) { int t = tid / C::TT, u = tid % C::TT; if (t < ns) lineB_step2<C>(&lines[t * LP], u); }
             for (int g = kp.stickoff[s0]; g < kp.stickoff[s0 + ns]; ++g) {
                 c128 v = lines[(kp.gstick[g] - s0) * LP + kp.gzpos[g]];
@@ -63,36 +65,39 @@ template <class C> struct Emu {
     // k_plane for one (band, p).  vt: relaid potential; box: natural-order box of this band
     template <int MODE> void plane(int p, c128 *W, const double *vt, c128 *box, double scale, int ncol) {
         const int X = kp.nx, rp = kp.rowpitch, S = kp.nsticks, n3 = ax.n, nthr = ncol * C::TT;
-        std::vector<c128> A((size_t)X * rp, c128{0, 0}), scr((size_t)ncol * SL);
+        // A is deliberately filled with garbage: the pruned y pass must never read an unoccupied position
+        std::vector<c128> A((size_t)X * rp, kp.zero_fill ? c128{0, 0} : c128{1e300, -1e300}), scr((size_t)ncol * SL);
         c128 *Wp = W + (size_t)p * S;
         if (MODE != 2) {
             for (int s = 0; s < S; ++s) A[kp.stickapos[s]] = Wp[s];
-            for (int task = 0; task < X * C::TT; ++task) lineA_step1<C>(&A[(task / C::TT) * rp], task % C::TT, tw.data());
+            for (int task = 0; task < X * C::TT; ++task) lineA_step1_pruned<C>(&A[(task / C::TT) * rp], task % C::TT, rowA(task % C::TT), kp.rowiv[task / C::TT]);
             for (int task = 0; task < X * C::TT; ++task) lineA_step2<C>(&A[(task / C::TT) * rp], task % C::TT);
         }
         const int z = (p / ax.r2) + ax.r1 * (p % ax.r2);
+        const XRows xr{kp.xiv.x, kp.xiv.y, kp.xiv.z, kp.xiv.w};
         for (int cbase = 0; cbase < C::N; cbase += ncol) {
             if (MODE != 2)
                 for (int tid = 0; tid < nthr; ++tid) {
                     int c = tid / C::TT, u = tid % C::TT, col = cbase + c;
-                    if (col < C::N) xcol_step1<C>(A.data(), rp, C::pos(col), kp.xrow.data(), &scr[(size_t)c * SL], u, tw.data());
+                    if (col < C::N) xcol_step1<C>(A.data(), rp, C::pos(col), xr, &scr[(size_t)c * SL], u, rowA(u));
                 }
             for (int tid = 0; tid < nthr; ++tid) {
                 int c = tid / C::TT, u = tid % C::TT, col = cbase + c;
                 if (col >= C::N) continue;
                 int y = (col / C::R2) + C::R1 * (col % C::R2);
-                const double *v = MODE == 0 ? vt + ((size_t)p * C::N + col) * C::N : nullptr;
+                VRow<C::R2> vr;
+                if (MODE == 0) load_vrow<C>(vr, vt + ((size_t)p * C::N + col) * C::N, u);
                 c128 *bx = MODE == 0 ? nullptr : box + (size_t)y * n3 + z;
-                xcol_step2<C, MODE>(&scr[(size_t)c * SL], u, tw.data(), v, bx, (long)C::N * n3, scale);
+                xcol_step2<C, MODE>(&scr[(size_t)c * SL], u, rowB(u), vr, bx, (long)C::N * n3, scale);
             }
             if (MODE != 1)
                 for (int tid = 0; tid < nthr; ++tid) {
                     int c = tid / C::TT, u = tid % C::TT, col = cbase + c;
-                    if (col < C::N) xcol_step3<C>(A.data(), rp, C::pos(col), kp.xrow.data(), &scr[(size_t)c * SL], u);
+                    if (col < C::N) xcol_step3<C>(A.data(), rp, C::pos(col), xr, &scr[(size_t)c * SL], u);
                 }
         }
         if (MODE != 1) {
-            for (int task = 0; task < X * C::TT; ++task) lineB_step1<C>(&A[(task / C::TT) * rp], task % C::TT, tw.data());
+            for (int task = 0; task < X * C::TT; ++task) lineB_step1<C>(&A[(task / C::TT) * rp], task % C::TT, rowB(task % C::TT));
             for (int task = 0; task < X * C::TT; ++task) lineB_step2<C>(&A[(task / C::TT) * rp], task % C::TT);
             for (int s = 0; s < S; ++s) Wp[s] = A[kp.stickapos[s]];
         }
