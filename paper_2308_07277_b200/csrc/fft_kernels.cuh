@@ -98,7 +98,8 @@ __device__ __forceinline__ void group_barrier(int grp) {
 
 template <class C, int MODE>
 __global__ void __launch_bounds__(384)
-k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ box, int ngroups, double scale)
+k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ box, int ngroups, double scale,
+        int stagger_ns)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int SL = C::L | 1;                         // scratch line pitch
@@ -106,7 +107,7 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
     const int X = kp.nx, rowpitch = kp.rowpitch, S = kp.nsticks;
     c128 *A = reinterpret_cast<c128 *>(smem_raw);
     c128 *scr = A + (size_t)X * rowpitch;
-    short4 *rowiv_s = reinterpret_cast<short4 *>(scr + (size_t)ngroups * TPG * SL);
+    int4 *rowinfo_s = reinterpret_cast<int4 *>(scr + (size_t)ngroups * TPG * SL);
     const XRows xr{kp.x_iv.x, kp.x_iv.y, kp.x_iv.z, kp.x_iv.w};
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int grp = tid / QM_GROUP, gl = tid % QM_GROUP;
@@ -125,18 +126,17 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
         if constexpr (C::R1 == C::R2) return twa; else return twb_store;
     }();
 
-    for (int i = tid; i < X; i += nthr) rowiv_s[i] = kp.row_iv[i];
+    for (int i = tid; i < X; i += nthr) rowinfo_s[i] = kp.row_info[i];
+    __syncthreads();
+    auto row_info = [&](int r) {
+        const int4 q = rowinfo_s[r];
+        return RowInfo{(int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, q.z};
+    };
     if constexpr (MODE != 2) {
-        if (kp.zero_fill) {
-            for (int i = tid; i < X * rowpitch; i += nthr) A[i] = c128{0.0, 0.0};
-            __syncthreads();
-        }
-        for (int s = tid; s < S; s += nthr) A[kp.stick_apos[s]] = Wp[s];
-        __syncthreads();
         for (int rc = grp; rc * TPG < X; rc += ngroups) {
             const int r = rc * TPG + team;
             const bool ok = team_ok && r < X;
-            if (ok) lineA_step1_pruned<C>(A + r * rowpitch, u, twa, rowiv_s[r]);
+            if (ok) lineA_step1_gin<C>(A + r * rowpitch, Wp, row_info(r), u, twa);
             group_barrier(grp);
             if (ok) lineA_step2<C>(A + r * rowpitch, u);
         }
@@ -147,6 +147,9 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
         c128 *myscr = scr + (size_t)(grp * TPG + team) * SL;
         const double *vplane = gd.vt + (size_t)p * C::N * C::N;
         VRow<C::R2> vr;
+        // De-phase the groups: they all do identical load -> FP64 -> store bursts, and when they run in
+        // lock step the shared-memory pipe and the FP64 pipe are used alternately instead of together.
+        if (stagger_ns > 0) __nanosleep((unsigned)(grp * stagger_ns));
         if constexpr (MODE == 0) {       // V of the first column: in flight while step 1 runs
             const int col0 = grp * TPG + team;
             if (team_ok && col0 < C::N) load_vrow<C>(vr, vplane + (size_t)col0 * C::N, u);
@@ -183,9 +186,7 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
             const bool ok = team_ok && r < X;
             if (ok) lineB_step1<C>(A + r * rowpitch, u, twb);
             group_barrier(grp);
-            if (ok) lineB_step2<C>(A + r * rowpitch, u);
+            if (ok) lineB_step2_gout<C>(A + r * rowpitch, Wp, row_info(r), u);
         }
-        __syncthreads();
-        for (int s = tid; s < S; s += nthr) Wp[s] = A[kp.stick_apos[s]];
     }
 }

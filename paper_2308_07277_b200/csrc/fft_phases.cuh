@@ -40,20 +40,41 @@ template <int R> QM_HD void load_twrow(TwRow<R> &t, const c128 *tw, int u, int l
     static_for<R>([&](auto I) { constexpr int j = decltype(I)::value; t.w[j] = (u < limit) ? tw[u * j] : c128{1.0, 0.0}; });
 }
 
-// iv: the line holds data only at natural indices [iv.x, iv.y] and [iv.z, iv.w]; everything else reads as zero
-// (so the plane array never needs a zero-fill pass)
-template <class C, class TW> QM_HD void lineA_step1_pruned(c128 *line, int u, const TW &tw, short4 iv) {
+// One plane row of the stick buffer: the occupied i2 indices are the intervals [a1,b1] and [a2,b2]
+// (convex sphere), stored back to back starting at stick index sbase.
+struct RowInfo {
+    int a1, b1, a2, b2, sbase;
+    QM_HD int stick(int i) const {      // stick index of natural index i, or -1 if the row has no stick there
+        return (i >= a1 && i <= b1) ? sbase + i - a1
+                                    : ((i >= a2 && i <= b2) ? sbase + (b1 - a1 + 1) + i - a2 : -1);
+    }
+};
+// Backward step 1 reading its (pruned) input straight from the stick plane in global memory:
+// the plane array needs neither a load pass nor a zero fill.
+template <class C, class TW> QM_HD void lineA_step1_gin(c128 *line, const c128 *Wp, const RowInfo ri, int u, const TW &tw) {
     if (u >= C::R2) return;
     c128 t[C::R1];
     static_for<C::R1>([&](auto I) {
         constexpr int n1 = decltype(I)::value;
-        const int i = n1 * C::R2 + u;
-        t[n1] = ((i >= iv.x && i <= iv.y) || (i >= iv.z && i <= iv.w)) ? line[n1 * C::R2P + u] : c128{0.0, 0.0};
+        const int s = ri.stick(n1 * C::R2 + u);
+        t[n1] = (s >= 0) ? Wp[s] : c128{0.0, 0.0};
     });
     Dft<C::R1, +1>::run(t);
     static_for<C::R1>([&](auto I) {
         constexpr int k1 = decltype(I)::value;
         line[k1 * C::R2P + u] = (k1 == 0) ? t[k1] : cmul_conj(t[k1], tw.template get<k1>());
+    });
+}
+// Forward step 2 writing only the occupied outputs straight to the stick plane in global memory.
+template <class C> QM_HD void lineB_step2_gout(const c128 *line, c128 *Wp, const RowInfo ri, int u) {
+    if (u >= C::R2) return;
+    c128 t[C::R1];
+    static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = line[a * C::R2P + u]; });
+    Dft<C::R1, -1>::run(t);
+    static_for<C::R1>([&](auto I) {
+        constexpr int c = decltype(I)::value;
+        const int s = ri.stick(c * C::R2 + u);
+        if (s >= 0) Wp[s] = t[c];
     });
 }
 

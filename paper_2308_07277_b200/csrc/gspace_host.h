@@ -48,9 +48,9 @@ struct QmKTables {
     std::vector<uint16_t> gzpos;
     std::vector<int16_t> xrow;
     std::vector<short4> rowiv;                 // per plane row: occupied i2 intervals
+    std::vector<int4> rowinfo;                 // packed (a1|b1<<16, a2|b2<<16, first stick of the row, 0)
     short4 xiv = {1, 0, 1, 0};                 // occupied i1 intervals (rows 0.. and following)
     bool x_contiguous = true;
-    int zero_fill = 0;
 };
 
 // returns 0, or -1 (sphere does not fit the grid) / -2 (empty sphere); msg gets the reason
@@ -154,11 +154,16 @@ static inline int qm_build_tables(const double *lattice, const double *recip, do
             else { iv.z = std::min<short>(iv.z, (short)i2); iv.w = std::max<short>(iv.w, (short)i2); }
         }
     }
-    kp->zero_fill = 0;
-    for (int r = 0; r < nx; ++r) {
-        const short4 iv = kp->rowiv[r];
-        const int span = (iv.x <= iv.y ? iv.y - iv.x + 1 : 0) + (iv.z <= iv.w ? iv.w - iv.z + 1 : 0);
-        if (span != rowcount[r]) kp->zero_fill = 1;
+    kp->rowinfo.resize(nx);
+    {
+        int s = 0;
+        for (int r = 0; r < nx; ++r) {
+            const short4 iv = kp->rowiv[r];
+            const int span = (iv.x <= iv.y ? iv.y - iv.x + 1 : 0) + (iv.z <= iv.w ? iv.w - iv.z + 1 : 0);
+            if (span != rowcount[r]) { *msg = "sticks of a plane row are not two contiguous intervals"; return -1; }
+            kp->rowinfo[r] = int4{(int)(unsigned short)iv.x | ((int)iv.y << 16), (int)(unsigned short)iv.z | ((int)iv.w << 16), s, 0};
+            s += span;      // sticks ascend in (i1, i2): the row's sticks are [s, s + span)
+        }
     }
     kp->stickapos.resize(S);
     for (int s = 0; s < S; ++s)

@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -50,7 +51,7 @@ struct KPoint : QmKTables {
     DevBuf<int32_t> d_gstick, d_stickoff, d_stickapos;
     DevBuf<uint16_t> d_gzpos;
     DevBuf<int16_t> d_xrow;
-    DevBuf<short4> d_rowiv;
+    DevBuf<int4> d_rowinfo;
     DevBuf<double> d_g2;
     // non-local
     bool nl_set = false;
@@ -63,7 +64,7 @@ struct KPoint : QmKTables {
         p.ng = ng; p.nsticks = nsticks; p.nx = nx; p.rowpitch = rowpitch;
         p.g_stick = d_gstick.p; p.g_zpos = d_gzpos.p; p.stick_off = d_stickoff.p;
         p.stick_apos = d_stickapos.p; p.xrow = d_xrow.p; p.g2 = d_g2.p;
-        p.row_iv = d_rowiv.p; p.zero_fill = zero_fill; p.x_iv = xiv;
+        p.row_info = d_rowinfo.p; p.x_iv = xiv;
         return p;
     }
 };
@@ -118,6 +119,7 @@ struct qm_gspace {
     unsigned long long launches = 0;
     int sm_count = 148;
     int max_smem = 0;
+    int plane_stagger_ns = 0;
     ~qm_gspace() { for (auto *k : kpts) delete k; }
 };
 
@@ -135,7 +137,7 @@ int build_kpoint(qm_gspace *g, KPoint *kp) {
     CU_TRY(kp->d_stickoff.upload(kp->stickoff));
     CU_TRY(kp->d_stickapos.upload(kp->stickapos));
     CU_TRY(kp->d_xrow.upload(kp->xrow));
-    CU_TRY(kp->d_rowiv.upload(kp->rowiv));
+    CU_TRY(kp->d_rowinfo.upload(kp->rowinfo));
     CU_TRY(kp->d_g2.upload(kp->g2));
     return QM_OK;
 }
@@ -146,7 +148,7 @@ size_t plane_smem(const qm_gspace *g, const KPoint *kp, int ngroups) {
     const size_t sl = (size_t)(ax.len | 1);
     const int tpg = PLANE_GROUP / std::max(ax.r1, ax.r2);
     return ((size_t)kp->nx * kp->rowpitch + (size_t)ngroups * tpg * sl) * sizeof(c128)
-           + (size_t)kp->nx * sizeof(short4) + 16;
+           + (size_t)kp->nx * sizeof(int4) + 16;
 }
 
 // number of independent 64-thread groups of the plane kernel: the fewest groups that reach the
@@ -203,7 +205,8 @@ template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *bo
     gd.vt = g->d_vt.p;
     dim3 grid(g->grid[2], nb);
     g->prof.begin(QM_K_PLANE, st);
-    k_plane<C, MODE><<<grid, ngroups * PLANE_GROUP, smem, st>>>(kp->plan(), gd, g->d_W.p, box, ngroups, scale);
+    k_plane<C, MODE><<<grid, ngroups * PLANE_GROUP, smem, st>>>(kp->plan(), gd, g->d_W.p, box, ngroups, scale,
+                                                                   g->plane_stagger_ns);
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
@@ -369,6 +372,7 @@ QM_API int qm_gspace_create(const double *lattice_bohr, double ecutwfc_ry, const
             return bail(QM_EGRID);
         }
     }
+    if (const char *e = getenv("QM_PLANE_STAGGER_NS")) g->plane_stagger_ns = atoi(e);
     *out = g;
     return QM_OK;
 }

@@ -20,8 +20,7 @@ struct QmKPlanDev {        // per k-point tables on the device
     const int32_t *stick_apos;   // [S]    position in the plane array: row*rowpitch + pos(i2)
     const int16_t *xrow;         // [n1]   compact row of box index i1, or -1
     short4 x_iv;                 //        occupied i1 intervals [x,y] -> rows 0.., [z,w] -> following rows
-    const short4 *row_iv;        // [X]    per plane row: occupied i2 intervals [x,y] and [z,w]
-    int zero_fill;               // 1 if some row's sticks do not fill its intervals (plane must be zeroed)
+    const int4 *row_info;        // [X]    per plane row: (a1 | b1<<16, a2 | b2<<16, first stick, 0): occupied i2 intervals
     const double *g2;            // [ng]   |k+G|^2
 };
 

@@ -65,12 +65,15 @@ template <class C> struct Emu {
     // k_plane for one (band, p).  vt: relaid potential; box: natural-order box of this band
     template <int MODE> void plane(int p, c128 *W, const double *vt, c128 *box, double scale, int ncol) {
         const int X = kp.nx, rp = kp.rowpitch, S = kp.nsticks, n3 = ax.n, nthr = ncol * C::TT;
-        // A is deliberately filled with garbage: the pruned y pass must never read an unoccupied position
-        std::vector<c128> A((size_t)X * rp, kp.zero_fill ? c128{0, 0} : c128{1e300, -1e300}), scr((size_t)ncol * SL);
+        // A is deliberately filled with garbage: every position must be written before it is read
+        std::vector<c128> A((size_t)X * rp, c128{1e300, -1e300}), scr((size_t)ncol * SL);
+        auto row_info = [&](int r) {
+            const int4 q = kp.rowinfo[r];
+            return RowInfo{(int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, q.z};
+        };
         c128 *Wp = W + (size_t)p * S;
         if (MODE != 2) {
-            for (int s = 0; s < S; ++s) A[kp.stickapos[s]] = Wp[s];
-            for (int task = 0; task < X * C::TT; ++task) lineA_step1_pruned<C>(&A[(task / C::TT) * rp], task % C::TT, rowA(task % C::TT), kp.rowiv[task / C::TT]);
+            for (int task = 0; task < X * C::TT; ++task) lineA_step1_gin<C>(&A[(task / C::TT) * rp], Wp, row_info(task / C::TT), task % C::TT, rowA(task % C::TT));
             for (int task = 0; task < X * C::TT; ++task) lineA_step2<C>(&A[(task / C::TT) * rp], task % C::TT);
         }
         const int z = (p / ax.r2) + ax.r1 * (p % ax.r2);
@@ -98,8 +101,7 @@ template <class C> struct Emu {
         }
         if (MODE != 1) {
             for (int task = 0; task < X * C::TT; ++task) lineB_step1<C>(&A[(task / C::TT) * rp], task % C::TT, rowB(task % C::TT));
-            for (int task = 0; task < X * C::TT; ++task) lineB_step2<C>(&A[(task / C::TT) * rp], task % C::TT);
-            for (int s = 0; s < S; ++s) Wp[s] = A[kp.stickapos[s]];
+            for (int task = 0; task < X * C::TT; ++task) lineB_step2_gout<C>(&A[(task / C::TT) * rp], Wp, row_info(task / C::TT), task % C::TT);
         }
     }
 };
