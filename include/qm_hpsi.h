@@ -104,6 +104,16 @@ QM_API int qm_apply_h(qm_gspace *g, const qm_c128 *psi_in_dev, qm_c128 *psi_out_
 QM_API int qm_apply_h_host(qm_gspace *g, const qm_c128 *psi_in_host, qm_c128 *psi_out_host,
                     int nbands, int k, void *stream);
 
+/* Asynchronous form of qm_apply_h_host for streaming many blocks: the call only enqueues
+ * (H2D on an internal copy stream, the apply on `stream`, D2H on a second internal copy stream,
+ * chained by events, two staging slots) and returns; consecutive calls therefore overlap the
+ * copies of one block with the compute of its neighbours.  psi_out_host is valid, and
+ * psi_in_host may be reused, after qm_host_synchronize (or after the matching block's D2H has
+ * completed).  Host buffers should be pinned, otherwise the copies are synchronous. */
+QM_API int qm_apply_h_host_async(qm_gspace *g, const qm_c128 *psi_in_host, qm_c128 *psi_out_host,
+                                 int nbands, int k, void *stream);
+QM_API int qm_host_synchronize(qm_gspace *g);
+
 /* Test hooks (not hot path) exercising the same kernels (A5):
  *  qm_debug_g2r : box_r[b][n1*n2*n3] = (1/N) sum_G psi_g[b][G] e^{+iG.r}   (scatter + backward FFT)
  *  qm_debug_r2g : psi_g[b][ng]       = sum_r box_r[b][r] e^{-iG.r}, taken on the sphere (unnormalised)

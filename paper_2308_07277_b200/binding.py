@@ -43,6 +43,8 @@ _SIGS = {
     "qm_set_nonlocal": [_vp, _i, _vp, _i, _vp, _i, _vp],
     "qm_apply_h": [_vp, _vp, _vp, _i, _i, _vp],
     "qm_apply_h_host": [_vp, _vp, _vp, _i, _i, _vp],
+    "qm_apply_h_host_async": [_vp, _vp, _vp, _i, _i, _vp],
+    "qm_host_synchronize": [_vp],
     "qm_debug_g2r": [_vp, _vp, _vp, _i, _i, _vp],
     "qm_debug_r2g": [_vp, _vp, _vp, _i, _i, _vp],
     "qm_get_launch_count": [_vp, ctypes.POINTER(ctypes.c_ulonglong)],
@@ -204,16 +206,31 @@ def qm_apply_h(h, psi_in_dev, psi_out_dev, k=0, stream=None):
     return psi_out_dev
 
 
-def qm_apply_h_host(h, psi_in_host, psi_out_host, k=0, stream=None):
-    """Host (ideally pinned) torch tensors [nb][ng] complex128; copies are done inside the C call."""
+def _host_call(fn, h, psi_in_host, psi_out_host, k, stream):
     import torch
     nb = _check_block(h, k, psi_in_host, "psi_in")
+    if tuple(psi_out_host.shape) != tuple(psi_in_host.shape):
+        raise TypeError("psi_out: shape differs from psi_in")
     for t in (psi_in_host, psi_out_host):
         if t.is_cuda or t.dtype != torch.complex128 or not t.is_contiguous():
             raise TypeError("qm_apply_h_host: expected contiguous complex128 host tensors")
-    _check(load_library().qm_apply_h_host(h, ctypes.c_void_p(psi_in_host.data_ptr()),
-                                          ctypes.c_void_p(psi_out_host.data_ptr()), nb, k, _stream_ptr(stream)))
+    _check(fn(h, ctypes.c_void_p(psi_in_host.data_ptr()), ctypes.c_void_p(psi_out_host.data_ptr()), nb, k,
+              _stream_ptr(stream)))
     return psi_out_host
+
+
+def qm_apply_h_host(h, psi_in_host, psi_out_host, k=0, stream=None):
+    """Host (ideally pinned) torch tensors [nb][ng] complex128; copies are done inside the C call."""
+    return _host_call(load_library().qm_apply_h_host, h, psi_in_host, psi_out_host, k, stream)
+
+
+def qm_apply_h_host_async(h, psi_in_host, psi_out_host, k=0, stream=None):
+    """Enqueue-only form; results are valid after qm_host_synchronize(h)."""
+    return _host_call(load_library().qm_apply_h_host_async, h, psi_in_host, psi_out_host, k, stream)
+
+
+def qm_host_synchronize(h):
+    _check(load_library().qm_host_synchronize(h))
 
 
 def qm_debug_g2r(h, psi_g_dev, box_r_dev, k=0, stream=None):
@@ -302,6 +319,11 @@ class GSpace:
 
     def apply_h_host(self, psi_in, psi_out, k=0, stream=None):
         return qm_apply_h_host(self._h, psi_in, psi_out, k, stream)
+
+    def apply_h_host_async(self, psi_in, psi_out, k=0, stream=None):
+        return qm_apply_h_host_async(self._h, psi_in, psi_out, k, stream)
+
+    def host_synchronize(self): qm_host_synchronize(self._h)
 
     def g2r(self, psi_g, k=0, stream=None):
         import torch

@@ -104,8 +104,23 @@ struct Profiler {
     void reset() { collect(); for (int i = 0; i < QM_K_COUNT; ++i) { total_ms[i] = 0; count[i] = 0; } }
 };
 
+struct HostPipe {       // two-slot staging pipeline behind qm_apply_h_host(_async)
+    bool init = false;
+    cudaStream_t s_in = nullptr, s_out = nullptr;
+    cudaEvent_t in_ready[2], compute_done[2], out_done[2];
+    bool used[2] = {false, false};
+    DevBuf<c128> in[2], out[2];
+    int slot = 0;
+    ~HostPipe() {
+        if (!init) return;
+        for (int i = 0; i < 2; ++i) { cudaEventDestroy(in_ready[i]); cudaEventDestroy(compute_done[i]); cudaEventDestroy(out_done[i]); }
+        cudaStreamDestroy(s_in); cudaStreamDestroy(s_out);
+    }
+};
+
 struct qm_gspace {
     Profiler prof;
+    HostPipe pipe;
     double lattice[9], recip[9];
     double ecut;
     int grid[3];
@@ -114,7 +129,7 @@ struct qm_gspace {
     DevBuf<c128> d_tw[3];
     DevBuf<double> d_vt;
     bool v_set = false;
-    DevBuf<c128> d_W, d_Ppart, d_P, d_stage_in, d_stage_out;
+    DevBuf<c128> d_W, d_Ppart, d_P;
     DevBuf<double> d_qt;
     unsigned long long launches = 0;
     int sm_count = 148;
@@ -474,22 +489,61 @@ QM_API int qm_apply_h(qm_gspace *g, const qm_c128 *psi_in_dev, qm_c128 *psi_out_
     return run_nonlocal(g, kp, in, out, nbands, st);
 }
 
-QM_API int qm_apply_h_host(qm_gspace *g, const qm_c128 *psi_in_host, qm_c128 *psi_out_host, int nbands, int k,
-                    void *stream) {
+QM_API int qm_host_synchronize(qm_gspace *g) {
+    if (!g) return fail(QM_EINVAL, "null handle");
+    if (!g->pipe.init) return QM_OK;
+    CU_TRY(cudaStreamSynchronize(g->pipe.s_in));
+    CU_TRY(cudaStreamSynchronize(g->pipe.s_out));
+    return QM_OK;
+}
+
+QM_API int qm_apply_h_host_async(qm_gspace *g, const qm_c128 *psi_in_host, qm_c128 *psi_out_host, int nbands, int k,
+                                 void *stream) {
     int rc = check_handle(g, k); if (rc) return rc;
     if (!psi_in_host || !psi_out_host || nbands <= 0) return fail(QM_EINVAL, "qm_apply_h_host: bad argument");
     KPoint *kp = g->kpts[k];
+    HostPipe &hp = g->pipe;
+    if (!hp.init) {
+        CU_TRY(cudaStreamCreateWithFlags(&hp.s_in, cudaStreamNonBlocking));
+        CU_TRY(cudaStreamCreateWithFlags(&hp.s_out, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            CU_TRY(cudaEventCreateWithFlags(&hp.in_ready[i], cudaEventDisableTiming));
+            CU_TRY(cudaEventCreateWithFlags(&hp.compute_done[i], cudaEventDisableTiming));
+            CU_TRY(cudaEventCreateWithFlags(&hp.out_done[i], cudaEventDisableTiming));
+        }
+        hp.init = true;
+    }
+    const int sl = hp.slot;
+    hp.slot ^= 1;
     const size_t count = (size_t)nbands * kp->ng;
-    CU_TRY(g->d_stage_in.resize(count));
-    CU_TRY(g->d_stage_out.resize(count));
+    if (hp.in[sl].n < count || hp.out[sl].n < count) {      // growing a slot: nothing may still be using it
+        rc = qm_host_synchronize(g); if (rc) return rc;
+        CU_TRY(cudaStreamSynchronize((cudaStream_t)stream));
+        CU_TRY(hp.in[sl].resize(count));
+        CU_TRY(hp.out[sl].resize(count));
+    }
     cudaStream_t st = (cudaStream_t)stream;
-    CU_TRY(cudaMemcpyAsync(g->d_stage_in.p, psi_in_host, count * sizeof(c128), cudaMemcpyHostToDevice, st));
-    rc = qm_apply_h(g, reinterpret_cast<const qm_c128 *>(g->d_stage_in.p),
-                    reinterpret_cast<qm_c128 *>(g->d_stage_out.p), nbands, k, stream);
+    if (hp.used[sl]) CU_TRY(cudaStreamWaitEvent(hp.s_in, hp.compute_done[sl], 0));    // slot's last apply has read it
+    CU_TRY(cudaMemcpyAsync(hp.in[sl].p, psi_in_host, count * sizeof(c128), cudaMemcpyHostToDevice, hp.s_in));
+    CU_TRY(cudaEventRecord(hp.in_ready[sl], hp.s_in));
+    CU_TRY(cudaStreamWaitEvent(st, hp.in_ready[sl], 0));
+    if (hp.used[sl]) CU_TRY(cudaStreamWaitEvent(st, hp.out_done[sl], 0));             // slot's last result has left
+    rc = qm_apply_h(g, reinterpret_cast<const qm_c128 *>(hp.in[sl].p), reinterpret_cast<qm_c128 *>(hp.out[sl].p),
+                    nbands, k, stream);
     if (rc) return rc;
-    CU_TRY(cudaMemcpyAsync(psi_out_host, g->d_stage_out.p, count * sizeof(c128), cudaMemcpyDeviceToHost, st));
-    CU_TRY(cudaStreamSynchronize(st));
+    CU_TRY(cudaEventRecord(hp.compute_done[sl], st));
+    CU_TRY(cudaStreamWaitEvent(hp.s_out, hp.compute_done[sl], 0));
+    CU_TRY(cudaMemcpyAsync(psi_out_host, hp.out[sl].p, count * sizeof(c128), cudaMemcpyDeviceToHost, hp.s_out));
+    CU_TRY(cudaEventRecord(hp.out_done[sl], hp.s_out));
+    hp.used[sl] = true;
     return QM_OK;
+}
+
+QM_API int qm_apply_h_host(qm_gspace *g, const qm_c128 *psi_in_host, qm_c128 *psi_out_host, int nbands, int k,
+                           void *stream) {
+    int rc = qm_apply_h_host_async(g, psi_in_host, psi_out_host, nbands, k, stream);
+    if (rc) return rc;
+    return qm_host_synchronize(g);
 }
 
 QM_API int qm_debug_g2r(qm_gspace *g, const qm_c128 *psi_g_dev, qm_c128 *box_r_dev, int nbands, int k, void *stream) {

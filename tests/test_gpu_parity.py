@@ -171,6 +171,25 @@ def test_host_entry_matches_device_entry(qm):
     gs.close()
 
 
+def test_async_host_pipeline_streams_many_blocks(qm):
+    """qm_apply_h_host_async: consecutive blocks overlap copies and compute (two staging slots); all
+    results must equal the device entry's, whatever the block sizes."""
+    torch, dev = _torch()
+    p = problem("cfg3")
+    gs = _gspace(qm, p)
+    want = _apply(qm, gs, p, p["psi"], "full")
+    hin = torch.from_numpy(p["psi"]).pin_memory()
+    hout = torch.zeros_like(hin).pin_memory()
+    edges = [0, 16, 17, 40, 48, 64]                      # ragged blocks, more blocks than slots
+    for rep in range(2):
+        hout.zero_()
+        for a, b in zip(edges[:-1], edges[1:]):
+            gs.apply_h_host_async(hin[a:b], hout[a:b])
+        gs.host_synchronize()
+        np.testing.assert_array_equal(hout.numpy(), want)
+    gs.close()
+
+
 def test_error_codes(qm):
     torch, dev = _torch()
     p = problem("cfg1")
