@@ -51,6 +51,7 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int LP = C::L | 1;
+    constexpr int GPT = 4;            // gather elements per thread kept in registers across the FFT
     c128 *lines = reinterpret_cast<c128 *>(smem_raw);
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int s0 = blockIdx.x * TS;
@@ -67,14 +68,35 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
         const int p = i / TS, tt = i % TS;
         if (tt < ns) lines[tt * LP + C::pos(p)] = Wb[(size_t)p * S + s0 + tt];
     }
+    // the gather's own inputs (positions, 1/2|k+G|^2 psi_in) are fetched now, behind the transform
+    const int g0 = kp.stick_off[s0], g1 = kp.stick_off[s0 + ns];
+    const size_t boff = (size_t)band * kp.ng;
+    int gpos[GPT];
+    c128 kin[GPT];
+#pragma unroll
+    for (int j = 0; j < GPT; ++j) {
+        const int g = g0 + tid + j * nthr;
+        gpos[j] = -1; kin[j] = c128{0.0, 0.0};
+        if (g < g1) {
+            gpos[j] = (kp.g_stick[g] - s0) * LP + kp.g_zpos[g];
+            if (kinetic) {
+                const c128 x = psi_in[boff + g];
+                const double h = 0.5 * kp.g2[g];
+                kin[j] = c128{h * x.x, h * x.y};
+            }
+        }
+    }
     __syncthreads();
     if (t < ns) lineB_step1<C>(lines + t * LP, u, twb);
     __syncthreads();
     if (t < ns) lineB_step2<C>(lines + t * LP, u);
     __syncthreads();
-    const int g0 = kp.stick_off[s0], g1 = kp.stick_off[s0 + ns];
-    const size_t boff = (size_t)band * kp.ng;
-    for (int g = g0 + tid; g < g1; g += nthr) {
+#pragma unroll
+    for (int j = 0; j < GPT; ++j) {
+        const int g = g0 + tid + j * nthr;
+        if (g < g1) out[boff + g] = lines[gpos[j]] + kin[j];
+    }
+    for (int g = g0 + tid + GPT * nthr; g < g1; g += nthr) {     // sticks longer than the register budget
         c128 v = lines[(kp.g_stick[g] - s0) * LP + kp.g_zpos[g]];
         if (kinetic) {
             const c128 x = psi_in[boff + g];
@@ -92,6 +114,9 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
 // synchronises with itself (named barrier), so the groups hide each other's latencies.  CTA-wide
 // barriers remain only between the four phases (load | y backward | x round trip | y forward | store).
 constexpr int QM_GROUP = 64;
+// Scratch lines of neighbouring teams: with 12-thread teams a quarter-warp straddles two teams as 4+4
+// threads, and their unit-stride 16-byte accesses are conflict free iff the pitch is 4 (mod 8); else odd.
+__host__ __device__ constexpr int qm_scratch_pitch(int len, int tt) { return tt == 12 ? len + ((12 - len % 8) % 8) : (len | 1); }
 __device__ __forceinline__ void group_barrier(int grp) {
     asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "r"(QM_GROUP) : "memory");
 }
@@ -102,7 +127,7 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
         int stagger_ns)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int SL = C::L | 1;                         // scratch line pitch
+    constexpr int SL = qm_scratch_pitch(C::L, C::TT);    // scratch line pitch
     constexpr int TPG = QM_GROUP / C::TT;                // teams (lines) per group
     const int X = kp.nx, rowpitch = kp.rowpitch, S = kp.nsticks;
     c128 *A = reinterpret_cast<c128 *>(smem_raw);
@@ -174,8 +199,10 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
             }
             group_barrier(grp);
             if constexpr (MODE != 1) {
+                // no barrier after step 3: the scratch column a thread reads here is exactly the one it
+                // overwrites in the next iteration's step 1 (MODE 2 has no step 1 and writes rows: barrier).
                 if (ok) xcol_step3<C>(A, rowpitch, colpos, xr, myscr, u);
-                group_barrier(grp);
+                if constexpr (MODE == 2) group_barrier(grp);
             }
         }
     }

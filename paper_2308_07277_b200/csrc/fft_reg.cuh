@@ -122,10 +122,36 @@ template <int RA, int RB, int DIR> struct DftComposite {
     }
 };
 
-template <int DIR> struct Dft<6, DIR> { static QM_HD void run(c128 (&x)[6]) { DftComposite<2, 3, DIR>::run(x); } };
+// Good-Thomas prime-factor form for coprime RA, RB: no internal twiddles at all.
+//   n = (RB*n1 + RA*n2) mod R,   k = (RB*(RB^-1 mod RA)*k1 + RA*(RA^-1 mod RB)*k2) mod R
+//   => w_R^{nk} = w_RA^{n1 k1} * w_RB^{n2 k2}
+__host__ __device__ constexpr int qm_modinv(int a, int m) { for (int x = 1; x < m; ++x) if ((a * x) % m == 1) return x; return 1; }
+template <int RA, int RB, int DIR> struct DftPFA {
+    static constexpr int R = RA * RB;
+    static constexpr int EA = RB * qm_modinv(RB % RA, RA), EB = RA * qm_modinv(RA % RB, RB);
+    static QM_HD void run(c128 (&x)[R]) {
+        c128 y[R];
+        static_for<RB>([&](auto N2) {
+            constexpr int n2 = decltype(N2)::value;
+            c128 t[RA];
+            static_for<RA>([&](auto N1) { constexpr int n1 = decltype(N1)::value; t[n1] = x[(RB * n1 + RA * n2) % R]; });
+            Dft<RA, DIR>::run(t);
+            static_for<RA>([&](auto K1) { constexpr int k1 = decltype(K1)::value; y[k1 * RB + n2] = t[k1]; });
+        });
+        static_for<RA>([&](auto K1) {
+            constexpr int k1 = decltype(K1)::value;
+            c128 t[RB];
+            static_for<RB>([&](auto N2) { constexpr int n2 = decltype(N2)::value; t[n2] = y[k1 * RB + n2]; });
+            Dft<RB, DIR>::run(t);
+            static_for<RB>([&](auto K2) { constexpr int k2 = decltype(K2)::value; x[(EA * k1 + EB * k2) % R] = t[k2]; });
+        });
+    }
+};
+
+template <int DIR> struct Dft<6, DIR> { static QM_HD void run(c128 (&x)[6]) { DftPFA<2, 3, DIR>::run(x); } };
 template <int DIR> struct Dft<8, DIR> { static QM_HD void run(c128 (&x)[8]) { DftComposite<2, 4, DIR>::run(x); } };
 template <int DIR> struct Dft<9, DIR> { static QM_HD void run(c128 (&x)[9]) { DftComposite<3, 3, DIR>::run(x); } };
-template <int DIR> struct Dft<10, DIR> { static QM_HD void run(c128 (&x)[10]) { DftComposite<2, 5, DIR>::run(x); } };
-template <int DIR> struct Dft<12, DIR> { static QM_HD void run(c128 (&x)[12]) { DftComposite<3, 4, DIR>::run(x); } };
-template <int DIR> struct Dft<15, DIR> { static QM_HD void run(c128 (&x)[15]) { DftComposite<3, 5, DIR>::run(x); } };
+template <int DIR> struct Dft<10, DIR> { static QM_HD void run(c128 (&x)[10]) { DftPFA<2, 5, DIR>::run(x); } };
+template <int DIR> struct Dft<12, DIR> { static QM_HD void run(c128 (&x)[12]) { DftPFA<3, 4, DIR>::run(x); } };
+template <int DIR> struct Dft<15, DIR> { static QM_HD void run(c128 (&x)[15]) { DftPFA<3, 5, DIR>::run(x); } };
 template <int DIR> struct Dft<16, DIR> { static QM_HD void run(c128 (&x)[16]) { DftComposite<4, 4, DIR>::run(x); } };

@@ -2,7 +2,7 @@
 //   a6  P = beta^H psi          PAPER.md:153-161 (eq. 14), 767 ("vdot" as ZGEMM)
 //   a7  Q = D P                 block-diagonal real-symmetric D (ONCV multi-projector)
 //   a8  out += beta Q
-// Complex products are four real DMMA chains (re/im split in registers; beta stays interleaved in HBM).
+// Complex products are three real DMMA chains (3M scheme; beta stays interleaved in HBM).
 #pragma once
 #include <cuda_runtime.h>
 #include "fft_reg.cuh"
@@ -17,149 +17,7 @@ __device__ __forceinline__ double2 ldg_c128(const c128 *p) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// v1 kernels: fragments loaded straight from global memory (L1/L2 give the reuse).
-// beta: [nproj_pad][ldb] zero padded (library copy).  psi: caller's [nb][ng].
-// Ppart: [nsplit][nproj_pad][nbp].
-template <int MT, int NT, int WARPS>
-__global__ void __launch_bounds__(WARPS * 32)
-k_proj1_direct(const c128 *__restrict__ beta, int ldb, const c128 *__restrict__ psi, int ng,
-               int nb, int band0, int nbp, int nproj_pad, c128 *__restrict__ Ppart, int kchunk)
-{
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int r = lane >> 2, c = lane & 3;
-    const int j0 = (blockIdx.x * WARPS + warp) * 8 * MT;
-    if (j0 >= nproj_pad) return;
-    const int kbeg = blockIdx.y * kchunk;
-    const int kend = min(ng, kbeg + kchunk);
-    double cre[MT][NT][2], cim[MT][NT][2];
-#pragma unroll
-    for (int i = 0; i < MT; ++i)
-#pragma unroll
-        for (int j = 0; j < NT; ++j) { cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0; }
-    const c128 *bp[MT];
-#pragma unroll
-    for (int i = 0; i < MT; ++i) bp[i] = beta + (size_t)(j0 + i * 8 + r) * ldb + c;
-    const c128 *pp[NT];
-#pragma unroll
-    for (int j = 0; j < NT; ++j) pp[j] = psi + (size_t)min(band0 + j * 8 + r, nb - 1) * ng + c;
-#pragma unroll 2
-    for (int k = kbeg; k < kend; k += 4) {
-        double2 a[MT], b[NT];
-        const bool ok = (k + c) < kend;
-#pragma unroll
-        for (int i = 0; i < MT; ++i) a[i] = ldg_c128(bp[i] + k);      // beta is zero padded past ng
-#pragma unroll
-        for (int j = 0; j < NT; ++j) b[j] = ok ? ldg_c128(pp[j] + k) : make_double2(0.0, 0.0);
-#pragma unroll
-        for (int i = 0; i < MT; ++i)
-#pragma unroll
-            for (int j = 0; j < NT; ++j) {
-                // conj(a) * b = (ar br + ai bi) + i (ar bi - ai br)
-                dmma884(cre[i][j][0], cre[i][j][1], a[i].x, b[j].x);
-                dmma884(cre[i][j][0], cre[i][j][1], a[i].y, b[j].y);
-                dmma884(cim[i][j][0], cim[i][j][1], a[i].x, b[j].y);
-                dmma884(cim[i][j][0], cim[i][j][1], a[i].y, -b[j].x);
-            }
-    }
-    c128 *P = Ppart + (size_t)blockIdx.y * nproj_pad * nbp;
-#pragma unroll
-    for (int i = 0; i < MT; ++i)
-#pragma unroll
-        for (int j = 0; j < NT; ++j) {
-            const int row = j0 + i * 8 + r, col = j * 8 + 2 * c;
-            P[(size_t)row * nbp + col] = c128{cre[i][j][0], cim[i][j][0]};
-            P[(size_t)row * nbp + col + 1] = c128{cre[i][j][1], cim[i][j][1]};
-        }
-}
-
-// P[j][n] = sum_s Ppart[s][j][n]  (fixed order => deterministic)
-__global__ void k_reduce_p(const c128 *__restrict__ Ppart, int nsplit, int count, c128 *__restrict__ P)
-{
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= count) return;
-    double sr = 0.0, si = 0.0;
-    for (int s = 0; s < nsplit; ++s) {
-        const double2 v = ldg_c128(Ppart + (size_t)s * count + i);
-        sr += v.x; si += v.y;
-    }
-    P[i] = c128{sr, si};
-}
-
-// Q[i][n] = sum_{j in block(i)} D[blk][i%db][j%db] P[j][n];  rows >= nproj are written as zero.
-__global__ void k_dmul(const double *__restrict__ D, int db, int nproj, int nproj_pad, int nbp,
-                       const c128 *__restrict__ P, c128 *__restrict__ Q)
-{
-    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= nproj_pad * nbp) return;
-    const int i = idx / nbp, n = idx % nbp;
-    double sr = 0.0, si = 0.0;
-    if (i < nproj) {
-        const int blk = i / db, ii = i % db;
-        const double *d = D + ((size_t)blk * db + ii) * db;
-        for (int j = 0; j < db; ++j) {
-            const double2 v = ldg_c128(P + (size_t)(blk * db + j) * nbp + n);
-            sr += d[j] * v.x; si += d[j] * v.y;
-        }
-    }
-    Q[idx] = c128{sr, si};
-}
-
-// out[n][g] += sum_i beta[i][g] Q[i][n]
-template <int MT, int NT, int WARPS>
-__global__ void __launch_bounds__(WARPS * 32)
-k_proj2_direct(const c128 *__restrict__ beta, int ldb, const c128 *__restrict__ Q, int nbp, int nproj_pad,
-               int ng, int nb, int band0, c128 *__restrict__ out)
-{
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int r = lane >> 2, c = lane & 3;
-    const int g0 = (blockIdx.x * WARPS + warp) * 8 * MT;
-    if (g0 >= ng) return;
-    double cre[MT][NT][2], cim[MT][NT][2];
-#pragma unroll
-    for (int i = 0; i < MT; ++i)
-#pragma unroll
-        for (int j = 0; j < NT; ++j) { cre[i][j][0] = cre[i][j][1] = cim[i][j][0] = cim[i][j][1] = 0.0; }
-    const c128 *bp = beta + (size_t)c * ldb + g0 + r;          // ldb >= roundup(ng, 8*MT*WARPS): in bounds
-    const c128 *qp = Q + (size_t)c * nbp + r;
-#pragma unroll 2
-    for (int k = 0; k < nproj_pad; k += 4) {
-        double2 a[MT], b[NT];
-#pragma unroll
-        for (int i = 0; i < MT; ++i) a[i] = ldg_c128(bp + (size_t)k * ldb + i * 8);
-#pragma unroll
-        for (int j = 0; j < NT; ++j) b[j] = ldg_c128(qp + (size_t)k * nbp + j * 8);
-#pragma unroll
-        for (int i = 0; i < MT; ++i)
-#pragma unroll
-            for (int j = 0; j < NT; ++j) {
-                // a * b = (ar br - ai bi) + i (ar bi + ai br)
-                dmma884(cre[i][j][0], cre[i][j][1], a[i].x, b[j].x);
-                dmma884(cre[i][j][0], cre[i][j][1], a[i].y, -b[j].y);
-                dmma884(cim[i][j][0], cim[i][j][1], a[i].x, b[j].y);
-                dmma884(cim[i][j][0], cim[i][j][1], a[i].y, b[j].x);
-            }
-    }
-#pragma unroll
-    for (int i = 0; i < MT; ++i) {
-        const int g = g0 + i * 8 + r;
-        if (g >= ng) continue;
-#pragma unroll
-        for (int j = 0; j < NT; ++j)
-#pragma unroll
-            for (int e = 0; e < 2; ++e) {
-                const int n = band0 + j * 8 + 2 * c + e;
-                if (n < nb) {
-                    c128 *o = out + (size_t)n * ng + g;
-                    c128 v = *o;
-                    v.x += cre[i][j][e]; v.y += cim[i][j][e];
-                    *o = v;
-                }
-            }
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// v2 kernels: shared-memory ring fed by cp.async.bulk (TMA engine, mbarrier complete_tx), one producer
+// Shared-memory ring fed by cp.async.bulk (TMA engine, mbarrier complete_tx), one producer
 // warp + consumer warps issuing DMMA; complex products by the 3M scheme (three real products:
 //   T1 = ar*br, T2 = ai*bi, T3 = (ar -/+ ai)*(br + bi)), which cuts the DMMA count by a quarter.
 // beta is kept in two library-owned tiled copies (qm_set_nonlocal "may re-lay-out"):
@@ -372,93 +230,138 @@ __global__ void k_dmul_tiles(const double *__restrict__ D, int db, int nproj, in
 }
 
 // GEMM 2:  out[band0+n][g] += sum_i beta[i][g] Q[i][n]
+// Stream-K: the (G tile, projector chunk) stages are flattened and cut into equal contiguous ranges, one
+// per CTA (two CTAs per SM), so every SM gets the same amount of work whatever N_G is.  A CTA whose range
+// starts or ends inside a G tile writes that tile's partial sum to a side buffer; k_proj2_fixup adds the
+// partials of each split tile to `out` in a fixed order (deterministic, no atomics).
+constexpr int P2_PART = P_NB * P2_G;      // c128 per partial tile
 __global__ void __launch_bounds__((P2_CW + 1) * 32, 2)
-k_proj2_pipe(const c128 *__restrict__ beta2, int nic, const double *__restrict__ qt, int ng, int nb, int band0,
-             c128 *__restrict__ out)
+k_proj2_sk(const c128 *__restrict__ beta2, int nic, int ngt, const double *__restrict__ qt, int ng, int nb, int band0,
+           c128 *__restrict__ out, c128 *__restrict__ part, int *__restrict__ pdesc)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + P2_ST * P2_STAGE_BYTES);
     uint64_t *empty = full + P2_ST;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int gt = blockIdx.x;
+    const long long total = (long long)ngt * nic;
+    const int s_begin = (int)(total * blockIdx.x / gridDim.x), s_end = (int)(total * (blockIdx.x + 1) / gridDim.x);
     if (threadIdx.x == 0) {
         for (int s = 0; s < P2_ST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], P2_CW); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        pdesc[2 * blockIdx.x] = -1; pdesc[2 * blockIdx.x + 1] = -1;
     }
     __syncthreads();
     if (warp == P2_CW) {
         if (lane == 0) {
-            for (int it = 0; it < nic; ++it) {
-                const int s = it % P2_ST;
+            for (int st = s_begin; st < s_end; ++st) {
+                const int it = st - s_begin, s = it % P2_ST;
                 if (it >= P2_ST) mbar_wait(&empty[s], ((it / P2_ST) - 1) & 1);
                 unsigned char *stage = smem + s * P2_STAGE_BYTES;
                 mbar_expect_tx(&full[s], P2_STAGE_BYTES);
-                bulk_g2s(stage, beta2 + ((size_t)gt * nic + it) * (P2_KS * P2_G), P2_BETA_BYTES, &full[s]);
-                bulk_g2s(stage + P2_BETA_BYTES, qt + (size_t)it * P2_Q_DOUBLES, P2_Q_BYTES, &full[s]);
+                bulk_g2s(stage, beta2 + (size_t)st * (P2_KS * P2_G), P2_BETA_BYTES, &full[s]);    // layout [gt][ic] == st
+                bulk_g2s(stage + P2_BETA_BYTES, qt + (size_t)(st % nic) * P2_Q_DOUBLES, P2_Q_BYTES, &full[s]);
             }
         }
     } else {
         const int r8 = lane >> 2, c = lane & 3;
-        double t1[2][2][2], t2[2][2][2], t3[2][2][2];
-#pragma unroll
-        for (int i = 0; i < 2; ++i)
-#pragma unroll
-            for (int j = 0; j < 2; ++j)
-#pragma unroll
-                for (int e = 0; e < 2; ++e) { t1[i][j][e] = 0.0; t2[i][j][e] = 0.0; t3[i][j][e] = 0.0; }
         int aoff[2], qoff[2];
 #pragma unroll
         for (int i = 0; i < 2; ++i) aoff[i] = (c * P2_G + 8 * (2 * warp + i) + (r8 ^ (2 * c))) * 16;
 #pragma unroll
         for (int j = 0; j < 2; ++j) qoff[j] = P2_BETA_BYTES + (c * P2_Q_PITCH + 8 * j + r8) * 8;
-        for (int it = 0; it < nic; ++it) {
-            const int s = it % P2_ST;
-            mbar_wait(&full[s], (it / P2_ST) & 1);
-            const unsigned char *stage = smem + s * P2_STAGE_BYTES;
+        int st = s_begin;
+        bool first_seg = true;
+        while (st < s_end) {
+            const int gt = st / nic, ic0 = st % nic;
+            const int ic1 = min(nic, ic0 + (s_end - st));
+            double t1[2][2][2], t2[2][2][2], t3[2][2][2];
 #pragma unroll
-            for (int kk = 0; kk < P2_KS / 4; ++kk) {
-                double2 a[2];
-                double qr[2], qi[2], qs[2];
+            for (int i = 0; i < 2; ++i)
 #pragma unroll
-                for (int i = 0; i < 2; ++i) a[i] = lds_c128(stage, aoff[i] + 4 * kk * P2_G * 16);
+                for (int j = 0; j < 2; ++j)
 #pragma unroll
-                for (int j = 0; j < 2; ++j) {
-                    const double *q = reinterpret_cast<const double *>(stage + qoff[j] + 4 * kk * P2_Q_PITCH * 8);
-                    qr[j] = q[0]; qi[j] = q[P2_KS * P2_Q_PITCH]; qs[j] = q[2 * P2_KS * P2_Q_PITCH];
-                }
+                    for (int e = 0; e < 2; ++e) { t1[i][j][e] = 0.0; t2[i][j][e] = 0.0; t3[i][j][e] = 0.0; }
+            for (int ic = ic0; ic < ic1; ++ic, ++st) {
+                const int it = st - s_begin, s = it % P2_ST;
+                mbar_wait(&full[s], (it / P2_ST) & 1);
+                const unsigned char *stage = smem + s * P2_STAGE_BYTES;
 #pragma unroll
-                for (int i = 0; i < 2; ++i) {
-                    const double as = a[i].x + a[i].y;
+                for (int kk = 0; kk < P2_KS / 4; ++kk) {
+                    double2 a[2];
+                    double qr[2], qi[2], qs[2];
+#pragma unroll
+                    for (int i = 0; i < 2; ++i) a[i] = lds_c128(stage, aoff[i] + 4 * kk * P2_G * 16);
 #pragma unroll
                     for (int j = 0; j < 2; ++j) {
-                        dmma884(t1[i][j][0], t1[i][j][1], a[i].x, qr[j]);
-                        dmma884(t2[i][j][0], t2[i][j][1], a[i].y, qi[j]);
-                        dmma884(t3[i][j][0], t3[i][j][1], as, qs[j]);
+                        const double *q = reinterpret_cast<const double *>(stage + qoff[j] + 4 * kk * P2_Q_PITCH * 8);
+                        qr[j] = q[0]; qi[j] = q[P2_KS * P2_Q_PITCH]; qs[j] = q[2 * P2_KS * P2_Q_PITCH];
+                    }
+#pragma unroll
+                    for (int i = 0; i < 2; ++i) {
+                        const double as = a[i].x + a[i].y;
+#pragma unroll
+                        for (int j = 0; j < 2; ++j) {
+                            dmma884(t1[i][j][0], t1[i][j][1], a[i].x, qr[j]);
+                            dmma884(t2[i][j][0], t2[i][j][1], a[i].y, qi[j]);
+                            dmma884(t3[i][j][0], t3[i][j][1], as, qs[j]);
+                        }
                     }
                 }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[s]);
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[s]);
-        }
-        // a q:  re = T1 - T2,  im = T3 - T1 - T2
+            // a q:  re = T1 - T2,  im = T3 - T1 - T2
+            const bool whole = (ic0 == 0 && ic1 == nic);
+            c128 *pslot = nullptr;
+            if (!whole) {
+                const int slot = 2 * blockIdx.x + (first_seg ? 0 : 1);
+                pslot = part + (size_t)slot * P2_PART;
+                if (warp == 0 && lane == 0) pdesc[slot] = gt;
+            }
 #pragma unroll
-        for (int i = 0; i < 2; ++i) {
-            const int g = gt * P2_G + 8 * (2 * warp + i) + r8;
-            if (g >= ng) continue;
+            for (int i = 0; i < 2; ++i) {
+                const int gl = 8 * (2 * warp + i) + r8, g = gt * P2_G + gl;
 #pragma unroll
-            for (int j = 0; j < 2; ++j)
+                for (int j = 0; j < 2; ++j)
 #pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const int n = band0 + j * 8 + 2 * c + e;
-                    if (n < nb) {
-                        c128 *o = out + (size_t)n * ng + g;
-                        c128 v = *o;
-                        v.x += t1[i][j][e] - t2[i][j][e];
-                        v.y += t3[i][j][e] - t1[i][j][e] - t2[i][j][e];
-                        *o = v;
+                    for (int e = 0; e < 2; ++e) {
+                        const int nl = j * 8 + 2 * c + e, n = band0 + nl;
+                        const c128 v = c128{t1[i][j][e] - t2[i][j][e], t3[i][j][e] - t1[i][j][e] - t2[i][j][e]};
+                        if (whole) {
+                            if (g < ng && n < nb) {
+                                c128 *o = out + (size_t)n * ng + g;
+                                *o = *o + v;
+                            }
+                        } else {
+                            pslot[nl * P2_G + gl] = v;
+                        }
                     }
-                }
+            }
+            first_seg = false;
         }
+    }
+}
+
+// One block per partial slot; the first slot of a split tile sums all that tile's partials into `out`.
+__global__ void k_proj2_fixup(const c128 *__restrict__ part, const int *__restrict__ pdesc, int nslots, int ng, int nb,
+                              int band0, c128 *__restrict__ out)
+{
+    const int b = blockIdx.x;
+    const int gt = pdesc[b];
+    if (gt < 0) return;
+    for (int j = b - 1; j >= 0 && j >= b - 4; --j) if (pdesc[j] == gt) return;     // not the first slot of this tile
+    for (int e = threadIdx.x; e < P2_PART; e += blockDim.x) {
+        const int nl = e / P2_G, gl = e % P2_G;
+        const int g = gt * P2_G + gl, n = band0 + nl;
+        if (g >= ng || n >= nb) continue;
+        double sr = 0.0, si = 0.0;
+        for (int j = b; j < nslots; ++j) {
+            const int d = pdesc[j];
+            if (d == gt) { const double2 v = ldg_c128(part + (size_t)j * P2_PART + e); sr += v.x; si += v.y; }
+            else if (d >= 0) break;
+        }
+        c128 *o = out + (size_t)n * ng + g;
+        c128 v = *o; v.x += sr; v.y += si; *o = v;
     }
 }
 

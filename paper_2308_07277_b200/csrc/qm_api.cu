@@ -131,10 +131,12 @@ struct qm_gspace {
     bool v_set = false;
     DevBuf<c128> d_W, d_Ppart, d_P;
     DevBuf<double> d_qt;
+    DevBuf<c128> d_part;
+    DevBuf<int> d_pdesc;
     unsigned long long launches = 0;
     int sm_count = 148;
     int max_smem = 0;
-    int plane_stagger_ns = 0;
+    int plane_stagger_ns = 100;     // de-phasing delay between the plane kernel's groups (QM_PLANE_STAGGER_NS)
     ~qm_gspace() { for (auto *k : kpts) delete k; }
 };
 
@@ -160,7 +162,7 @@ int build_kpoint(qm_gspace *g, KPoint *kp) {
 constexpr int PLANE_GROUP = 64;
 size_t plane_smem(const qm_gspace *g, const KPoint *kp, int ngroups) {
     const QmAxis &ax = g->ax[0];
-    const size_t sl = (size_t)(ax.len | 1);
+    const size_t sl = (size_t)qm_scratch_pitch(ax.len, std::max(ax.r1, ax.r2));
     const int tpg = PLANE_GROUP / std::max(ax.r1, ax.r2);
     return ((size_t)kp->nx * kp->rowpitch + (size_t)ngroups * tpg * sl) * sizeof(c128)
            + (size_t)kp->nx * sizeof(int4) + 16;
@@ -290,7 +292,7 @@ int run_nonlocal(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb
     static bool attr = false;
     if (!attr) {
         CU_TRY(cudaFuncSetAttribute(k_proj1_pipe, cudaFuncAttributeMaxDynamicSharedMemorySize, P1_SMEM));
-        CU_TRY(cudaFuncSetAttribute(k_proj2_pipe, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM));
+        CU_TRY(cudaFuncSetAttribute(k_proj2_sk, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM));
         attr = true;
     }
     const int nsplit = std::max(1, std::min(kp->nkc, g->sm_count / kp->nmblk));
@@ -299,6 +301,10 @@ int run_nonlocal(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb
     CU_TRY(g->d_Ppart.resize(pcount * nsplit));
     CU_TRY(g->d_P.resize(pcount));
     CU_TRY(g->d_qt.resize((size_t)kp->nic * P2_Q_DOUBLES));
+    const long long stages2 = (long long)kp->ngt * kp->nic;
+    const int ncta2 = (int)std::min<long long>(stages2, 2LL * g->sm_count);
+    CU_TRY(g->d_part.resize((size_t)2 * ncta2 * P2_PART));
+    CU_TRY(g->d_pdesc.resize((size_t)2 * ncta2));
     for (int band0 = 0; band0 < nb; band0 += P_NB) {
         g->prof.begin(QM_K_PROJ1, st);
         k_proj1_pipe<<<dim3(kp->nmblk, nsplit), (P1_CW + 1) * 32, P1_SMEM, st>>>(
@@ -313,10 +319,11 @@ int run_nonlocal(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb
                                                           g->d_qt.p);
         g->prof.end(st);
         g->prof.begin(QM_K_PROJ2, st);
-        k_proj2_pipe<<<kp->ngt, (P2_CW + 1) * 32, P2_SMEM, st>>>(kp->d_beta2.p, kp->nic, g->d_qt.p, kp->ng, nb, band0,
-                                                                 out);
+        k_proj2_sk<<<ncta2, (P2_CW + 1) * 32, P2_SMEM, st>>>(kp->d_beta2.p, kp->nic, kp->ngt, g->d_qt.p, kp->ng, nb,
+                                                             band0, out, g->d_part.p, g->d_pdesc.p);
+        k_proj2_fixup<<<2 * ncta2, 256, 0, st>>>(g->d_part.p, g->d_pdesc.p, 2 * ncta2, kp->ng, nb, band0, out);
         g->prof.end(st);
-        g->launches += 4;
+        g->launches += 5;
     }
     CU_TRY(cudaGetLastError());
     return QM_OK;
