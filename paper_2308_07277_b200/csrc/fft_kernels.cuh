@@ -114,6 +114,9 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
 // synchronises with itself (named barrier), so the groups hide each other's latencies.  CTA-wide
 // barriers remain only between the four phases (load | y backward | x round trip | y forward | store).
 constexpr int QM_GROUP = 64;
+#ifndef QM_PLANE_MAX_THREADS
+#define QM_PLANE_MAX_THREADS 384
+#endif
 // Scratch lines of neighbouring teams: with 12-thread teams a quarter-warp straddles two teams as 4+4
 // threads, and their unit-stride 16-byte accesses are conflict free iff the pitch is 4 (mod 8); else odd.
 __host__ __device__ constexpr int qm_scratch_pitch(int len, int tt) { return tt == 12 ? len + ((12 - len % 8) % 8) : (len | 1); }
@@ -122,7 +125,7 @@ __device__ __forceinline__ void group_barrier(int grp) {
 }
 
 template <class C, int MODE>
-__global__ void __launch_bounds__(384)
+__global__ void __launch_bounds__(QM_PLANE_MAX_THREADS)
 k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ box, int ngroups, double scale,
         int stagger_ns)
 {

@@ -174,7 +174,7 @@ int plane_groups(const qm_gspace *g, const KPoint *kp) {
     const QmAxis &ax = g->ax[0];
     const int tpg = PLANE_GROUP / std::max(ax.r1, ax.r2);
     const int nchunks = (ax.n + tpg - 1) / tpg;
-    int gmax = std::min(384 / PLANE_GROUP, nchunks);
+    int gmax = std::min(QM_PLANE_MAX_THREADS / PLANE_GROUP, nchunks);
     while (gmax > 1 && plane_smem(g, kp, gmax) > (size_t)g->max_smem) --gmax;
     const int rounds = (nchunks + gmax - 1) / gmax;
     int best = gmax;
@@ -231,10 +231,14 @@ template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *bo
 }
 
 // dispatch on FFT length ---------------------------------------------------------------------
+#ifdef QM_DEV_SIZES      /* developer builds: only the lengths of the five BASELINE.json configs (fast compile) */
+#define QM_FOR_SIZES(X) X(24, 4, 6) X(32, 4, 8) X(48, 6, 8) X(96, 8, 12) X(144, 12, 12)
+#else
 #define QM_FOR_SIZES(X)                                                                              \
     X(8, 2, 4) X(12, 3, 4) X(16, 4, 4) X(18, 3, 6) X(20, 4, 5) X(24, 4, 6) X(30, 5, 6) X(32, 4, 8)   \
     X(36, 6, 6) X(40, 5, 8) X(48, 6, 8) X(60, 6, 10) X(64, 8, 8) X(72, 8, 9) X(80, 8, 10)            \
     X(96, 8, 12) X(100, 10, 10) X(108, 9, 12) X(120, 10, 12) X(128, 8, 16) X(144, 12, 12)
+#endif
 
 int dispatch_zinv(qm_gspace *g, KPoint *kp, const c128 *psi, int nb, cudaStream_t st) {
     switch (g->grid[2]) {
