@@ -6,145 +6,147 @@
 #pragma once
 #include <cuda_runtime.h>
 #include "fft_phases.cuh"
+#include "async_copy.cuh"
 #include "qm_plan.h"
 
+// z kernels.  A CTA owns tiles of QM_ZT adjacent sticks of one band (looping over tiles gridDim.x apart, so
+// the per-thread twiddle row is loaded once).  Both kernels are global -> registers -> first radix pass ->
+// shared memory -> second radix pass -> registers -> global: one shared-memory round trip, no zero fill, no
+// table-driven scatter (the G of a stick are two contiguous index runs, Pruned).  Thread mapping is
+// (stick, u) with u fastest where the sphere side is touched (contiguous psi runs) and (u, stick) with the
+// stick fastest where the stick planes W[p][S] are touched (contiguous 256-byte segments).
+constexpr int QM_ZT = 16;
+template <class C> __host__ __device__ constexpr int qm_z_threads() { return QM_ZT * C::TT; }
+
 template <class C>
-__global__ void __launch_bounds__(256)
-k_zinv(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ psi,
-       c128 *__restrict__ W, int TS)
+__global__ void __launch_bounds__(QM_ZT * C::TT, 3)
+k_zinv(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ psi, c128 *__restrict__ W, int ntiles)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int LP = C::L | 1;
     c128 *lines = reinterpret_cast<c128 *>(smem_raw);
-    const int tid = threadIdx.x, nthr = blockDim.x;
-    const int s0 = blockIdx.x * TS;
-    const int ns = min(TS, kp.nsticks - s0);
-    const int band = blockIdx.y;
-    const int S = kp.nsticks;
-    const int t = tid / C::TT, u = tid % C::TT;
-    c128 *tw_s = lines + TS * LP;
-    const TwTable twa{tw_s, u};
-
-    for (int i = tid; i < C::N; i += nthr) tw_s[i] = tw[i];
-    for (int i = tid; i < TS * LP; i += nthr) lines[i] = c128{0.0, 0.0};
-    __syncthreads();
-    const int g0 = kp.stick_off[s0], g1 = kp.stick_off[s0 + ns];
+    const int tid = threadIdx.x;
+    const int S = kp.nsticks, band = blockIdx.y;
+    const int t1 = tid / C::TT, u1 = tid % C::TT;      // pass 1: u fastest
+    const int t2 = tid % QM_ZT, u2 = tid / QM_ZT;      // pass 2: stick fastest
+    TwRow<C::R1> twa;
+    load_twrow(twa, tw, u1, C::R2);
     const c128 *psib = psi + (size_t)band * kp.ng;
-    for (int g = g0 + tid; g < g1; g += nthr)
-        lines[(kp.g_stick[g] - s0) * LP + kp.g_zpos[g]] = psib[g];
-    __syncthreads();
-    if (t < ns) lineA_step1<C>(lines + t * LP, u, twa);
-    __syncthreads();
-    if (t < ns) lineA_step2<C>(lines + t * LP, u);
-    __syncthreads();
     c128 *Wb = W + (size_t)band * C::N * S;
-    for (int i = tid; i < C::N * TS; i += nthr) {
-        const int p = i / TS, tt = i % TS;
-        if (tt < ns) Wb[(size_t)p * S + s0 + tt] = lines[tt * LP + C::pos(p)];
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int s0 = tile * QM_ZT;
+        const int ns = min(QM_ZT, S - s0);
+        if (t1 < ns) {
+            const int4 q = kp.stick_info[s0 + t1];
+            const Pruned pr = make_pruned<C>((int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, u1, 1);
+            prunedA_step1<C>(SpaceGlobal{}, psib + q.z, C::R2, pr, lines + t1 * LP, u1, twa);
+        }
+        __syncthreads();
+        if (t2 < ns) zinv_step2_store<C>(lines + t2 * LP, Wb + s0 + t2, S, u2);
+        __syncthreads();
     }
 }
 
 template <class C>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(QM_ZT * C::TT, 3)
 k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
-       const c128 *__restrict__ psi_in, c128 *__restrict__ out, int TS, int kinetic)
+       const c128 *__restrict__ psi_in, c128 *__restrict__ out, int ntiles, int kinetic)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int LP = C::L | 1;
-    constexpr int GPT = 4;            // gather elements per thread kept in registers across the FFT
     c128 *lines = reinterpret_cast<c128 *>(smem_raw);
-    const int tid = threadIdx.x, nthr = blockDim.x;
-    const int s0 = blockIdx.x * TS;
-    const int ns = min(TS, kp.nsticks - s0);
-    const int band = blockIdx.y;
-    const int S = kp.nsticks;
-    const int t = tid / C::TT, u = tid % C::TT;
-    c128 *tw_s = lines + TS * LP;
-    const TwTable twb{tw_s, u};
-    for (int i = tid; i < C::N; i += nthr) tw_s[i] = tw[i];
-
+    const int tid = threadIdx.x;
+    const int S = kp.nsticks, band = blockIdx.y;
+    const int t1 = tid / C::TT, u1 = tid % C::TT;      // pass 2 (gather side): u fastest
+    const int t2 = tid % QM_ZT, u2 = tid / QM_ZT;      // pass 1 (stick-plane side): stick fastest
+    TwRow<C::R2> twb;
+    load_twrow(twb, tw, u2, C::R1);
     const c128 *Wb = W + (size_t)band * C::N * S;
-    for (int i = tid; i < C::N * TS; i += nthr) {
-        const int p = i / TS, tt = i % TS;
-        if (tt < ns) lines[tt * LP + C::pos(p)] = Wb[(size_t)p * S + s0 + tt];
-    }
-    // the gather's own inputs (positions, 1/2|k+G|^2 psi_in) are fetched now, behind the transform
-    const int g0 = kp.stick_off[s0], g1 = kp.stick_off[s0 + ns];
     const size_t boff = (size_t)band * kp.ng;
-    int gpos[GPT];
-    c128 kin[GPT];
-#pragma unroll
-    for (int j = 0; j < GPT; ++j) {
-        const int g = g0 + tid + j * nthr;
-        gpos[j] = -1; kin[j] = c128{0.0, 0.0};
-        if (g < g1) {
-            gpos[j] = (kp.g_stick[g] - s0) * LP + kp.g_zpos[g];
-            if (kinetic) {
-                const c128 x = psi_in[boff + g];
-                const double h = 0.5 * kp.g2[g];
-                kin[j] = c128{h * x.x, h * x.y};
-            }
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int s0 = tile * QM_ZT;
+        const int ns = min(QM_ZT, S - s0);
+        if (t2 < ns) zfwd_step1_load<C>(Wb + s0 + t2, S, lines + t2 * LP, u2, twb);
+        __syncthreads();
+        if (t1 < ns) {
+            const int4 q = kp.stick_info[s0 + t1];
+            const Pruned pr = make_pruned<C>((int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, u1, 1);
+            zfwd_step2_gather<C>(lines + t1 * LP, out + boff + q.z, kinetic ? psi_in + boff + q.z : nullptr, kp.g2 + q.z, pr, u1,
+                                 kinetic != 0);
         }
-    }
-    __syncthreads();
-    if (t < ns) lineB_step1<C>(lines + t * LP, u, twb);
-    __syncthreads();
-    if (t < ns) lineB_step2<C>(lines + t * LP, u);
-    __syncthreads();
-#pragma unroll
-    for (int j = 0; j < GPT; ++j) {
-        const int g = g0 + tid + j * nthr;
-        if (g < g1) out[boff + g] = lines[gpos[j]] + kin[j];
-    }
-    for (int g = g0 + tid + GPT * nthr; g < g1; g += nthr) {     // sticks longer than the register budget
-        c128 v = lines[(kp.g_stick[g] - s0) * LP + kp.g_zpos[g]];
-        if (kinetic) {
-            const c128 x = psi_in[boff + g];
-            const double h = 0.5 * kp.g2[g];
-            v.x += h * x.x; v.y += h * x.y;
-        }
-        out[boff + g] = v;
+        __syncthreads();
     }
 }
 
 // MODE 0 apply, 1 g2r (write natural-order box), 2 r2g (read natural-order box)
 //
-// One CTA per (band, z-plane).  The CTA is split into independent groups of 64 threads (two warps =
-// 64/TT teams of TT threads, one team per line); a group walks its own rows / columns and only
-// synchronises with itself (named barrier), so the groups hide each other's latencies.  CTA-wide
-// barriers remain only between the four phases (load | y backward | x round trip | y forward | store).
-constexpr int QM_GROUP = 64;
+// One CTA per (band, z-plane).  The CTA is split into independent groups of G threads (G/TT teams of TT
+// threads, one team per line); a group walks its own rows / columns and only synchronises with itself
+// (named barrier, or __syncwarp when G == 32), so the groups hide each other's latencies.  CTA-wide
+// barriers remain only between the phases (y backward | x round trip | y forward).
+// All pruned-access masks and offsets are hoisted: per kernel for the x direction (Pruned px), per row for
+// the y direction; the accesses themselves are predicated 16-byte loads/stores at base + immediate.
 #ifndef QM_PLANE_MAX_THREADS
 #define QM_PLANE_MAX_THREADS 384
 #endif
+#ifndef QM_PLANE_GROUP
+#define QM_PLANE_GROUP 96
+#endif
+constexpr int QM_GROUP = QM_PLANE_GROUP;
 // Scratch lines of neighbouring teams: with 12-thread teams a quarter-warp straddles two teams as 4+4
 // threads, and their unit-stride 16-byte accesses are conflict free iff the pitch is 4 (mod 8); else odd.
 __host__ __device__ constexpr int qm_scratch_pitch(int len, int tt) { return tt == 12 ? len + ((12 - len % 8) % 8) : (len | 1); }
-__device__ __forceinline__ void group_barrier(int grp) {
-    asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "r"(QM_GROUP) : "memory");
+// Which line of its group's chunk a team works on.  With 12-thread teams in 96-thread groups the quarter-warps
+// that straddle two teams hold teams (0,1), (2,3), (4,5), (6,7): giving each pair lines 4 apart makes their
+// 16-byte accesses to odd-pitch plane rows (pitch = 5 mod 8) and to columns 4 apart fall in disjoint banks.
+template <int TT, int TPG> __host__ __device__ constexpr int qm_team_slot(int team) {
+    return (TT == 12 && TPG == 8) ? ((team >> 1) + 4 * (team & 1)) : team;
 }
+template <int G> __device__ __forceinline__ void group_barrier(int grp) {
+#ifdef QM_ABLATE_GBAR     /* timing experiment only: results are wrong */
+    return;
+#endif
+    if constexpr (G == 32) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "r"(G) : "memory");
+}
+
+// Shared-memory carve-up of the plane kernel (bytes): plane array A | scratch lines, which double as the two
+// stick-plane staging buffers outside the x phase | row table | mbarrier.
+__host__ __device__ constexpr size_t qm_stage_elems(int S) { return ((size_t)S + 7) & ~(size_t)7; }   // 128-byte multiple
 
 template <class C, int MODE>
 __global__ void __launch_bounds__(QM_PLANE_MAX_THREADS)
 k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ box, int ngroups, double scale,
-        int stagger_ns)
+        int stagger_ns, int nplanes, int scr_elems)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr int G = QM_GROUP;
     constexpr int SL = qm_scratch_pitch(C::L, C::TT);    // scratch line pitch
-    constexpr int TPG = QM_GROUP / C::TT;                // teams (lines) per group
-    const int X = kp.nx, rowpitch = kp.rowpitch, S = kp.nsticks;
+    constexpr int TPG = G / C::TT;                       // teams (lines) per group
+    constexpr int RP = C::L | 1;                         // plane row pitch (== kp.rowpitch, host checks)
+    const int X = kp.nx, S = kp.nsticks;
     c128 *A = reinterpret_cast<c128 *>(smem_raw);
-    c128 *scr = A + (size_t)X * rowpitch;
-    int4 *rowinfo_s = reinterpret_cast<int4 *>(scr + (size_t)ngroups * TPG * SL);
-    const XRows xr{kp.x_iv.x, kp.x_iv.y, kp.x_iv.z, kp.x_iv.w};
+    c128 *scr = A + (((size_t)X * RP + 7) & ~(size_t)7);
+    c128 *stage_in = scr, *stage_out = scr + qm_stage_elems(S);      // valid outside the x phase only
+    int4 *rowinfo_s = reinterpret_cast<int4 *>(scr + scr_elems);
+    uint64_t *wbar = reinterpret_cast<uint64_t *>(rowinfo_s + X);
     const int tid = threadIdx.x, nthr = blockDim.x;
-    const int grp = tid / QM_GROUP, gl = tid % QM_GROUP;
+    const int grp = tid / G, gl = tid % G;
     const int team = gl / C::TT, u = gl % C::TT;
     const bool team_ok = team < TPG;
-    const int p = blockIdx.x, band = blockIdx.y;
+    const int slot = qm_team_slot<C::TT, TPG>(team);     // line of the group's chunk this team works on
     const int n3 = gd.ax[2].n;
-    c128 *Wp = W + ((size_t)band * n3 + p) * S;
+    const uint32_t wbytes = (uint32_t)S * 16u;
+    const Pruned px = make_pruned<C>(kp.x_iv.x, kp.x_iv.y, kp.x_iv.z, kp.x_iv.w, u, RP);
 
+    if (tid == 0) {
+        mbar_init(wbar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        if constexpr (MODE != 2) {       // stick plane of the first (band, z-plane): one bulk copy, in flight during set-up
+            mbar_expect_tx(wbar, wbytes);
+            bulk_g2s(stage_in, W + (size_t)blockIdx.x * S, wbytes, wbar);
+        }
+    }
     // per-thread twiddle rows (u is fixed for the whole kernel)
     TwRow<C::R1> twa;
     load_twrow(twa, gd.tw[0], u, C::R2);
@@ -156,67 +158,95 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
 
     for (int i = tid; i < X; i += nthr) rowinfo_s[i] = kp.row_info[i];
     __syncthreads();
-    auto row_info = [&](int r) {
+    auto row_pruned = [&](int r, int &sbase) {
         const int4 q = rowinfo_s[r];
-        return RowInfo{(int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, q.z};
+        sbase = q.z;
+        return make_pruned<C>((int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, u, 1);
     };
-    if constexpr (MODE != 2) {
-        for (int rc = grp; rc * TPG < X; rc += ngroups) {
-            const int r = rc * TPG + team;
-            const bool ok = team_ok && r < X;
-            if (ok) lineA_step1_gin<C>(A + r * rowpitch, Wp, row_info(r), u, twa);
-            group_barrier(grp);
-            if (ok) lineA_step2<C>(A + r * rowpitch, u);
+    // persistent loop over (band, z-plane) pairs: plane pl = band * n3 + p, its sticks are W[pl][0..S)
+    for (int pl = blockIdx.x, it = 0; pl < nplanes; pl += gridDim.x, ++it) {
+        const int band = pl / n3, p = pl - band * n3;
+        c128 *Wp = W + (size_t)pl * S;
+        if constexpr (MODE != 2) {
+            mbar_wait(wbar, (uint32_t)(it & 1));
+            for (int r = grp * TPG + slot; r - slot < X; r += ngroups * TPG) {
+                const bool ok = team_ok && r < X;
+                if (ok) {
+                    int sbase;
+                    const Pruned pr = row_pruned(r, sbase);
+                    prunedA_step1<C>(SpaceShared{}, stage_in + sbase, C::R2, pr, A + r * RP, u, twa);
+                }
+                group_barrier<G>(grp);
+                if (ok) lineA_step2<C>(A + r * RP, u);
+            }
+        }
+        if (tid == 0) bulk_wait_read0();      // the previous plane's bulk store has read stage_out: scratch is free
+        __syncthreads();
+        {
+            const int z = (p / gd.ax[2].r2) + gd.ax[2].r1 * (p % gd.ax[2].r2);
+            c128 *myscr = scr + (size_t)(grp * TPG + team) * SL;
+            const double *vplane = gd.vt + (size_t)p * C::N * VLayout<C>::COL;
+            VRow<C::R2> vr;
+            // De-phase the groups: they all do identical load -> FP64 -> store bursts, and when they run in
+            // lock step the shared-memory pipe and the FP64 pipe are used alternately instead of together.
+            if (stagger_ns > 0) __nanosleep((unsigned)(grp * stagger_ns));
+            const int col0 = grp * TPG + slot;
+            if constexpr (MODE == 0) {       // V of the first column: in flight while step 1 runs
+                if (team_ok && col0 < C::N) load_vrow<C>(vr, vplane + (size_t)col0 * VLayout<C>::COL, u);
+            }
+            for (int col = col0; col - slot < C::N; col += ngroups * TPG) {
+                const bool ok = team_ok && col < C::N;
+                c128 *Acol = A + C::pos(col);
+                if constexpr (MODE != 2) {
+                    if (ok) prunedA_step1<C>(SpaceShared{}, Acol, C::R2 * RP, px, myscr, u, twa);
+                    group_barrier<G>(grp);
+                }
+                if (ok) {
+                    const int y = (col / C::R2) + C::R1 * (col % C::R2);
+                    c128 *bx = nullptr;
+                    if constexpr (MODE != 0) bx = box + (size_t)band * C::N * C::N * n3 + (size_t)y * n3 + z;
+                    xcol_step2<C, MODE>(myscr, u, twb, vr, bx, (long)C::N * n3, scale);
+                }
+                if constexpr (MODE == 0) {   // prefetch V of this team's next column behind steps 3 and 1
+                    const int ncol = col + ngroups * TPG;
+                    if (team_ok && ncol < C::N) load_vrow<C>(vr, vplane + (size_t)ncol * VLayout<C>::COL, u);
+                }
+                group_barrier<G>(grp);
+                if constexpr (MODE != 1) {
+                    // no barrier after step 3: the scratch column a thread reads here is exactly the one it
+                    // overwrites in the next iteration's step 1 (MODE 2 has no step 1 and writes rows: barrier).
+                    if (ok) prunedB_step2<C>(SpaceShared{}, myscr, Acol, C::R2 * RP, px, u);
+                    if constexpr (MODE == 2) group_barrier<G>(grp);
+                }
+            }
+        }
+        fence_async_smem();                   // scratch was written through the generic proxy; bulk copies reuse it
+        __syncthreads();
+        if constexpr (MODE != 2) {            // the next plane's sticks arrive while this plane's y forward pass runs
+            const int nxt = pl + gridDim.x;
+            if (tid == 0 && nxt < nplanes) {
+                fence_async_smem();
+                mbar_expect_tx(wbar, wbytes);
+                bulk_g2s(stage_in, W + (size_t)nxt * S, wbytes, wbar);
+            }
+        }
+        if constexpr (MODE != 1) {
+            for (int r = grp * TPG + slot; r - slot < X; r += ngroups * TPG) {
+                const bool ok = team_ok && r < X;
+                if (ok) lineB_step1<C>(A + r * RP, u, twb);
+                group_barrier<G>(grp);
+                if (ok) {
+                    int sbase;
+                    const Pruned pr = row_pruned(r, sbase);
+                    prunedB_step2<C>(SpaceShared{}, A + r * RP, stage_out + sbase, C::R2, pr, u);
+                }
+            }
+            fence_async_smem();
+            __syncthreads();
+            if (tid == 0) { bulk_s2g(Wp, stage_out, wbytes); bulk_commit(); }
+        } else {
+            __syncthreads();                  // MODE 1: A is rewritten by the next plane's y backward pass
         }
     }
-    __syncthreads();
-    {
-        const int z = (p / gd.ax[2].r2) + gd.ax[2].r1 * (p % gd.ax[2].r2);
-        c128 *myscr = scr + (size_t)(grp * TPG + team) * SL;
-        const double *vplane = gd.vt + (size_t)p * C::N * C::N;
-        VRow<C::R2> vr;
-        // De-phase the groups: they all do identical load -> FP64 -> store bursts, and when they run in
-        // lock step the shared-memory pipe and the FP64 pipe are used alternately instead of together.
-        if (stagger_ns > 0) __nanosleep((unsigned)(grp * stagger_ns));
-        if constexpr (MODE == 0) {       // V of the first column: in flight while step 1 runs
-            const int col0 = grp * TPG + team;
-            if (team_ok && col0 < C::N) load_vrow<C>(vr, vplane + (size_t)col0 * C::N, u);
-        }
-        for (int cc = grp; cc * TPG < C::N; cc += ngroups) {
-            const int col = cc * TPG + team;
-            const bool ok = team_ok && col < C::N;
-            const int colpos = C::pos(col);
-            if constexpr (MODE != 2) {
-                if (ok) xcol_step1<C>(A, rowpitch, colpos, xr, myscr, u, twa);
-                group_barrier(grp);
-            }
-            if (ok) {
-                const int y = (col / C::R2) + C::R1 * (col % C::R2);
-                c128 *bx = nullptr;
-                if constexpr (MODE != 0) bx = box + (size_t)band * C::N * C::N * n3 + (size_t)y * n3 + z;
-                xcol_step2<C, MODE>(myscr, u, twb, vr, bx, (long)C::N * n3, scale);
-            }
-            if constexpr (MODE == 0) {   // prefetch V of this team's next column behind steps 3 and 1
-                const int ncol = col + ngroups * TPG;
-                if (team_ok && ncol < C::N) load_vrow<C>(vr, vplane + (size_t)ncol * C::N, u);
-            }
-            group_barrier(grp);
-            if constexpr (MODE != 1) {
-                // no barrier after step 3: the scratch column a thread reads here is exactly the one it
-                // overwrites in the next iteration's step 1 (MODE 2 has no step 1 and writes rows: barrier).
-                if (ok) xcol_step3<C>(A, rowpitch, colpos, xr, myscr, u);
-                if constexpr (MODE == 2) group_barrier(grp);
-            }
-        }
-    }
-    __syncthreads();
-    if constexpr (MODE != 1) {
-        for (int rc = grp; rc * TPG < X; rc += ngroups) {
-            const int r = rc * TPG + team;
-            const bool ok = team_ok && r < X;
-            if (ok) lineB_step1<C>(A + r * rowpitch, u, twb);
-            group_barrier(grp);
-            if (ok) lineB_step2_gout<C>(A + r * rowpitch, Wp, row_info(r), u);
-        }
-    }
+    if (tid == 0) bulk_wait0();
 }

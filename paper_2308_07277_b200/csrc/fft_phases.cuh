@@ -78,6 +78,101 @@ template <class C> QM_HD void lineB_step2_gout(const c128 *line, c128 *Wp, const
     });
 }
 
+// ---- pruned passes with hoisted addressing ---------------------------------------------------------
+// A thread with fixed u touches the line elements i = n*R2 + u (n = 0..R1-1).  When only two index
+// intervals [a1,b1], [a2,b2] of the line exist (stored back to back with element stride `stride`), the
+// elements that exist and their addresses depend on (u, intervals) only: they are worked out once
+// (per kernel for the x direction, per row for the y direction) instead of once per access.
+struct Pruned {
+    unsigned m1, m2;      // bit n set: i = n*R2+u lies in interval 1 / interval 2
+    int c1, c2;           // element offset of i: n*R2*stride + c1 (interval 1), + c2 (interval 2)
+};
+QM_HD unsigned qm_range_mask(int a, int b, int u, int r2, int r1) {   // { n : a <= n*r2 + u <= b }
+    int lo = a - u, hi = b - u;
+    if (hi < 0 || b < a) return 0u;
+    lo = lo <= 0 ? 0 : (lo + r2 - 1) / r2;
+    hi = hi / r2;
+    if (hi > r1 - 1) hi = r1 - 1;
+    return lo > hi ? 0u : ((2u << hi) - (1u << lo));
+}
+template <class C> QM_HD Pruned make_pruned(int a1, int b1, int a2, int b2, int u, int stride) {
+    const int cnt1 = b1 >= a1 ? b1 - a1 + 1 : 0;
+    return Pruned{qm_range_mask(a1, b1, u, C::R2, C::R1), qm_range_mask(a2, b2, u, C::R2, C::R1),
+                  (u - a1) * stride, (u - a2 + cnt1) * stride};
+}
+// predicated 16-byte accesses (no branch, no address arithmetic beyond base + immediate)
+struct SpaceShared {}; struct SpaceGlobal {};
+QM_HD c128 ld_pred(SpaceShared, const c128 *p, bool pred) {
+#ifdef __CUDA_ARCH__
+    c128 v;
+    asm volatile("{ .reg .pred q; setp.ne.u32 q, %3, 0; mov.f64 %0, 0d0000000000000000; mov.f64 %1, 0d0000000000000000;\n"
+                 "  @q ld.shared.v2.f64 {%0, %1}, [%2]; }"
+                 : "=d"(v.x), "=d"(v.y) : "r"((unsigned)__cvta_generic_to_shared(p)), "r"((unsigned)pred) : "memory");
+    return v;
+#else
+    return pred ? *p : c128{0.0, 0.0};
+#endif
+}
+QM_HD c128 ld_pred(SpaceGlobal, const c128 *p, bool pred) {
+#ifdef __CUDA_ARCH__
+    c128 v;
+    asm volatile("{ .reg .pred q; setp.ne.u32 q, %3, 0; mov.f64 %0, 0d0000000000000000; mov.f64 %1, 0d0000000000000000;\n"
+                 "  @q ld.global.v2.f64 {%0, %1}, [%2]; }"
+                 : "=d"(v.x), "=d"(v.y) : "l"(p), "r"((unsigned)pred) : "memory");
+    return v;
+#else
+    return pred ? *p : c128{0.0, 0.0};
+#endif
+}
+QM_HD void st_pred(SpaceShared, c128 *p, c128 v, bool pred) {
+#ifdef __CUDA_ARCH__
+    asm volatile("{ .reg .pred q; setp.ne.u32 q, %3, 0; @q st.shared.v2.f64 [%0], {%1, %2}; }"
+                 :: "r"((unsigned)__cvta_generic_to_shared(p)), "d"(v.x), "d"(v.y), "r"((unsigned)pred) : "memory");
+#else
+    if (pred) *p = v;
+#endif
+}
+QM_HD void st_pred(SpaceGlobal, c128 *p, c128 v, bool pred) {
+#ifdef __CUDA_ARCH__
+    asm volatile("{ .reg .pred q; setp.ne.u32 q, %3, 0; @q st.global.v2.f64 [%0], {%1, %2}; }"
+                 :: "l"(p), "d"(v.x), "d"(v.y), "r"((unsigned)pred) : "memory");
+#else
+    if (pred) *p = v;
+#endif
+}
+// Backward step 1 with pruned input: src = first stored element of the line, estride = R2*stride (elements
+// between n and n+1); writes the full padded line `dst`.
+template <class C, class SP, class TW>
+QM_HD void prunedA_step1(SP sp, const c128 *src, int estride, const Pruned pr, c128 *dst, int u, const TW &tw) {
+    if (u >= C::R2) return;
+    c128 t[C::R1];
+    const c128 *p1 = src + pr.c1, *p2 = src + pr.c2;
+    static_for<C::R1>([&](auto I) {
+        constexpr int n1 = decltype(I)::value;
+        const bool in2 = (pr.m2 >> n1) & 1u, in1 = (pr.m1 >> n1) & 1u;
+        t[n1] = ld_pred(sp, (in2 ? p2 : p1) + n1 * estride, in1 || in2);
+    });
+    Dft<C::R1, +1>::run(t);
+    static_for<C::R1>([&](auto I) {
+        constexpr int k1 = decltype(I)::value;
+        dst[k1 * C::R2P + u] = (k1 == 0) ? t[k1] : cmul_conj(t[k1], tw.template get<k1>());
+    });
+}
+// Forward step 2 with pruned output: reads the full padded line `srcline`, stores only what exists.
+template <class C, class SP>
+QM_HD void prunedB_step2(SP sp, const c128 *srcline, c128 *dst, int estride, const Pruned pr, int u) {
+    if (u >= C::R2) return;
+    c128 t[C::R1];
+    static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = srcline[a * C::R2P + u]; });
+    Dft<C::R1, -1>::run(t);
+    c128 *p1 = dst + pr.c1, *p2 = dst + pr.c2;
+    static_for<C::R1>([&](auto I) {
+        constexpr int c = decltype(I)::value;
+        const bool in2 = (pr.m2 >> c) & 1u, in1 = (pr.m1 >> c) & 1u;
+        st_pred(sp, (in2 ? p2 : p1) + c * estride, t[c], in1 || in2);
+    });
+}
+
 template <class C, class TW> QM_HD void lineA_step1(c128 *line, int u, const TW &tw) {
     if (u >= C::R2) return;
     c128 t[C::R1];
@@ -113,6 +208,47 @@ template <class C> QM_HD void lineB_step2(c128 *line, int u) {
     static_for<C::R1>([&](auto I) { constexpr int c = decltype(I)::value; line[c * C::R2P + u] = t[c]; });
 }
 
+// ---- z kernels: one shared-memory round trip per stick ------------------------------------------------
+// zinv pass 2: thread (stick t, row u) finishes the backward transform and writes the stick planes
+// W[p = u*R2 + k2][s] straight from registers (lanes run over sticks => contiguous 16-byte stores).
+template <class C> QM_HD void zinv_step2_store(const c128 *line, c128 *Wcol, long pstride, int u) {
+    if (u >= C::R1) return;
+    c128 t[C::R2];
+    static_for<C::R2>([&](auto I) { constexpr int n2 = decltype(I)::value; t[n2] = line[u * C::R2P + n2]; });
+    Dft<C::R2, +1>::run(t);
+    static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; Wcol[(long)(u * C::R2 + k2) * pstride] = t[k2]; });
+}
+// zfwd pass 1: thread (stick t, row u) reads W[p = u*R2 + b][s] into registers and starts the forward transform.
+template <class C, class TW> QM_HD void zfwd_step1_load(const c128 *Wcol, long pstride, c128 *line, int u, const TW &tw) {
+    if (u >= C::R1) return;
+    c128 t[C::R2];
+    static_for<C::R2>([&](auto I) { constexpr int b = decltype(I)::value; t[b] = Wcol[(long)(u * C::R2 + b) * pstride]; });
+    Dft<C::R2, -1>::run(t);
+    static_for<C::R2>([&](auto I) {
+        constexpr int d = decltype(I)::value;
+        line[u * C::R2P + d] = (d == 0) ? t[d] : cmul(t[d], tw.template get<d>());
+    });
+}
+// zfwd pass 2: finishes the forward transform and gathers to the sphere with the kinetic term fused
+// (PAPER.md:668-674): out[g] = (V psi)(G) + 1/2 |k+G|^2 psi_in[g] for the G of this stick only.
+template <class C> QM_HD void zfwd_step2_gather(const c128 *line, c128 *out, const c128 *psi_in, const double *g2,
+                                                 const Pruned pr, int u, bool kinetic) {
+    if (u >= C::R2) return;
+    c128 t[C::R1];
+    static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = line[a * C::R2P + u]; });
+    Dft<C::R1, -1>::run(t);
+    static_for<C::R1>([&](auto I) {
+        constexpr int c = decltype(I)::value;
+        const bool in2 = (pr.m2 >> c) & 1u, in1 = (pr.m1 >> c) & 1u;
+        const int off = (in2 ? pr.c2 : pr.c1) + c * C::R2;
+        if (in1 || in2) {
+            c128 v = t[c];
+            if (kinetic) { const double h = 0.5 * g2[off]; const c128 x = psi_in[off]; v.x = fma(h, x.x, v.x); v.y = fma(h, x.y, v.y); }
+            out[off] = v;
+        }
+    });
+}
+
 // ---- x direction of the plane kernel: X compact rows <-> full length-N1 line in scratch -------------
 // A: plane array [X][rowpitch].  The occupied box indices i1 form two intervals (the sphere is convex):
 // [a1,b1] -> rows 0.., [a2,b2] -> rows (b1-a1+1)..; everything else is not stored (zero).
@@ -143,9 +279,23 @@ template <class C, class TW> QM_HD void xcol_step1(const c128 *A, int rowpitch, 
 // v: this thread's R2 potential values V(x = u + R1*k2), already in registers (prefetched by the caller).
 // box: pointer to element x=0 of this column in a natural-order box, xstride = n2*n3.
 template <int R> struct VRow { double v[R]; };
-template <class C> QM_HD void load_vrow(VRow<C::R2> &vr, const double *v, int u) {
+// V of one plane column is stored in pairs: vcol[(j * R1 + u) * 2 + e] = V(x = u + R1*(2j + e)), j < R2E/2
+// (R2E = R2 rounded up to even, the pad is zero), so a thread reads its R2 values with 16-byte loads and the
+// lanes of a team read contiguous 16-byte words.
+template <class C> struct VLayout { static constexpr int R2E = C::R2 + (C::R2 & 1), COL = C::R1 * R2E; };
+template <class C> QM_HD void load_vrow(VRow<C::R2> &vr, const double *vcol, int u) {
     if (u >= C::R1) return;
-    static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; vr.v[k2] = v[u + C::R1 * k2]; });
+#ifdef QM_ABLATE_V        /* timing experiment only */
+    static_for<C::R2>([&](auto I) { vr.v[decltype(I)::value] = 1.0; });
+    return;
+#endif
+    const double2 *q = reinterpret_cast<const double2 *>(vcol) + u;
+    static_for<VLayout<C>::R2E / 2>([&](auto I) {
+        constexpr int j = decltype(I)::value;
+        const double2 d = q[j * C::R1];
+        vr.v[2 * j] = d.x;
+        if constexpr (2 * j + 1 < C::R2) vr.v[2 * j + 1] = d.y;
+    });
 }
 template <class C, int MODE, class TW> QM_HD void xcol_step2(c128 *scr, int u, const TW &tw, const VRow<C::R2> &vr,
                                                              c128 *box, long xstride, double scale) {

@@ -49,6 +49,7 @@ struct QmKTables {
     std::vector<int16_t> xrow;
     std::vector<short4> rowiv;                 // per plane row: occupied i2 intervals
     std::vector<int4> rowinfo;                 // packed (a1|b1<<16, a2|b2<<16, first stick of the row, 0)
+    std::vector<int4> stickinfo;               // per stick: packed occupied i3 intervals (a1|b1<<16, a2|b2<<16), first G, 0
     short4 xiv = {1, 0, 1, 0};                 // occupied i1 intervals (rows 0.. and following)
     bool x_contiguous = true;
 };
@@ -164,6 +165,21 @@ static inline int qm_build_tables(const double *lattice, const double *recip, do
             kp->rowinfo[r] = int4{(int)(unsigned short)iv.x | ((int)iv.y << 16), (int)(unsigned short)iv.z | ((int)iv.w << 16), s, 0};
             s += span;      // sticks ascend in (i1, i2): the row's sticks are [s, s + span)
         }
+    }
+    // occupied i3 intervals of every stick: [0..m3max] and [n3+m3min..n3-1]; the G of a stick are stored in
+    // ascending i3, i.e. interval 1 then interval 2 back to back (what the z kernels' pruned passes assume)
+    kp->stickinfo.resize(S);
+    for (int s = 0; s < S; ++s) {
+        short4 iv = {1, 0, 1, 0};
+        for (int g = kp->stickoff[s]; g < kp->stickoff[s + 1]; ++g) {
+            const int i3 = kp->idx[g] % n3;
+            if (2 * i3 < n3) { if (iv.x > iv.y) iv.x = (short)i3; iv.y = (short)i3; }
+            else { if (iv.z > iv.w) iv.z = (short)i3; iv.w = (short)i3; }
+        }
+        const int span = (iv.x <= iv.y ? iv.y - iv.x + 1 : 0) + (iv.z <= iv.w ? iv.w - iv.z + 1 : 0);
+        if (span != kp->stickoff[s + 1] - kp->stickoff[s]) { *msg = "G of a stick are not two contiguous intervals"; return -1; }
+        kp->stickinfo[s] = int4{(int)(unsigned short)iv.x | ((int)iv.y << 16), (int)(unsigned short)iv.z | ((int)iv.w << 16),
+                                kp->stickoff[s], 0};
     }
     kp->stickapos.resize(S);
     for (int s = 0; s < S; ++s)

@@ -51,7 +51,7 @@ struct KPoint : QmKTables {
     DevBuf<int32_t> d_gstick, d_stickoff, d_stickapos;
     DevBuf<uint16_t> d_gzpos;
     DevBuf<int16_t> d_xrow;
-    DevBuf<int4> d_rowinfo;
+    DevBuf<int4> d_rowinfo, d_stickinfo;
     DevBuf<double> d_g2;
     // non-local
     bool nl_set = false;
@@ -64,7 +64,7 @@ struct KPoint : QmKTables {
         p.ng = ng; p.nsticks = nsticks; p.nx = nx; p.rowpitch = rowpitch;
         p.g_stick = d_gstick.p; p.g_zpos = d_gzpos.p; p.stick_off = d_stickoff.p;
         p.stick_apos = d_stickapos.p; p.xrow = d_xrow.p; p.g2 = d_g2.p;
-        p.row_info = d_rowinfo.p; p.x_iv = xiv;
+        p.row_info = d_rowinfo.p; p.x_iv = xiv; p.stick_info = d_stickinfo.p;
         return p;
     }
 };
@@ -136,13 +136,13 @@ struct qm_gspace {
     unsigned long long launches = 0;
     int sm_count = 148;
     int max_smem = 0;
+    int z_cta_per_sm = 3;           // resident z-kernel CTAs per SM the grid is sized for (QM_Z_CTA_PER_SM)
     int plane_stagger_ns = 100;     // de-phasing delay between the plane kernel's groups (QM_PLANE_STAGGER_NS)
     ~qm_gspace() { for (auto *k : kpts) delete k; }
 };
 
 namespace {
 
-constexpr int ZT_STICKS = 16;                         // sticks per CTA in the z kernels
 
 int build_kpoint(qm_gspace *g, KPoint *kp) {
     std::string msg;
@@ -155,17 +155,22 @@ int build_kpoint(qm_gspace *g, KPoint *kp) {
     CU_TRY(kp->d_stickapos.upload(kp->stickapos));
     CU_TRY(kp->d_xrow.upload(kp->xrow));
     CU_TRY(kp->d_rowinfo.upload(kp->rowinfo));
+    CU_TRY(kp->d_stickinfo.upload(kp->stickinfo));
     CU_TRY(kp->d_g2.upload(kp->g2));
     return QM_OK;
 }
 
-constexpr int PLANE_GROUP = 64;
-size_t plane_smem(const qm_gspace *g, const KPoint *kp, int ngroups) {
+constexpr int PLANE_GROUP = QM_GROUP;
+size_t plane_scr_elems(const qm_gspace *g, const KPoint *kp, int ngroups) {
     const QmAxis &ax = g->ax[0];
     const size_t sl = (size_t)qm_scratch_pitch(ax.len, std::max(ax.r1, ax.r2));
     const int tpg = PLANE_GROUP / std::max(ax.r1, ax.r2);
-    return ((size_t)kp->nx * kp->rowpitch + (size_t)ngroups * tpg * sl) * sizeof(c128)
-           + (size_t)kp->nx * sizeof(int4) + 16;
+    // scratch lines of the x phase; outside it the same region stages one stick plane in and one out
+    return (std::max((size_t)ngroups * tpg * sl, 2 * qm_stage_elems(kp->nsticks)) + 7) & ~(size_t)7;
+}
+size_t plane_smem(const qm_gspace *g, const KPoint *kp, int ngroups) {
+    const size_t a_elems = ((size_t)kp->nx * kp->rowpitch + 7) & ~(size_t)7;
+    return (a_elems + plane_scr_elems(g, kp, ngroups)) * sizeof(c128) + (size_t)kp->nx * sizeof(int4) + 16;
 }
 
 // number of independent 64-thread groups of the plane kernel: the fewest groups that reach the
@@ -183,14 +188,23 @@ int plane_groups(const qm_gspace *g, const KPoint *kp) {
     return best;
 }
 
+// z kernels: grid.x tiles-in-flight per band chosen so that the whole grid is close to a whole number of
+// resident CTAs per SM (each CTA then loops over ~ntiles / grid.x tiles)
+int z_grid_x(const qm_gspace *g, int ntiles, int nb, int cta_per_sm) {
+    const int slots = g->sm_count * cta_per_sm;
+    int gx = std::max(1, slots / std::max(1, nb));
+    if (gx >= ntiles) return ntiles;
+    const int rounds = (ntiles + gx - 1) / gx;          // fewest CTAs that keep the same number of rounds
+    return (ntiles + rounds - 1) / rounds;
+}
 template <class C> int launch_zinv(qm_gspace *g, KPoint *kp, const c128 *psi, int nb, cudaStream_t st) {
-    const int TS = ZT_STICKS;
-    const size_t smem = ((size_t)C::N + (size_t)TS * (C::L | 1)) * sizeof(c128);
+    const size_t smem = (size_t)QM_ZT * (C::L | 1) * sizeof(c128);
     static bool attr = false;
     if (!attr) { CU_TRY(cudaFuncSetAttribute(k_zinv<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
-    dim3 grid((kp->nsticks + TS - 1) / TS, nb);
+    const int ntiles = (kp->nsticks + QM_ZT - 1) / QM_ZT;
+    dim3 grid(z_grid_x(g, ntiles, nb, g->z_cta_per_sm), nb);
     g->prof.begin(QM_K_ZINV, st);
-    k_zinv<C><<<grid, TS * C::TT, smem, st>>>(kp->plan(), g->d_tw[2].p, psi, g->d_W.p, TS);
+    k_zinv<C><<<grid, QM_ZT * C::TT, smem, st>>>(kp->plan(), g->d_tw[2].p, psi, g->d_W.p, ntiles);
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
@@ -198,13 +212,13 @@ template <class C> int launch_zinv(qm_gspace *g, KPoint *kp, const c128 *psi, in
 }
 template <class C> int launch_zfwd(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb, int kinetic,
                                    cudaStream_t st) {
-    const int TS = ZT_STICKS;
-    const size_t smem = ((size_t)C::N + (size_t)TS * (C::L | 1)) * sizeof(c128);
+    const size_t smem = (size_t)QM_ZT * (C::L | 1) * sizeof(c128);
     static bool attr = false;
     if (!attr) { CU_TRY(cudaFuncSetAttribute(k_zfwd<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
-    dim3 grid((kp->nsticks + TS - 1) / TS, nb);
+    const int ntiles = (kp->nsticks + QM_ZT - 1) / QM_ZT;
+    dim3 grid(z_grid_x(g, ntiles, nb, g->z_cta_per_sm), nb);
     g->prof.begin(QM_K_ZFWD, st);
-    k_zfwd<C><<<grid, TS * C::TT, smem, st>>>(kp->plan(), g->d_tw[2].p, g->d_W.p, psi_in, out, TS, kinetic);
+    k_zfwd<C><<<grid, QM_ZT * C::TT, smem, st>>>(kp->plan(), g->d_tw[2].p, g->d_W.p, psi_in, out, ntiles, kinetic);
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
@@ -220,10 +234,12 @@ template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *bo
     QmGridDev gd;
     for (int i = 0; i < 3; ++i) { gd.ax[i] = g->ax[i]; gd.tw[i] = g->d_tw[i].p; }
     gd.vt = g->d_vt.p;
-    dim3 grid(g->grid[2], nb);
+    const int nplanes = g->grid[2] * nb;
+    const int grid = std::min(nplanes, g->sm_count);      // persistent: one CTA per SM walks the (band, z-plane) list
     g->prof.begin(QM_K_PLANE, st);
     k_plane<C, MODE><<<grid, ngroups * PLANE_GROUP, smem, st>>>(kp->plan(), gd, g->d_W.p, box, ngroups, scale,
-                                                                   g->plane_stagger_ns);
+                                                                   g->plane_stagger_ns, nplanes,
+                                                                   (int)plane_scr_elems(g, kp, ngroups));
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
@@ -268,15 +284,18 @@ template <int MODE> int dispatch_plane(qm_gspace *g, KPoint *kp, c128 *box, int 
 __global__ void k_relayout_v(const double *__restrict__ v, double *__restrict__ vt, QmAxis a1, QmAxis a2, QmAxis a3,
                              double scale)
 {
-    // vt[p][col][x] = scale * v[x][y(col)][z(p)]
-    const size_t total = (size_t)a1.n * a2.n * a3.n;
+    // vt[p][col][j][u][e] = scale * v[x = u + r1*(2j+e)][y(col)][z(p)]   (pairs; fft_phases.cuh VLayout)
+    const int r2e = a1.r2 + (a1.r2 & 1), colsz = a1.r1 * r2e;
+    const size_t total = (size_t)a3.n * a2.n * colsz;
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
-        const int x = (int)(i % a1.n);
-        const int col = (int)((i / a1.n) % a2.n);
-        const int p = (int)(i / ((size_t)a1.n * a2.n));
+        const int e = (int)(i % colsz);
+        const int u = (e >> 1) % a1.r1, k2 = 2 * ((e >> 1) / a1.r1) + (e & 1);
+        const int col = (int)((i / colsz) % a2.n);
+        const int p = (int)(i / ((size_t)colsz * a2.n));
+        const int x = u + a1.r1 * k2;
         const int y = (col / a2.r2) + a2.r1 * (col % a2.r2);
         const int z = (p / a3.r2) + a3.r1 * (p % a3.r2);
-        vt[i] = scale * v[((size_t)x * a2.n + y) * a3.n + z];
+        vt[i] = (k2 < a1.r2) ? scale * v[((size_t)x * a2.n + y) * a3.n + z] : 0.0;
     }
 }
 
@@ -399,6 +418,7 @@ QM_API int qm_gspace_create(const double *lattice_bohr, double ecutwfc_ry, const
         }
     }
     if (const char *e = getenv("QM_PLANE_STAGGER_NS")) g->plane_stagger_ns = atoi(e);
+    if (const char *e = getenv("QM_Z_CTA_PER_SM")) g->z_cta_per_sm = std::max(1, atoi(e));
     *out = g;
     return QM_OK;
 }
@@ -446,7 +466,8 @@ QM_API int qm_gspace_alias_free(const qm_gspace *g, int k, int *flag) {
 QM_API int qm_set_vloc(qm_gspace *g, const double *V_r_dev, void *stream) {
     if (!g || !V_r_dev) return fail(QM_EINVAL, "qm_set_vloc: null argument");
     const size_t n = (size_t)g->grid[0] * g->grid[1] * g->grid[2];
-    CU_TRY(g->d_vt.resize(n));
+    const size_t r2e = (size_t)g->ax[0].r2 + (g->ax[0].r2 & 1);
+    CU_TRY(g->d_vt.resize((size_t)g->grid[2] * g->grid[1] * g->ax[0].r1 * r2e));
     k_relayout_v<<<g->sm_count * 4, 256, 0, (cudaStream_t)stream>>>(V_r_dev, g->d_vt.p, g->ax[0], g->ax[1], g->ax[2],
                                                                    1.0 / (double)n);
     g->launches++;

@@ -21,6 +21,7 @@ struct QmKPlanDev {        // per k-point tables on the device
     const int16_t *xrow;         // [n1]   compact row of box index i1, or -1
     short4 x_iv;                 //        occupied i1 intervals [x,y] -> rows 0.., [z,w] -> following rows
     const int4 *row_info;        // [X]    per plane row: (a1 | b1<<16, a2 | b2<<16, first stick, 0): occupied i2 intervals
+    const int4 *stick_info;      // [S]    per stick: (a1 | b1<<16, a2 | b2<<16, first G, 0): occupied i3 intervals
     const double *g2;            // [ng]   |k+G|^2
 };
 

@@ -34,31 +34,37 @@ template <class C> struct Emu {
     }
     TwRow<C::R1> rowA(int u) { TwRow<C::R1> t; load_twrow(t, tw.data(), u, C::R2); return t; }
     TwRow<C::R2> rowB(int u) { TwRow<C::R2> t; load_twrow(t, tw.data(), u, C::R1); return t; }
-    // k_zinv for one band: psi[ng] -> W[N][S]
+    static Pruned stick_pruned(const int4 q, int u) {
+        return make_pruned<C>((int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, u, 1);
+    }
+    // k_zinv for one band: psi[ng] -> W[N][S]   (same thread mappings as the kernel)
     void zinv(const c128 *psi, c128 *W) {
         const int S = kp.nsticks, nthr = TS * C::TT;
         for (int s0 = 0; s0 < S; s0 += TS) {
             const int ns = std::min(TS, S - s0);
-            std::vector<c128> lines(TS * LP, c128{0, 0});
-            for (int g = kp.stickoff[s0]; g < kp.stickoff[s0 + ns]; ++g)
-                lines[(kp.gstick[g] - s0) * LP + kp.gzpos[g]] = psi[g];
-            for (int tid = 0; tid < nthr; ++tid) { int t = tid / C::TT, u = tid % C::TT; if (t < ns) lineA_step1<C>(&lines[t * LP], u, rowA(u)); }
-            for (int tid = 0; tid < nthr; ++tid) { int t = tid / C::TT, u = tid % C::TT; if (t < ns) lineA_step2<C>(&lines[t * LP], u); }
-            for (int i = 0; i < C::N * TS; ++i) { int p = i / TS, tt = i % TS; if (tt < ns) W[(size_t)p * S + s0 + tt] = lines[tt * LP + C::pos(p)]; }
+            std::vector<c128> lines(TS * LP, c128{1e300, -1e300});
+            for (int tid = 0; tid < nthr; ++tid) {
+                int t = tid / C::TT, u = tid % C::TT;
+                if (t < ns) { const int4 q = kp.stickinfo[s0 + t]; prunedA_step1<C>(SpaceGlobal{}, psi + q.z, C::R2, stick_pruned(q, u), &lines[t * LP], u, rowA(u)); }
+            }
+            for (int tid = 0; tid < nthr; ++tid) {
+                int t = tid % TS, u = tid / TS;
+                if (t < ns) zinv_step2_store<C>(&lines[t * LP], W + s0 + t, S, u);
+            }
         }
     }
     void zfwd(const c128 *W, const c128 *psi_in, c128 *out, bool kinetic) {
         const int S = kp.nsticks, nthr = TS * C::TT;
         for (int s0 = 0; s0 < S; s0 += TS) {
             const int ns = std::min(TS, S - s0);
-            std::vector<c128> lines(TS * LP, c128{0, 0});
-            for (int i = 0; i < C::N * TS; ++i) { int p = i / TS, tt = i % TS; if (tt < ns) lines[tt * LP + C::pos(p)] = W[(size_t)p * S + s0 + tt]; }
-            for (int tid = 0; tid < nthr; ++tid) { int t = tid / C::TT, u = tid % C::TT; if (t < ns) lineB_step1<C>(&lines[t * LP], u, rowB(u)); }
-            for (int tid = 0; tid < nthr; ++tid) { int t = tid / C::TT, u = tid % C::TT; if (t < ns) lineB_step2<C>(&lines[t * LP], u); }
-            for (int g = kp.stickoff[s0]; g < kp.stickoff[s0 + ns]; ++g) {
-                c128 v = lines[(kp.gstick[g] - s0) * LP + kp.gzpos[g]];
-                if (kinetic) { double h = 0.5 * kp.g2[g]; v.x += h * psi_in[g].x; v.y += h * psi_in[g].y; }
-                out[g] = v;
+            std::vector<c128> lines(TS * LP, c128{1e300, -1e300});
+            for (int tid = 0; tid < nthr; ++tid) {
+                int t = tid % TS, u = tid / TS;
+                if (t < ns) zfwd_step1_load<C>(W + s0 + t, S, &lines[t * LP], u, rowB(u));
+            }
+            for (int tid = 0; tid < nthr; ++tid) {
+                int t = tid / C::TT, u = tid % C::TT;
+                if (t < ns) { const int4 q = kp.stickinfo[s0 + t]; zfwd_step2_gather<C>(&lines[t * LP], out + q.z, kinetic ? psi_in + q.z : nullptr, kp.g2.data() + q.z, stick_pruned(q, u), u, kinetic); }
             }
         }
     }
@@ -73,7 +79,12 @@ template <class C> struct Emu {
         };
         c128 *Wp = W + (size_t)p * S;
         if (MODE != 2) {
-            for (int task = 0; task < X * C::TT; ++task) lineA_step1_gin<C>(&A[(task / C::TT) * rp], Wp, row_info(task / C::TT), task % C::TT, rowA(task % C::TT));
+            for (int task = 0; task < X * C::TT; ++task) {
+                const RowInfo ri = row_info(task / C::TT);
+                const int u = task % C::TT;
+                const Pruned pr = make_pruned<C>(ri.a1, ri.b1, ri.a2, ri.b2, u, 1);
+                prunedA_step1<C>(SpaceGlobal{}, Wp + ri.sbase, C::R2, pr, &A[(task / C::TT) * rp], u, rowA(u));
+            }
             for (int task = 0; task < X * C::TT; ++task) lineA_step2<C>(&A[(task / C::TT) * rp], task % C::TT);
         }
         const int z = (p / ax.r2) + ax.r1 * (p % ax.r2);
@@ -82,26 +93,30 @@ template <class C> struct Emu {
             if (MODE != 2)
                 for (int tid = 0; tid < nthr; ++tid) {
                     int c = tid / C::TT, u = tid % C::TT, col = cbase + c;
-                    if (col < C::N) xcol_step1<C>(A.data(), rp, C::pos(col), xr, &scr[(size_t)c * SL], u, rowA(u));
+                    if (col < C::N) prunedA_step1<C>(SpaceShared{}, A.data() + C::pos(col), C::R2 * rp, make_pruned<C>(xr.a1, xr.b1, xr.a2, xr.b2, u, rp), &scr[(size_t)c * SL], u, rowA(u));
                 }
             for (int tid = 0; tid < nthr; ++tid) {
                 int c = tid / C::TT, u = tid % C::TT, col = cbase + c;
                 if (col >= C::N) continue;
                 int y = (col / C::R2) + C::R1 * (col % C::R2);
                 VRow<C::R2> vr;
-                if (MODE == 0) load_vrow<C>(vr, vt + ((size_t)p * C::N + col) * C::N, u);
+                if (MODE == 0) load_vrow<C>(vr, vt + ((size_t)p * C::N + col) * VLayout<C>::COL, u);
                 c128 *bx = MODE == 0 ? nullptr : box + (size_t)y * n3 + z;
                 xcol_step2<C, MODE>(&scr[(size_t)c * SL], u, rowB(u), vr, bx, (long)C::N * n3, scale);
             }
             if (MODE != 1)
                 for (int tid = 0; tid < nthr; ++tid) {
                     int c = tid / C::TT, u = tid % C::TT, col = cbase + c;
-                    if (col < C::N) xcol_step3<C>(A.data(), rp, C::pos(col), xr, &scr[(size_t)c * SL], u);
+                    if (col < C::N) prunedB_step2<C>(SpaceShared{}, &scr[(size_t)c * SL], A.data() + C::pos(col), C::R2 * rp, make_pruned<C>(xr.a1, xr.b1, xr.a2, xr.b2, u, rp), u);
                 }
         }
         if (MODE != 1) {
             for (int task = 0; task < X * C::TT; ++task) lineB_step1<C>(&A[(task / C::TT) * rp], task % C::TT, rowB(task % C::TT));
-            for (int task = 0; task < X * C::TT; ++task) lineB_step2_gout<C>(&A[(task / C::TT) * rp], Wp, row_info(task / C::TT), task % C::TT);
+            for (int task = 0; task < X * C::TT; ++task) {
+                const RowInfo ri = row_info(task / C::TT);
+                const int u = task % C::TT;
+                prunedB_step2<C>(SpaceGlobal{}, &A[(task / C::TT) * rp], Wp + ri.sbase, C::R2, make_pruned<C>(ri.a1, ri.b1, ri.a2, ri.b2, u, 1), u);
+            }
         }
     }
 };
@@ -120,11 +135,13 @@ template <class C> int run(int n, const double *lat, double ecut, const double *
     auto v = slurp<double>(v_path);
     if ((int)psi.size() != nb * kp.ng || (int)v.size() != n * n * n) { fprintf(stderr, "size mismatch ng=%d\n", kp.ng); return 4; }
     const size_t n3 = (size_t)n * n * n;
-    std::vector<double> vt(n3);
-    for (size_t i = 0; i < n3; ++i) {
-        int x = i % n, col = (i / n) % n, p = i / ((size_t)n * n);
+    const int r2e = VLayout<C>::R2E, colsz = VLayout<C>::COL;
+    std::vector<double> vt((size_t)n * n * colsz, 0.0);
+    for (size_t i = 0; i < vt.size(); ++i) {
+        int e = i % colsz, u = (e >> 1) % ax[0].r1, k2 = 2 * ((e >> 1) / ax[0].r1) + (e & 1), col = (i / colsz) % n, p = i / ((size_t)colsz * n);
+        int x = u + ax[0].r1 * k2;
         int y = (col / ax[1].r2) + ax[1].r1 * (col % ax[1].r2), z = (p / ax[2].r2) + ax[2].r1 * (p % ax[2].r2);
-        vt[i] = v[((size_t)x * n + y) * n + z] / (double)n3;
+        if (k2 < ax[0].r2) vt[i] = v[((size_t)x * n + y) * n + z] / (double)n3;
     }
     Emu<C> emu(kp, ax[2]);
     const int S = kp.nsticks, ncol = 5;     // odd column count on purpose: exercises the ragged last pass
