@@ -35,6 +35,14 @@ def _peaks():
     return 6650.0, 1590.0, "fallback (B200_PROFILING.md)"
 
 
+def _ncu_traffic(cfg_name, kernel):
+    """DRAM bytes per launch of `kernel` from the committed `ncu --set full` capture (profiles/), or None."""
+    p = os.path.join(ROOT, "profiles", f"ncu_traffic_{cfg_name}.json")
+    if not os.path.exists(p):
+        return None
+    return json.load(open(p)).get(kernel)
+
+
 class ClockSampler(threading.Thread):
     """Samples SM clock / throttle reasons with NVML while the timed region runs."""
 
@@ -90,8 +98,9 @@ def _cpu_oracle_rate(cfg, inputs, target_s=12.0):
         oh.apply_h_rows(ps, miller, g2, vhat, cfg.grid, beta, d, rows=rows)
         return time.perf_counter() - t, rows.size
 
-    t1, r1 = run(32)
-    t2, r2 = run(128)
+    run(16)                 # thread-pool / page warm-up, not used
+    t1, r1 = run(64)
+    t2, r2 = run(256)
     per_row = max((t2 - t1) / (r2 - r1), 1e-9)
     fixed = max(t1 - per_row * r1, 0.0)
     r3 = int(min(ng, max(256, (target_s - fixed) / per_row)))
@@ -301,7 +310,8 @@ def run_ours(args):
         dom = max((k for k in kernels if "bound" in kernels[k]), key=lambda k: kernels[k]["share"])
         d = kernels[dom]
         roofline = {"kernel": dom, "bound": d["bound"], "achieved": d["achieved"], "peak": d["peak"],
-                    "unit": d["unit"], "frac": d["frac"], "traffic": None, "share_of_step": d["share"],
+                    "unit": d["unit"], "frac": d["frac"], "traffic": _ncu_traffic(cfg.name, dom),
+                    "share_of_step": d["share"],
                     "peak_source": ("FP64 DMMA m8n8k4 register-resident probe run in this process; DMMA and DFMA "
                                     "share this issue budget (MEASURED_PEAKS.json has no FP64 entry)"
                                     if d["bound"] in ("tensor", "alu") else peak_src)}

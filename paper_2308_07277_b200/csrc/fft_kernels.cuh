@@ -5,6 +5,7 @@
 //   k_zfwd  : a4(z)+a5  forward z-FFT, gather to the sphere, + 1/2|k+G|^2 psi_in
 #pragma once
 #include <cuda_runtime.h>
+#include <cstdio>
 #include "fft_phases.cuh"
 #include "async_copy.cuh"
 #include "qm_plan.h"
@@ -22,7 +23,7 @@ template <class C>
 __global__ void __launch_bounds__(QM_ZT * C::TT, 3)
 k_zinv(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ psi, c128 *__restrict__ W, int ntiles)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int LP = C::L | 1;
     c128 *lines = reinterpret_cast<c128 *>(smem_raw);
     const int tid = threadIdx.x;
@@ -52,7 +53,7 @@ __global__ void __launch_bounds__(QM_ZT * C::TT, 3)
 k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
        const c128 *__restrict__ psi_in, c128 *__restrict__ out, int ntiles, int kinetic)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int LP = C::L | 1;
     c128 *lines = reinterpret_cast<c128 *>(smem_raw);
     const int tid = threadIdx.x;
@@ -163,12 +164,19 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
         sbase = q.z;
         return make_pruned<C>((int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, u, 1);
     };
+#ifdef QM_PLANE_TIMING
+    long long tacc[5] = {0, 0, 0, 0, 0}, t0 = clock64(), t1;
+#define QM_TICK(i) do { t1 = clock64(); tacc[i] += t1 - t0; t0 = t1; } while (0)
+#else
+#define QM_TICK(i) do {} while (0)
+#endif
     // persistent loop over (band, z-plane) pairs: plane pl = band * n3 + p, its sticks are W[pl][0..S)
     for (int pl = blockIdx.x, it = 0; pl < nplanes; pl += gridDim.x, ++it) {
         const int band = pl / n3, p = pl - band * n3;
         c128 *Wp = W + (size_t)pl * S;
         if constexpr (MODE != 2) {
             mbar_wait(wbar, (uint32_t)(it & 1));
+            QM_TICK(0);
             for (int r = grp * TPG + slot; r - slot < X; r += ngroups * TPG) {
                 const bool ok = team_ok && r < X;
                 if (ok) {
@@ -182,6 +190,7 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
         }
         if (tid == 0) bulk_wait_read0();      // the previous plane's bulk store has read stage_out: scratch is free
         __syncthreads();
+        QM_TICK(1);
         {
             const int z = (p / gd.ax[2].r2) + gd.ax[2].r1 * (p % gd.ax[2].r2);
             c128 *myscr = scr + (size_t)(grp * TPG + team) * SL;
@@ -222,6 +231,7 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
         }
         fence_async_smem();                   // scratch was written through the generic proxy; bulk copies reuse it
         __syncthreads();
+        QM_TICK(2);
         if constexpr (MODE != 2) {            // the next plane's sticks arrive while this plane's y forward pass runs
             const int nxt = pl + gridDim.x;
             if (tid == 0 && nxt < nplanes) {
@@ -244,9 +254,15 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
             fence_async_smem();
             __syncthreads();
             if (tid == 0) { bulk_s2g(Wp, stage_out, wbytes); bulk_commit(); }
+            QM_TICK(3);
         } else {
             __syncthreads();                  // MODE 1: A is rewritten by the next plane's y backward pass
         }
     }
     if (tid == 0) bulk_wait0();
+#ifdef QM_PLANE_TIMING
+    QM_TICK(4);
+    if (tid == 0 && (blockIdx.x == 0 || blockIdx.x == 77 || blockIdx.x == 147))
+        printf("cta %d clk: wait %lld yback %lld x %lld yfwd %lld tail %lld\n", blockIdx.x, tacc[0], tacc[1], tacc[2], tacc[3], tacc[4]);
+#endif
 }
