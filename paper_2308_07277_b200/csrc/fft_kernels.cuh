@@ -111,43 +111,34 @@ template <int G> __device__ __forceinline__ void group_barrier(int grp) {
     else asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "r"(G) : "memory");
 }
 
-// Shared-memory carve-up of the plane kernel (bytes): plane array A | scratch lines, which double as the two
-// stick-plane staging buffers outside the x phase | row table | mbarrier.
-__host__ __device__ constexpr size_t qm_stage_elems(int S) { return ((size_t)S + 7) & ~(size_t)7; }   // 128-byte multiple
-
+// Persistent: a CTA walks the (band, z-plane) pairs pl = blockIdx.x, blockIdx.x + gridDim.x, ...  Between two x phases
+// the y-forward pass of the plane just finished and the y-backward pass of the next plane run as ONE loop over
+// row chunks (a row of the plane array is consumed and refilled by the same team), so there are two CTA-wide
+// barriers per plane.  The next plane's stick values of a row are fetched into registers (quarter rule,
+// prefetch_quarter) before the y-forward work of that row starts, which hides their latency.
 template <class C, int MODE>
 __global__ void __launch_bounds__(QM_PLANE_MAX_THREADS)
 k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ box, int ngroups, double scale,
-        int stagger_ns, int nplanes, int scr_elems)
+        int stagger_ns, int nplanes, int quarter)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int G = QM_GROUP;
     constexpr int SL = qm_scratch_pitch(C::L, C::TT);    // scratch line pitch
     constexpr int TPG = G / C::TT;                       // teams (lines) per group
     constexpr int RP = C::L | 1;                         // plane row pitch (== kp.rowpitch, host checks)
+    constexpr int NPRE = 2 * Quarter<C>::Q;
+    constexpr bool HAS_BACK = MODE != 2, HAS_FWD = MODE != 1;
     const int X = kp.nx, S = kp.nsticks;
     c128 *A = reinterpret_cast<c128 *>(smem_raw);
     c128 *scr = A + (((size_t)X * RP + 7) & ~(size_t)7);
-    c128 *stage_in = scr, *stage_out = scr + qm_stage_elems(S);      // valid outside the x phase only
-    int4 *rowinfo_s = reinterpret_cast<int4 *>(scr + scr_elems);
-    uint64_t *wbar = reinterpret_cast<uint64_t *>(rowinfo_s + X);
+    int4 *rowinfo_s = reinterpret_cast<int4 *>(scr + (size_t)ngroups * TPG * SL);
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int grp = tid / G, gl = tid % G;
     const int team = gl / C::TT, u = gl % C::TT;
     const bool team_ok = team < TPG;
     const int slot = qm_team_slot<C::TT, TPG>(team);     // line of the group's chunk this team works on
     const int n3 = gd.ax[2].n;
-    const uint32_t wbytes = (uint32_t)S * 16u;
-    const Pruned px = make_pruned<C>(kp.x_iv.x, kp.x_iv.y, kp.x_iv.z, kp.x_iv.w, u, RP);
 
-    if (tid == 0) {
-        mbar_init(wbar, 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        if constexpr (MODE != 2) {       // stick plane of the first (band, z-plane): one bulk copy, in flight during set-up
-            mbar_expect_tx(wbar, wbytes);
-            bulk_g2s(stage_in, W + (size_t)blockIdx.x * S, wbytes, wbar);
-        }
-    }
     // per-thread twiddle rows (u is fixed for the whole kernel)
     TwRow<C::R1> twa;
     load_twrow(twa, gd.tw[0], u, C::R2);
@@ -165,33 +156,50 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
         return make_pruned<C>((int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, u, 1);
     };
 #ifdef QM_PLANE_TIMING
-    long long tacc[5] = {0, 0, 0, 0, 0}, t0 = clock64(), t1;
+    long long tacc[3] = {0, 0, 0}, t0 = clock64(), t1;
 #define QM_TICK(i) do { t1 = clock64(); tacc[i] += t1 - t0; t0 = t1; } while (0)
 #else
 #define QM_TICK(i) do {} while (0)
 #endif
-    // persistent loop over (band, z-plane) pairs: plane pl = band * n3 + p, its sticks are W[pl][0..S)
-    for (int pl = blockIdx.x, it = 0; pl < nplanes; pl += gridDim.x, ++it) {
-        const int band = pl / n3, p = pl - band * n3;
-        c128 *Wp = W + (size_t)pl * S;
-        if constexpr (MODE != 2) {
-            mbar_wait(wbar, (uint32_t)(it & 1));
-            QM_TICK(0);
-            for (int r = grp * TPG + slot; r - slot < X; r += ngroups * TPG) {
+    const int row0 = grp * TPG + slot, rstride = ngroups * TPG;
+    for (int pl = blockIdx.x, prev = -1;; prev = pl, pl += gridDim.x) {
+        const bool have_cur = pl < nplanes;
+        const bool do_back = HAS_BACK && have_cur, do_fwd = HAS_FWD && prev >= 0;
+        // ---- merged y phase: y-forward of plane `prev`, y-backward of plane `pl`, row chunk by row chunk ----
+        if (do_back || do_fwd) {
+            const c128 *Wcur = W + (size_t)(have_cur ? pl : 0) * S;
+            c128 *Wprev = W + (size_t)(prev >= 0 ? prev : 0) * S;
+            for (int r = row0; r - slot < X; r += rstride) {
                 const bool ok = team_ok && r < X;
-                if (ok) {
-                    int sbase;
-                    const Pruned pr = row_pruned(r, sbase);
-                    prunedA_step1<C>(SpaceShared{}, stage_in + sbase, C::R2, pr, A + r * RP, u, twa);
+                int sbase = 0;
+                Pruned pr{0u, 0u, 0, 0};
+                if (ok) pr = row_pruned(r, sbase);
+                c128 pre[NPRE];
+                if (do_back && quarter && ok) prefetch_quarter<C>(SpaceGlobal{}, Wcur + sbase, C::R2, pr, pre);
+                if (do_fwd) {
+                    if (ok) lineB_step1<C>(A + r * RP, u, twb);
+                    group_barrier<G>(grp);
+                    if (ok) prunedB_step2<C>(SpaceGlobal{}, A + r * RP, Wprev + sbase, C::R2, pr, u);
                 }
-                group_barrier<G>(grp);
-                if (ok) lineA_step2<C>(A + r * RP, u);
+                if (do_back) {
+                    // the team that read row r in the step above is the one that refills it: no barrier needed
+                    if (ok) {
+                        if (quarter) prunedA_step1_pre<C>(pre, A + r * RP, u, twa);
+                        else prunedA_step1<C>(SpaceGlobal{}, Wcur + sbase, C::R2, pr, A + r * RP, u, twa);
+                    }
+                    group_barrier<G>(grp);
+                    if (ok) lineA_step2<C>(A + r * RP, u);
+                }
             }
         }
-        if (tid == 0) bulk_wait_read0();      // the previous plane's bulk store has read stage_out: scratch is free
+        if (!have_cur) break;
         __syncthreads();
-        QM_TICK(1);
+        QM_TICK(0);
+        // ---- x phase of plane `pl` ----
         {
+            // (re)derived per plane on purpose: keeping it live through the y phase costs registers there
+            const Pruned px = make_pruned<C>(kp.x_iv.x, kp.x_iv.y, kp.x_iv.z, kp.x_iv.w, u, RP);
+            const int band = pl / n3, p = pl - band * n3;
             const int z = (p / gd.ax[2].r2) + gd.ax[2].r1 * (p % gd.ax[2].r2);
             c128 *myscr = scr + (size_t)(grp * TPG + team) * SL;
             const double *vplane = gd.vt + (size_t)p * C::N * VLayout<C>::COL;
@@ -229,40 +237,12 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
                 }
             }
         }
-        fence_async_smem();                   // scratch was written through the generic proxy; bulk copies reuse it
         __syncthreads();
-        QM_TICK(2);
-        if constexpr (MODE != 2) {            // the next plane's sticks arrive while this plane's y forward pass runs
-            const int nxt = pl + gridDim.x;
-            if (tid == 0 && nxt < nplanes) {
-                fence_async_smem();
-                mbar_expect_tx(wbar, wbytes);
-                bulk_g2s(stage_in, W + (size_t)nxt * S, wbytes, wbar);
-            }
-        }
-        if constexpr (MODE != 1) {
-            for (int r = grp * TPG + slot; r - slot < X; r += ngroups * TPG) {
-                const bool ok = team_ok && r < X;
-                if (ok) lineB_step1<C>(A + r * RP, u, twb);
-                group_barrier<G>(grp);
-                if (ok) {
-                    int sbase;
-                    const Pruned pr = row_pruned(r, sbase);
-                    prunedB_step2<C>(SpaceShared{}, A + r * RP, stage_out + sbase, C::R2, pr, u);
-                }
-            }
-            fence_async_smem();
-            __syncthreads();
-            if (tid == 0) { bulk_s2g(Wp, stage_out, wbytes); bulk_commit(); }
-            QM_TICK(3);
-        } else {
-            __syncthreads();                  // MODE 1: A is rewritten by the next plane's y backward pass
-        }
+        QM_TICK(1);
     }
-    if (tid == 0) bulk_wait0();
 #ifdef QM_PLANE_TIMING
-    QM_TICK(4);
+    QM_TICK(2);
     if (tid == 0 && (blockIdx.x == 0 || blockIdx.x == 77 || blockIdx.x == 147))
-        printf("cta %d clk: wait %lld yback %lld x %lld yfwd %lld tail %lld\n", blockIdx.x, tacc[0], tacc[1], tacc[2], tacc[3], tacc[4]);
+        printf("cta %d clk: y %lld x %lld tail %lld\n", blockIdx.x, tacc[0], tacc[1], tacc[2]);
 #endif
 }

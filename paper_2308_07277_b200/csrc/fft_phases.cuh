@@ -158,6 +158,38 @@ QM_HD void prunedA_step1(SP sp, const c128 *src, int estride, const Pruned pr, c
         dst[k1 * C::R2P + u] = (k1 == 0) ? t[k1] : cmul_conj(t[k1], tw.template get<k1>());
     });
 }
+// "Quarter" form of the pruned backward step 1: when every occupied index lies below N/4 or at/above 3N/4
+// (true for every alias-free grid, 4 m + 1 <= n), only the first Q and the last Q first-pass inputs of a thread
+// can exist, Q = ceil(R1 / 4).  They are fetched ahead of time into 2Q registers (prefetch_quarter) and the
+// transform is started later from those registers (prunedA_step1_pre).
+template <class C> struct Quarter { static constexpr int Q = (C::R1 + 3) / 4; };
+template <class C, class SP>
+QM_HD void prefetch_quarter(SP sp, const c128 *src, int estride, const Pruned pr, c128 (&pre)[2 * Quarter<C>::Q]) {
+    constexpr int Q = Quarter<C>::Q;
+    const c128 *p1 = src + pr.c1, *p2 = src + pr.c2;
+    static_for<Q>([&](auto I) {
+        constexpr int j = decltype(I)::value;
+        pre[j] = ld_pred(sp, p1 + j * estride, (pr.m1 >> j) & 1u);
+        pre[Q + j] = ld_pred(sp, p2 + (C::R1 - Q + j) * estride, (pr.m2 >> (C::R1 - Q + j)) & 1u);
+    });
+}
+template <class C, class TW>
+QM_HD void prunedA_step1_pre(const c128 (&pre)[2 * Quarter<C>::Q], c128 *dst, int u, const TW &tw) {
+    if (u >= C::R2) return;
+    constexpr int Q = Quarter<C>::Q;
+    c128 t[C::R1];
+    static_for<C::R1>([&](auto I) {
+        constexpr int n1 = decltype(I)::value;
+        if constexpr (n1 < Q) t[n1] = pre[n1];
+        else if constexpr (n1 >= C::R1 - Q) t[n1] = pre[Q + n1 - (C::R1 - Q)];
+        else t[n1] = c128{0.0, 0.0};
+    });
+    Dft<C::R1, +1>::run(t);
+    static_for<C::R1>([&](auto I) {
+        constexpr int k1 = decltype(I)::value;
+        dst[k1 * C::R2P + u] = (k1 == 0) ? t[k1] : cmul_conj(t[k1], tw.template get<k1>());
+    });
+}
 // Forward step 2 with pruned output: reads the full padded line `srcline`, stores only what exists.
 template <class C, class SP>
 QM_HD void prunedB_step2(SP sp, const c128 *srcline, c128 *dst, int estride, const Pruned pr, int u) {

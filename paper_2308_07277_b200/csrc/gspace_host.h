@@ -52,6 +52,7 @@ struct QmKTables {
     std::vector<int4> stickinfo;               // per stick: packed occupied i3 intervals (a1|b1<<16, a2|b2<<16), first G, 0
     short4 xiv = {1, 0, 1, 0};                 // occupied i1 intervals (rows 0.. and following)
     bool x_contiguous = true;
+    bool y_quarter = false;                    // every occupied i2 of every row lies in the first / last quarter-block (fft_phases.cuh Quarter)
 };
 
 // returns 0, or -1 (sphere does not fit the grid) / -2 (empty sphere); msg gets the reason
@@ -180,6 +181,15 @@ static inline int qm_build_tables(const double *lattice, const double *recip, do
         if (span != kp->stickoff[s + 1] - kp->stickoff[s]) { *msg = "G of a stick are not two contiguous intervals"; return -1; }
         kp->stickinfo[s] = int4{(int)(unsigned short)iv.x | ((int)iv.y << 16), (int)(unsigned short)iv.z | ((int)iv.w << 16),
                                 kp->stickoff[s], 0};
+    }
+    {   // quarter rule for the plane kernel's register prefetch: i2 < Q*r2 or i2 >= (r1-Q)*r2, Q = ceil(r1/4)
+        const int q = (ax[1].r1 + 3) / 4;
+        kp->y_quarter = true;
+        for (int r = 0; r < nx; ++r) {
+            const short4 iv = kp->rowiv[r];
+            if (iv.x <= iv.y && iv.y >= q * ax[1].r2) kp->y_quarter = false;
+            if (iv.z <= iv.w && iv.z < (ax[1].r1 - q) * ax[1].r2) kp->y_quarter = false;
+        }
     }
     kp->stickapos.resize(S);
     for (int s = 0; s < S; ++s)

@@ -137,7 +137,7 @@ struct qm_gspace {
     int sm_count = 148;
     int max_smem = 0;
     int z_cta_per_sm = 3;           // resident z-kernel CTAs per SM the grid is sized for (QM_Z_CTA_PER_SM)
-    int plane_stagger_ns = 100;     // de-phasing delay between the plane kernel's groups (QM_PLANE_STAGGER_NS)
+    int plane_stagger_ns = 300;     // de-phasing delay between the plane kernel's groups (QM_PLANE_STAGGER_NS)
     ~qm_gspace() { for (auto *k : kpts) delete k; }
 };
 
@@ -161,16 +161,12 @@ int build_kpoint(qm_gspace *g, KPoint *kp) {
 }
 
 constexpr int PLANE_GROUP = QM_GROUP;
-size_t plane_scr_elems(const qm_gspace *g, const KPoint *kp, int ngroups) {
+size_t plane_smem(const qm_gspace *g, const KPoint *kp, int ngroups) {
     const QmAxis &ax = g->ax[0];
     const size_t sl = (size_t)qm_scratch_pitch(ax.len, std::max(ax.r1, ax.r2));
     const int tpg = PLANE_GROUP / std::max(ax.r1, ax.r2);
-    // scratch lines of the x phase; outside it the same region stages one stick plane in and one out
-    return (std::max((size_t)ngroups * tpg * sl, 2 * qm_stage_elems(kp->nsticks)) + 7) & ~(size_t)7;
-}
-size_t plane_smem(const qm_gspace *g, const KPoint *kp, int ngroups) {
     const size_t a_elems = ((size_t)kp->nx * kp->rowpitch + 7) & ~(size_t)7;
-    return (a_elems + plane_scr_elems(g, kp, ngroups)) * sizeof(c128) + (size_t)kp->nx * sizeof(int4) + 16;
+    return (a_elems + (size_t)ngroups * tpg * sl) * sizeof(c128) + (size_t)kp->nx * sizeof(int4) + 16;
 }
 
 // number of independent 64-thread groups of the plane kernel: the fewest groups that reach the
@@ -239,7 +235,7 @@ template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *bo
     g->prof.begin(QM_K_PLANE, st);
     k_plane<C, MODE><<<grid, ngroups * PLANE_GROUP, smem, st>>>(kp->plan(), gd, g->d_W.p, box, ngroups, scale,
                                                                    g->plane_stagger_ns, nplanes,
-                                                                   (int)plane_scr_elems(g, kp, ngroups));
+                                                                   kp->y_quarter ? 1 : 0);
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
