@@ -10,22 +10,26 @@
 #include "async_copy.cuh"
 #include "qm_plan.h"
 
-// z kernels.  A CTA owns tiles of QM_ZT adjacent sticks of one band (looping over tiles gridDim.x apart, so
-// the per-thread twiddle row is loaded once).  Both kernels are global -> registers -> first radix pass ->
-// shared memory -> second radix pass -> registers -> global: one shared-memory round trip, no zero fill, no
-// table-driven scatter (the G of a stick are two contiguous index runs, Pruned).  Thread mapping is
-// (stick, u) with u fastest where the sphere side is touched (contiguous psi runs) and (u, stick) with the
-// stick fastest where the stick planes W[p][S] are touched (contiguous 256-byte segments).
-constexpr int QM_ZT = 16;
-template <class C> __host__ __device__ constexpr int qm_z_threads() { return QM_ZT * C::TT; }
+// z kernels.  A CTA owns tiles of QM_ZT adjacent sticks of one band (looping over tiles gridDim.x apart, so the
+// per-thread twiddle row is loaded once).  The stick-plane workspace W is blocked by tile (WView): a tile's
+// N3 x QM_ZT block is contiguous and moves with ONE bulk asynchronous copy (TMA engine) through a shared-memory
+// staging buffer.  Sphere side: the G of a stick are two contiguous runs of psi (Pruned), loaded straight into
+// registers one tile ahead (quarter rule), no zero fill, no table-driven scatter.  Thread mapping is (stick, u)
+// with u fastest on the sphere side and (u, stick) with the stick fastest on the staging side.
+template <class C> __host__ __device__ constexpr size_t qm_z_smem() {
+    return ((size_t)QM_ZT * (C::L | 1) + (size_t)C::N * QM_ZT) * sizeof(c128) + 16;
+}
 
 template <class C>
-__global__ void __launch_bounds__(QM_ZT * C::TT, 3)
-k_zinv(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ psi, c128 *__restrict__ W, int ntiles)
+__global__ void __launch_bounds__(QM_ZT * C::TT, 2)
+k_zinv(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ psi, c128 *__restrict__ W, int ntiles,
+       int quarter)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int LP = C::L | 1;
-    c128 *lines = reinterpret_cast<c128 *>(smem_raw);
+    constexpr int NPRE = 2 * Quarter<C>::Q;
+    c128 *stage = reinterpret_cast<c128 *>(smem_raw);                 // [N][QM_ZT], 128-byte aligned
+    c128 *lines = stage + (size_t)C::N * QM_ZT;
     const int tid = threadIdx.x;
     const int S = kp.nsticks, band = blockIdx.y;
     const int t1 = tid / C::TT, u1 = tid % C::TT;      // pass 1: u fastest
@@ -33,47 +37,85 @@ k_zinv(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ psi,
     TwRow<C::R1> twa;
     load_twrow(twa, tw, u1, C::R2);
     const c128 *psib = psi + (size_t)band * kp.ng;
-    c128 *Wb = W + (size_t)band * C::N * S;
+    c128 *Wb = W + (size_t)band * ntiles * C::N * QM_ZT;
+    auto info = [&](int tile) {
+        const int s = tile * QM_ZT + t1;
+        return (tile < ntiles && s < S) ? kp.stick_info[s] : int4{1, 1, 0, 0};   // both intervals empty
+    };
+    auto pruned_of = [&](const int4 q) {
+        return make_pruned<C>((int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, u1, 1);
+    };
+    int4 q = info(blockIdx.x), qn = info(blockIdx.x + gridDim.x);
+    Pruned pr = pruned_of(q);
+    c128 pre[NPRE];
+    if (quarter) prefetch_quarter<C>(SpaceGlobal{}, psib + q.z, C::R2, pr, pre);
     for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const int s0 = tile * QM_ZT;
-        const int ns = min(QM_ZT, S - s0);
+        const int ns = min(QM_ZT, S - tile * QM_ZT);
         if (t1 < ns) {
-            const int4 q = kp.stick_info[s0 + t1];
-            const Pruned pr = make_pruned<C>((int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, u1, 1);
-            prunedA_step1<C>(SpaceGlobal{}, psib + q.z, C::R2, pr, lines + t1 * LP, u1, twa);
+            if (quarter) prunedA_step1_pre<C>(pre, lines + t1 * LP, u1, twa);
+            else prunedA_step1<C>(SpaceGlobal{}, psib + q.z, C::R2, pr, lines + t1 * LP, u1, twa);
         }
+        // advance the two-deep prefetch: data of the next tile, table entry of the one after
+        q = qn; pr = pruned_of(q);
+        if (quarter) prefetch_quarter<C>(SpaceGlobal{}, psib + q.z, C::R2, pr, pre);
+        qn = info(tile + 2 * gridDim.x);
+        if (tid == 0) bulk_wait_read0();      // the previous tile's bulk store has read the staging buffer
         __syncthreads();
-        if (t2 < ns) zinv_step2_store<C>(lines + t2 * LP, Wb + s0 + t2, S, u2);
+        if (t2 < ns) zinv_step2_store<C>(lines + t2 * LP, stage + t2, QM_ZT, u2);
+        fence_async_smem();
         __syncthreads();
+        if (tid == 0) { bulk_s2g(Wb + (size_t)tile * C::N * QM_ZT, stage, (uint32_t)(C::N * QM_ZT * sizeof(c128))); bulk_commit(); }
     }
+    if (tid == 0) bulk_wait0();
 }
 
 template <class C>
-__global__ void __launch_bounds__(QM_ZT * C::TT, 3)
+__global__ void __launch_bounds__(QM_ZT * C::TT, 2)
 k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
-       const c128 *__restrict__ psi_in, c128 *__restrict__ out, int ntiles, int kinetic)
+       const c128 *__restrict__ psi_in, c128 *__restrict__ out, int ntiles, int kinetic, int quarter)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int LP = C::L | 1;
-    c128 *lines = reinterpret_cast<c128 *>(smem_raw);
+    constexpr int NPRE = 2 * Quarter<C>::Q;
+    constexpr uint32_t TILE_BYTES = (uint32_t)(C::N * QM_ZT * sizeof(c128));
+    c128 *stage = reinterpret_cast<c128 *>(smem_raw);                 // [N][QM_ZT]
+    c128 *lines = stage + (size_t)C::N * QM_ZT;
+    uint64_t *wbar = reinterpret_cast<uint64_t *>(lines + (size_t)QM_ZT * LP);
     const int tid = threadIdx.x;
     const int S = kp.nsticks, band = blockIdx.y;
     const int t1 = tid / C::TT, u1 = tid % C::TT;      // pass 2 (gather side): u fastest
-    const int t2 = tid % QM_ZT, u2 = tid / QM_ZT;      // pass 1 (stick-plane side): stick fastest
+    const int t2 = tid % QM_ZT, u2 = tid / QM_ZT;      // pass 1 (staging side): stick fastest
+    const c128 *Wb = W + (size_t)band * ntiles * C::N * QM_ZT;
+    if (tid == 0) {
+        mbar_init(wbar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_expect_tx(wbar, TILE_BYTES);
+        bulk_g2s(stage, Wb + (size_t)blockIdx.x * C::N * QM_ZT, TILE_BYTES, wbar);
+    }
     TwRow<C::R2> twb;
     load_twrow(twb, tw, u2, C::R1);
-    const c128 *Wb = W + (size_t)band * C::N * S;
     const size_t boff = (size_t)band * kp.ng;
-    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const int s0 = tile * QM_ZT;
-        const int ns = min(QM_ZT, S - s0);
-        if (t2 < ns) zfwd_step1_load<C>(Wb + s0 + t2, S, lines + t2 * LP, u2, twb);
-        __syncthreads();
+    __syncthreads();
+    for (int tile = blockIdx.x, it = 0; tile < ntiles; tile += gridDim.x, ++it) {
+        const int ns = min(QM_ZT, S - tile * QM_ZT);
+        // gather-side inputs of this tile: in flight behind the wait and the first pass
+        int4 q = int4{1, 1, 0, 0};             // both intervals empty
+        if (t1 < ns) q = kp.stick_info[tile * QM_ZT + t1];
+        const Pruned pr = make_pruned<C>((int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, u1, 1);
+        c128 kin[NPRE];
+        if (quarter) prefetch_kin<C>(psi_in + boff + q.z, kp.g2 + q.z, pr, kinetic != 0 && t1 < ns, kin);
+        mbar_wait(wbar, (uint32_t)(it & 1));
+        zfwd_step1_load<C>(stage + t2, QM_ZT, lines + t2 * LP, u2, twb);
+        __syncthreads();                       // staging buffer consumed, lines complete
+        if (tid == 0 && tile + (int)gridDim.x < ntiles) {
+            fence_async_smem();
+            mbar_expect_tx(wbar, TILE_BYTES);
+            bulk_g2s(stage, Wb + (size_t)(tile + gridDim.x) * C::N * QM_ZT, TILE_BYTES, wbar);
+        }
         if (t1 < ns) {
-            const int4 q = kp.stick_info[s0 + t1];
-            const Pruned pr = make_pruned<C>((int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, u1, 1);
-            zfwd_step2_gather<C>(lines + t1 * LP, out + boff + q.z, kinetic ? psi_in + boff + q.z : nullptr, kp.g2 + q.z, pr, u1,
-                                 kinetic != 0);
+            if (quarter) zfwd_step2_gather_pre<C>(lines + t1 * LP, out + boff + q.z, pr, u1, kin);
+            else zfwd_step2_gather<C>(lines + t1 * LP, out + boff + q.z, kinetic ? psi_in + boff + q.z : nullptr, kp.g2 + q.z,
+                                      pr, u1, kinetic != 0);
         }
         __syncthreads();
     }
@@ -116,6 +158,136 @@ template <int G> __device__ __forceinline__ void group_barrier(int grp) {
 // row chunks (a row of the plane array is consumed and refilled by the same team), so there are two CTA-wide
 // barriers per plane.  The next plane's stick values of a row are fetched into registers (quarter rule,
 // prefetch_quarter) before the y-forward work of that row starts, which hides their latency.
+// The two phases are separate __noinline__ functions on purpose: each gets its own register allocation (the
+// x loop sits at the 168-register cap and is sensitive to anything else that is live); the per-thread twiddle
+// rows are re-read from a shared-memory copy of the table at the start of each phase.
+struct PlaneCtx {
+    c128 *A, *scr;
+    const int4 *rowinfo_s;
+    const c128 *tw_s;
+    int X, ngroups, n3, quarter;
+    size_t wband;
+};
+template <class C> struct PlaneIds {
+    static constexpr int G = QM_GROUP, TPG = G / C::TT;
+    int grp, team, u, slot; bool team_ok;
+    __device__ PlaneIds() {
+        const int tid = threadIdx.x, gl = tid % G;
+        grp = tid / G; team = gl / C::TT; u = gl % C::TT;
+        team_ok = team < TPG;
+        slot = qm_team_slot<C::TT, TPG>(team);
+    }
+};
+
+template <class C, int MODE>
+__device__ __forceinline__ void plane_y_phase(const PlaneCtx cx, c128 *__restrict__ W, int pl, int prev, bool have_cur)
+{
+    constexpr int G = QM_GROUP, TPG = G / C::TT, RP = C::L | 1, NPRE = 2 * Quarter<C>::Q;
+    constexpr bool HAS_BACK = MODE != 2, HAS_FWD = MODE != 1;
+    const PlaneIds<C> id;
+    const int u = id.u, grp = id.grp, slot = id.slot, X = cx.X, n3 = cx.n3, quarter = cx.quarter;
+    const bool do_back = HAS_BACK && have_cur, do_fwd = HAS_FWD && prev >= 0;
+    if (!(do_back || do_fwd)) return;
+    TwRow<C::R1> twa;
+    load_twrow(twa, cx.tw_s, u, C::R2);
+    TwRow<C::R2> twb_store;
+    if constexpr (C::R1 != C::R2) load_twrow(twb_store, cx.tw_s, u, C::R1);
+    const auto &twb = [&]() -> const TwRow<C::R2> & {
+        if constexpr (C::R1 == C::R2) return twa; else return twb_store;
+    }();
+    c128 *A = cx.A;
+    const int pc = have_cur ? pl : 0, pp = prev >= 0 ? prev : 0;
+    const WView Wcur = qm_wview(W + (size_t)(pc / n3) * cx.wband, pc % n3, n3);
+    const WView Wprev = qm_wview(W + (size_t)(pp / n3) * cx.wband, pp % n3, n3);
+    for (int r = grp * TPG + slot; r - slot < X; r += cx.ngroups * TPG) {
+        const bool ok = id.team_ok && r < X;
+        int sbase = 0;
+        Pruned pr{0u, 0u, 0, 0};
+        if (ok) {
+            const int4 q = cx.rowinfo_s[r];
+            sbase = q.z;
+            pr = make_pruned<C>((int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, u, 1);
+        }
+        c128 pre[NPRE];
+        if (do_back && quarter && ok) prefetch_quarter<C>(SpaceGlobal{}, Wcur + sbase, C::R2, pr, pre);
+        if (do_fwd) {
+            if (ok) lineB_step1<C>(A + r * RP, u, twb);
+            group_barrier<G>(grp);
+            if (ok) {
+                if (quarter) prunedB_step2_quarter<C>(SpaceGlobal{}, A + r * RP, Wprev + sbase, C::R2, pr, u);
+                else prunedB_step2<C>(SpaceGlobal{}, A + r * RP, Wprev + sbase, C::R2, pr, u);
+            }
+        }
+        if (do_back) {
+            // the team that read row r in the step above is the one that refills it: no barrier needed
+            if (ok) {
+                if (quarter) prunedA_step1_pre<C>(pre, A + r * RP, u, twa);
+                else prunedA_step1<C>(SpaceGlobal{}, Wcur + sbase, C::R2, pr, A + r * RP, u, twa);
+            }
+            group_barrier<G>(grp);
+            if (ok) lineA_step2<C>(A + r * RP, u);
+        }
+    }
+}
+
+template <class C, int MODE>
+__device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_iv, const double *__restrict__ vt,
+                                           c128 *__restrict__ box, int pl, double scale, int stagger_ns)
+{
+    constexpr int G = QM_GROUP, TPG = G / C::TT, RP = C::L | 1;
+    constexpr int SL = qm_scratch_pitch(C::L, C::TT);    // scratch line pitch
+    const PlaneIds<C> id;
+    const int u = id.u, grp = id.grp, slot = id.slot, n3 = cx.n3, ngroups = cx.ngroups;
+    const bool team_ok = id.team_ok;
+    TwRow<C::R1> twa;
+    load_twrow(twa, cx.tw_s, u, C::R2);
+    TwRow<C::R2> twb_store;
+    if constexpr (C::R1 != C::R2) load_twrow(twb_store, cx.tw_s, u, C::R1);
+    const auto &twb = [&]() -> const TwRow<C::R2> & {
+        if constexpr (C::R1 == C::R2) return twa; else return twb_store;
+    }();
+    c128 *A = cx.A;
+    const Pruned px = make_pruned<C>(x_iv.x, x_iv.y, x_iv.z, x_iv.w, u, RP);
+    const int band = pl / n3, p = pl - band * n3;
+    c128 *myscr = cx.scr + (size_t)(grp * TPG + id.team) * SL;
+    const double *vplane = vt + (size_t)p * C::N * VLayout<C>::COL;
+    VRow<C::R2> vr;
+    // De-phase the groups: they all do identical load -> FP64 -> store bursts, and when they run in
+    // lock step the shared-memory pipe and the FP64 pipe are used alternately instead of together.
+    if (stagger_ns > 0) __nanosleep((unsigned)(grp * stagger_ns));
+    const int col0 = grp * TPG + slot;
+    if constexpr (MODE == 0) {       // V of the first column: in flight while step 1 runs
+        if (team_ok && col0 < C::N) load_vrow<C>(vr, vplane + (size_t)col0 * VLayout<C>::COL, u);
+    }
+    for (int col = col0; col - slot < C::N; col += ngroups * TPG) {
+        const bool ok = team_ok && col < C::N;
+        c128 *Acol = A + C::pos(col);
+        if constexpr (MODE != 2) {
+            if (ok) prunedA_step1<C>(SpaceShared{}, Acol, C::R2 * RP, px, myscr, u, twa);
+            group_barrier<G>(grp);
+        }
+        if (ok) {
+            c128 *bx = nullptr;
+            if constexpr (MODE != 0) {
+                const int y = (col / C::R2) + C::R1 * (col % C::R2);
+                bx = box + (size_t)band * C::N * C::N * n3 + (size_t)y * n3;     // + z added by the caller through `box`
+            }
+            xcol_step2<C, MODE>(myscr, u, twb, vr, bx, (long)C::N * n3, scale);
+        }
+        if constexpr (MODE == 0) {   // prefetch V of this team's next column behind steps 3 and 1
+            const int ncol = col + ngroups * TPG;
+            if (team_ok && ncol < C::N) load_vrow<C>(vr, vplane + (size_t)ncol * VLayout<C>::COL, u);
+        }
+        group_barrier<G>(grp);
+        if constexpr (MODE != 1) {
+            // no barrier after step 3: the scratch column a thread reads here is exactly the one it
+            // overwrites in the next iteration's step 1 (MODE 2 has no step 1 and writes rows: barrier).
+            if (ok) prunedB_step2<C>(SpaceShared{}, myscr, Acol, C::R2 * RP, px, u);
+            if constexpr (MODE == 2) group_barrier<G>(grp);
+        }
+    }
+}
+
 template <class C, int MODE>
 __global__ void __launch_bounds__(QM_PLANE_MAX_THREADS)
 k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ box, int ngroups, double scale,
@@ -123,126 +295,42 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int G = QM_GROUP;
-    constexpr int SL = qm_scratch_pitch(C::L, C::TT);    // scratch line pitch
-    constexpr int TPG = G / C::TT;                       // teams (lines) per group
+    constexpr int SL = qm_scratch_pitch(C::L, C::TT);
+    constexpr int TPG = G / C::TT;
     constexpr int RP = C::L | 1;                         // plane row pitch (== kp.rowpitch, host checks)
-    constexpr int NPRE = 2 * Quarter<C>::Q;
-    constexpr bool HAS_BACK = MODE != 2, HAS_FWD = MODE != 1;
-    const int X = kp.nx, S = kp.nsticks;
-    c128 *A = reinterpret_cast<c128 *>(smem_raw);
-    c128 *scr = A + (((size_t)X * RP + 7) & ~(size_t)7);
-    int4 *rowinfo_s = reinterpret_cast<int4 *>(scr + (size_t)ngroups * TPG * SL);
-    const int tid = threadIdx.x, nthr = blockDim.x;
-    const int grp = tid / G, gl = tid % G;
-    const int team = gl / C::TT, u = gl % C::TT;
-    const bool team_ok = team < TPG;
-    const int slot = qm_team_slot<C::TT, TPG>(team);     // line of the group's chunk this team works on
-    const int n3 = gd.ax[2].n;
-
-    // per-thread twiddle rows (u is fixed for the whole kernel)
-    TwRow<C::R1> twa;
-    load_twrow(twa, gd.tw[0], u, C::R2);
-    TwRow<C::R2> twb_store;
-    if constexpr (C::R1 != C::R2) load_twrow(twb_store, gd.tw[0], u, C::R1);
-    const auto &twb = [&]() -> const TwRow<C::R2> & {
-        if constexpr (C::R1 == C::R2) return twa; else return twb_store;
-    }();
-
-    for (int i = tid; i < X; i += nthr) rowinfo_s[i] = kp.row_info[i];
+    PlaneCtx cx;
+    cx.X = kp.nx; cx.ngroups = ngroups; cx.n3 = gd.ax[2].n; cx.quarter = quarter;
+    cx.wband = (size_t)((kp.nsticks + QM_ZT - 1) / QM_ZT) * QM_ZT * gd.ax[2].n;   // W elements per band
+    cx.A = reinterpret_cast<c128 *>(smem_raw);
+    cx.scr = cx.A + (((size_t)cx.X * RP + 7) & ~(size_t)7);
+    c128 *tw_s = cx.scr + (size_t)ngroups * TPG * SL;
+    int4 *rowinfo_s = reinterpret_cast<int4 *>(tw_s + C::N);
+    cx.tw_s = tw_s; cx.rowinfo_s = rowinfo_s;
+    for (int i = threadIdx.x; i < cx.X; i += blockDim.x) rowinfo_s[i] = kp.row_info[i];
+    for (int i = threadIdx.x; i < C::N; i += blockDim.x) tw_s[i] = gd.tw[0][i];
     __syncthreads();
-    auto row_pruned = [&](int r, int &sbase) {
-        const int4 q = rowinfo_s[r];
-        sbase = q.z;
-        return make_pruned<C>((int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, u, 1);
-    };
 #ifdef QM_PLANE_TIMING
     long long tacc[3] = {0, 0, 0}, t0 = clock64(), t1;
 #define QM_TICK(i) do { t1 = clock64(); tacc[i] += t1 - t0; t0 = t1; } while (0)
 #else
 #define QM_TICK(i) do {} while (0)
 #endif
-    const int row0 = grp * TPG + slot, rstride = ngroups * TPG;
+    const int n3 = cx.n3;
     for (int pl = blockIdx.x, prev = -1;; prev = pl, pl += gridDim.x) {
         const bool have_cur = pl < nplanes;
-        const bool do_back = HAS_BACK && have_cur, do_fwd = HAS_FWD && prev >= 0;
-        // ---- merged y phase: y-forward of plane `prev`, y-backward of plane `pl`, row chunk by row chunk ----
-        if (do_back || do_fwd) {
-            const c128 *Wcur = W + (size_t)(have_cur ? pl : 0) * S;
-            c128 *Wprev = W + (size_t)(prev >= 0 ? prev : 0) * S;
-            for (int r = row0; r - slot < X; r += rstride) {
-                const bool ok = team_ok && r < X;
-                int sbase = 0;
-                Pruned pr{0u, 0u, 0, 0};
-                if (ok) pr = row_pruned(r, sbase);
-                c128 pre[NPRE];
-                if (do_back && quarter && ok) prefetch_quarter<C>(SpaceGlobal{}, Wcur + sbase, C::R2, pr, pre);
-                if (do_fwd) {
-                    if (ok) lineB_step1<C>(A + r * RP, u, twb);
-                    group_barrier<G>(grp);
-                    if (ok) prunedB_step2<C>(SpaceGlobal{}, A + r * RP, Wprev + sbase, C::R2, pr, u);
-                }
-                if (do_back) {
-                    // the team that read row r in the step above is the one that refills it: no barrier needed
-                    if (ok) {
-                        if (quarter) prunedA_step1_pre<C>(pre, A + r * RP, u, twa);
-                        else prunedA_step1<C>(SpaceGlobal{}, Wcur + sbase, C::R2, pr, A + r * RP, u, twa);
-                    }
-                    group_barrier<G>(grp);
-                    if (ok) lineA_step2<C>(A + r * RP, u);
-                }
-            }
-        }
+        plane_y_phase<C, MODE>(cx, W, pl, prev, have_cur);
         if (!have_cur) break;
         __syncthreads();
         QM_TICK(0);
-        // ---- x phase of plane `pl` ----
-        {
-            // (re)derived per plane on purpose: keeping it live through the y phase costs registers there
-            const Pruned px = make_pruned<C>(kp.x_iv.x, kp.x_iv.y, kp.x_iv.z, kp.x_iv.w, u, RP);
-            const int band = pl / n3, p = pl - band * n3;
-            const int z = (p / gd.ax[2].r2) + gd.ax[2].r1 * (p % gd.ax[2].r2);
-            c128 *myscr = scr + (size_t)(grp * TPG + team) * SL;
-            const double *vplane = gd.vt + (size_t)p * C::N * VLayout<C>::COL;
-            VRow<C::R2> vr;
-            // De-phase the groups: they all do identical load -> FP64 -> store bursts, and when they run in
-            // lock step the shared-memory pipe and the FP64 pipe are used alternately instead of together.
-            if (stagger_ns > 0) __nanosleep((unsigned)(grp * stagger_ns));
-            const int col0 = grp * TPG + slot;
-            if constexpr (MODE == 0) {       // V of the first column: in flight while step 1 runs
-                if (team_ok && col0 < C::N) load_vrow<C>(vr, vplane + (size_t)col0 * VLayout<C>::COL, u);
-            }
-            for (int col = col0; col - slot < C::N; col += ngroups * TPG) {
-                const bool ok = team_ok && col < C::N;
-                c128 *Acol = A + C::pos(col);
-                if constexpr (MODE != 2) {
-                    if (ok) prunedA_step1<C>(SpaceShared{}, Acol, C::R2 * RP, px, myscr, u, twa);
-                    group_barrier<G>(grp);
-                }
-                if (ok) {
-                    const int y = (col / C::R2) + C::R1 * (col % C::R2);
-                    c128 *bx = nullptr;
-                    if constexpr (MODE != 0) bx = box + (size_t)band * C::N * C::N * n3 + (size_t)y * n3 + z;
-                    xcol_step2<C, MODE>(myscr, u, twb, vr, bx, (long)C::N * n3, scale);
-                }
-                if constexpr (MODE == 0) {   // prefetch V of this team's next column behind steps 3 and 1
-                    const int ncol = col + ngroups * TPG;
-                    if (team_ok && ncol < C::N) load_vrow<C>(vr, vplane + (size_t)ncol * VLayout<C>::COL, u);
-                }
-                group_barrier<G>(grp);
-                if constexpr (MODE != 1) {
-                    // no barrier after step 3: the scratch column a thread reads here is exactly the one it
-                    // overwrites in the next iteration's step 1 (MODE 2 has no step 1 and writes rows: barrier).
-                    if (ok) prunedB_step2<C>(SpaceShared{}, myscr, Acol, C::R2 * RP, px, u);
-                    if constexpr (MODE == 2) group_barrier<G>(grp);
-                }
-            }
-        }
+        const int p = pl % n3;
+        const int z = (p / gd.ax[2].r2) + gd.ax[2].r1 * (p % gd.ax[2].r2);
+        plane_x_phase<C, MODE>(cx, kp.x_iv, gd.vt, box ? box + z : nullptr, pl, scale, stagger_ns);
         __syncthreads();
         QM_TICK(1);
     }
 #ifdef QM_PLANE_TIMING
     QM_TICK(2);
-    if (tid == 0 && (blockIdx.x == 0 || blockIdx.x == 77 || blockIdx.x == 147))
+    if (threadIdx.x == 0 && (blockIdx.x == 0 || blockIdx.x == 77 || blockIdx.x == 147))
         printf("cta %d clk: y %lld x %lld tail %lld\n", blockIdx.x, tacc[0], tacc[1], tacc[2]);
 #endif
 }

@@ -100,6 +100,22 @@ template <class C> QM_HD Pruned make_pruned(int a1, int b1, int a2, int b2, int 
     return Pruned{qm_range_mask(a1, b1, u, C::R2, C::R1), qm_range_mask(a2, b2, u, C::R2, C::R1),
                   (u - a1) * stride, (u - a2 + cnt1) * stride};
 }
+// Stick-plane workspace W of one band, blocked by tiles of QM_ZT sticks: element (plane label p, stick s) lives at
+// base[((s / QM_ZT) * n3 + p) * QM_ZT + s % QM_ZT].  A tile's N3 x QM_ZT block is contiguous (what the z kernels move
+// with one bulk copy); the plane kernel addresses single elements through this pointer-like view (p fixed).
+constexpr int QM_ZT = 16;
+struct WView {
+    c128 *base;            // element (p, stick 0) of the band: band base + p * QM_ZT
+    unsigned tstride;      // elements between consecutive tiles: n3 * QM_ZT
+    int s;                 // stick
+    QM_HD WView operator+(int e) const { return WView{base, tstride, s + e}; }
+    QM_HD c128 *ptr() const { const unsigned us = (unsigned)s; return base + ((us / QM_ZT) * tstride + (us % QM_ZT)); }
+};
+QM_HD WView qm_wview(c128 *band_base, int p, int n3) { return WView{band_base + p * QM_ZT, (unsigned)(n3 * QM_ZT), 0}; }
+QM_HD const c128 *qm_ptr(const c128 *p) { return p; }
+QM_HD c128 *qm_ptr(c128 *p) { return p; }
+QM_HD c128 *qm_ptr(const WView &w) { return w.ptr(); }
+
 // predicated 16-byte accesses (no branch, no address arithmetic beyond base + immediate)
 struct SpaceShared {}; struct SpaceGlobal {};
 QM_HD c128 ld_pred(SpaceShared, const c128 *p, bool pred) {
@@ -142,15 +158,22 @@ QM_HD void st_pred(SpaceGlobal, c128 *p, c128 v, bool pred) {
 }
 // Backward step 1 with pruned input: src = first stored element of the line, estride = R2*stride (elements
 // between n and n+1); writes the full padded line `dst`.
-template <class C, class SP, class TW>
-QM_HD void prunedA_step1(SP sp, const c128 *src, int estride, const Pruned pr, c128 *dst, int u, const TW &tw) {
+template <class C, class SP, class P, class TW>
+QM_HD void prunedA_step1(SP sp, const P src, int estride, const Pruned pr, c128 *dst, int u, const TW &tw) {
     if (u >= C::R2) return;
     c128 t[C::R1];
-    const c128 *p1 = src + pr.c1, *p2 = src + pr.c2;
+    // interval 1 lies below N/2 and interval 2 at or above it (host tables), so for most n1 the interval is
+    // known at compile time and the access is base + immediate under one mask-bit test
+    const P p1 = src + pr.c1, p2 = src + pr.c2;
+    const unsigned mm = pr.m1 | pr.m2;
     static_for<C::R1>([&](auto I) {
         constexpr int n1 = decltype(I)::value;
-        const bool in2 = (pr.m2 >> n1) & 1u, in1 = (pr.m1 >> n1) & 1u;
-        t[n1] = ld_pred(sp, (in2 ? p2 : p1) + n1 * estride, in1 || in2);
+        if constexpr (2 * (n1 + 1) * C::R2 <= C::N) t[n1] = ld_pred(sp, qm_ptr(p1 + n1 * estride), (mm & (1u << n1)) != 0u);
+        else if constexpr (2 * n1 * C::R2 >= C::N) t[n1] = ld_pred(sp, qm_ptr(p2 + n1 * estride), (mm & (1u << n1)) != 0u);
+        else {
+            const bool in2 = (pr.m2 >> n1) & 1u;
+            t[n1] = ld_pred(sp, qm_ptr((in2 ? p2 : p1) + n1 * estride), (mm & (1u << n1)) != 0u);
+        }
     });
     Dft<C::R1, +1>::run(t);
     static_for<C::R1>([&](auto I) {
@@ -163,14 +186,14 @@ QM_HD void prunedA_step1(SP sp, const c128 *src, int estride, const Pruned pr, c
 // can exist, Q = ceil(R1 / 4).  They are fetched ahead of time into 2Q registers (prefetch_quarter) and the
 // transform is started later from those registers (prunedA_step1_pre).
 template <class C> struct Quarter { static constexpr int Q = (C::R1 + 3) / 4; };
-template <class C, class SP>
-QM_HD void prefetch_quarter(SP sp, const c128 *src, int estride, const Pruned pr, c128 (&pre)[2 * Quarter<C>::Q]) {
+template <class C, class SP, class P>
+QM_HD void prefetch_quarter(SP sp, const P src, int estride, const Pruned pr, c128 (&pre)[2 * Quarter<C>::Q]) {
     constexpr int Q = Quarter<C>::Q;
-    const c128 *p1 = src + pr.c1, *p2 = src + pr.c2;
+    const P p1 = src + pr.c1, p2 = src + pr.c2;
     static_for<Q>([&](auto I) {
         constexpr int j = decltype(I)::value;
-        pre[j] = ld_pred(sp, p1 + j * estride, (pr.m1 >> j) & 1u);
-        pre[Q + j] = ld_pred(sp, p2 + (C::R1 - Q + j) * estride, (pr.m2 >> (C::R1 - Q + j)) & 1u);
+        pre[j] = ld_pred(sp, qm_ptr(p1 + j * estride), (pr.m1 >> j) & 1u);
+        pre[Q + j] = ld_pred(sp, qm_ptr(p2 + (C::R1 - Q + j) * estride), (pr.m2 >> (C::R1 - Q + j)) & 1u);
     });
 }
 template <class C, class TW>
@@ -191,17 +214,38 @@ QM_HD void prunedA_step1_pre(const c128 (&pre)[2 * Quarter<C>::Q], c128 *dst, in
     });
 }
 // Forward step 2 with pruned output: reads the full padded line `srcline`, stores only what exists.
-template <class C, class SP>
-QM_HD void prunedB_step2(SP sp, const c128 *srcline, c128 *dst, int estride, const Pruned pr, int u) {
+template <class C, class SP, class P>
+QM_HD void prunedB_step2(SP sp, const c128 *srcline, const P dst, int estride, const Pruned pr, int u) {
     if (u >= C::R2) return;
     c128 t[C::R1];
     static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = srcline[a * C::R2P + u]; });
     Dft<C::R1, -1>::run(t);
-    c128 *p1 = dst + pr.c1, *p2 = dst + pr.c2;
+    const P p1 = dst + pr.c1, p2 = dst + pr.c2;
+    const unsigned mm = pr.m1 | pr.m2;
     static_for<C::R1>([&](auto I) {
         constexpr int c = decltype(I)::value;
-        const bool in2 = (pr.m2 >> c) & 1u, in1 = (pr.m1 >> c) & 1u;
-        st_pred(sp, (in2 ? p2 : p1) + c * estride, t[c], in1 || in2);
+        if constexpr (2 * (c + 1) * C::R2 <= C::N) st_pred(sp, qm_ptr(p1 + c * estride), t[c], (mm & (1u << c)) != 0u);
+        else if constexpr (2 * c * C::R2 >= C::N) st_pred(sp, qm_ptr(p2 + c * estride), t[c], (mm & (1u << c)) != 0u);
+        else {
+            const bool in2 = (pr.m2 >> c) & 1u;
+            st_pred(sp, qm_ptr((in2 ? p2 : p1) + c * estride), t[c], (mm & (1u << c)) != 0u);
+        }
+    });
+}
+// Quarter-rule form of the pruned forward step 2: only the first Q and last Q outputs of a thread can exist.
+template <class C, class SP, class P>
+QM_HD void prunedB_step2_quarter(SP sp, const c128 *srcline, const P dst, int estride, const Pruned pr, int u) {
+    if (u >= C::R2) return;
+    constexpr int Q = Quarter<C>::Q;
+    c128 t[C::R1];
+    static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = srcline[a * C::R2P + u]; });
+    Dft<C::R1, -1>::run(t);
+    const P p1 = dst + pr.c1, p2 = dst + pr.c2;
+    static_for<Q>([&](auto I) {
+        constexpr int j = decltype(I)::value;
+        constexpr int c2 = C::R1 - Q + j;
+        st_pred(sp, qm_ptr(p1 + j * estride), t[j], (pr.m1 >> j) & 1u);
+        st_pred(sp, qm_ptr(p2 + c2 * estride), t[c2], (pr.m2 >> c2) & 1u);
     });
 }
 
@@ -278,6 +322,36 @@ template <class C> QM_HD void zfwd_step2_gather(const c128 *line, c128 *out, con
             if (kinetic) { const double h = 0.5 * g2[off]; const c128 x = psi_in[off]; v.x = fma(h, x.x, v.x); v.y = fma(h, x.y, v.y); }
             out[off] = v;
         }
+    });
+}
+
+// Quarter-rule forms of the gather (see Quarter): the 1/2|k+G|^2 psi_in terms of the <= 2Q outputs a thread can
+// own are fetched ahead of the transform (prefetch_kin) and added when the outputs are stored.
+template <class C> QM_HD void prefetch_kin(const c128 *psi_in, const double *g2, const Pruned pr, bool kinetic,
+                                            c128 (&kin)[2 * Quarter<C>::Q]) {
+    constexpr int Q = Quarter<C>::Q;
+    static_for<Q>([&](auto I) {
+        constexpr int j = decltype(I)::value;
+        const int o1 = pr.c1 + j * C::R2, o2 = pr.c2 + (C::R1 - Q + j) * C::R2;
+        const bool q1 = kinetic && ((pr.m1 >> j) & 1u), q2 = kinetic && ((pr.m2 >> (C::R1 - Q + j)) & 1u);
+        const c128 x1 = ld_pred(SpaceGlobal{}, psi_in + o1, q1), x2 = ld_pred(SpaceGlobal{}, psi_in + o2, q2);
+        const double h1 = q1 ? 0.5 * g2[o1] : 0.0, h2 = q2 ? 0.5 * g2[o2] : 0.0;
+        kin[j] = c128{h1 * x1.x, h1 * x1.y};
+        kin[Q + j] = c128{h2 * x2.x, h2 * x2.y};
+    });
+}
+template <class C> QM_HD void zfwd_step2_gather_pre(const c128 *line, c128 *out, const Pruned pr, int u,
+                                                     const c128 (&kin)[2 * Quarter<C>::Q]) {
+    if (u >= C::R2) return;
+    constexpr int Q = Quarter<C>::Q;
+    c128 t[C::R1];
+    static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = line[a * C::R2P + u]; });
+    Dft<C::R1, -1>::run(t);
+    static_for<Q>([&](auto I) {
+        constexpr int j = decltype(I)::value;
+        constexpr int c2 = C::R1 - Q + j;
+        st_pred(SpaceGlobal{}, out + pr.c1 + j * C::R2, t[j] + kin[j], (pr.m1 >> j) & 1u);
+        st_pred(SpaceGlobal{}, out + pr.c2 + c2 * C::R2, t[c2] + kin[Q + j], (pr.m2 >> c2) & 1u);
     });
 }
 

@@ -52,6 +52,7 @@ struct QmKTables {
     std::vector<int4> stickinfo;               // per stick: packed occupied i3 intervals (a1|b1<<16, a2|b2<<16), first G, 0
     short4 xiv = {1, 0, 1, 0};                 // occupied i1 intervals (rows 0.. and following)
     bool x_contiguous = true;
+    bool z_quarter = false;                    // same rule for the occupied i3 of every stick (z kernels)
     bool y_quarter = false;                    // every occupied i2 of every row lies in the first / last quarter-block (fft_phases.cuh Quarter)
 };
 
@@ -170,6 +171,8 @@ static inline int qm_build_tables(const double *lattice, const double *recip, do
     // occupied i3 intervals of every stick: [0..m3max] and [n3+m3min..n3-1]; the G of a stick are stored in
     // ascending i3, i.e. interval 1 then interval 2 back to back (what the z kernels' pruned passes assume)
     kp->stickinfo.resize(S);
+    kp->z_quarter = true;
+    const int zq = (ax[2].r1 + 3) / 4;
     for (int s = 0; s < S; ++s) {
         short4 iv = {1, 0, 1, 0};
         for (int g = kp->stickoff[s]; g < kp->stickoff[s + 1]; ++g) {
@@ -179,6 +182,8 @@ static inline int qm_build_tables(const double *lattice, const double *recip, do
         }
         const int span = (iv.x <= iv.y ? iv.y - iv.x + 1 : 0) + (iv.z <= iv.w ? iv.w - iv.z + 1 : 0);
         if (span != kp->stickoff[s + 1] - kp->stickoff[s]) { *msg = "G of a stick are not two contiguous intervals"; return -1; }
+        if (iv.x <= iv.y && iv.y >= zq * ax[2].r2) kp->z_quarter = false;
+        if (iv.z <= iv.w && iv.z < (ax[2].r1 - zq) * ax[2].r2) kp->z_quarter = false;
         kp->stickinfo[s] = int4{(int)(unsigned short)iv.x | ((int)iv.y << 16), (int)(unsigned short)iv.z | ((int)iv.w << 16),
                                 kp->stickoff[s], 0};
     }

@@ -136,7 +136,7 @@ struct qm_gspace {
     unsigned long long launches = 0;
     int sm_count = 148;
     int max_smem = 0;
-    int z_cta_per_sm = 3;           // resident z-kernel CTAs per SM the grid is sized for (QM_Z_CTA_PER_SM)
+    int z_cta_per_sm = 2;           // resident z-kernel CTAs per SM the grid is sized for (QM_Z_CTA_PER_SM)
     int plane_stagger_ns = 300;     // de-phasing delay between the plane kernel's groups (QM_PLANE_STAGGER_NS)
     ~qm_gspace() { for (auto *k : kpts) delete k; }
 };
@@ -166,7 +166,7 @@ size_t plane_smem(const qm_gspace *g, const KPoint *kp, int ngroups) {
     const size_t sl = (size_t)qm_scratch_pitch(ax.len, std::max(ax.r1, ax.r2));
     const int tpg = PLANE_GROUP / std::max(ax.r1, ax.r2);
     const size_t a_elems = ((size_t)kp->nx * kp->rowpitch + 7) & ~(size_t)7;
-    return (a_elems + (size_t)ngroups * tpg * sl) * sizeof(c128) + (size_t)kp->nx * sizeof(int4) + 16;
+    return (a_elems + (size_t)ngroups * tpg * sl + ax.n) * sizeof(c128) + (size_t)kp->nx * sizeof(int4) + 16;   // + twiddle table
 }
 
 // number of independent 64-thread groups of the plane kernel: the fewest groups that reach the
@@ -194,13 +194,13 @@ int z_grid_x(const qm_gspace *g, int ntiles, int nb, int cta_per_sm) {
     return (ntiles + rounds - 1) / rounds;
 }
 template <class C> int launch_zinv(qm_gspace *g, KPoint *kp, const c128 *psi, int nb, cudaStream_t st) {
-    const size_t smem = (size_t)QM_ZT * (C::L | 1) * sizeof(c128);
+    const size_t smem = qm_z_smem<C>();
     static bool attr = false;
     if (!attr) { CU_TRY(cudaFuncSetAttribute(k_zinv<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
     const int ntiles = (kp->nsticks + QM_ZT - 1) / QM_ZT;
     dim3 grid(z_grid_x(g, ntiles, nb, g->z_cta_per_sm), nb);
     g->prof.begin(QM_K_ZINV, st);
-    k_zinv<C><<<grid, QM_ZT * C::TT, smem, st>>>(kp->plan(), g->d_tw[2].p, psi, g->d_W.p, ntiles);
+    k_zinv<C><<<grid, QM_ZT * C::TT, smem, st>>>(kp->plan(), g->d_tw[2].p, psi, g->d_W.p, ntiles, kp->z_quarter ? 1 : 0);
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
@@ -208,13 +208,14 @@ template <class C> int launch_zinv(qm_gspace *g, KPoint *kp, const c128 *psi, in
 }
 template <class C> int launch_zfwd(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb, int kinetic,
                                    cudaStream_t st) {
-    const size_t smem = (size_t)QM_ZT * (C::L | 1) * sizeof(c128);
+    const size_t smem = qm_z_smem<C>();
     static bool attr = false;
     if (!attr) { CU_TRY(cudaFuncSetAttribute(k_zfwd<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
     const int ntiles = (kp->nsticks + QM_ZT - 1) / QM_ZT;
     dim3 grid(z_grid_x(g, ntiles, nb, g->z_cta_per_sm), nb);
     g->prof.begin(QM_K_ZFWD, st);
-    k_zfwd<C><<<grid, QM_ZT * C::TT, smem, st>>>(kp->plan(), g->d_tw[2].p, g->d_W.p, psi_in, out, ntiles, kinetic);
+    k_zfwd<C><<<grid, QM_ZT * C::TT, smem, st>>>(kp->plan(), g->d_tw[2].p, g->d_W.p, psi_in, out, ntiles, kinetic,
+                                                  kp->z_quarter ? 1 : 0);
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
@@ -244,7 +245,7 @@ template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *bo
 
 // dispatch on FFT length ---------------------------------------------------------------------
 #ifdef QM_DEV_SIZES      /* developer builds: only the lengths of the five BASELINE.json configs (fast compile) */
-#define QM_FOR_SIZES(X) X(24, 4, 6) X(32, 4, 8) X(48, 6, 8) X(96, 8, 12) X(144, 12, 12)
+#define QM_FOR_SIZES(X) X(12, 3, 4) X(24, 4, 6) X(32, 4, 8) X(48, 6, 8) X(96, 8, 12) X(144, 12, 12)
 #else
 #define QM_FOR_SIZES(X)                                                                              \
     X(8, 2, 4) X(12, 3, 4) X(16, 4, 4) X(18, 3, 6) X(20, 4, 5) X(24, 4, 6) X(30, 5, 6) X(32, 4, 8)   \
@@ -302,7 +303,8 @@ int check_handle(const qm_gspace *g, int k) {
 }
 
 int ensure_workspace(qm_gspace *g, const KPoint *kp, int nb) {
-    CU_TRY(g->d_W.resize((size_t)nb * g->grid[2] * kp->nsticks));
+    const size_t ntiles = ((size_t)kp->nsticks + QM_ZT - 1) / QM_ZT;      // W is blocked by stick tile (WView)
+    CU_TRY(g->d_W.resize((size_t)nb * ntiles * QM_ZT * g->grid[2]));
     return QM_OK;
 }
 

@@ -49,7 +49,7 @@ template <class C> struct Emu {
             }
             for (int tid = 0; tid < nthr; ++tid) {
                 int t = tid % TS, u = tid / TS;
-                if (t < ns) zinv_step2_store<C>(&lines[t * LP], W + s0 + t, S, u);
+                if (t < ns) zinv_step2_store<C>(&lines[t * LP], W + (size_t)(s0 / TS) * C::N * QM_ZT + t, QM_ZT, u);
             }
         }
     }
@@ -60,7 +60,7 @@ template <class C> struct Emu {
             std::vector<c128> lines(TS * LP, c128{1e300, -1e300});
             for (int tid = 0; tid < nthr; ++tid) {
                 int t = tid % TS, u = tid / TS;
-                if (t < ns) zfwd_step1_load<C>(W + s0 + t, S, &lines[t * LP], u, rowB(u));
+                if (t < ns) zfwd_step1_load<C>(W + (size_t)(s0 / TS) * C::N * QM_ZT + t, QM_ZT, &lines[t * LP], u, rowB(u));
             }
             for (int tid = 0; tid < nthr; ++tid) {
                 int t = tid / C::TT, u = tid % C::TT;
@@ -77,7 +77,7 @@ template <class C> struct Emu {
             const int4 q = kp.rowinfo[r];
             return RowInfo{(int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, q.z};
         };
-        c128 *Wp = W + (size_t)p * S;
+        const WView Wp = qm_wview(W, p, n3);
         if (MODE != 2) {
             for (int task = 0; task < X * C::TT; ++task) {
                 const RowInfo ri = row_info(task / C::TT);
@@ -145,7 +145,7 @@ template <class C> int run(int n, const double *lat, double ecut, const double *
     }
     Emu<C> emu(kp, ax[2]);
     const int S = kp.nsticks, ncol = 5;     // odd column count on purpose: exercises the ragged last pass
-    std::vector<c128> hloc((size_t)nb * kp.ng), g2r(nb * n3), r2g((size_t)nb * kp.ng), W((size_t)n * S);
+    std::vector<c128> hloc((size_t)nb * kp.ng), g2r(nb * n3), r2g((size_t)nb * kp.ng), W((size_t)n * ((S + QM_ZT - 1) / QM_ZT) * QM_ZT);
     for (int b = 0; b < nb; ++b) {
         emu.zinv(&psi[(size_t)b * kp.ng], W.data());
         for (int p = 0; p < n; ++p) emu.template plane<0>(p, W.data(), vt.data(), nullptr, 1.0, ncol);

@@ -147,6 +147,32 @@ def test_parity_sampled_rows_full_size(qm, name, nb):
     gs.close()
 
 
+def test_parity_aliased_grid_general_path(qm):
+    """A legal but aliased grid (2m+1 <= n < 4m+1, reading A8): the oracle's modulo lookup still defines the
+    result, the library reports alias_free == 0, and the plane kernel runs its general (non-quarter) y pass."""
+    import dataclasses
+    from workloads import CONFIGS, cell_for, make_beta, make_dmatrix, make_psi
+    from oracle import gsphere as og
+    cfg = dataclasses.replace(CONFIGS["cfg1"], name="cfg1_aliased", grid=(12, 12, 12))
+    lat, pos = cell_for(cfg)
+    miller, idx, g2 = og.gsphere(lat, cfg.ecutwfc_ry, cfg.grid, np.zeros(3))
+    assert 4 * np.abs(miller).max() + 1 > 12 >= 2 * np.abs(miller).max() + 1
+    v = np.random.default_rng(5).standard_normal(12 ** 3)       # any real V(r) will do on this grid (the A9
+    v /= np.max(np.abs(v))                                      # generator needs room for the 4*ecut sphere)
+    p = dict(cfg=cfg, lat=lat, k=np.zeros(3), kpts=np.zeros((1, 3)), miller=miller, idx=idx, g2=g2, v=v,
+             vhat=oh.vhat_box(v, cfg.grid), beta=make_beta(cfg, lat, pos, np.zeros(3), miller),
+             dblk=make_dmatrix(cfg), psi=make_psi(cfg, 0, idx.size))
+    gs = _gspace(qm, p)
+    assert np.array_equal(gs.index_map(0), idx)
+    assert not gs.alias_free(0)
+    for variant in ("full", "d0"):
+        got = _apply(qm, gs, p, p["psi"], variant)
+        ref = _oracle(p, p["psi"], variant)
+        e_inf, e_2 = band_errors(got, ref)
+        assert e_inf <= TOL and e_2 <= TOL, (variant, e_inf, e_2)
+    gs.close()
+
+
 @pytest.mark.parametrize("nb", [1, 3, 17])
 def test_ragged_band_counts(qm, nb):
     p = problem("cfg3")
