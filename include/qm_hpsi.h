@@ -133,8 +133,8 @@ typedef enum {
     QM_K_PLANE = 1,     /* fused xy-plane kernel incl. V_loc multiply   (a2, a3, a4) */
     QM_K_ZFWD = 2,      /* forward z-FFT + gather + kinetic             (a4, a5) */
     QM_K_PROJ1 = 3,     /* P = beta^H psi   (DMMA)                      (a6) */
-    QM_K_PREDUCE = 4,   /* split-K reduction of P */
-    QM_K_DMUL = 5,      /* Q = D P                                      (a7) */
+    QM_K_PREDUCE = 4,   /* split-K reduction of P; with D blocks that divide 16 also Q = D P, fused  (a7) */
+    QM_K_DMUL = 5,      /* Q = D P, general block size (separate launch)  (a7) */
     QM_K_PROJ2 = 6,     /* out += beta Q    (DMMA)                      (a8) */
     QM_K_COUNT = 7
 } qm_kernel_kind;

@@ -25,7 +25,17 @@ __device__ __forceinline__ double2 ldg_c128(const c128 *p) {
 //   beta1[mblk][kc][128 rows][16 k]  element (r,k) at r*16 + (k ^ ((r&1)<<2))      (GEMM 1, one 32 KB copy/stage)
 //   beta2[gt][ic][16 i][64 G]        element (i,g) at i*64 + (g ^ ((i&3)<<1))      (GEMM 2, one 16 KB copy/stage)
 // The XOR swizzles make every DMMA fragment load (one 16-byte LDS per thread) bank-conflict free.
-constexpr int P1_ROWS = 128, P1_KS = 16, P1_CW = 8, P1_ST = 4, P1_PSI_PITCH = 20, P_NB = 16;
+#ifndef QM_P1_ROWS
+#define QM_P1_ROWS 128      /* projector rows per CTA of GEMM 1 (16 per consumer warp) */
+#endif
+#ifndef QM_P1_STAGES
+#define QM_P1_STAGES 4
+#endif
+#ifndef QM_P1_OCC
+#define QM_P1_OCC 1         /* CTAs of GEMM 1 per SM the split-K factor is sized for */
+#endif
+constexpr int P1_ROWS = QM_P1_ROWS, P1_KS = 16, P1_CW = P1_ROWS / 16, P1_ST = QM_P1_STAGES, P1_OCC = QM_P1_OCC,
+              P1_PSI_PITCH = 20, P_NB = 16;
 constexpr int P1_BETA_BYTES = P1_ROWS * P1_KS * 16;                 // 32768
 constexpr int P1_PSI_BYTES = P_NB * P1_PSI_PITCH * 16;              // 5120
 constexpr int P1_STAGE_BYTES = P1_BETA_BYTES + P1_PSI_BYTES;
@@ -70,7 +80,7 @@ __global__ void k_tile_beta2(const c128 *__restrict__ src, int ng, int nproj, c1
 }
 
 // GEMM 1:  Ppart[split][row][n] = sum_{k in split} conj(beta[row][k]) psi[band0+n][k]
-__global__ void __launch_bounds__((P1_CW + 1) * 32, 1)
+__global__ void __launch_bounds__((P1_CW + 1) * 32, P1_OCC)
 k_proj1_pipe(const c128 *__restrict__ beta1, int nkc, const c128 *__restrict__ psi, int ng, int nb, int band0,
              c128 *__restrict__ Ppart, int nrows_pad, int nsplit)
 {
@@ -203,6 +213,37 @@ __global__ void k_dmul_tiles(const double *__restrict__ D, int db, int nproj, in
     }
     double *t = qt + (size_t)(i / P2_KS) * P2_Q_DOUBLES + (i % P2_KS) * P2_Q_PITCH + n;
     t[0] = sr; t[P2_KS * P2_Q_PITCH] = si; t[2 * P2_KS * P2_Q_PITCH] = sr + si;
+}
+
+// Fused split-K reduction + D multiply for block sizes that divide 16 (every BASELINE.json config has 4x4 blocks):
+// a CTA owns 16 projector rows x 16 bands, sums the split partials in a fixed order (deterministic), keeps P in
+// shared memory and writes the Q tiles (Qr, Qi, Qr+Qi) GEMM 2 consumes.
+__global__ void __launch_bounds__(256)
+k_reduce_dmul(const c128 *__restrict__ Ppart, int nsplit, int nrows_pad, const double *__restrict__ D, int db, int nproj,
+              double *__restrict__ qt)
+{
+    __shared__ double2 Ps[16][P_NB + 1];
+    const int n = threadIdx.x % P_NB, rl = threadIdx.x / P_NB;
+    const int row = blockIdx.x * 16 + rl;
+    const size_t count = (size_t)nrows_pad * P_NB;
+    const c128 *src = Ppart + (size_t)row * P_NB + n;
+    double sr[4] = {0.0, 0.0, 0.0, 0.0}, si[4] = {0.0, 0.0, 0.0, 0.0};
+    int s = 0;
+    for (; s + 4 <= nsplit; s += 4) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) { const double2 v = ldg_c128(src + (size_t)(s + j) * count); sr[j] += v.x; si[j] += v.y; }
+    }
+    for (; s < nsplit; ++s) { const double2 v = ldg_c128(src + (size_t)s * count); sr[0] += v.x; si[0] += v.y; }
+    Ps[rl][n] = make_double2((sr[0] + sr[1]) + (sr[2] + sr[3]), (si[0] + si[1]) + (si[2] + si[3]));
+    __syncthreads();
+    double qr = 0.0, qi = 0.0;
+    if (row < nproj) {
+        const int blk = row / db, ii = row % db, r0 = rl - ii;       // the block's rows sit in this CTA (db divides 16)
+        const double *d = D + ((size_t)blk * db + ii) * db;
+        for (int j = 0; j < db; ++j) { const double2 v = Ps[r0 + j][n]; const double dj = __ldg(d + j); qr += dj * v.x; qi += dj * v.y; }
+    }
+    double *t = qt + (size_t)(row / P2_KS) * P2_Q_DOUBLES + (row % P2_KS) * P2_Q_PITCH + n;
+    t[0] = qr; t[P2_KS * P2_Q_PITCH] = qi; t[2 * P2_KS * P2_Q_PITCH] = qr + qi;
 }
 
 // GEMM 2:  out[band0+n][g] += sum_i beta[i][g] Q[i][n]

@@ -316,7 +316,7 @@ int run_nonlocal(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb
         CU_TRY(cudaFuncSetAttribute(k_proj2_sk, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM));
         attr = true;
     }
-    const int nsplit = std::max(1, std::min(kp->nkc, g->sm_count / kp->nmblk));
+    const int nsplit = std::max(1, std::min(kp->nkc, g->sm_count * P1_OCC / kp->nmblk));
     const int nrows_pad = kp->nmblk * P1_ROWS;
     const size_t pcount = (size_t)nrows_pad * P_NB;
     CU_TRY(g->d_Ppart.resize(pcount * nsplit));
@@ -331,20 +331,29 @@ int run_nonlocal(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb
         k_proj1_pipe<<<dim3(kp->nmblk, nsplit), (P1_CW + 1) * 32, P1_SMEM, st>>>(
             kp->d_beta1.p, kp->nkc, psi_in, kp->ng, nb, band0, g->d_Ppart.p, nrows_pad, nsplit);
         g->prof.end(st);
-        g->prof.begin(QM_K_PREDUCE, st);
-        k_reduce_p2<<<(unsigned)((pcount + 255) / 256), 256, 0, st>>>(g->d_Ppart.p, nsplit, (int)pcount, g->d_P.p);
-        g->prof.end(st);
-        g->prof.begin(QM_K_DMUL, st);
         const int qcount = kp->nic * P2_KS * P_NB;
-        k_dmul_tiles<<<(qcount + 255) / 256, 256, 0, st>>>(kp->d_D.p, kp->dblock, kp->nproj, kp->nic, g->d_P.p,
-                                                          g->d_qt.p);
-        g->prof.end(st);
+        if (16 % kp->dblock == 0 && kp->nic * P2_KS <= nrows_pad) {
+            g->prof.begin(QM_K_PREDUCE, st);      // fused split-K reduction + D multiply
+            k_reduce_dmul<<<(kp->nic * P2_KS) / 16, 256, 0, st>>>(g->d_Ppart.p, nsplit, nrows_pad, kp->d_D.p, kp->dblock,
+                                                                   kp->nproj, g->d_qt.p);
+            g->prof.end(st);
+            g->launches += 1;
+        } else {
+            g->prof.begin(QM_K_PREDUCE, st);
+            k_reduce_p2<<<(unsigned)((pcount + 255) / 256), 256, 0, st>>>(g->d_Ppart.p, nsplit, (int)pcount, g->d_P.p);
+            g->prof.end(st);
+            g->prof.begin(QM_K_DMUL, st);
+            k_dmul_tiles<<<(qcount + 255) / 256, 256, 0, st>>>(kp->d_D.p, kp->dblock, kp->nproj, kp->nic, g->d_P.p,
+                                                              g->d_qt.p);
+            g->prof.end(st);
+            g->launches += 2;
+        }
         g->prof.begin(QM_K_PROJ2, st);
         k_proj2_sk<<<ncta2, (P2_CW + 1) * 32, P2_SMEM, st>>>(kp->d_beta2.p, kp->nic, kp->ngt, g->d_qt.p, kp->ng, nb,
                                                              band0, out, g->d_part.p, g->d_pdesc.p);
         k_proj2_fixup<<<2 * ncta2, 256, 0, st>>>(g->d_part.p, g->d_pdesc.p, 2 * ncta2, kp->ng, nb, band0, out);
         g->prof.end(st);
-        g->launches += 5;
+        g->launches += 3;
     }
     CU_TRY(cudaGetLastError());
     return QM_OK;

@@ -173,6 +173,25 @@ def test_parity_aliased_grid_general_path(qm):
     gs.close()
 
 
+@pytest.mark.parametrize("name,db", [("cfg1", 8), ("cfg3", 32), ("cfg3", 2)])
+def test_parity_other_d_block_sizes(qm, name, db):
+    """d_block == nproj is one dense Hermitian (real symmetric) D; block sizes that divide 16 take the
+    fused reduction + D kernel, the others the general two-kernel path."""
+    torch, dev = _torch()
+    p = problem(name)
+    nproj = p["beta"].shape[0]
+    a = np.random.default_rng(11).standard_normal((nproj // db, db, db))
+    dblk = 0.5 * (a + np.transpose(a, (0, 2, 1)))
+    gs = _gspace(qm, p)
+    gs.set_vloc(torch.from_numpy(p["v"]).to(dev))
+    gs.set_nonlocal(0, torch.from_numpy(p["beta"]).to(dev), torch.from_numpy(dblk).to(dev))
+    got = gs.apply_h(torch.from_numpy(p["psi"]).to(dev)).cpu().numpy()
+    ref = oh.apply_h_rows(p["psi"], p["miller"], p["g2"], p["vhat"], p["cfg"].grid, p["beta"], oh.expand_d(dblk))
+    e_inf, e_2 = band_errors(got, ref)
+    assert e_inf <= TOL and e_2 <= TOL, (e_inf, e_2)
+    gs.close()
+
+
 @pytest.mark.parametrize("nb", [1, 3, 17])
 def test_ragged_band_counts(qm, nb):
     p = problem("cfg3")
