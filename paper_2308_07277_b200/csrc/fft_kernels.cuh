@@ -48,20 +48,21 @@ k_zinv(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ psi,
     int4 q = info(blockIdx.x), qn = info(blockIdx.x + gridDim.x);
     Pruned pr = pruned_of(q);
     c128 pre[NPRE];
-    if (quarter) prefetch_quarter<C>(SpaceGlobal{}, psib + q.z, C::R2, pr, pre);
+    if (quarter) prefetch_quarter<C>(psib + q.z, C::R2, pr, pre);
+    const SLine lines_s = qm_sline(lines), stage_s = qm_sline(stage);
     for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const int ns = min(QM_ZT, S - tile * QM_ZT);
         if (t1 < ns) {
-            if (quarter) prunedA_step1_pre<C>(pre, lines + t1 * LP, u1, twa);
-            else prunedA_step1<C>(SpaceGlobal{}, psib + q.z, C::R2, pr, lines + t1 * LP, u1, twa);
+            if (quarter) prunedA_step1_pre<C>(pre, lines_s + t1 * LP, u1, twa);
+            else prunedA_step1<C>(psib + q.z, C::R2, pr, lines_s + t1 * LP, u1, twa);
         }
         // advance the two-deep prefetch: data of the next tile, table entry of the one after
         q = qn; pr = pruned_of(q);
-        if (quarter) prefetch_quarter<C>(SpaceGlobal{}, psib + q.z, C::R2, pr, pre);
+        if (quarter) prefetch_quarter<C>(psib + q.z, C::R2, pr, pre);
         qn = info(tile + 2 * gridDim.x);
         if (tid == 0) bulk_wait_read0();      // the previous tile's bulk store has read the staging buffer
         __syncthreads();
-        if (t2 < ns) zinv_step2_store<C>(lines + t2 * LP, stage + t2, QM_ZT, u2);
+        if (t2 < ns) zinv_step2_store<C>(lines_s + t2 * LP, stage_s + t2, QM_ZT, u2);
         fence_async_smem();
         __syncthreads();
         if (tid == 0) { bulk_s2g(Wb + (size_t)tile * C::N * QM_ZT, stage, (uint32_t)(C::N * QM_ZT * sizeof(c128))); bulk_commit(); }
@@ -96,6 +97,7 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
     load_twrow(twb, tw, u2, C::R1);
     const size_t boff = (size_t)band * kp.ng;
     __syncthreads();
+    const SLine lines_s = qm_sline(lines), stage_s = qm_sline(stage);
     for (int tile = blockIdx.x, it = 0; tile < ntiles; tile += gridDim.x, ++it) {
         const int ns = min(QM_ZT, S - tile * QM_ZT);
         // gather-side inputs of this tile: in flight behind the wait and the first pass
@@ -105,7 +107,7 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
         c128 kin[NPRE];
         if (quarter) prefetch_kin<C>(psi_in + boff + q.z, kp.g2 + q.z, pr, kinetic != 0 && t1 < ns, kin);
         mbar_wait(wbar, (uint32_t)(it & 1));
-        zfwd_step1_load<C>(stage + t2, QM_ZT, lines + t2 * LP, u2, twb);
+        zfwd_step1_load<C>(stage_s + t2, QM_ZT, lines_s + t2 * LP, u2, twb);
         __syncthreads();                       // staging buffer consumed, lines complete
         if (tid == 0 && tile + (int)gridDim.x < ntiles) {
             fence_async_smem();
@@ -113,8 +115,8 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
             bulk_g2s(stage, Wb + (size_t)(tile + gridDim.x) * C::N * QM_ZT, TILE_BYTES, wbar);
         }
         if (t1 < ns) {
-            if (quarter) zfwd_step2_gather_pre<C>(lines + t1 * LP, out + boff + q.z, pr, u1, kin);
-            else zfwd_step2_gather<C>(lines + t1 * LP, out + boff + q.z, kinetic ? psi_in + boff + q.z : nullptr, kp.g2 + q.z,
+            if (quarter) zfwd_step2_gather_pre<C>(lines_s + t1 * LP, out + boff + q.z, pr, u1, kin);
+            else zfwd_step2_gather<C>(lines_s + t1 * LP, out + boff + q.z, kinetic ? psi_in + boff + q.z : nullptr, kp.g2 + q.z,
                                       pr, u1, kinetic != 0);
         }
         __syncthreads();
@@ -195,7 +197,7 @@ __device__ __forceinline__ void plane_y_phase(const PlaneCtx cx, c128 *__restric
     const auto &twb = [&]() -> const TwRow<C::R2> & {
         if constexpr (C::R1 == C::R2) return twa; else return twb_store;
     }();
-    c128 *A = cx.A;
+    const SLine As = qm_sline(cx.A);
     const int pc = have_cur ? pl : 0, pp = prev >= 0 ? prev : 0;
     const WView Wcur = qm_wview(W + (size_t)(pc / n3) * cx.wband, pc % n3, n3);
     const WView Wprev = qm_wview(W + (size_t)(pp / n3) * cx.wband, pp % n3, n3);
@@ -209,23 +211,24 @@ __device__ __forceinline__ void plane_y_phase(const PlaneCtx cx, c128 *__restric
             pr = make_pruned<C>((int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, u, 1);
         }
         c128 pre[NPRE];
-        if (do_back && quarter && ok) prefetch_quarter<C>(SpaceGlobal{}, Wcur + sbase, C::R2, pr, pre);
+        const SLine Arow = As + r * RP;
+        if (do_back && quarter && ok) prefetch_quarter<C>(Wcur + sbase, C::R2, pr, pre);
         if (do_fwd) {
-            if (ok) lineB_step1<C>(A + r * RP, u, twb);
+            if (ok) lineB_step1<C>(Arow, u, twb);
             group_barrier<G>(grp);
             if (ok) {
-                if (quarter) prunedB_step2_quarter<C>(SpaceGlobal{}, A + r * RP, Wprev + sbase, C::R2, pr, u);
-                else prunedB_step2<C>(SpaceGlobal{}, A + r * RP, Wprev + sbase, C::R2, pr, u);
+                if (quarter) prunedB_step2_quarter<C>(Arow, Wprev + sbase, C::R2, pr, u);
+                else prunedB_step2<C>(Arow, Wprev + sbase, C::R2, pr, u);
             }
         }
         if (do_back) {
             // the team that read row r in the step above is the one that refills it: no barrier needed
             if (ok) {
-                if (quarter) prunedA_step1_pre<C>(pre, A + r * RP, u, twa);
-                else prunedA_step1<C>(SpaceGlobal{}, Wcur + sbase, C::R2, pr, A + r * RP, u, twa);
+                if (quarter) prunedA_step1_pre<C>(pre, Arow, u, twa);
+                else prunedA_step1<C>(Wcur + sbase, C::R2, pr, Arow, u, twa);
             }
             group_barrier<G>(grp);
-            if (ok) lineA_step2<C>(A + r * RP, u);
+            if (ok) lineA_step2<C>(Arow, u);
         }
     }
 }
@@ -246,10 +249,10 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
     const auto &twb = [&]() -> const TwRow<C::R2> & {
         if constexpr (C::R1 == C::R2) return twa; else return twb_store;
     }();
-    c128 *A = cx.A;
+    const SLine As = qm_sline(cx.A);
     const Pruned px = make_pruned<C>(x_iv.x, x_iv.y, x_iv.z, x_iv.w, u, RP);
     const int band = pl / n3, p = pl - band * n3;
-    c128 *myscr = cx.scr + (size_t)(grp * TPG + id.team) * SL;
+    const SLine myscr = qm_sline(cx.scr + (size_t)(grp * TPG + id.team) * SL);
     const double *vplane = vt + (size_t)p * C::N * VLayout<C>::COL;
     VRow<C::R2> vr;
     // De-phase the groups: they all do identical load -> FP64 -> store bursts, and when they run in
@@ -261,9 +264,9 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
     }
     for (int col = col0; col - slot < C::N; col += ngroups * TPG) {
         const bool ok = team_ok && col < C::N;
-        c128 *Acol = A + C::pos(col);
+        const SLine Acol = As + C::pos(col);
         if constexpr (MODE != 2) {
-            if (ok) prunedA_step1<C>(SpaceShared{}, Acol, C::R2 * RP, px, myscr, u, twa);
+            if (ok) prunedA_step1<C>(Acol, C::R2 * RP, px, myscr, u, twa);
             group_barrier<G>(grp);
         }
         if (ok) {
@@ -282,7 +285,7 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
         if constexpr (MODE != 1) {
             // no barrier after step 3: the scratch column a thread reads here is exactly the one it
             // overwrites in the next iteration's step 1 (MODE 2 has no step 1 and writes rows: barrier).
-            if (ok) prunedB_step2<C>(SpaceShared{}, myscr, Acol, C::R2 * RP, px, u);
+            if (ok) prunedB_step2<C>(myscr, Acol, C::R2 * RP, px, u);
             if constexpr (MODE == 2) group_barrier<G>(grp);
         }
     }

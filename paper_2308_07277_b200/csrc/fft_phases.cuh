@@ -26,63 +26,86 @@ template <int R1_, int R2_> struct LineCfg {
 
 // Per-thread twiddle rows held in registers: TW[j] = exp(-2 pi i u j / N) for the thread's fixed u.
 // (Looking them up in shared memory at stride j costs up to 8-way bank conflicts; every thread keeps
-//  the same u for the whole kernel, so the row is loaded once.)
+//  the same u for a whole phase, so the row is loaded once per phase.)
 template <int R> struct TwRow {
     c128 w[R];
     template <int J> QM_HD c128 get() const { return w[J]; }
-};
-// Same interface, but looked up in a table on every use (kernels that use each twiddle only once).
-struct TwTable {
-    const c128 *tw; int u;
-    template <int J> QM_HD c128 get() const { return tw[u * J]; }
 };
 template <int R> QM_HD void load_twrow(TwRow<R> &t, const c128 *tw, int u, int limit) {
     static_for<R>([&](auto I) { constexpr int j = decltype(I)::value; t.w[j] = (u < limit) ? tw[u * j] : c128{1.0, 0.0}; });
 }
 
-// One plane row of the stick buffer: the occupied i2 indices are the intervals [a1,b1] and [a2,b2]
-// (convex sphere), stored back to back starting at stick index sbase.
-struct RowInfo {
-    int a1, b1, a2, b2, sbase;
-    QM_HD int stick(int i) const {      // stick index of natural index i, or -1 if the row has no stick there
-        return (i >= a1 && i <= b1) ? sbase + i - a1
-                                    : ((i >= a2 && i <= b2) ? sbase + (b1 - a1 + 1) + i - a2 : -1);
-    }
+// ---- shared-memory lines -----------------------------------------------------------------------------
+// A line in shared memory as its own pointer-like type, so that the pruned passes can tell it from a global
+// pointer (predicated accesses need the state space).  Plain accesses go through the generic pointer: explicit
+// ld/st.shared asm for them was measured 4 % slower in the plane kernel (it pins the instruction order).
+struct SLine {
+    c128 *p;
+    QM_HD c128 &operator[](int i) const { return p[i]; }
+    QM_HD SLine operator+(int e) const { return SLine{p + e}; }
 };
-// Backward step 1 reading its (pruned) input straight from the stick plane in global memory:
-// the plane array needs neither a load pass nor a zero fill.
-template <class C, class TW> QM_HD void lineA_step1_gin(c128 *line, const c128 *Wp, const RowInfo ri, int u, const TW &tw) {
-    if (u >= C::R2) return;
-    c128 t[C::R1];
-    static_for<C::R1>([&](auto I) {
-        constexpr int n1 = decltype(I)::value;
-        const int s = ri.stick(n1 * C::R2 + u);
-        t[n1] = (s >= 0) ? Wp[s] : c128{0.0, 0.0};
-    });
-    Dft<C::R1, +1>::run(t);
-    static_for<C::R1>([&](auto I) {
-        constexpr int k1 = decltype(I)::value;
-        line[k1 * C::R2P + u] = (k1 == 0) ? t[k1] : cmul_conj(t[k1], tw.template get<k1>());
-    });
+QM_HD SLine qm_sline(const c128 *p) { return SLine{const_cast<c128 *>(p)}; }
+
+// Stick-plane workspace W of one band, blocked by tiles of QM_ZT sticks: element (plane label p, stick s) lives at
+// band_base[((s / QM_ZT) * n3 + p) * QM_ZT + s % QM_ZT].  A tile's N3 x QM_ZT block is contiguous (what the z kernels
+// move with one bulk copy); the plane kernel addresses single elements through this pointer-like view (p fixed).
+constexpr int QM_ZT = 16;
+struct WView {
+    c128 *base;            // element (p, stick 0) of the band: band base + p * QM_ZT
+    unsigned tstride;      // elements between consecutive tiles: n3 * QM_ZT
+    int s;                 // stick
+    QM_HD WView operator+(int e) const { return WView{base, tstride, s + e}; }
+    QM_HD c128 *ptr() const { const unsigned us = (unsigned)s; return base + ((us / QM_ZT) * tstride + (us % QM_ZT)); }
+};
+QM_HD WView qm_wview(c128 *band_base, int p, int n3) { return WView{band_base + p * QM_ZT, (unsigned)(n3 * QM_ZT), 0}; }
+
+// ---- predicated 16-byte accesses (no branch) ------------------------------------------------------------
+QM_HD c128 ld_pred(const c128 *p, bool pred) {
+#ifdef __CUDA_ARCH__
+    c128 v;
+    asm volatile("{ .reg .pred q; setp.ne.u32 q, %3, 0; mov.f64 %0, 0d0000000000000000; mov.f64 %1, 0d0000000000000000;\n"
+                 "  @q ld.global.v2.f64 {%0, %1}, [%2]; }"
+                 : "=d"(v.x), "=d"(v.y) : "l"(p), "r"((unsigned)pred) : "memory");
+    return v;
+#else
+    return pred ? *p : c128{0.0, 0.0};
+#endif
 }
-// Forward step 2 writing only the occupied outputs straight to the stick plane in global memory.
-template <class C> QM_HD void lineB_step2_gout(const c128 *line, c128 *Wp, const RowInfo ri, int u) {
-    if (u >= C::R2) return;
-    c128 t[C::R1];
-    static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = line[a * C::R2P + u]; });
-    Dft<C::R1, -1>::run(t);
-    static_for<C::R1>([&](auto I) {
-        constexpr int c = decltype(I)::value;
-        const int s = ri.stick(c * C::R2 + u);
-        if (s >= 0) Wp[s] = t[c];
-    });
+QM_HD c128 ld_pred(const WView &w, bool pred) { return ld_pred((const c128 *)w.ptr(), pred); }
+QM_HD c128 ld_pred(const SLine &l, bool pred) {
+#ifdef __CUDA_ARCH__
+    c128 v;
+    asm volatile("{ .reg .pred q; setp.ne.u32 q, %3, 0; mov.f64 %0, 0d0000000000000000; mov.f64 %1, 0d0000000000000000;\n"
+                 "  @q ld.shared.v2.f64 {%0, %1}, [%2]; }"
+                 : "=d"(v.x), "=d"(v.y) : "r"((unsigned)__cvta_generic_to_shared(l.p)), "r"((unsigned)pred) : "memory");
+    return v;
+#else
+    return pred ? *l.p : c128{0.0, 0.0};
+#endif
+}
+QM_HD void st_pred(c128 *p, c128 v, bool pred) {
+#ifdef __CUDA_ARCH__
+    asm volatile("{ .reg .pred q; setp.ne.u32 q, %3, 0; @q st.global.v2.f64 [%0], {%1, %2}; }"
+                 :: "l"(p), "d"(v.x), "d"(v.y), "r"((unsigned)pred) : "memory");
+#else
+    if (pred) *p = v;
+#endif
+}
+QM_HD void st_pred(const WView &w, c128 v, bool pred) { st_pred(w.ptr(), v, pred); }
+QM_HD void st_pred(const SLine &l, c128 v, bool pred) {
+#ifdef __CUDA_ARCH__
+    asm volatile("{ .reg .pred q; setp.ne.u32 q, %3, 0; @q st.shared.v2.f64 [%0], {%1, %2}; }"
+                 :: "r"((unsigned)__cvta_generic_to_shared(l.p)), "d"(v.x), "d"(v.y), "r"((unsigned)pred) : "memory");
+#else
+    if (pred) *l.p = v;
+#endif
 }
 
 // ---- pruned passes with hoisted addressing ---------------------------------------------------------
 // A thread with fixed u touches the line elements i = n*R2 + u (n = 0..R1-1).  When only two index
 // intervals [a1,b1], [a2,b2] of the line exist (stored back to back with element stride `stride`), the
 // elements that exist and their addresses depend on (u, intervals) only: they are worked out once
-// (per kernel for the x direction, per row for the y direction) instead of once per access.
+// (per kernel for the x direction, per row / stick for the y and z directions) instead of once per access.
 struct Pruned {
     unsigned m1, m2;      // bit n set: i = n*R2+u lies in interval 1 / interval 2
     int c1, c2;           // element offset of i: n*R2*stride + c1 (interval 1), + c2 (interval 2)
@@ -100,79 +123,28 @@ template <class C> QM_HD Pruned make_pruned(int a1, int b1, int a2, int b2, int 
     return Pruned{qm_range_mask(a1, b1, u, C::R2, C::R1), qm_range_mask(a2, b2, u, C::R2, C::R1),
                   (u - a1) * stride, (u - a2 + cnt1) * stride};
 }
-// Stick-plane workspace W of one band, blocked by tiles of QM_ZT sticks: element (plane label p, stick s) lives at
-// base[((s / QM_ZT) * n3 + p) * QM_ZT + s % QM_ZT].  A tile's N3 x QM_ZT block is contiguous (what the z kernels move
-// with one bulk copy); the plane kernel addresses single elements through this pointer-like view (p fixed).
-constexpr int QM_ZT = 16;
-struct WView {
-    c128 *base;            // element (p, stick 0) of the band: band base + p * QM_ZT
-    unsigned tstride;      // elements between consecutive tiles: n3 * QM_ZT
-    int s;                 // stick
-    QM_HD WView operator+(int e) const { return WView{base, tstride, s + e}; }
-    QM_HD c128 *ptr() const { const unsigned us = (unsigned)s; return base + ((us / QM_ZT) * tstride + (us % QM_ZT)); }
-};
-QM_HD WView qm_wview(c128 *band_base, int p, int n3) { return WView{band_base + p * QM_ZT, (unsigned)(n3 * QM_ZT), 0}; }
-QM_HD const c128 *qm_ptr(const c128 *p) { return p; }
-QM_HD c128 *qm_ptr(c128 *p) { return p; }
-QM_HD c128 *qm_ptr(const WView &w) { return w.ptr(); }
+// intervals packed as in the host tables: x = a1 | b1 << 16, y = a2 | b2 << 16
+template <class C> QM_HD Pruned make_pruned_packed(int x, int y, int u, int stride) {
+    return make_pruned<C>((int)(short)(x & 0xffff), x >> 16, (int)(short)(y & 0xffff), y >> 16, u, stride);
+}
 
-// predicated 16-byte accesses (no branch, no address arithmetic beyond base + immediate)
-struct SpaceShared {}; struct SpaceGlobal {};
-QM_HD c128 ld_pred(SpaceShared, const c128 *p, bool pred) {
-#ifdef __CUDA_ARCH__
-    c128 v;
-    asm volatile("{ .reg .pred q; setp.ne.u32 q, %3, 0; mov.f64 %0, 0d0000000000000000; mov.f64 %1, 0d0000000000000000;\n"
-                 "  @q ld.shared.v2.f64 {%0, %1}, [%2]; }"
-                 : "=d"(v.x), "=d"(v.y) : "r"((unsigned)__cvta_generic_to_shared(p)), "r"((unsigned)pred) : "memory");
-    return v;
-#else
-    return pred ? *p : c128{0.0, 0.0};
-#endif
-}
-QM_HD c128 ld_pred(SpaceGlobal, const c128 *p, bool pred) {
-#ifdef __CUDA_ARCH__
-    c128 v;
-    asm volatile("{ .reg .pred q; setp.ne.u32 q, %3, 0; mov.f64 %0, 0d0000000000000000; mov.f64 %1, 0d0000000000000000;\n"
-                 "  @q ld.global.v2.f64 {%0, %1}, [%2]; }"
-                 : "=d"(v.x), "=d"(v.y) : "l"(p), "r"((unsigned)pred) : "memory");
-    return v;
-#else
-    return pred ? *p : c128{0.0, 0.0};
-#endif
-}
-QM_HD void st_pred(SpaceShared, c128 *p, c128 v, bool pred) {
-#ifdef __CUDA_ARCH__
-    asm volatile("{ .reg .pred q; setp.ne.u32 q, %3, 0; @q st.shared.v2.f64 [%0], {%1, %2}; }"
-                 :: "r"((unsigned)__cvta_generic_to_shared(p)), "d"(v.x), "d"(v.y), "r"((unsigned)pred) : "memory");
-#else
-    if (pred) *p = v;
-#endif
-}
-QM_HD void st_pred(SpaceGlobal, c128 *p, c128 v, bool pred) {
-#ifdef __CUDA_ARCH__
-    asm volatile("{ .reg .pred q; setp.ne.u32 q, %3, 0; @q st.global.v2.f64 [%0], {%1, %2}; }"
-                 :: "l"(p), "d"(v.x), "d"(v.y), "r"((unsigned)pred) : "memory");
-#else
-    if (pred) *p = v;
-#endif
-}
-// Backward step 1 with pruned input: src = first stored element of the line, estride = R2*stride (elements
-// between n and n+1); writes the full padded line `dst`.
-template <class C, class SP, class P, class TW>
-QM_HD void prunedA_step1(SP sp, const P src, int estride, const Pruned pr, c128 *dst, int u, const TW &tw) {
+// Backward step 1 with pruned input.  src: pointer-like (const c128 *, WView, SLine) to the first stored element
+// of the line, estride = R2*stride (elements between n and n+1); writes the full padded line `dst`.
+// Interval 1 lies below N/2 and interval 2 at or above it (host tables), so for most n the interval is known at
+// compile time and the access is base + immediate under one mask-bit test.
+template <class C, class P, class L, class TW>
+QM_HD void prunedA_step1(const P src, int estride, const Pruned pr, const L dst, int u, const TW &tw) {
     if (u >= C::R2) return;
     c128 t[C::R1];
-    // interval 1 lies below N/2 and interval 2 at or above it (host tables), so for most n1 the interval is
-    // known at compile time and the access is base + immediate under one mask-bit test
     const P p1 = src + pr.c1, p2 = src + pr.c2;
     const unsigned mm = pr.m1 | pr.m2;
     static_for<C::R1>([&](auto I) {
         constexpr int n1 = decltype(I)::value;
-        if constexpr (2 * (n1 + 1) * C::R2 <= C::N) t[n1] = ld_pred(sp, qm_ptr(p1 + n1 * estride), (mm & (1u << n1)) != 0u);
-        else if constexpr (2 * n1 * C::R2 >= C::N) t[n1] = ld_pred(sp, qm_ptr(p2 + n1 * estride), (mm & (1u << n1)) != 0u);
+        if constexpr (2 * (n1 + 1) * C::R2 <= C::N) t[n1] = ld_pred(p1 + n1 * estride, (mm & (1u << n1)) != 0u);
+        else if constexpr (2 * n1 * C::R2 >= C::N) t[n1] = ld_pred(p2 + n1 * estride, (mm & (1u << n1)) != 0u);
         else {
             const bool in2 = (pr.m2 >> n1) & 1u;
-            t[n1] = ld_pred(sp, qm_ptr((in2 ? p2 : p1) + n1 * estride), (mm & (1u << n1)) != 0u);
+            t[n1] = ld_pred((in2 ? p2 : p1) + n1 * estride, (mm & (1u << n1)) != 0u);
         }
     });
     Dft<C::R1, +1>::run(t);
@@ -186,18 +158,18 @@ QM_HD void prunedA_step1(SP sp, const P src, int estride, const Pruned pr, c128 
 // can exist, Q = ceil(R1 / 4).  They are fetched ahead of time into 2Q registers (prefetch_quarter) and the
 // transform is started later from those registers (prunedA_step1_pre).
 template <class C> struct Quarter { static constexpr int Q = (C::R1 + 3) / 4; };
-template <class C, class SP, class P>
-QM_HD void prefetch_quarter(SP sp, const P src, int estride, const Pruned pr, c128 (&pre)[2 * Quarter<C>::Q]) {
+template <class C, class P>
+QM_HD void prefetch_quarter(const P src, int estride, const Pruned pr, c128 (&pre)[2 * Quarter<C>::Q]) {
     constexpr int Q = Quarter<C>::Q;
     const P p1 = src + pr.c1, p2 = src + pr.c2;
     static_for<Q>([&](auto I) {
         constexpr int j = decltype(I)::value;
-        pre[j] = ld_pred(sp, qm_ptr(p1 + j * estride), (pr.m1 >> j) & 1u);
-        pre[Q + j] = ld_pred(sp, qm_ptr(p2 + (C::R1 - Q + j) * estride), (pr.m2 >> (C::R1 - Q + j)) & 1u);
+        pre[j] = ld_pred(p1 + j * estride, (pr.m1 >> j) & 1u);
+        pre[Q + j] = ld_pred(p2 + (C::R1 - Q + j) * estride, (pr.m2 >> (C::R1 - Q + j)) & 1u);
     });
 }
-template <class C, class TW>
-QM_HD void prunedA_step1_pre(const c128 (&pre)[2 * Quarter<C>::Q], c128 *dst, int u, const TW &tw) {
+template <class C, class L, class TW>
+QM_HD void prunedA_step1_pre(const c128 (&pre)[2 * Quarter<C>::Q], const L dst, int u, const TW &tw) {
     if (u >= C::R2) return;
     constexpr int Q = Quarter<C>::Q;
     c128 t[C::R1];
@@ -214,8 +186,8 @@ QM_HD void prunedA_step1_pre(const c128 (&pre)[2 * Quarter<C>::Q], c128 *dst, in
     });
 }
 // Forward step 2 with pruned output: reads the full padded line `srcline`, stores only what exists.
-template <class C, class SP, class P>
-QM_HD void prunedB_step2(SP sp, const c128 *srcline, const P dst, int estride, const Pruned pr, int u) {
+template <class C, class L, class P>
+QM_HD void prunedB_step2(const L srcline, const P dst, int estride, const Pruned pr, int u) {
     if (u >= C::R2) return;
     c128 t[C::R1];
     static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = srcline[a * C::R2P + u]; });
@@ -224,17 +196,17 @@ QM_HD void prunedB_step2(SP sp, const c128 *srcline, const P dst, int estride, c
     const unsigned mm = pr.m1 | pr.m2;
     static_for<C::R1>([&](auto I) {
         constexpr int c = decltype(I)::value;
-        if constexpr (2 * (c + 1) * C::R2 <= C::N) st_pred(sp, qm_ptr(p1 + c * estride), t[c], (mm & (1u << c)) != 0u);
-        else if constexpr (2 * c * C::R2 >= C::N) st_pred(sp, qm_ptr(p2 + c * estride), t[c], (mm & (1u << c)) != 0u);
+        if constexpr (2 * (c + 1) * C::R2 <= C::N) st_pred(p1 + c * estride, t[c], (mm & (1u << c)) != 0u);
+        else if constexpr (2 * c * C::R2 >= C::N) st_pred(p2 + c * estride, t[c], (mm & (1u << c)) != 0u);
         else {
             const bool in2 = (pr.m2 >> c) & 1u;
-            st_pred(sp, qm_ptr((in2 ? p2 : p1) + c * estride), t[c], (mm & (1u << c)) != 0u);
+            st_pred((in2 ? p2 : p1) + c * estride, t[c], (mm & (1u << c)) != 0u);
         }
     });
 }
 // Quarter-rule form of the pruned forward step 2: only the first Q and last Q outputs of a thread can exist.
-template <class C, class SP, class P>
-QM_HD void prunedB_step2_quarter(SP sp, const c128 *srcline, const P dst, int estride, const Pruned pr, int u) {
+template <class C, class L, class P>
+QM_HD void prunedB_step2_quarter(const L srcline, const P dst, int estride, const Pruned pr, int u) {
     if (u >= C::R2) return;
     constexpr int Q = Quarter<C>::Q;
     c128 t[C::R1];
@@ -244,29 +216,20 @@ QM_HD void prunedB_step2_quarter(SP sp, const c128 *srcline, const P dst, int es
     static_for<Q>([&](auto I) {
         constexpr int j = decltype(I)::value;
         constexpr int c2 = C::R1 - Q + j;
-        st_pred(sp, qm_ptr(p1 + j * estride), t[j], (pr.m1 >> j) & 1u);
-        st_pred(sp, qm_ptr(p2 + c2 * estride), t[c2], (pr.m2 >> c2) & 1u);
+        st_pred(p1 + j * estride, t[j], (pr.m1 >> j) & 1u);
+        st_pred(p2 + c2 * estride, t[c2], (pr.m2 >> c2) & 1u);
     });
 }
 
-template <class C, class TW> QM_HD void lineA_step1(c128 *line, int u, const TW &tw) {
-    if (u >= C::R2) return;
-    c128 t[C::R1];
-    static_for<C::R1>([&](auto I) { constexpr int n1 = decltype(I)::value; t[n1] = line[n1 * C::R2P + u]; });
-    Dft<C::R1, +1>::run(t);
-    static_for<C::R1>([&](auto I) {
-        constexpr int k1 = decltype(I)::value;
-        line[k1 * C::R2P + u] = (k1 == 0) ? t[k1] : cmul_conj(t[k1], tw.template get<k1>());
-    });
-}
-template <class C> QM_HD void lineA_step2(c128 *line, int u) {
+// ---- full (unpruned) in-place passes ---------------------------------------------------------------------
+template <class C, class L> QM_HD void lineA_step2(const L line, int u) {
     if (u >= C::R1) return;
     c128 t[C::R2];
     static_for<C::R2>([&](auto I) { constexpr int n2 = decltype(I)::value; t[n2] = line[u * C::R2P + n2]; });
     Dft<C::R2, +1>::run(t);
     static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; line[u * C::R2P + k2] = t[k2]; });
 }
-template <class C, class TW> QM_HD void lineB_step1(c128 *line, int u, const TW &tw) {
+template <class C, class L, class TW> QM_HD void lineB_step1(const L line, int u, const TW &tw) {
     if (u >= C::R1) return;
     c128 t[C::R2];
     static_for<C::R2>([&](auto I) { constexpr int b = decltype(I)::value; t[b] = line[u * C::R2P + b]; });
@@ -276,29 +239,23 @@ template <class C, class TW> QM_HD void lineB_step1(c128 *line, int u, const TW 
         line[u * C::R2P + d] = (d == 0) ? t[d] : cmul(t[d], tw.template get<d>());
     });
 }
-template <class C> QM_HD void lineB_step2(c128 *line, int u) {
-    if (u >= C::R2) return;
-    c128 t[C::R1];
-    static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = line[a * C::R2P + u]; });
-    Dft<C::R1, -1>::run(t);
-    static_for<C::R1>([&](auto I) { constexpr int c = decltype(I)::value; line[c * C::R2P + u] = t[c]; });
-}
 
 // ---- z kernels: one shared-memory round trip per stick ------------------------------------------------
-// zinv pass 2: thread (stick t, row u) finishes the backward transform and writes the stick planes
-// W[p = u*R2 + k2][s] straight from registers (lanes run over sticks => contiguous 16-byte stores).
-template <class C> QM_HD void zinv_step2_store(const c128 *line, c128 *Wcol, long pstride, int u) {
+// zinv pass 2: thread (stick t, row u) finishes the backward transform and writes plane labels p = u*R2 + k2
+// of its stick into the staging block [N][QM_ZT] (lanes run over sticks => contiguous 16-byte stores).
+template <class C, class L> QM_HD void zinv_step2_store(const L line, const L stagecol, int pstride, int u) {
     if (u >= C::R1) return;
     c128 t[C::R2];
     static_for<C::R2>([&](auto I) { constexpr int n2 = decltype(I)::value; t[n2] = line[u * C::R2P + n2]; });
     Dft<C::R2, +1>::run(t);
-    static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; Wcol[(long)(u * C::R2 + k2) * pstride] = t[k2]; });
+    static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; stagecol[(u * C::R2 + k2) * pstride] = t[k2]; });
 }
-// zfwd pass 1: thread (stick t, row u) reads W[p = u*R2 + b][s] into registers and starts the forward transform.
-template <class C, class TW> QM_HD void zfwd_step1_load(const c128 *Wcol, long pstride, c128 *line, int u, const TW &tw) {
+// zfwd pass 1: thread (stick t, row u) reads plane labels p = u*R2 + b of its stick from the staging block and
+// starts the forward transform.
+template <class C, class L, class TW> QM_HD void zfwd_step1_load(const L stagecol, int pstride, const L line, int u, const TW &tw) {
     if (u >= C::R1) return;
     c128 t[C::R2];
-    static_for<C::R2>([&](auto I) { constexpr int b = decltype(I)::value; t[b] = Wcol[(long)(u * C::R2 + b) * pstride]; });
+    static_for<C::R2>([&](auto I) { constexpr int b = decltype(I)::value; t[b] = stagecol[(u * C::R2 + b) * pstride]; });
     Dft<C::R2, -1>::run(t);
     static_for<C::R2>([&](auto I) {
         constexpr int d = decltype(I)::value;
@@ -307,8 +264,8 @@ template <class C, class TW> QM_HD void zfwd_step1_load(const c128 *Wcol, long p
 }
 // zfwd pass 2: finishes the forward transform and gathers to the sphere with the kinetic term fused
 // (PAPER.md:668-674): out[g] = (V psi)(G) + 1/2 |k+G|^2 psi_in[g] for the G of this stick only.
-template <class C> QM_HD void zfwd_step2_gather(const c128 *line, c128 *out, const c128 *psi_in, const double *g2,
-                                                 const Pruned pr, int u, bool kinetic) {
+template <class C, class L> QM_HD void zfwd_step2_gather(const L line, c128 *out, const c128 *psi_in, const double *g2,
+                                                          const Pruned pr, int u, bool kinetic) {
     if (u >= C::R2) return;
     c128 t[C::R1];
     static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = line[a * C::R2P + u]; });
@@ -324,7 +281,6 @@ template <class C> QM_HD void zfwd_step2_gather(const c128 *line, c128 *out, con
         }
     });
 }
-
 // Quarter-rule forms of the gather (see Quarter): the 1/2|k+G|^2 psi_in terms of the <= 2Q outputs a thread can
 // own are fetched ahead of the transform (prefetch_kin) and added when the outputs are stored.
 template <class C> QM_HD void prefetch_kin(const c128 *psi_in, const double *g2, const Pruned pr, bool kinetic,
@@ -334,14 +290,14 @@ template <class C> QM_HD void prefetch_kin(const c128 *psi_in, const double *g2,
         constexpr int j = decltype(I)::value;
         const int o1 = pr.c1 + j * C::R2, o2 = pr.c2 + (C::R1 - Q + j) * C::R2;
         const bool q1 = kinetic && ((pr.m1 >> j) & 1u), q2 = kinetic && ((pr.m2 >> (C::R1 - Q + j)) & 1u);
-        const c128 x1 = ld_pred(SpaceGlobal{}, psi_in + o1, q1), x2 = ld_pred(SpaceGlobal{}, psi_in + o2, q2);
+        const c128 x1 = ld_pred(psi_in + o1, q1), x2 = ld_pred(psi_in + o2, q2);
         const double h1 = q1 ? 0.5 * g2[o1] : 0.0, h2 = q2 ? 0.5 * g2[o2] : 0.0;
         kin[j] = c128{h1 * x1.x, h1 * x1.y};
         kin[Q + j] = c128{h2 * x2.x, h2 * x2.y};
     });
 }
-template <class C> QM_HD void zfwd_step2_gather_pre(const c128 *line, c128 *out, const Pruned pr, int u,
-                                                     const c128 (&kin)[2 * Quarter<C>::Q]) {
+template <class C, class L> QM_HD void zfwd_step2_gather_pre(const L line, c128 *out, const Pruned pr, int u,
+                                                              const c128 (&kin)[2 * Quarter<C>::Q]) {
     if (u >= C::R2) return;
     constexpr int Q = Quarter<C>::Q;
     c128 t[C::R1];
@@ -350,35 +306,15 @@ template <class C> QM_HD void zfwd_step2_gather_pre(const c128 *line, c128 *out,
     static_for<Q>([&](auto I) {
         constexpr int j = decltype(I)::value;
         constexpr int c2 = C::R1 - Q + j;
-        st_pred(SpaceGlobal{}, out + pr.c1 + j * C::R2, t[j] + kin[j], (pr.m1 >> j) & 1u);
-        st_pred(SpaceGlobal{}, out + pr.c2 + c2 * C::R2, t[c2] + kin[Q + j], (pr.m2 >> c2) & 1u);
+        st_pred(out + pr.c1 + j * C::R2, t[j] + kin[j], (pr.m1 >> j) & 1u);
+        st_pred(out + pr.c2 + c2 * C::R2, t[c2] + kin[Q + j], (pr.m2 >> c2) & 1u);
     });
 }
 
-// ---- x direction of the plane kernel: X compact rows <-> full length-N1 line in scratch -------------
-// A: plane array [X][rowpitch].  The occupied box indices i1 form two intervals (the sphere is convex):
-// [a1,b1] -> rows 0.., [a2,b2] -> rows (b1-a1+1)..; everything else is not stored (zero).
-struct XRows {
-    int a1, b1, a2, b2;
-    QM_HD int row(int i1) const {
-        return (i1 >= a1 && i1 <= b1) ? i1 - a1 : ((i1 >= a2 && i1 <= b2) ? i1 - a2 + (b1 - a1 + 1) : -1);
-    }
-};
-template <class C, class TW> QM_HD void xcol_step1(const c128 *A, int rowpitch, int colpos, const XRows xr,
-                                                   c128 *scr, int u, const TW &tw) {
-    if (u >= C::R2) return;
-    c128 t[C::R1];
-    static_for<C::R1>([&](auto I) {
-        constexpr int n1 = decltype(I)::value;
-        const int r = xr.row(n1 * C::R2 + u);
-        t[n1] = (r >= 0) ? A[r * rowpitch + colpos] : c128{0.0, 0.0};
-    });
-    Dft<C::R1, +1>::run(t);
-    static_for<C::R1>([&](auto I) {
-        constexpr int k1 = decltype(I)::value;
-        scr[k1 * C::R2P + u] = (k1 == 0) ? t[k1] : cmul_conj(t[k1], tw.template get<k1>());
-    });
-}
+// ---- x direction of the plane kernel -----------------------------------------------------------------------
+// The occupied box indices i1 form two intervals (the sphere is convex): [a1,b1] -> plane rows 0..,
+// [a2,b2] -> the following rows; everything else is not stored (zero).  Steps 1 and 3 of a column are
+// prunedA_step1 / prunedB_step2 on the plane array with stride = row pitch; step 2 works on the scratch line:
 // MODE 0: apply  (backward step 2, multiply by v[x], forward step 1)      PAPER.md:659-662 (eq. 47)
 // MODE 1: g2r    (backward step 2, write psi(r)*scale to box, stop)
 // MODE 2: r2g    (read box, forward step 1)
@@ -403,8 +339,8 @@ template <class C> QM_HD void load_vrow(VRow<C::R2> &vr, const double *vcol, int
         if constexpr (2 * j + 1 < C::R2) vr.v[2 * j + 1] = d.y;
     });
 }
-template <class C, int MODE, class TW> QM_HD void xcol_step2(c128 *scr, int u, const TW &tw, const VRow<C::R2> &vr,
-                                                             c128 *box, long xstride, double scale) {
+template <class C, int MODE, class L, class TW>
+QM_HD void xcol_step2(const L scr, int u, const TW &tw, const VRow<C::R2> &vr, c128 *box, long xstride, double scale) {
     if (u >= C::R1) return;
     c128 t[C::R2];
     if constexpr (MODE == 2) {
@@ -423,17 +359,5 @@ template <class C, int MODE, class TW> QM_HD void xcol_step2(c128 *scr, int u, c
     static_for<C::R2>([&](auto I) {
         constexpr int d = decltype(I)::value;
         scr[u * C::R2P + d] = (d == 0) ? t[d] : cmul(t[d], tw.template get<d>());
-    });
-}
-template <class C> QM_HD void xcol_step3(c128 *A, int rowpitch, int colpos, const XRows xr,
-                                         const c128 *scr, int u) {
-    if (u >= C::R2) return;
-    c128 t[C::R1];
-    static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = scr[a * C::R2P + u]; });
-    Dft<C::R1, -1>::run(t);
-    static_for<C::R1>([&](auto I) {
-        constexpr int c = decltype(I)::value;
-        const int r = xr.row(u + C::R2 * c);
-        if (r >= 0) A[r * rowpitch + colpos] = t[c];
     });
 }

@@ -23,6 +23,9 @@ template <class T> void dump(const std::string &path, const std::vector<T> &v) {
     FILE *f = fopen(path.c_str(), "wb"); fwrite(v.data(), sizeof(T), v.size(), f); fclose(f);
 }
 
+struct RowInfo { int a1, b1, a2, b2, sbase; };
+struct XRows { int a1, b1, a2, b2; };
+
 template <class C> struct Emu {
     static constexpr int LP = C::L | 1, SL = C::L | 1, TS = 16;
     const QmKTables &kp; QmAxis ax; std::vector<c128> tw;
@@ -45,11 +48,11 @@ template <class C> struct Emu {
             std::vector<c128> lines(TS * LP, c128{1e300, -1e300});
             for (int tid = 0; tid < nthr; ++tid) {
                 int t = tid / C::TT, u = tid % C::TT;
-                if (t < ns) { const int4 q = kp.stickinfo[s0 + t]; prunedA_step1<C>(SpaceGlobal{}, psi + q.z, C::R2, stick_pruned(q, u), &lines[t * LP], u, rowA(u)); }
+                if (t < ns) { const int4 q = kp.stickinfo[s0 + t]; prunedA_step1<C>(psi + q.z, C::R2, stick_pruned(q, u), qm_sline(&lines[t * LP]), u, rowA(u)); }
             }
             for (int tid = 0; tid < nthr; ++tid) {
                 int t = tid % TS, u = tid / TS;
-                if (t < ns) zinv_step2_store<C>(&lines[t * LP], W + (size_t)(s0 / TS) * C::N * QM_ZT + t, QM_ZT, u);
+                if (t < ns) zinv_step2_store<C>(qm_sline(&lines[t * LP]), qm_sline(W + (size_t)(s0 / TS) * C::N * QM_ZT + t), QM_ZT, u);
             }
         }
     }
@@ -60,11 +63,11 @@ template <class C> struct Emu {
             std::vector<c128> lines(TS * LP, c128{1e300, -1e300});
             for (int tid = 0; tid < nthr; ++tid) {
                 int t = tid % TS, u = tid / TS;
-                if (t < ns) zfwd_step1_load<C>(W + (size_t)(s0 / TS) * C::N * QM_ZT + t, QM_ZT, &lines[t * LP], u, rowB(u));
+                if (t < ns) zfwd_step1_load<C>(qm_sline(W + (size_t)(s0 / TS) * C::N * QM_ZT + t), QM_ZT, qm_sline(&lines[t * LP]), u, rowB(u));
             }
             for (int tid = 0; tid < nthr; ++tid) {
                 int t = tid / C::TT, u = tid % C::TT;
-                if (t < ns) { const int4 q = kp.stickinfo[s0 + t]; zfwd_step2_gather<C>(&lines[t * LP], out + q.z, kinetic ? psi_in + q.z : nullptr, kp.g2.data() + q.z, stick_pruned(q, u), u, kinetic); }
+                if (t < ns) { const int4 q = kp.stickinfo[s0 + t]; zfwd_step2_gather<C>(qm_sline(&lines[t * LP]), out + q.z, kinetic ? psi_in + q.z : nullptr, kp.g2.data() + q.z, stick_pruned(q, u), u, kinetic); }
             }
         }
     }
@@ -83,9 +86,9 @@ template <class C> struct Emu {
                 const RowInfo ri = row_info(task / C::TT);
                 const int u = task % C::TT;
                 const Pruned pr = make_pruned<C>(ri.a1, ri.b1, ri.a2, ri.b2, u, 1);
-                prunedA_step1<C>(SpaceGlobal{}, Wp + ri.sbase, C::R2, pr, &A[(task / C::TT) * rp], u, rowA(u));
+                prunedA_step1<C>(Wp + ri.sbase, C::R2, pr, qm_sline(&A[(task / C::TT) * rp]), u, rowA(u));
             }
-            for (int task = 0; task < X * C::TT; ++task) lineA_step2<C>(&A[(task / C::TT) * rp], task % C::TT);
+            for (int task = 0; task < X * C::TT; ++task) lineA_step2<C>(qm_sline(&A[(task / C::TT) * rp]), task % C::TT);
         }
         const int z = (p / ax.r2) + ax.r1 * (p % ax.r2);
         const XRows xr{kp.xiv.x, kp.xiv.y, kp.xiv.z, kp.xiv.w};
@@ -93,7 +96,7 @@ template <class C> struct Emu {
             if (MODE != 2)
                 for (int tid = 0; tid < nthr; ++tid) {
                     int c = tid / C::TT, u = tid % C::TT, col = cbase + c;
-                    if (col < C::N) prunedA_step1<C>(SpaceShared{}, A.data() + C::pos(col), C::R2 * rp, make_pruned<C>(xr.a1, xr.b1, xr.a2, xr.b2, u, rp), &scr[(size_t)c * SL], u, rowA(u));
+                    if (col < C::N) prunedA_step1<C>(qm_sline(A.data() + C::pos(col)), C::R2 * rp, make_pruned<C>(xr.a1, xr.b1, xr.a2, xr.b2, u, rp), qm_sline(&scr[(size_t)c * SL]), u, rowA(u));
                 }
             for (int tid = 0; tid < nthr; ++tid) {
                 int c = tid / C::TT, u = tid % C::TT, col = cbase + c;
@@ -102,20 +105,20 @@ template <class C> struct Emu {
                 VRow<C::R2> vr;
                 if (MODE == 0) load_vrow<C>(vr, vt + ((size_t)p * C::N + col) * VLayout<C>::COL, u);
                 c128 *bx = MODE == 0 ? nullptr : box + (size_t)y * n3 + z;
-                xcol_step2<C, MODE>(&scr[(size_t)c * SL], u, rowB(u), vr, bx, (long)C::N * n3, scale);
+                xcol_step2<C, MODE>(qm_sline(&scr[(size_t)c * SL]), u, rowB(u), vr, bx, (long)C::N * n3, scale);
             }
             if (MODE != 1)
                 for (int tid = 0; tid < nthr; ++tid) {
                     int c = tid / C::TT, u = tid % C::TT, col = cbase + c;
-                    if (col < C::N) prunedB_step2<C>(SpaceShared{}, &scr[(size_t)c * SL], A.data() + C::pos(col), C::R2 * rp, make_pruned<C>(xr.a1, xr.b1, xr.a2, xr.b2, u, rp), u);
+                    if (col < C::N) prunedB_step2<C>(qm_sline(&scr[(size_t)c * SL]), qm_sline(A.data() + C::pos(col)), C::R2 * rp, make_pruned<C>(xr.a1, xr.b1, xr.a2, xr.b2, u, rp), u);
                 }
         }
         if (MODE != 1) {
-            for (int task = 0; task < X * C::TT; ++task) lineB_step1<C>(&A[(task / C::TT) * rp], task % C::TT, rowB(task % C::TT));
+            for (int task = 0; task < X * C::TT; ++task) lineB_step1<C>(qm_sline(&A[(task / C::TT) * rp]), task % C::TT, rowB(task % C::TT));
             for (int task = 0; task < X * C::TT; ++task) {
                 const RowInfo ri = row_info(task / C::TT);
                 const int u = task % C::TT;
-                prunedB_step2<C>(SpaceGlobal{}, &A[(task / C::TT) * rp], Wp + ri.sbase, C::R2, make_pruned<C>(ri.a1, ri.b1, ri.a2, ri.b2, u, 1), u);
+                prunedB_step2<C>(qm_sline(&A[(task / C::TT) * rp]), Wp + ri.sbase, C::R2, make_pruned<C>(ri.a1, ri.b1, ri.a2, ri.b2, u, 1), u);
             }
         }
     }
