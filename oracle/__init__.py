@@ -12,11 +12,13 @@ Parts:
                       (dense-matrix numpy form for small N_G; the same triple
                       sum as explicit C loops in hpsi_direct.c for large N_G)
   O3  dft.py          naive DFT straight from the definition (8^3-size checks)
+  O5  subspace.py     subspace products <psi_i|phi_j>
 
 Pins (tests/test_oracle_*.py, ``-m "not gpu"``): the paper's printed bcc
 example, closed-form plane-wave
 eigenvalues, single-Fourier-component shift, rank-1 projector, Hermiticity,
-naive-DFT brute force on 8^3, numpy fftn identity.
+naive-DFT brute force on 8^3, numpy fftn identity; for O5 unit
+vectors, a geometric-sequence closed form, the inner-product axioms, np.vdot.
 Parity unpinned: none of the functions here; absolute physical energies of
 real Si are out of scope (no pseudopotential data).
 """
