@@ -246,6 +246,22 @@ def run_ours(args):
     prof = qm.qm_profile_read(gs.handle)
     qm.qm_profile_enable(gs.handle, False)
 
+    # next row of the scope table: subspace products <psi_i|H psi_j>, all bands x all bands and one
+    # call batch x one call batch, device-timed outside the step timing above (own figure, not part of `value`)
+    sub = {}
+    for tag, n_sub in (("all_bands", nb), ("call_batch", cb)):
+        a_sub, b_sub = psi_dev[0][:n_sub], out_dev[0][:n_sub]
+        s_sub = gs.subspace(a_sub, b_sub)
+        torch.cuda.synchronize()
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 3
+        s0.record()
+        for _ in range(reps):
+            gs.subspace(a_sub, b_sub, s_sub)
+        s1.record()
+        torch.cuda.synchronize()
+        sub[tag] = (n_sub, s0.elapsed_time(s1) / reps)
+
     # end to end through the host entry: pinned host buffers, copies inside the timed region
     hin = [p.cpu().pin_memory() for p in psi_dev]
     hout = [torch.empty_like(h).pin_memory() for h in hin]
@@ -336,6 +352,10 @@ def run_ours(args):
                 "gpu_launches": int(launches),
                 "roofline": roofline, "fft_path": fft_path, "kernels": kernels,
                 "fp64_peaks_tflops": {"dmma_probe": dmma_peak, "dfma_probe": dfma_peak},
+                "subspace": {tag: {"na": n, "nb": n, "ng": ng, "ms": t_ms, "bound": "tensor",
+                                   "achieved": 8.0 * n * n * ng / (t_ms * 1e-3) / 1e12, "peak": dmma_peak,
+                                   "unit": "TFLOP/s", "frac": 8.0 * n * n * ng / (t_ms * 1e-3) / 1e12 / dmma_peak}
+                             for tag, (n, t_ms) in sub.items()},
                 "cpu_baseline": cpu}
         print(json.dumps(line))
     if world > 1:

@@ -98,6 +98,16 @@ QM_API int qm_set_nonlocal(qm_gspace *g, int k, const qm_c128 *beta_kG_dev, int 
 QM_API int qm_apply_h(qm_gspace *g, const qm_c128 *psi_in_dev, qm_c128 *psi_out_dev,
                int nbands, int k, void *stream);
 
+/* Subspace products S[i][j] = <a_i|b_j> = sum_G conj(a_i(G)) b_j(G) over the sphere of k-point k: the step right
+ * after h_psi in the Davidson solver, the paper's WavefunG.vdot(psi, phi) = ZGEMM.
+ * With b = H a this is the subspace Hamiltonian, with b = a the overlap matrix.  Plain sum, no volume factor.
+ *  a_dev  DEVICE  [na][ng(k)] row-major complex128     b_dev  DEVICE  [nb][ng(k)] row-major complex128
+ *  s_dev  DEVICE  [na][nb] row-major complex128, overwritten; must not overlap a or b.  a == b is allowed.
+ * FP64 tensor cores (DMMA), split-K with a fixed-order reduction (bitwise reproducible).  Only enqueues on `stream`;
+ * the split-K workspace is library owned and grown on first use. */
+QM_API int qm_subspace(qm_gspace *g, int k, const qm_c128 *a_dev, int na, const qm_c128 *b_dev, int nb,
+                qm_c128 *s_dev, void *stream);
+
 /* Same operation with HOST buffers (pinned memory recommended): the library copies psi_in to
  * a library-owned device buffer, applies H, copies the result back, all on `stream`, then
  * synchronises the stream.  This is the end-to-end entry bench.py times. */
@@ -136,7 +146,9 @@ typedef enum {
     QM_K_PREDUCE = 4,   /* split-K reduction of P; with D blocks that divide 16 also Q = D P, fused  (a7) */
     QM_K_DMUL = 5,      /* Q = D P, general block size (separate launch)  (a7) */
     QM_K_PROJ2 = 6,     /* out += beta Q    (DMMA)                      (a8) */
-    QM_K_COUNT = 7
+    QM_K_SUBGEMM = 7,   /* S = A^H B (DMMA, split-K)                     (8(f) rank 1) */
+    QM_K_SUBREDUCE = 8, /* split-K reduction of S */
+    QM_K_COUNT = 9
 } qm_kernel_kind;
 QM_API int qm_profile_enable(qm_gspace *g, int on);
 QM_API int qm_profile_reset(qm_gspace *g);

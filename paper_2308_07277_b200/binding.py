@@ -42,6 +42,7 @@ _SIGS = {
     "qm_set_vloc": [_vp, _vp, _vp],
     "qm_set_nonlocal": [_vp, _i, _vp, _i, _vp, _i, _vp],
     "qm_apply_h": [_vp, _vp, _vp, _i, _i, _vp],
+    "qm_subspace": [_vp, _i, _vp, _i, _vp, _i, _vp, _vp],
     "qm_apply_h_host": [_vp, _vp, _vp, _i, _i, _vp],
     "qm_apply_h_host_async": [_vp, _vp, _vp, _i, _i, _vp],
     "qm_host_synchronize": [_vp],
@@ -54,7 +55,7 @@ _SIGS = {
     "qm_profile_read": [_vp, _i, ctypes.POINTER(_d), ctypes.POINTER(ctypes.c_ulonglong)],
 }
 EXPORTS = sorted(list(_SIGS) + ["qm_last_error", "qm_version", "qm_kernel_name"])
-QM_K_COUNT = 7
+QM_K_COUNT = 9
 
 
 def load_library():
@@ -206,6 +207,21 @@ def qm_apply_h(h, psi_in_dev, psi_out_dev, k=0, stream=None):
     return psi_out_dev
 
 
+def qm_subspace(h, a_dev, b_dev, s_dev=None, k=0, stream=None):
+    """S[i][j] = <a_i|b_j> over the sphere of k-point k (include/qm_hpsi.h); returns the [na][nb] device tensor."""
+    import torch
+    na = _check_block(h, k, a_dev, "a")
+    nb = _check_block(h, k, b_dev, "b")
+    if s_dev is None:
+        s_dev = torch.empty((na, nb), dtype=torch.complex128, device=a_dev.device)
+    if tuple(s_dev.shape) != (na, nb):
+        raise TypeError("s: expected shape [na][nb]")
+    _check(load_library().qm_subspace(h, k, _dev_ptr(a_dev, torch.complex128, "a"), na,
+                                      _dev_ptr(b_dev, torch.complex128, "b"), nb,
+                                      _dev_ptr(s_dev, torch.complex128, "s"), _stream_ptr(stream)))
+    return s_dev
+
+
 def _host_call(fn, h, psi_in_host, psi_out_host, k, stream):
     import torch
     nb = _check_block(h, k, psi_in_host, "psi_in")
@@ -316,6 +332,8 @@ class GSpace:
         if psi_out is None:
             psi_out = torch.empty_like(psi_in)
         return qm_apply_h(self._h, psi_in, psi_out, k, stream)
+
+    def subspace(self, a, b, s=None, k=0, stream=None): return qm_subspace(self._h, a, b, s, k, stream)
 
     def apply_h_host(self, psi_in, psi_out, k=0, stream=None):
         return qm_apply_h_host(self._h, psi_in, psi_out, k, stream)

@@ -13,6 +13,7 @@
 #include "../../include/qm_hpsi.h"
 #include "fft_kernels.cuh"
 #include "proj_kernels.cuh"
+#include "subspace_kernels.cuh"
 #include "qm_plan.h"
 #include "gspace_host.h"
 
@@ -131,7 +132,7 @@ struct qm_gspace {
     bool v_set = false;
     DevBuf<c128> d_W, d_Ppart, d_P;
     DevBuf<double> d_qt;
-    DevBuf<c128> d_part;
+    DevBuf<c128> d_part, d_subpart;
     DevBuf<int> d_pdesc;
     unsigned long long launches = 0;
     int sm_count = 148;
@@ -578,6 +579,35 @@ QM_API int qm_apply_h_host_async(qm_gspace *g, const qm_c128 *psi_in_host, qm_c1
     return QM_OK;
 }
 
+QM_API int qm_subspace(qm_gspace *g, int k, const qm_c128 *a_dev, int na, const qm_c128 *b_dev, int nb,
+                qm_c128 *s_dev, void *stream)
+{
+    int rc = check_handle(g, k); if (rc) return rc;
+    if (!a_dev || !b_dev || !s_dev || na <= 0 || nb <= 0) return fail(QM_EINVAL, "qm_subspace: bad argument");
+    KPoint *kp = g->kpts[k];
+    cudaStream_t st = (cudaStream_t)stream;
+    static bool attr = false;
+    if (!attr) { CU_TRY(cudaFuncSetAttribute(k_sub_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, SG_SMEM)); attr = true; }
+    const int ntm = (na + SG_T - 1) / SG_T, ntn = (nb + SG_T - 1) / SG_T;
+    const int nkc = (kp->ng + SG_KS - 1) / SG_KS;
+    const int nsplit = std::max(1, std::min(nkc, g->sm_count / (ntm * ntn)));
+    const int ldp = ntn * SG_T;
+    const size_t plane = (size_t)ntm * SG_T * ldp;
+    CU_TRY(g->d_subpart.resize(plane * nsplit));
+    g->prof.begin(QM_K_SUBGEMM, st);
+    k_sub_gemm<<<dim3(ntm * ntn, nsplit), (SG_CW + 1) * 32, SG_SMEM, st>>>(
+        reinterpret_cast<const c128 *>(a_dev), na, reinterpret_cast<const c128 *>(b_dev), nb, kp->ng, ntn, nsplit,
+        g->d_subpart.p, ldp);
+    g->prof.end(st);
+    g->prof.begin(QM_K_SUBREDUCE, st);
+    k_sub_reduce<<<(na * nb + 255) / 256, 256, 0, st>>>(g->d_subpart.p, nsplit, plane, ldp, na, nb,
+                                                       reinterpret_cast<c128 *>(s_dev));
+    g->prof.end(st);
+    g->launches += 2;
+    CU_TRY(cudaGetLastError());
+    return QM_OK;
+}
+
 QM_API int qm_apply_h_host(qm_gspace *g, const qm_c128 *psi_in_host, qm_c128 *psi_out_host, int nbands, int k,
                            void *stream) {
     int rc = qm_apply_h_host_async(g, psi_in_host, psi_out_host, nbands, k, stream);
@@ -632,7 +662,7 @@ QM_API int qm_profile_read(qm_gspace *g, int kind, double *total_ms, unsigned lo
 }
 QM_API const char *qm_kernel_name(int kind) {
     static const char *names[QM_K_COUNT] = {"k_zinv", "k_plane", "k_zfwd", "k_proj1", "k_reduce_p", "k_dmul",
-                                            "k_proj2"};
+                                            "k_proj2", "k_sub_gemm", "k_sub_reduce"};
     return (kind >= 0 && kind < QM_K_COUNT) ? names[kind] : "?";
 }
 
