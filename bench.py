@@ -262,6 +262,25 @@ def run_ours(args):
         torch.cuda.synchronize()
         sub[tag] = (n_sub, s0.elapsed_time(s1) / reps)
 
+    # 8(f) rank 2: density accumulation n(r) += f_i |psi_i(r)|^2, one call batch of bands per call, all bands of the config
+    occ_dev = torch.full((nb,), 2.0, dtype=torch.float64, device=dev)
+    rho_dev = torch.empty(int(np.prod(cfg.grid)), dtype=torch.float64, device=dev)
+
+    def density_pass():
+        gs.density_reset()
+        for b0 in range(0, nb, cb):
+            gs.density_accumulate(psi_dev[0][b0:b0 + cb], occ_dev[b0:b0 + cb])
+        gs.density_get(rho_dev)
+
+    density_pass()
+    torch.cuda.synchronize()
+    d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    d0.record()
+    density_pass()
+    d1.record()
+    torch.cuda.synchronize()
+    density_ms = d0.elapsed_time(d1)
+
     # end to end through the host entry: pinned host buffers, copies inside the timed region
     hin = [p.cpu().pin_memory() for p in psi_dev]
     hout = [torch.empty_like(h).pin_memory() for h in hin]
@@ -353,6 +372,10 @@ def run_ours(args):
                 "gpu_launches": int(launches),
                 "roofline": roofline, "fft_path": fft_path, "kernels": kernels,
                 "fp64_peaks_tflops": {"dmma_probe": dmma_peak, "dfma_probe": dfma_peak},
+                "density": {"note": "frac = achieved / peak", "bands": nb, "call_batch": cb, "ms": density_ms, "bands_per_s": nb / (density_ms * 1e-3),
+                            "bound": "alu", "unit": "TFLOP/s", "peak": dmma_peak,
+                            "achieved": nb * N3 * ((nx + cfg.grid[0]) * 5.0 * cfg.grid[0] * np.log2(cfg.grid[0])
+                                                   + 3.0 * cfg.grid[0] * cfg.grid[1]) / (density_ms * 1e-3) / 1e12},
                 "subspace": {tag: {"na": n, "nb": n, "ng": ng, "ms": t_ms, "bound": "tensor",
                                    "achieved": 8.0 * n * n * ng / (t_ms * 1e-3) / 1e12, "peak": dmma_peak,
                                    "unit": "TFLOP/s", "frac": 8.0 * n * n * ng / (t_ms * 1e-3) / 1e12 / dmma_peak}

@@ -98,6 +98,22 @@ QM_API int qm_set_nonlocal(qm_gspace *g, int k, const qm_c128 *beta_kG_dev, int 
 QM_API int qm_apply_h(qm_gspace *g, const qm_c128 *psi_in_dev, qm_c128 *psi_out_dev,
                int nbands, int k, void *stream);
 
+/* Electron density from Bloch states (eq. 2, 1008):  n(r_j) = sum_i f_i |psi_i(r_j)|^2 with
+ * psi_i(r_j) = sum_{G in sphere(k)} psi_i(G) exp(+i G.r_j) (unnormalised synthesis, reading A5/A20; the Bloch phase
+ * exp(i k.r) drops out of |psi|^2), r_j = sum_a (j_a/n_a) a_a.  Scatter, pruned backward FFT and |.|^2 are fused; the
+ * full box of psi(r) is never written.  The running sum lives in library memory between calls:
+ *   qm_density_reset      zero it (allocates on first use);
+ *   qm_density_accumulate add weight * occ[i] * |psi_i(r)|^2 for a block of nbands states at k-point k
+ *                         (call it once per band batch and k-point; weight = the k-point weight);
+ *   qm_density_get        rho[j] = scale * running sum, flat C order over (n1,n2,n3), overwritten.
+ *  psi_dev  DEVICE [nbands][ng(k)] complex128    occ_dev  DEVICE [nbands] doubles    rho_dev  DEVICE [n1*n2*n3] doubles
+ * Every z-plane of the sum is accumulated by one thread block in band order: bitwise reproducible, no atomics.
+ * QM_ENOTSET if accumulate / get come before reset.  All three only enqueue on `stream`. */
+QM_API int qm_density_reset(qm_gspace *g, void *stream);
+QM_API int qm_density_accumulate(qm_gspace *g, int k, const qm_c128 *psi_dev, int nbands, const double *occ_dev,
+                          double weight, void *stream);
+QM_API int qm_density_get(qm_gspace *g, double *rho_dev, double scale, void *stream);
+
 /* Subspace products S[i][j] = <a_i|b_j> = sum_G conj(a_i(G)) b_j(G) over the sphere of k-point k: the step right
  * after h_psi in the Davidson solver, the paper's WavefunG.vdot(psi, phi) = ZGEMM.
  * With b = H a this is the subspace Hamiltonian, with b = a the overlap matrix.  Plain sum, no volume factor.

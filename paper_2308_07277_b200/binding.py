@@ -43,6 +43,9 @@ _SIGS = {
     "qm_set_nonlocal": [_vp, _i, _vp, _i, _vp, _i, _vp],
     "qm_apply_h": [_vp, _vp, _vp, _i, _i, _vp],
     "qm_subspace": [_vp, _i, _vp, _i, _vp, _i, _vp, _vp],
+    "qm_density_reset": [_vp, _vp],
+    "qm_density_accumulate": [_vp, _i, _vp, _i, _vp, _d, _vp],
+    "qm_density_get": [_vp, _vp, _d, _vp],
     "qm_apply_h_host": [_vp, _vp, _vp, _i, _i, _vp],
     "qm_apply_h_host_async": [_vp, _vp, _vp, _i, _i, _vp],
     "qm_host_synchronize": [_vp],
@@ -222,6 +225,26 @@ def qm_subspace(h, a_dev, b_dev, s_dev=None, k=0, stream=None):
     return s_dev
 
 
+def qm_density_reset(h, stream=None):
+    _check(load_library().qm_density_reset(h, _stream_ptr(stream)))
+
+
+def qm_density_accumulate(h, psi_dev, occ_dev, weight=1.0, k=0, stream=None):
+    import torch
+    nb = _check_block(h, k, psi_dev, "psi")
+    if occ_dev.dim() != 1 or occ_dev.shape[0] != nb:
+        raise TypeError("occ: expected shape [nbands]")
+    _check(load_library().qm_density_accumulate(h, k, _dev_ptr(psi_dev, torch.complex128, "psi"), nb,
+                                                _dev_ptr(occ_dev, torch.float64, "occ"), float(weight),
+                                                _stream_ptr(stream)))
+
+
+def qm_density_get(h, rho_dev, scale=1.0, stream=None):
+    import torch
+    _check(load_library().qm_density_get(h, _dev_ptr(rho_dev, torch.float64, "rho"), float(scale), _stream_ptr(stream)))
+    return rho_dev
+
+
 def _host_call(fn, h, psi_in_host, psi_out_host, k, stream):
     import torch
     nb = _check_block(h, k, psi_in_host, "psi_in")
@@ -334,6 +357,18 @@ class GSpace:
         return qm_apply_h(self._h, psi_in, psi_out, k, stream)
 
     def subspace(self, a, b, s=None, k=0, stream=None): return qm_subspace(self._h, a, b, s, k, stream)
+
+    def density_reset(self, stream=None): qm_density_reset(self._h, stream)
+
+    def density_accumulate(self, psi, occ, weight=1.0, k=0, stream=None):
+        qm_density_accumulate(self._h, psi, occ, weight, k, stream)
+
+    def density_get(self, rho=None, scale=1.0, stream=None):
+        import torch
+        if rho is None:
+            rho = torch.empty(int(self.grid[0]) * int(self.grid[1]) * int(self.grid[2]), dtype=torch.float64,
+                              device=torch.device("cuda", torch.cuda.current_device()))
+        return qm_density_get(self._h, rho, scale, stream)
 
     def apply_h_host(self, psi_in, psi_out, k=0, stream=None):
         return qm_apply_h_host(self._h, psi_in, psi_out, k, stream)

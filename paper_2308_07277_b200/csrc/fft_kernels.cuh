@@ -123,7 +123,7 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
     }
 }
 
-// MODE 0 apply, 1 g2r (write natural-order box), 2 r2g (read natural-order box)
+// MODE 0 apply, 1 g2r (write natural-order box), 2 r2g (read natural-order box), 3 density (rho += w |psi(r)|^2)
 //
 // One CTA per (band, z-plane).  The CTA is split into independent groups of G threads (G/TT teams of TT
 // threads, one team per line); a group walks its own rows / columns and only synchronises with itself
@@ -185,7 +185,7 @@ template <class C, int MODE>
 __device__ __forceinline__ void plane_y_phase(const PlaneCtx cx, c128 *__restrict__ W, int pl, int prev, bool have_cur)
 {
     constexpr int G = QM_GROUP, TPG = G / C::TT, RP = C::L | 1, NPRE = 2 * Quarter<C>::Q;
-    constexpr bool HAS_BACK = MODE != 2, HAS_FWD = MODE != 1;
+    constexpr bool HAS_BACK = MODE != 2, HAS_FWD = MODE != 1 && MODE != 3;
     const PlaneIds<C> id;
     const int u = id.u, grp = id.grp, slot = id.slot, X = cx.X, n3 = cx.n3, quarter = cx.quarter;
     const bool do_back = HAS_BACK && have_cur, do_fwd = HAS_FWD && prev >= 0;
@@ -235,7 +235,8 @@ __device__ __forceinline__ void plane_y_phase(const PlaneCtx cx, c128 *__restric
 
 template <class C, int MODE>
 __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_iv, const double *__restrict__ vt,
-                                           c128 *__restrict__ box, int pl, double scale, int stagger_ns)
+                                           c128 *__restrict__ box, int pl, double scale, int stagger_ns,
+                                           double *__restrict__ rhot)
 {
     constexpr int G = QM_GROUP, TPG = G / C::TT, RP = C::L | 1;
     constexpr int SL = qm_scratch_pitch(C::L, C::TT);    // scratch line pitch
@@ -269,7 +270,10 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
             if (ok) prunedA_step1<C>(Acol, C::R2 * RP, px, myscr, u, twa);
             group_barrier<G>(grp);
         }
-        if (ok) {
+        if constexpr (MODE == 3) {
+            // scale = weight * occupation of this band; rhot = running density of this plane in the V layout
+            if (ok) xcol_density<C>(myscr, u, rhot + ((size_t)p * C::N + col) * VLayout<C>::COL, scale);
+        } else if (ok) {
             c128 *bx = nullptr;
             if constexpr (MODE != 0) {
                 const int y = (col / C::R2) + C::R1 * (col % C::R2);
@@ -282,7 +286,7 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
             if (team_ok && ncol < C::N) load_vrow<C>(vr, vplane + (size_t)ncol * VLayout<C>::COL, u);
         }
         group_barrier<G>(grp);
-        if constexpr (MODE != 1) {
+        if constexpr (MODE != 1 && MODE != 3) {
             // no barrier after step 3: the scratch column a thread reads here is exactly the one it
             // overwrites in the next iteration's step 1 (MODE 2 has no step 1 and writes rows: barrier).
             if (ok) prunedB_step2<C>(myscr, Acol, C::R2 * RP, px, u);
@@ -294,7 +298,7 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
 template <class C, int MODE>
 __global__ void __launch_bounds__(QM_PLANE_MAX_THREADS)
 k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ box, int ngroups, double scale,
-        int stagger_ns, int nplanes, int quarter)
+        int stagger_ns, int nplanes, int quarter, const double *__restrict__ occ, double *__restrict__ rhot)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int G = QM_GROUP;
@@ -319,7 +323,21 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
 #define QM_TICK(i) do {} while (0)
 #endif
     const int n3 = cx.n3;
-    for (int pl = blockIdx.x, prev = -1;; prev = pl, pl += gridDim.x) {
+    // plane sequence of this CTA.  Apply / debug modes: pl = blockIdx.x, + gridDim.x, ... (pl = band * n3 + p).
+    // Density mode: the CTA owns z-planes p = blockIdx.x, + gridDim.x, ... and walks ALL bands of a plane before
+    // the next one, so every plane of rho is accumulated by one CTA in band order (deterministic, no atomics).
+    const int nbands = nplanes / n3;
+    auto plane_at = [&](int it) -> int {
+        if constexpr (MODE == 3) {
+            const int p = (int)blockIdx.x + (it / nbands) * (int)gridDim.x;
+            return p < n3 ? (it % nbands) * n3 + p : nplanes;
+        } else {
+            const long long v = (long long)blockIdx.x + (long long)it * gridDim.x;
+            return v < nplanes ? (int)v : nplanes;
+        }
+    };
+    for (int it = 0, prev = -1;; ++it) {
+        const int pl = plane_at(it);
         const bool have_cur = pl < nplanes;
         plane_y_phase<C, MODE>(cx, W, pl, prev, have_cur);
         if (!have_cur) break;
@@ -327,9 +345,12 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
         QM_TICK(0);
         const int p = pl % n3;
         const int z = (p / gd.ax[2].r2) + gd.ax[2].r1 * (p % gd.ax[2].r2);
-        plane_x_phase<C, MODE>(cx, kp.x_iv, gd.vt, box ? box + z : nullptr, pl, scale, stagger_ns);
+        double sc = scale;
+        if constexpr (MODE == 3) sc = scale * occ[pl / n3];
+        plane_x_phase<C, MODE>(cx, kp.x_iv, gd.vt, box ? box + z : nullptr, pl, sc, stagger_ns, rhot);
         __syncthreads();
         QM_TICK(1);
+        prev = pl;
     }
 #ifdef QM_PLANE_TIMING
     QM_TICK(2);

@@ -361,3 +361,20 @@ QM_HD void xcol_step2(const L scr, int u, const TW &tw, const VRow<C::R2> &vr, c
         scr[u * C::R2P + d] = (d == 0) ? t[d] : cmul(t[d], tw.template get<d>());
     });
 }
+// MODE 3 of the plane kernel (density, eq. 2): backward step 2, then rho(x) += w |psi(x)|^2 on this
+// thread's R2 points.  The running density of a plane column is kept in the V layout (VLayout), so the read-modify-
+// write is 16-byte and lane-contiguous; one CTA owns a plane for all bands, so the order of the sums is fixed.
+template <class C, class L> QM_HD void xcol_density(const L scr, int u, double *rhocol, double w) {
+    if (u >= C::R1) return;
+    c128 t[C::R2];
+    static_for<C::R2>([&](auto I) { constexpr int n2 = decltype(I)::value; t[n2] = scr[u * C::R2P + n2]; });
+    Dft<C::R2, +1>::run(t);                          // t[k2] = psi(x = u + R1*k2)
+    double2 *q = reinterpret_cast<double2 *>(rhocol) + u;
+    static_for<VLayout<C>::R2E / 2>([&](auto I) {
+        constexpr int j = decltype(I)::value;
+        double2 d = q[j * C::R1];
+        d.x = fma(w, t[2 * j].x * t[2 * j].x + t[2 * j].y * t[2 * j].y, d.x);
+        if constexpr (2 * j + 1 < C::R2) d.y = fma(w, t[2 * j + 1].x * t[2 * j + 1].x + t[2 * j + 1].y * t[2 * j + 1].y, d.y);
+        q[j * C::R1] = d;
+    });
+}

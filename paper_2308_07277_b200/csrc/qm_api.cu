@@ -128,7 +128,8 @@ struct qm_gspace {
     QmAxis ax[3];
     std::vector<KPoint *> kpts;
     DevBuf<c128> d_tw[3];
-    DevBuf<double> d_vt;
+    DevBuf<double> d_vt, d_rhot;
+    bool rho_open = false;
     bool v_set = false;
     DevBuf<c128> d_W, d_Ppart, d_P;
     DevBuf<double> d_qt;
@@ -223,7 +224,7 @@ template <class C> int launch_zfwd(qm_gspace *g, KPoint *kp, const c128 *psi_in,
     return QM_OK;
 }
 template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *box, int nb, double scale,
-                                              cudaStream_t st) {
+                                              cudaStream_t st, const double *occ = nullptr, double *rhot = nullptr) {
     const int ngroups = plane_groups(g, kp);
     const size_t smem = plane_smem(g, kp, ngroups);
     if (smem > (size_t)g->max_smem)
@@ -233,11 +234,12 @@ template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *bo
     for (int i = 0; i < 3; ++i) { gd.ax[i] = g->ax[i]; gd.tw[i] = g->d_tw[i].p; }
     gd.vt = g->d_vt.p;
     const int nplanes = g->grid[2] * nb;
-    const int grid = std::min(nplanes, g->sm_count);      // persistent: one CTA per SM walks the (band, z-plane) list
+    // persistent: one CTA per SM walks the (band, z-plane) list; density mode: one CTA per z-plane, all bands
+    const int grid = MODE == 3 ? std::min(g->grid[2], g->sm_count) : std::min(nplanes, g->sm_count);
     g->prof.begin(QM_K_PLANE, st);
     k_plane<C, MODE><<<grid, ngroups * PLANE_GROUP, smem, st>>>(kp->plan(), gd, g->d_W.p, box, ngroups, scale,
                                                                    g->plane_stagger_ns, nplanes,
-                                                                   kp->y_quarter ? 1 : 0);
+                                                                   kp->y_quarter ? 1 : 0, occ, rhot);
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
@@ -270,13 +272,33 @@ int dispatch_zfwd(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int n
     }
     return fail(QM_EGRID, "unsupported FFT length (axis 3)");
 }
-template <int MODE> int dispatch_plane(qm_gspace *g, KPoint *kp, c128 *box, int nb, double scale, cudaStream_t st) {
+template <int MODE> int dispatch_plane(qm_gspace *g, KPoint *kp, c128 *box, int nb, double scale, cudaStream_t st,
+                                       const double *occ = nullptr, double *rhot = nullptr) {
     switch (g->grid[0]) {
-#define X(N, A, B) case N: return launch_plane<LineCfg<A, B>, MODE>(g, kp, box, nb, scale, st);
+#define X(N, A, B) case N: return launch_plane<LineCfg<A, B>, MODE>(g, kp, box, nb, scale, st, occ, rhot);
         QM_FOR_SIZES(X)
 #undef X
     }
     return fail(QM_EGRID, "unsupported FFT length (axes 1,2)");
+}
+
+// rho[x][y][z] = scale * rhot[p][col][j][u][e]   (inverse of k_relayout_v's index map; fft_phases.cuh VLayout)
+__global__ void k_density_out(const double *__restrict__ rhot, double *__restrict__ rho, QmAxis a1, QmAxis a2, QmAxis a3,
+                              double scale)
+{
+    const int r2e = a1.r2 + (a1.r2 & 1), colsz = a1.r1 * r2e;
+    const size_t total = (size_t)a3.n * a2.n * colsz;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const int e = (int)(i % colsz);
+        const int u = (e >> 1) % a1.r1, k2 = 2 * ((e >> 1) / a1.r1) + (e & 1);
+        if (k2 >= a1.r2) continue;
+        const int col = (int)((i / colsz) % a2.n);
+        const int p = (int)(i / ((size_t)colsz * a2.n));
+        const int x = u + a1.r1 * k2;
+        const int y = (col / a2.r2) + a2.r1 * (col % a2.r2);
+        const int z = (p / a3.r2) + a3.r1 * (p % a3.r2);
+        rho[((size_t)x * a2.n + y) * a3.n + z] = scale * rhot[i];
+    }
 }
 
 __global__ void k_relayout_v(const double *__restrict__ v, double *__restrict__ vt, QmAxis a1, QmAxis a2, QmAxis a3,
@@ -604,6 +626,38 @@ QM_API int qm_subspace(qm_gspace *g, int k, const qm_c128 *a_dev, int na, const 
                                                        reinterpret_cast<c128 *>(s_dev));
     g->prof.end(st);
     g->launches += 2;
+    CU_TRY(cudaGetLastError());
+    return QM_OK;
+}
+
+static size_t qm_rhot_elems(const qm_gspace *g) {
+    const size_t r2e = (size_t)g->ax[0].r2 + (g->ax[0].r2 & 1);
+    return (size_t)g->grid[2] * g->grid[1] * g->ax[0].r1 * r2e;
+}
+QM_API int qm_density_reset(qm_gspace *g, void *stream) {
+    if (!g) return fail(QM_EINVAL, "null handle");
+    const size_t n = qm_rhot_elems(g);
+    CU_TRY(g->d_rhot.resize(n));
+    CU_TRY(cudaMemsetAsync(g->d_rhot.p, 0, n * sizeof(double), (cudaStream_t)stream));
+    g->rho_open = true;
+    return QM_OK;
+}
+QM_API int qm_density_accumulate(qm_gspace *g, int k, const qm_c128 *psi_dev, int nbands, const double *occ_dev,
+                          double weight, void *stream) {
+    int rc = check_handle(g, k); if (rc) return rc;
+    if (!psi_dev || !occ_dev || nbands <= 0) return fail(QM_EINVAL, "qm_density_accumulate: bad argument");
+    if (!g->rho_open) return fail(QM_ENOTSET, "qm_density_accumulate before qm_density_reset");
+    KPoint *kp = g->kpts[k];
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = ensure_workspace(g, kp, nbands); if (rc) return rc;
+    rc = dispatch_zinv(g, kp, reinterpret_cast<const c128 *>(psi_dev), nbands, st); if (rc) return rc;
+    return dispatch_plane<3>(g, kp, nullptr, nbands, weight, st, occ_dev, g->d_rhot.p);
+}
+QM_API int qm_density_get(qm_gspace *g, double *rho_dev, double scale, void *stream) {
+    if (!g || !rho_dev) return fail(QM_EINVAL, "qm_density_get: null argument");
+    if (!g->rho_open) return fail(QM_ENOTSET, "qm_density_get before qm_density_reset");
+    k_density_out<<<g->sm_count * 4, 256, 0, (cudaStream_t)stream>>>(g->d_rhot.p, rho_dev, g->ax[0], g->ax[1], g->ax[2], scale);
+    g->launches++;
     CU_TRY(cudaGetLastError());
     return QM_OK;
 }
