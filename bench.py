@@ -281,6 +281,20 @@ def run_ours(args):
     torch.cuda.synchronize()
     density_ms = d0.elapsed_time(d1)
 
+    # 8(f) rank 3: Taylor propagator of order 4 (eq. 52) over all bands, one call batch per call
+    def taylor_pass():
+        for b0 in range(0, nb, cb):
+            gs.taylor_propagate(psi_dev[0][b0:b0 + cb], 0.02, 4, out_dev[0][b0:b0 + cb])
+
+    taylor_pass()
+    torch.cuda.synchronize()
+    y0, y1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    y0.record()
+    taylor_pass()
+    y1.record()
+    torch.cuda.synchronize()
+    taylor_ms = y0.elapsed_time(y1)
+
     # end to end through the host entry: pinned host buffers, copies inside the timed region
     hin = [p.cpu().pin_memory() for p in psi_dev]
     hout = [torch.empty_like(h).pin_memory() for h in hin]
@@ -372,6 +386,9 @@ def run_ours(args):
                 "gpu_launches": int(launches),
                 "roofline": roofline, "fft_path": fft_path, "kernels": kernels,
                 "fp64_peaks_tflops": {"dmma_probe": dmma_peak, "dfma_probe": dfma_peak},
+                "taylor": {"order": 4, "bands": nb, "call_batch": cb, "ms": taylor_ms,
+                           "band_steps_per_s": nb / (taylor_ms * 1e-3),
+                           "h_applies_per_s": 4 * nb / (taylor_ms * 1e-3)},
                 "density": {"note": "frac = achieved / peak", "bands": nb, "call_batch": cb, "ms": density_ms, "bands_per_s": nb / (density_ms * 1e-3),
                             "bound": "alu", "unit": "TFLOP/s", "peak": dmma_peak,
                             "achieved": nb * N3 * ((nx + cfg.grid[0]) * 5.0 * cfg.grid[0] * np.log2(cfg.grid[0])

@@ -114,6 +114,14 @@ QM_API int qm_density_accumulate(qm_gspace *g, int k, const qm_c128 *psi_dev, in
                           double weight, void *stream);
 QM_API int qm_density_get(qm_gspace *g, double *rho_dev, double scale, void *stream);
 
+/* Taylor-series propagator of the TDKS equation (eq. 52; the paper's prop_psi()):
+ *   psi_out = sum_{r=0}^{order} (-i dt)^r / r!  H^r psi_in          (dt in atomic units of time, H in Hartree)
+ * as `order` chained qm_apply_h calls with a fused scale-and-accumulate kernel between them; needs qm_set_vloc /
+ * qm_set_nonlocal like qm_apply_h.  psi_in_dev, psi_out_dev DEVICE [nbands][ng(k)] complex128, must not overlap;
+ * psi_out is overwritten.  order == 0 copies.  Two library-owned blocks of the same size are grown on first use. */
+QM_API int qm_taylor_propagate(qm_gspace *g, int k, const qm_c128 *psi_in_dev, qm_c128 *psi_out_dev, int nbands, double dt,
+                        int order, void *stream);
+
 /* Subspace products S[i][j] = <a_i|b_j> = sum_G conj(a_i(G)) b_j(G) over the sphere of k-point k: the step right
  * after h_psi in the Davidson solver, the paper's WavefunG.vdot(psi, phi) = ZGEMM.
  * With b = H a this is the subspace Hamiltonian, with b = a the overlap matrix.  Plain sum, no volume factor.

@@ -9,7 +9,7 @@ from .binding import (  # noqa: F401
     qm_version, qm_fft_size_supported,
     qm_gspace_create, qm_gspace_destroy, qm_gspace_num_k, qm_gspace_num_g, qm_gspace_num_sticks,
     qm_gspace_get_index_map, qm_gspace_get_miller, qm_gspace_get_g2, qm_gspace_alias_free,
-    qm_set_vloc, qm_set_nonlocal, qm_apply_h, qm_subspace, qm_density_reset, qm_density_accumulate, qm_density_get, qm_apply_h_host, qm_apply_h_host_async, qm_host_synchronize, qm_debug_g2r, qm_debug_r2g,
+    qm_set_vloc, qm_set_nonlocal, qm_apply_h, qm_subspace, qm_taylor_propagate, qm_density_reset, qm_density_accumulate, qm_density_get, qm_apply_h_host, qm_apply_h_host_async, qm_host_synchronize, qm_debug_g2r, qm_debug_r2g,
     qm_get_launch_count, qm_probe_fp64_tensor_peak,
     qm_profile_enable, qm_profile_reset, qm_profile_read, qm_kernel_name,
 )

@@ -43,6 +43,7 @@ _SIGS = {
     "qm_set_nonlocal": [_vp, _i, _vp, _i, _vp, _i, _vp],
     "qm_apply_h": [_vp, _vp, _vp, _i, _i, _vp],
     "qm_subspace": [_vp, _i, _vp, _i, _vp, _i, _vp, _vp],
+    "qm_taylor_propagate": [_vp, _i, _vp, _vp, _i, _d, _i, _vp],
     "qm_density_reset": [_vp, _vp],
     "qm_density_accumulate": [_vp, _i, _vp, _i, _vp, _d, _vp],
     "qm_density_get": [_vp, _vp, _d, _vp],
@@ -225,6 +226,17 @@ def qm_subspace(h, a_dev, b_dev, s_dev=None, k=0, stream=None):
     return s_dev
 
 
+def qm_taylor_propagate(h, psi_in_dev, psi_out_dev, dt, order, k=0, stream=None):
+    import torch
+    nb = _check_block(h, k, psi_in_dev, "psi_in")
+    if tuple(psi_out_dev.shape) != tuple(psi_in_dev.shape):
+        raise TypeError("psi_out: shape differs from psi_in")
+    _check(load_library().qm_taylor_propagate(h, k, _dev_ptr(psi_in_dev, torch.complex128, "psi_in"),
+                                              _dev_ptr(psi_out_dev, torch.complex128, "psi_out"), nb, float(dt),
+                                              int(order), _stream_ptr(stream)))
+    return psi_out_dev
+
+
 def qm_density_reset(h, stream=None):
     _check(load_library().qm_density_reset(h, _stream_ptr(stream)))
 
@@ -357,6 +369,12 @@ class GSpace:
         return qm_apply_h(self._h, psi_in, psi_out, k, stream)
 
     def subspace(self, a, b, s=None, k=0, stream=None): return qm_subspace(self._h, a, b, s, k, stream)
+
+    def taylor_propagate(self, psi_in, dt, order, psi_out=None, k=0, stream=None):
+        import torch
+        if psi_out is None:
+            psi_out = torch.empty_like(psi_in)
+        return qm_taylor_propagate(self._h, psi_in, psi_out, dt, order, k, stream)
 
     def density_reset(self, stream=None): qm_density_reset(self._h, stream)
 

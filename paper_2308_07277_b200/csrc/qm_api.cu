@@ -133,7 +133,7 @@ struct qm_gspace {
     bool v_set = false;
     DevBuf<c128> d_W, d_Ppart, d_P;
     DevBuf<double> d_qt;
-    DevBuf<c128> d_part, d_subpart;
+    DevBuf<c128> d_part, d_subpart, d_tay_h, d_tay_t;
     DevBuf<int> d_pdesc;
     unsigned long long launches = 0;
     int sm_count = 148;
@@ -626,6 +626,43 @@ QM_API int qm_subspace(qm_gspace *g, int k, const qm_c128 *a_dev, int na, const 
                                                        reinterpret_cast<c128 *>(s_dev));
     g->prof.end(st);
     g->launches += 2;
+    CU_TRY(cudaGetLastError());
+    return QM_OK;
+}
+
+// one term of the Taylor series: t = c * h (the next power's input), out += t
+__global__ void k_taylor_axpy(const c128 *__restrict__ h, double cr, double ci, c128 *__restrict__ t, c128 *__restrict__ out,
+                              size_t n, int keep_t)
+{
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const c128 x = h[i];
+        const c128 v = c128{cr * x.x - ci * x.y, cr * x.y + ci * x.x};
+        if (keep_t) t[i] = v;
+        c128 o = out[i];
+        o.x += v.x; o.y += v.y;
+        out[i] = o;
+    }
+}
+
+QM_API int qm_taylor_propagate(qm_gspace *g, int k, const qm_c128 *psi_in_dev, qm_c128 *psi_out_dev, int nbands, double dt,
+                        int order, void *stream) {
+    int rc = check_handle(g, k); if (rc) return rc;
+    if (!psi_in_dev || !psi_out_dev || nbands <= 0 || order < 0) return fail(QM_EINVAL, "qm_taylor_propagate: bad argument");
+    KPoint *kp = g->kpts[k];
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n = (size_t)nbands * kp->ng;
+    CU_TRY(g->d_tay_h.resize(n));
+    CU_TRY(g->d_tay_t.resize(n));
+    CU_TRY(cudaMemcpyAsync(psi_out_dev, psi_in_dev, n * sizeof(c128), cudaMemcpyDeviceToDevice, st));     // r = 0 term
+    const qm_c128 *src = psi_in_dev;
+    for (int r = 1; r <= order; ++r) {
+        rc = qm_apply_h(g, src, reinterpret_cast<qm_c128 *>(g->d_tay_h.p), nbands, k, stream); if (rc) return rc;
+        // t_r = (-i dt / r) H t_{r-1}  =>  t_r = (-i dt)^r / r!  H^r psi     (eq. 52)
+        k_taylor_axpy<<<g->sm_count * 8, 256, 0, st>>>(g->d_tay_h.p, 0.0, -dt / r, g->d_tay_t.p,
+                                                       reinterpret_cast<c128 *>(psi_out_dev), n, r < order ? 1 : 0);
+        g->launches++;
+        src = reinterpret_cast<const qm_c128 *>(g->d_tay_t.p);
+    }
     CU_TRY(cudaGetLastError());
     return QM_OK;
 }
