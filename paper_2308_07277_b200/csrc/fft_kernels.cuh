@@ -160,13 +160,11 @@ template <int G> __device__ __forceinline__ void group_barrier(int grp) {
 // row chunks (a row of the plane array is consumed and refilled by the same team), so there are two CTA-wide
 // barriers per plane.  The next plane's stick values of a row are fetched into registers (quarter rule,
 // prefetch_quarter) before the y-forward work of that row starts, which hides their latency.
-// The two phases are separate __noinline__ functions on purpose: each gets its own register allocation (the
-// x loop sits at the 168-register cap and is sensitive to anything else that is live); the per-thread twiddle
-// rows are re-read from a shared-memory copy of the table at the start of each phase.
+// The two phases are separate (force-inlined) functions; making them __noinline__ to separate their register
+// allocation was measured 25 % slower (the x loop then spills at the 168-register cap).
 struct PlaneCtx {
     c128 *A, *scr;
     const int4 *rowinfo_s;
-    const c128 *tw_s;
     int X, ngroups, n3, quarter;
     size_t wband;
 };
@@ -182,7 +180,8 @@ template <class C> struct PlaneIds {
 };
 
 template <class C, int MODE>
-__device__ __forceinline__ void plane_y_phase(const PlaneCtx cx, c128 *__restrict__ W, int pl, int prev, bool have_cur)
+__device__ __forceinline__ void plane_y_phase(const PlaneCtx cx, c128 *__restrict__ W, int pl, int prev, bool have_cur,
+                                              const TwRow<C::R1> &twa, const TwRow<C::R2> &twb)
 {
     constexpr int G = QM_GROUP, TPG = G / C::TT, RP = C::L | 1, NPRE = 2 * Quarter<C>::Q;
     constexpr bool HAS_BACK = MODE != 2, HAS_FWD = MODE != 1 && MODE != 3;
@@ -190,13 +189,6 @@ __device__ __forceinline__ void plane_y_phase(const PlaneCtx cx, c128 *__restric
     const int u = id.u, grp = id.grp, slot = id.slot, X = cx.X, n3 = cx.n3, quarter = cx.quarter;
     const bool do_back = HAS_BACK && have_cur, do_fwd = HAS_FWD && prev >= 0;
     if (!(do_back || do_fwd)) return;
-    TwRow<C::R1> twa;
-    load_twrow(twa, cx.tw_s, u, C::R2);
-    TwRow<C::R2> twb_store;
-    if constexpr (C::R1 != C::R2) load_twrow(twb_store, cx.tw_s, u, C::R1);
-    const auto &twb = [&]() -> const TwRow<C::R2> & {
-        if constexpr (C::R1 == C::R2) return twa; else return twb_store;
-    }();
     const SLine As = qm_sline(cx.A);
     const int pc = have_cur ? pl : 0, pp = prev >= 0 ? prev : 0;
     const WView Wcur = qm_wview(W + (size_t)(pc / n3) * cx.wband, pc % n3, n3);
@@ -236,20 +228,13 @@ __device__ __forceinline__ void plane_y_phase(const PlaneCtx cx, c128 *__restric
 template <class C, int MODE>
 __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_iv, const double *__restrict__ vt,
                                            c128 *__restrict__ box, int pl, double scale, int stagger_ns,
-                                           double *__restrict__ rhot)
+                                           double *__restrict__ rhot, const TwRow<C::R1> &twa, const TwRow<C::R2> &twb)
 {
     constexpr int G = QM_GROUP, TPG = G / C::TT, RP = C::L | 1;
     constexpr int SL = qm_scratch_pitch(C::L, C::TT);    // scratch line pitch
     const PlaneIds<C> id;
     const int u = id.u, grp = id.grp, slot = id.slot, n3 = cx.n3, ngroups = cx.ngroups;
     const bool team_ok = id.team_ok;
-    TwRow<C::R1> twa;
-    load_twrow(twa, cx.tw_s, u, C::R2);
-    TwRow<C::R2> twb_store;
-    if constexpr (C::R1 != C::R2) load_twrow(twb_store, cx.tw_s, u, C::R1);
-    const auto &twb = [&]() -> const TwRow<C::R2> & {
-        if constexpr (C::R1 == C::R2) return twa; else return twb_store;
-    }();
     const SLine As = qm_sline(cx.A);
     const Pruned px = make_pruned<C>(x_iv.x, x_iv.y, x_iv.z, x_iv.w, u, RP);
     const int band = pl / n3, p = pl - band * n3;
@@ -310,11 +295,9 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
     cx.wband = (size_t)((kp.nsticks + QM_ZT - 1) / QM_ZT) * QM_ZT * gd.ax[2].n;   // W elements per band
     cx.A = reinterpret_cast<c128 *>(smem_raw);
     cx.scr = cx.A + (((size_t)cx.X * RP + 7) & ~(size_t)7);
-    c128 *tw_s = cx.scr + (size_t)ngroups * TPG * SL;
-    int4 *rowinfo_s = reinterpret_cast<int4 *>(tw_s + C::N);
-    cx.tw_s = tw_s; cx.rowinfo_s = rowinfo_s;
+    int4 *rowinfo_s = reinterpret_cast<int4 *>(cx.scr + (size_t)ngroups * TPG * SL);
+    cx.rowinfo_s = rowinfo_s;
     for (int i = threadIdx.x; i < cx.X; i += blockDim.x) rowinfo_s[i] = kp.row_info[i];
-    for (int i = threadIdx.x; i < C::N; i += blockDim.x) tw_s[i] = gd.tw[0][i];
     __syncthreads();
 #ifdef QM_PLANE_TIMING
     long long tacc[3] = {0, 0, 0}, t0 = clock64(), t1;
@@ -322,6 +305,15 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
 #else
 #define QM_TICK(i) do {} while (0)
 #endif
+    // per-thread twiddle rows, loaded once (u is fixed for the whole kernel)
+    const int u_tw = (int)(threadIdx.x % G) % C::TT;
+    TwRow<C::R1> twa;
+    load_twrow(twa, gd.tw[0], u_tw, C::R2);
+    TwRow<C::R2> twb_store;
+    if constexpr (C::R1 != C::R2) load_twrow(twb_store, gd.tw[0], u_tw, C::R1);
+    const auto &twb = [&]() -> const TwRow<C::R2> & {
+        if constexpr (C::R1 == C::R2) return twa; else return twb_store;
+    }();
     const int n3 = cx.n3;
     // plane sequence of this CTA.  Apply / debug modes: pl = blockIdx.x, + gridDim.x, ... (pl = band * n3 + p).
     // Density mode: the CTA owns z-planes p = blockIdx.x, + gridDim.x, ... and walks ALL bands of a plane before
@@ -339,7 +331,7 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
     for (int it = 0, prev = -1;; ++it) {
         const int pl = plane_at(it);
         const bool have_cur = pl < nplanes;
-        plane_y_phase<C, MODE>(cx, W, pl, prev, have_cur);
+        plane_y_phase<C, MODE>(cx, W, pl, prev, have_cur, twa, twb);
         if (!have_cur) break;
         __syncthreads();
         QM_TICK(0);
@@ -347,7 +339,7 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
         const int z = (p / gd.ax[2].r2) + gd.ax[2].r1 * (p % gd.ax[2].r2);
         double sc = scale;
         if constexpr (MODE == 3) sc = scale * occ[pl / n3];
-        plane_x_phase<C, MODE>(cx, kp.x_iv, gd.vt, box ? box + z : nullptr, pl, sc, stagger_ns, rhot);
+        plane_x_phase<C, MODE>(cx, kp.x_iv, gd.vt, box ? box + z : nullptr, pl, sc, stagger_ns, rhot, twa, twb);
         __syncthreads();
         QM_TICK(1);
         prev = pl;

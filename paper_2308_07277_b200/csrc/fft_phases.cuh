@@ -49,7 +49,10 @@ QM_HD SLine qm_sline(const c128 *p) { return SLine{const_cast<c128 *>(p)}; }
 // Stick-plane workspace W of one band, blocked by tiles of QM_ZT sticks: element (plane label p, stick s) lives at
 // band_base[((s / QM_ZT) * n3 + p) * QM_ZT + s % QM_ZT].  A tile's N3 x QM_ZT block is contiguous (what the z kernels
 // move with one bulk copy); the plane kernel addresses single elements through this pointer-like view (p fixed).
-constexpr int QM_ZT = 16;
+#ifndef QM_ZT_STICKS
+#define QM_ZT_STICKS 16
+#endif
+constexpr int QM_ZT = QM_ZT_STICKS;
 struct WView {
     c128 *base;            // element (p, stick 0) of the band: band base + p * QM_ZT
     unsigned tstride;      // elements between consecutive tiles: n3 * QM_ZT

@@ -34,8 +34,11 @@ __device__ __forceinline__ double2 ldg_c128(const c128 *p) {
 #ifndef QM_P1_OCC
 #define QM_P1_OCC 1         /* CTAs of GEMM 1 per SM the split-K factor is sized for */
 #endif
-constexpr int P1_ROWS = QM_P1_ROWS, P1_KS = 16, P1_CW = P1_ROWS / 16, P1_ST = QM_P1_STAGES, P1_OCC = QM_P1_OCC,
-              P1_PSI_PITCH = 20, P_NB = 16;
+#ifndef QM_P1_KS
+#define QM_P1_KS 16         /* K slice per stage of GEMM 1 */
+#endif
+constexpr int P1_ROWS = QM_P1_ROWS, P1_KS = QM_P1_KS, P1_CW = P1_ROWS / 16, P1_ST = QM_P1_STAGES, P1_OCC = QM_P1_OCC,
+              P1_PSI_PITCH = P1_KS + 4, P_NB = 16;
 constexpr int P1_BETA_BYTES = P1_ROWS * P1_KS * 16;                 // 32768
 constexpr int P1_PSI_BYTES = P_NB * P1_PSI_PITCH * 16;              // 5120
 constexpr int P1_STAGE_BYTES = P1_BETA_BYTES + P1_PSI_BYTES;

@@ -168,7 +168,7 @@ size_t plane_smem(const qm_gspace *g, const KPoint *kp, int ngroups) {
     const size_t sl = (size_t)qm_scratch_pitch(ax.len, std::max(ax.r1, ax.r2));
     const int tpg = PLANE_GROUP / std::max(ax.r1, ax.r2);
     const size_t a_elems = ((size_t)kp->nx * kp->rowpitch + 7) & ~(size_t)7;
-    return (a_elems + (size_t)ngroups * tpg * sl + ax.n) * sizeof(c128) + (size_t)kp->nx * sizeof(int4) + 16;   // + twiddle table
+    return (a_elems + (size_t)ngroups * tpg * sl) * sizeof(c128) + (size_t)kp->nx * sizeof(int4) + 16;
 }
 
 // number of independent 64-thread groups of the plane kernel: the fewest groups that reach the

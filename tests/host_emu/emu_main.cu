@@ -27,7 +27,7 @@ struct RowInfo { int a1, b1, a2, b2, sbase; };
 struct XRows { int a1, b1, a2, b2; };
 
 template <class C> struct Emu {
-    static constexpr int LP = C::L | 1, SL = C::L | 1, TS = 16;
+    static constexpr int LP = C::L | 1, SL = C::L | 1, TS = QM_ZT;
     const QmKTables &kp; QmAxis ax; std::vector<c128> tw;
     Emu(const QmKTables &k, QmAxis a) : kp(k), ax(a), tw(C::N) {
         for (int j = 0; j < C::N; ++j) {
