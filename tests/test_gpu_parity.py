@@ -204,6 +204,24 @@ def test_ragged_band_counts(qm, nb):
     gs.close()
 
 
+@pytest.mark.parametrize("name,nb", [("cfg3", 64), ("cfg5", 16)])
+def test_apply_is_bitwise_reproducible(qm, name, nb):
+    """No atomics and fixed-order reductions everywhere (split-K, stream-K fix-up): repeated applies agree bit for bit.
+    Doubles as a race detector for the barrier-free hand-offs inside the plane kernel (compute-sanitizer is not
+    available on the GPU pool)."""
+    torch, dev = _torch()
+    p = problem(name, 0, nbands=nb, orthonormalise=False)
+    gs = _gspace(qm, p)
+    gs.set_vloc(torch.from_numpy(p["v"]).to(dev))
+    gs.set_nonlocal(0, torch.from_numpy(p["beta"]).to(dev), torch.from_numpy(p["dblk"]).to(dev))
+    psi = torch.from_numpy(p["psi"]).to(dev)
+    first = gs.apply_h(psi).clone()
+    for _ in range(10):
+        again = gs.apply_h(psi)
+        assert torch.equal(first, again)
+    gs.close()
+
+
 def test_host_entry_matches_device_entry(qm):
     torch, dev = _torch()
     p = problem("cfg1")
