@@ -117,6 +117,24 @@ def _cpu_oracle_rate(cfg, inputs, target_s=12.0):
                       f"extrapolated affinely to all rows"}
 
 
+def _cpu_fft_rate(cfg, inputs, idx):
+    """SURVEY 8(d) CPU number (1): the paper's own CPU method -- scatter, library inverse FFT, x V, forward FFT, gather +
+    kinetic, projectors as two BLAS products (oracle/hpsi_fft.py) -- on one call batch."""
+    from oracle import hpsi as oh
+    from oracle import hpsi_fft as of
+    lat, miller, g2, v, beta, dblk, psi = inputs
+    nb = cfg.call_batch
+    d = oh.expand_d(dblk)
+    ps = np.ascontiguousarray(psi[:nb])
+    of.apply_h_fft(ps[:1], idx, g2, v, cfg.grid, beta, d)            # warm-up (plans, threads)
+    t = time.perf_counter()
+    of.apply_h_fft(ps, idx, g2, v, cfg.grid, beta, d)
+    dt = time.perf_counter() - t
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else os.cpu_count()
+    return {"value": nb / dt, "unit": UNIT, "cores": cores, "kind": "oracle-fft (scipy.fft + BLAS zgemm route)",
+            "sample": f"{cfg.name}: one {nb}-band call batch, all rows, {dt:.2f} s measured"}
+
+
 def _build_inputs(cfg, miller_fn):
     from workloads import cell_for, make_beta, make_dmatrix, make_kpoints, make_psi, make_vloc
     lat, pos = cell_for(cfg)
@@ -371,11 +389,12 @@ def run_ours(args):
         fft_path = {"achieved_GBps": fft_bytes / (fft_ms * 1e-3) / 1e9 if fft_ms else None, "peak_GBps": hbm_peak,
                     "frac": fft_bytes / (fft_ms * 1e-3) / 1e9 / hbm_peak if fft_ms else None,
                     "alg_bytes_per_call": fft_bytes, "ms_per_call": fft_ms, "peak_source": peak_src}
-        cpu = None
+        cpu = cpu_fft = None
         if world == 1 and not args.no_cpu_baseline:
             from oracle import gsphere as og    # cpu_baseline leg only
             miller, idx, g2 = og.gsphere(lat, cfg.ecutwfc_ry, cfg.grid, kpts[0])
             cpu = _cpu_oracle_rate(cfg, (lat, miller, g2, v, per_k[0][1], dblk, per_k[0][2]))
+            cpu_fft = _cpu_fft_rate(cfg, (lat, miller, g2, v, per_k[0][1], dblk, per_k[0][2]), idx)
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "complex128", "data": "synthetic",
@@ -397,7 +416,7 @@ def run_ours(args):
                                    "achieved": 8.0 * n * n * ng / (t_ms * 1e-3) / 1e12, "peak": dmma_peak,
                                    "unit": "TFLOP/s", "frac": 8.0 * n * n * ng / (t_ms * 1e-3) / 1e12 / dmma_peak}
                              for tag, (n, t_ms) in sub.items()},
-                "cpu_baseline": cpu}
+                "cpu_baseline": cpu, "cpu_fft_baseline": cpu_fft}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
