@@ -137,6 +137,9 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
 #ifndef QM_PLANE_GROUP
 #define QM_PLANE_GROUP 96
 #endif
+#ifndef QM_PLANE_YROWS
+#define QM_PLANE_YROWS 1        /* plane rows a team works on between two group barriers of the y phase (2: spills, 343 vs 300 us) */
+#endif
 constexpr int QM_GROUP = QM_PLANE_GROUP;
 // Scratch lines of neighbouring teams: with 12-thread teams a quarter-warp straddles two teams as 4+4
 // threads, and their unit-stride 16-byte accesses are conflict free iff the pitch is 4 (mod 8); else odd.
@@ -193,34 +196,52 @@ __device__ __forceinline__ void plane_y_phase(const PlaneCtx cx, c128 *__restric
     const int pc = have_cur ? pl : 0, pp = prev >= 0 ? prev : 0;
     const WView Wcur = qm_wview(W + (size_t)(pc / n3) * cx.wband, pc % n3, n3);
     const WView Wprev = qm_wview(W + (size_t)(pp / n3) * cx.wband, pp % n3, n3);
-    for (int r = grp * TPG + slot; r - slot < X; r += cx.ngroups * TPG) {
-        const bool ok = id.team_ok && r < X;
-        int sbase = 0;
-        Pruned pr{0u, 0u, 0, 0};
-        if (ok) {
-            const int4 q = cx.rowinfo_s[r];
-            sbase = q.z;
-            pr = make_pruned<C>((int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, u, 1);
+    // A team works on NR rows per round (rows r, r + rstride, ...): the same number of row steps with 1/NR of the
+    // group barriers and NR independent load -> transform -> store chains between two barriers.
+    constexpr int NR = QM_PLANE_YROWS;
+    const int rstride = cx.ngroups * TPG;
+    for (int r0 = grp * TPG + slot; r0 - slot < X; r0 += NR * rstride) {
+        bool ok[NR];
+        int sbase[NR];
+        Pruned pr[NR];
+        c128 pre[NR][NPRE];
+#pragma unroll
+        for (int i = 0; i < NR; ++i) {
+            const int r = r0 + i * rstride;
+            ok[i] = id.team_ok && r < X;
+            sbase[i] = 0;
+            pr[i] = Pruned{0u, 0u, 0, 0};
+            if (ok[i]) {
+                const int4 q = cx.rowinfo_s[r];
+                sbase[i] = q.z;
+                pr[i] = make_pruned_packed<C>(q.x, q.y, u, 1);
+            }
+            if (do_back && quarter && ok[i]) prefetch_quarter<C>(Wcur + sbase[i], C::R2, pr[i], pre[i]);
         }
-        c128 pre[NPRE];
-        const SLine Arow = As + r * RP;
-        if (do_back && quarter && ok) prefetch_quarter<C>(Wcur + sbase, C::R2, pr, pre);
         if (do_fwd) {
-            if (ok) lineB_step1<C>(Arow, u, twb);
+#pragma unroll
+            for (int i = 0; i < NR; ++i)
+                if (ok[i]) lineB_step1<C>(As + (r0 + i * rstride) * RP, u, twb);
             group_barrier<G>(grp);
-            if (ok) {
-                if (quarter) prunedB_step2_quarter<C>(Arow, Wprev + sbase, C::R2, pr, u);
-                else prunedB_step2<C>(Arow, Wprev + sbase, C::R2, pr, u);
+        }
+#pragma unroll
+        for (int i = 0; i < NR; ++i) {
+            const SLine Arow = As + (r0 + i * rstride) * RP;
+            if (do_fwd && ok[i]) {
+                if (quarter) prunedB_step2_quarter<C>(Arow, Wprev + sbase[i], C::R2, pr[i], u);
+                else prunedB_step2<C>(Arow, Wprev + sbase[i], C::R2, pr[i], u);
+            }
+            // the team that read the row in the step above is the one that refills it: no barrier needed
+            if (do_back && ok[i]) {
+                if (quarter) prunedA_step1_pre<C>(pre[i], Arow, u, twa);
+                else prunedA_step1<C>(Wcur + sbase[i], C::R2, pr[i], Arow, u, twa);
             }
         }
         if (do_back) {
-            // the team that read row r in the step above is the one that refills it: no barrier needed
-            if (ok) {
-                if (quarter) prunedA_step1_pre<C>(pre, Arow, u, twa);
-                else prunedA_step1<C>(Wcur + sbase, C::R2, pr, Arow, u, twa);
-            }
             group_barrier<G>(grp);
-            if (ok) lineA_step2<C>(Arow, u);
+#pragma unroll
+            for (int i = 0; i < NR; ++i)
+                if (ok[i]) lineA_step2<C>(As + (r0 + i * rstride) * RP, u);
         }
     }
 }
