@@ -58,6 +58,8 @@ typedef enum {
  *  lattice_bohr  HOST  9 doubles, rows a1,a2,a3
  *  ecutwfc_ry          cut-off in Rydberg
  *  fft_grid      HOST  3 ints n1,n2,n3; each must be a supported FFT length (see qm_fft_size_supported)
+ *                      and n1 == n2 (the fused xy-plane kernel uses one line factorisation for both axes; n3 is free).
+ *                      Anything else returns QM_EGRID.
  *  kpts_cryst    HOST  nk*3 doubles (may be NULL iff nk==1 => Gamma)
  *  out                 receives the handle; destroy with qm_gspace_destroy.
  * Uploads the tables to the current CUDA device (synchronously; this is set-up, not hot path). */
