@@ -275,3 +275,45 @@ def test_error_codes(qm):
         qm.GSpace(p["lat"], 25.0, (8, 8, 8))
     assert e.value.code == -3                                    # sphere does not fit
     gs.close()
+
+
+# every supported FFT length (each is its own template instantiation: team sizes 4..16, odd second radix, ...)
+_FCC = 0.5 * np.array([[-1.0, 0, 1], [0, 1, 1], [-1, 1, 0]])
+_SIZE_CASES = [
+    (8, 10.26 * _FCC, 5.0, (0.0, 0.0, 0.0)), (12, 10.26 * _FCC, 8.0, (0.1, -0.2, 0.3)),
+    (16, 10.26 * _FCC, 14.0, (0.0, 0.0, 0.0)), (18, 10.26 * _FCC, 14.0, (0.0, 0.0, 0.0)),
+    (20, 10.26 * _FCC, 20.0, (0.0, 0.0, 0.0)), (30, 10.26 * _FCC, 30.0, (0.3, 0.3, -0.4)),
+    (36, 10.26 * np.eye(3), 20.0, (0.0, 0.0, 0.0)), (40, 10.26 * np.eye(3), 25.0, (0.0, 0.0, 0.0)),
+    (60, 14.0 * np.eye(3), 30.0, (0.0, 0.0, 0.0)), (64, 14.0 * np.eye(3), 30.0, (0.0, 0.0, 0.0)),
+    (72, 16.0 * np.eye(3), 30.0, (0.0, 0.0, 0.0)), (80, 18.0 * np.eye(3), 30.0, (0.0, 0.0, 0.0)),
+    (100, 20.52 * np.eye(3), 30.0, (0.2, 0.1, -0.3)), (108, 22.0 * np.eye(3), 30.0, (0.0, 0.0, 0.0)),
+    (120, 24.0 * np.eye(3), 30.0, (0.0, 0.0, 0.0)), (128, 26.0 * np.eye(3), 30.0, (0.0, 0.0, 0.0)),
+]
+
+
+@pytest.mark.parametrize("n,lat,ecut,k", _SIZE_CASES, ids=[f"n{c[0]}" for c in _SIZE_CASES])
+def test_every_fft_length_local_and_kinetic_terms(qm, n, lat, ecut, k):
+    """T + L on every supported grid edge against the paper's FFT route with library FFTs (oracle/hpsi_fft.py, itself
+    tied to the direct-sum oracle in tests/test_oracle_hpsi.py); small grids also against the direct sum."""
+    from oracle import gsphere as og
+    torch, dev = _torch()
+    grid = (n, n, n)
+    kk = np.array(k, dtype=float)
+    miller, idx, g2 = og.gsphere(lat, ecut, grid, kk)
+    rng = np.random.default_rng(n)
+    nb = 3
+    psi = rng.standard_normal((nb, idx.size)) + 1j * rng.standard_normal((nb, idx.size))
+    v = rng.standard_normal(n ** 3)
+    gs = qm.GSpace(lat, ecut, grid, kk[None, :])
+    assert np.array_equal(gs.index_map(0), idx)
+    gs.set_vloc(torch.from_numpy(v).to(dev))
+    gs.set_nonlocal(0, None, None)
+    got = gs.apply_h(torch.from_numpy(psi).to(dev)).cpu().numpy()
+    ref = of.apply_h_fft(psi, idx, g2, v, grid)
+    e_inf, e_2 = band_errors(got, ref)
+    assert e_inf <= TOL and e_2 <= TOL, (e_inf, e_2)
+    if n <= 20:
+        ref2 = oh.apply_h_rows(psi, miller, g2, oh.vhat_box(v, grid), grid)
+        e_inf, e_2 = band_errors(got, ref2)
+        assert e_inf <= TOL and e_2 <= TOL, (e_inf, e_2)
+    gs.close()
