@@ -389,6 +389,15 @@ def run_ours(args):
         fft_path = {"achieved_GBps": fft_bytes / (fft_ms * 1e-3) / 1e9 if fft_ms else None, "peak_GBps": hbm_peak,
                     "frac": fft_bytes / (fft_ms * 1e-3) / 1e9 / hbm_peak if fft_ms else None,
                     "alg_bytes_per_call": fft_bytes, "ms_per_call": fft_ms, "peak_source": peak_src}
+        # the same time charged with the bytes of the unfused one-pass-per-axis design (SURVEY 8(d) model D1: psi -> sticks,
+        # sticks -> slab, slab -> x-FFT.V.x-FFT -> slab, slab -> sticks, sticks -> out): what an HBM-bound implementation
+        # of the path would have to move; the north_star's ">= 60 % of HBM" refers to such passes
+        slab = nx * cfg.grid[1] * N3 * 16
+        d1_bytes = cb * (ng * 16 + N3 * S * 16 + (N3 * S * 16 + slab) + 2 * slab + (slab + N3 * S * 16)
+                         + (N3 * S * 16 + 2 * ng * 16)) + nvox * 8
+        fft_path["d1_model"] = {"alg_bytes_per_call": d1_bytes,
+                                "achieved_GBps": d1_bytes / (fft_ms * 1e-3) / 1e9 if fft_ms else None,
+                                "frac": d1_bytes / (fft_ms * 1e-3) / 1e9 / hbm_peak if fft_ms else None}
         cpu = cpu_fft = None
         if world == 1 and not args.no_cpu_baseline:
             from oracle import gsphere as og    # cpu_baseline leg only
