@@ -189,7 +189,7 @@ __device__ __forceinline__ void plane_y_phase(const PlaneCtx cx, c128 *__restric
     constexpr int G = QM_GROUP, TPG = G / C::TT, RP = C::L | 1, NPRE = 2 * Quarter<C>::Q;
     constexpr bool HAS_BACK = MODE != 2, HAS_FWD = MODE != 1 && MODE != 3;
     const PlaneIds<C> id;
-    const int u = id.u, grp = id.grp, slot = id.slot, X = cx.X, n3 = cx.n3, quarter = cx.quarter;
+    const int u = id.u, grp = id.grp, slot = id.slot, X = cx.X, n3 = cx.n3, quarter = cx.quarter & 1;
     const bool do_back = HAS_BACK && have_cur, do_fwd = HAS_FWD && prev >= 0;
     if (!(do_back || do_fwd)) return;
     const SLine As = qm_sline(cx.A);
@@ -256,6 +256,7 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
     const PlaneIds<C> id;
     const int u = id.u, grp = id.grp, slot = id.slot, n3 = cx.n3, ngroups = cx.ngroups;
     const bool team_ok = id.team_ok;
+    const bool xq = (cx.quarter & 2) != 0;               // quarter rule holds for the x rows: 2Q loads / stores per column
     const SLine As = qm_sline(cx.A);
     const Pruned px = make_pruned<C>(x_iv.x, x_iv.y, x_iv.z, x_iv.w, u, RP);
     const int band = pl / n3, p = pl - band * n3;
@@ -273,7 +274,10 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
         const bool ok = team_ok && col < C::N;
         const SLine Acol = As + C::pos(col);
         if constexpr (MODE != 2) {
-            if (ok) prunedA_step1<C>(Acol, C::R2 * RP, px, myscr, u, twa);
+            if (ok) {
+                if (xq) prunedA_step1_quarter<C>(Acol, C::R2 * RP, px, myscr, u, twa);
+                else prunedA_step1<C>(Acol, C::R2 * RP, px, myscr, u, twa);
+            }
             group_barrier<G>(grp);
         }
         if constexpr (MODE == 3) {
@@ -295,7 +299,10 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
         if constexpr (MODE != 1 && MODE != 3) {
             // no barrier after step 3: the scratch column a thread reads here is exactly the one it
             // overwrites in the next iteration's step 1 (MODE 2 has no step 1 and writes rows: barrier).
-            if (ok) prunedB_step2<C>(myscr, Acol, C::R2 * RP, px, u);
+            if (ok) {
+                if (xq) prunedB_step2_quarter<C>(myscr, Acol, C::R2 * RP, px, u);
+                else prunedB_step2<C>(myscr, Acol, C::R2 * RP, px, u);
+            }
             if constexpr (MODE == 2) group_barrier<G>(grp);
         }
     }

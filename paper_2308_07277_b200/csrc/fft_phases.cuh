@@ -182,11 +182,18 @@ QM_HD void prunedA_step1_pre(const c128 (&pre)[2 * Quarter<C>::Q], const L dst, 
         else if constexpr (n1 >= C::R1 - Q) t[n1] = pre[Q + n1 - (C::R1 - Q)];
         else t[n1] = c128{0.0, 0.0};
     });
-    Dft<C::R1, +1>::run(t);
+    DftQuarterIn<C::R1, +1>::run(t);
     static_for<C::R1>([&](auto I) {
         constexpr int k1 = decltype(I)::value;
         dst[k1 * C::R2P + u] = (k1 == 0) ? t[k1] : cmul_conj(t[k1], tw.template get<k1>());
     });
+}
+template <class C, class P, class L, class TW>
+QM_HD void prunedA_step1_quarter(const P src, int estride, const Pruned pr, const L dst, int u, const TW &tw) {
+    if (u >= C::R2) return;
+    c128 pre[2 * Quarter<C>::Q];
+    prefetch_quarter<C>(src, estride, pr, pre);
+    prunedA_step1_pre<C>(pre, dst, u, tw);
 }
 // Forward step 2 with pruned output: reads the full padded line `srcline`, stores only what exists.
 template <class C, class L, class P>
@@ -214,7 +221,7 @@ QM_HD void prunedB_step2_quarter(const L srcline, const P dst, int estride, cons
     constexpr int Q = Quarter<C>::Q;
     c128 t[C::R1];
     static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = srcline[a * C::R2P + u]; });
-    Dft<C::R1, -1>::run(t);
+    DftQuarterOut<C::R1, -1>::run(t);
     const P p1 = dst + pr.c1, p2 = dst + pr.c2;
     static_for<Q>([&](auto I) {
         constexpr int j = decltype(I)::value;
@@ -305,7 +312,7 @@ template <class C, class L> QM_HD void zfwd_step2_gather_pre(const L line, c128 
     constexpr int Q = Quarter<C>::Q;
     c128 t[C::R1];
     static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = line[a * C::R2P + u]; });
-    Dft<C::R1, -1>::run(t);
+    DftQuarterOut<C::R1, -1>::run(t);
     static_for<Q>([&](auto I) {
         constexpr int j = decltype(I)::value;
         constexpr int c2 = C::R1 - Q + j;

@@ -158,3 +158,85 @@ template <int DIR> struct Dft<10, DIR> { static QM_HD void run(c128 (&x)[10]) { 
 template <int DIR> struct Dft<12, DIR> { static QM_HD void run(c128 (&x)[12]) { DftPFA<3, 4, DIR>::run(x); } };
 template <int DIR> struct Dft<15, DIR> { static QM_HD void run(c128 (&x)[15]) { DftPFA<3, 5, DIR>::run(x); } };
 template <int DIR> struct Dft<16, DIR> { static QM_HD void run(c128 (&x)[16]) { DftComposite<4, 4, DIR>::run(x); } };
+
+// ---- quarter-pruned codelets -------------------------------------------------------------------------------
+// On an alias-free grid only the first and last quarter of a line's first-pass inputs (backward) / last-pass
+// outputs (forward) exist (fft_phases.cuh, Quarter).  For radix 12 that is indices {0,1,2,9,10,11}: the six middle
+// inputs are exact zeros, the six middle outputs are never stored.  The prime-factor forms below skip the work on
+// them (72 and 80 FP64 instructions instead of 96); other radices fall back to the full codelet.
+template <int R, int DIR> struct DftQuarterIn  { static QM_HD void run(c128 (&x)[R]) { Dft<R, DIR>::run(x); } };
+template <int R, int DIR> struct DftQuarterOut { static QM_HD void run(c128 (&x)[R]) { Dft<R, DIR>::run(x); } };
+
+// x[3..8] are zero on entry (their values are ignored); all 12 outputs are produced.
+template <int DIR> struct DftQuarterIn<12, DIR> {
+    static QM_HD void run(c128 (&x)[12]) {
+        constexpr double s3 = (DIR > 0 ? 1.0 : -1.0) * 0.8660254037844386;     // Im w, w = exp(DIR 2 pi i / 3)
+        // PFA 3x4, stage 1: DFT3 over n1 of x[(4 n1 + 3 n2) % 12]; y[k1][n2]
+        c128 y[3][4];
+        // n2 = 0: (x0, 0, 0)
+        y[0][0] = x[0]; y[1][0] = x[0]; y[2][0] = x[0];
+        {   // n2 = 1: (0, 0, c = x11):  X0 = c, X1 = c w^2, X2 = c w
+            const c128 c = x[11];
+            const c128 h = {-0.5 * c.x, -0.5 * c.y};
+            y[0][1] = c;
+            y[1][1] = {h.x + s3 * c.y, h.y - s3 * c.x};
+            y[2][1] = {h.x - s3 * c.y, h.y + s3 * c.x};
+        }
+        {   // n2 = 2: (0, b = x10, c = x2):  X0 = b + c, X1 = b w + c w^2, X2 = b w^2 + c w
+            const c128 s = x[10] + x[2], d = x[10] - x[2];
+            const c128 h = {-0.5 * s.x, -0.5 * s.y};
+            y[0][2] = s;
+            y[1][2] = {h.x - s3 * d.y, h.y + s3 * d.x};
+            y[2][2] = {h.x + s3 * d.y, h.y - s3 * d.x};
+        }
+        {   // n2 = 3: (a = x9, b = x1, 0):  X0 = a + b, X1 = a + b w, X2 = a + b w^2
+            const c128 a = x[9], b = x[1];
+            const c128 h = {a.x - 0.5 * b.x, a.y - 0.5 * b.y};
+            y[0][3] = a + b;
+            y[1][3] = {h.x - s3 * b.y, h.y + s3 * b.x};
+            y[2][3] = {h.x + s3 * b.y, h.y - s3 * b.x};
+        }
+        // stage 2: DFT4 over n2, output index (4 k1 + 9 k2) % 12
+        static_for<3>([&](auto K1) {
+            constexpr int k1 = decltype(K1)::value;
+            c128 t[4] = {y[k1][0], y[k1][1], y[k1][2], y[k1][3]};
+            Dft<4, DIR>::run(t);
+            static_for<4>([&](auto K2) { constexpr int k2 = decltype(K2)::value; x[(4 * k1 + 9 * k2) % 12] = t[k2]; });
+        });
+    }
+};
+
+// all 12 inputs are used; only x[0,1,2,9,10,11] hold results on exit (the others are unspecified).
+template <int DIR> struct DftQuarterOut<12, DIR> {
+    static QM_HD void run(c128 (&x)[12]) {
+        constexpr double s3 = (DIR > 0 ? 1.0 : -1.0) * 0.8660254037844386;
+        // PFA 4x3, stage 1: DFT4 over n1 of x[(3 n1 + 4 n2) % 12]; y[k1][n2]
+        c128 y[4][3];
+        static_for<3>([&](auto N2) {
+            constexpr int n2 = decltype(N2)::value;
+            c128 t[4];
+            static_for<4>([&](auto N1) { constexpr int n1 = decltype(N1)::value; t[n1] = x[(3 * n1 + 4 * n2) % 12]; });
+            Dft<4, DIR>::run(t);
+            static_for<4>([&](auto K1) { constexpr int k1 = decltype(K1)::value; y[k1][n2] = t[k1]; });
+        });
+        // stage 2: DFT3 over n2 for each k1, output index (9 k1 + 4 k2) % 12; needed (k1,k2):
+        //   0:(0,0)  1:(1,1)  2:(2,2)  9:(1,0)  10:(2,1)  11:(3,2)
+        x[0] = y[0][0] + y[0][1] + y[0][2];
+        {   // k1 = 1: k2 = 0 -> 9, k2 = 1 -> 1
+            const c128 a = y[1][0], s = y[1][1] + y[1][2], d = y[1][1] - y[1][2];
+            const c128 h = {a.x - 0.5 * s.x, a.y - 0.5 * s.y};
+            x[9] = a + s;
+            x[1] = {h.x - s3 * d.y, h.y + s3 * d.x};
+        }
+        {   // k1 = 2: k2 = 1 -> 10, k2 = 2 -> 2
+            const c128 a = y[2][0], s = y[2][1] + y[2][2], d = y[2][1] - y[2][2];
+            const c128 h = {a.x - 0.5 * s.x, a.y - 0.5 * s.y};
+            x[10] = {h.x - s3 * d.y, h.y + s3 * d.x};
+            x[2] = {h.x + s3 * d.y, h.y - s3 * d.x};
+        }
+        {   // k1 = 3: k2 = 2 -> 11
+            const c128 a = y[3][0], s = y[3][1] + y[3][2], d = y[3][1] - y[3][2];
+            x[11] = {a.x - 0.5 * s.x + s3 * d.y, a.y - 0.5 * s.y - s3 * d.x};
+        }
+    }
+};

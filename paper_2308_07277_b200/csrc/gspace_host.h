@@ -52,6 +52,7 @@ struct QmKTables {
     std::vector<int4> stickinfo;               // per stick: packed occupied i3 intervals (a1|b1<<16, a2|b2<<16), first G, 0
     short4 xiv = {1, 0, 1, 0};                 // occupied i1 intervals (rows 0.. and following)
     bool x_contiguous = true;
+    bool x_quarter = false;                    // the same rule for the occupied i1 (x rows of the plane kernel)
     bool z_quarter = false;                    // same rule for the occupied i3 of every stick (z kernels)
     bool y_quarter = false;                    // every occupied i2 of every row lies in the first / last quarter-block (fft_phases.cuh Quarter)
 };
@@ -186,6 +187,11 @@ static inline int qm_build_tables(const double *lattice, const double *recip, do
         if (iv.z <= iv.w && iv.z < (ax[2].r1 - zq) * ax[2].r2) kp->z_quarter = false;
         kp->stickinfo[s] = int4{(int)(unsigned short)iv.x | ((int)iv.y << 16), (int)(unsigned short)iv.z | ((int)iv.w << 16),
                                 kp->stickoff[s], 0};
+    }
+    {
+        const int q = (ax[0].r1 + 3) / 4;
+        const short4 iv = kp->xiv;
+        kp->x_quarter = !(iv.x <= iv.y && iv.y >= q * ax[0].r2) && !(iv.z <= iv.w && iv.z < (ax[0].r1 - q) * ax[0].r2);
     }
     {   // quarter rule for the plane kernel's register prefetch: i2 < Q*r2 or i2 >= (r1-Q)*r2, Q = ceil(r1/4)
         const int q = (ax[1].r1 + 3) / 4;

@@ -239,7 +239,7 @@ template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *bo
     g->prof.begin(QM_K_PLANE, st);
     k_plane<C, MODE><<<grid, ngroups * PLANE_GROUP, smem, st>>>(kp->plan(), gd, g->d_W.p, box, ngroups, scale,
                                                                    g->plane_stagger_ns, nplanes,
-                                                                   kp->y_quarter ? 1 : 0, occ, rhot);
+                                                                   (kp->y_quarter ? 1 : 0) | (kp->x_quarter ? 2 : 0), occ, rhot);
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());

@@ -48,7 +48,14 @@ template <class C> struct Emu {
             std::vector<c128> lines(TS * LP, c128{1e300, -1e300});
             for (int tid = 0; tid < nthr; ++tid) {
                 int t = tid / C::TT, u = tid % C::TT;
-                if (t < ns) { const int4 q = kp.stickinfo[s0 + t]; prunedA_step1<C>(psi + q.z, C::R2, stick_pruned(q, u), qm_sline(&lines[t * LP]), u, rowA(u)); }
+                if (t < ns) {
+                    const int4 q = kp.stickinfo[s0 + t];
+                    if (kp.z_quarter) {
+                        c128 pre[2 * Quarter<C>::Q];
+                        prefetch_quarter<C>(psi + q.z, C::R2, stick_pruned(q, u), pre);
+                        prunedA_step1_pre<C>(pre, qm_sline(&lines[t * LP]), u, rowA(u));
+                    } else prunedA_step1<C>(psi + q.z, C::R2, stick_pruned(q, u), qm_sline(&lines[t * LP]), u, rowA(u));
+                }
             }
             for (int tid = 0; tid < nthr; ++tid) {
                 int t = tid % TS, u = tid / TS;
@@ -67,7 +74,14 @@ template <class C> struct Emu {
             }
             for (int tid = 0; tid < nthr; ++tid) {
                 int t = tid / C::TT, u = tid % C::TT;
-                if (t < ns) { const int4 q = kp.stickinfo[s0 + t]; zfwd_step2_gather<C>(qm_sline(&lines[t * LP]), out + q.z, kinetic ? psi_in + q.z : nullptr, kp.g2.data() + q.z, stick_pruned(q, u), u, kinetic); }
+                if (t < ns) {
+                    const int4 q = kp.stickinfo[s0 + t];
+                    if (kp.z_quarter) {
+                        c128 kin[2 * Quarter<C>::Q];
+                        prefetch_kin<C>(psi_in + q.z, kp.g2.data() + q.z, stick_pruned(q, u), kinetic, kin);
+                        zfwd_step2_gather_pre<C>(qm_sline(&lines[t * LP]), out + q.z, stick_pruned(q, u), u, kin);
+                    } else zfwd_step2_gather<C>(qm_sline(&lines[t * LP]), out + q.z, kinetic ? psi_in + q.z : nullptr, kp.g2.data() + q.z, stick_pruned(q, u), u, kinetic);
+                }
             }
         }
     }
@@ -86,7 +100,8 @@ template <class C> struct Emu {
                 const RowInfo ri = row_info(task / C::TT);
                 const int u = task % C::TT;
                 const Pruned pr = make_pruned<C>(ri.a1, ri.b1, ri.a2, ri.b2, u, 1);
-                prunedA_step1<C>(Wp + ri.sbase, C::R2, pr, qm_sline(&A[(task / C::TT) * rp]), u, rowA(u));
+                if (kp.y_quarter) prunedA_step1_quarter<C>(Wp + ri.sbase, C::R2, pr, qm_sline(&A[(task / C::TT) * rp]), u, rowA(u));
+                else prunedA_step1<C>(Wp + ri.sbase, C::R2, pr, qm_sline(&A[(task / C::TT) * rp]), u, rowA(u));
             }
             for (int task = 0; task < X * C::TT; ++task) lineA_step2<C>(qm_sline(&A[(task / C::TT) * rp]), task % C::TT);
         }
@@ -96,7 +111,10 @@ template <class C> struct Emu {
             if (MODE != 2)
                 for (int tid = 0; tid < nthr; ++tid) {
                     int c = tid / C::TT, u = tid % C::TT, col = cbase + c;
-                    if (col < C::N) prunedA_step1<C>(qm_sline(A.data() + C::pos(col)), C::R2 * rp, make_pruned<C>(xr.a1, xr.b1, xr.a2, xr.b2, u, rp), qm_sline(&scr[(size_t)c * SL]), u, rowA(u));
+                    if (col < C::N) {
+                        if (kp.x_quarter) prunedA_step1_quarter<C>(qm_sline(A.data() + C::pos(col)), C::R2 * rp, make_pruned<C>(xr.a1, xr.b1, xr.a2, xr.b2, u, rp), qm_sline(&scr[(size_t)c * SL]), u, rowA(u));
+                        else prunedA_step1<C>(qm_sline(A.data() + C::pos(col)), C::R2 * rp, make_pruned<C>(xr.a1, xr.b1, xr.a2, xr.b2, u, rp), qm_sline(&scr[(size_t)c * SL]), u, rowA(u));
+                    }
                 }
             for (int tid = 0; tid < nthr; ++tid) {
                 int c = tid / C::TT, u = tid % C::TT, col = cbase + c;
@@ -110,7 +128,10 @@ template <class C> struct Emu {
             if (MODE != 1)
                 for (int tid = 0; tid < nthr; ++tid) {
                     int c = tid / C::TT, u = tid % C::TT, col = cbase + c;
-                    if (col < C::N) prunedB_step2<C>(qm_sline(&scr[(size_t)c * SL]), qm_sline(A.data() + C::pos(col)), C::R2 * rp, make_pruned<C>(xr.a1, xr.b1, xr.a2, xr.b2, u, rp), u);
+                    if (col < C::N) {
+                        if (kp.x_quarter) prunedB_step2_quarter<C>(qm_sline(&scr[(size_t)c * SL]), qm_sline(A.data() + C::pos(col)), C::R2 * rp, make_pruned<C>(xr.a1, xr.b1, xr.a2, xr.b2, u, rp), u);
+                        else prunedB_step2<C>(qm_sline(&scr[(size_t)c * SL]), qm_sline(A.data() + C::pos(col)), C::R2 * rp, make_pruned<C>(xr.a1, xr.b1, xr.a2, xr.b2, u, rp), u);
+                    }
                 }
         }
         if (MODE != 1) {
@@ -118,7 +139,8 @@ template <class C> struct Emu {
             for (int task = 0; task < X * C::TT; ++task) {
                 const RowInfo ri = row_info(task / C::TT);
                 const int u = task % C::TT;
-                prunedB_step2<C>(qm_sline(&A[(task / C::TT) * rp]), Wp + ri.sbase, C::R2, make_pruned<C>(ri.a1, ri.b1, ri.a2, ri.b2, u, 1), u);
+                if (kp.y_quarter) prunedB_step2_quarter<C>(qm_sline(&A[(task / C::TT) * rp]), Wp + ri.sbase, C::R2, make_pruned<C>(ri.a1, ri.b1, ri.a2, ri.b2, u, 1), u);
+                else prunedB_step2<C>(qm_sline(&A[(task / C::TT) * rp]), Wp + ri.sbase, C::R2, make_pruned<C>(ri.a1, ri.b1, ri.a2, ri.b2, u, 1), u);
             }
         }
     }
@@ -159,7 +181,7 @@ template <class C> int run(int n, const double *lat, double ecut, const double *
         emu.zfwd(W.data(), nullptr, &r2g[(size_t)b * kp.ng], false);
     }
     dump(prefix + ".idx", kp.idx); dump(prefix + ".hloc", hloc); dump(prefix + ".g2r", g2r); dump(prefix + ".r2g", r2g);
-    printf("ng %d sticks %d nx %d\n", kp.ng, kp.nsticks, kp.nx);
+    printf("ng %d sticks %d nx %d quarter x%d y%d z%d\n", kp.ng, kp.nsticks, kp.nx, (int)kp.x_quarter, (int)kp.y_quarter, (int)kp.z_quarter);
     return 0;
 }
 
