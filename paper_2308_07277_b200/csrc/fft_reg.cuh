@@ -240,3 +240,41 @@ template <int DIR> struct DftQuarterOut<12, DIR> {
         }
     }
 };
+
+// Radix 8 (grids 64, 72, 80, 96, 128): existing inputs / wanted outputs are {0,1,6,7}.  Composite 2x4 form of Dft<8>
+// with the work on the zero inputs (40 instead of 56 FP64 instructions) or on the unwanted outputs (48) removed.
+template <int DIR> struct DftQuarterIn<8, DIR> {
+    static QM_HD void run(c128 (&x)[8]) {
+        // stage 1: DFT2 over n1 of (x[n2], x[4+n2]) with one of the two zero, then the root w8^(n2*k1)
+        c128 y[2][4];
+        y[0][0] = x[0];                 y[1][0] = x[0];
+        y[0][1] = x[1];                 y[1][1] = mul_root<8, 1, DIR>(x[1]);
+        y[0][2] = x[6];                 y[1][2] = mul_root<8, 2, DIR>(c128{-x[6].x, -x[6].y});
+        y[0][3] = x[7];                 y[1][3] = mul_root<8, 3, DIR>(c128{-x[7].x, -x[7].y});
+        static_for<2>([&](auto K1) {
+            constexpr int k1 = decltype(K1)::value;
+            c128 t[4] = {y[k1][0], y[k1][1], y[k1][2], y[k1][3]};
+            Dft<4, DIR>::run(t);
+            static_for<4>([&](auto K2) { constexpr int k2 = decltype(K2)::value; x[k1 + 2 * k2] = t[k2]; });
+        });
+    }
+};
+template <int DIR> struct DftQuarterOut<8, DIR> {
+    static QM_HD void run(c128 (&x)[8]) {
+        c128 y[2][4];
+        static_for<4>([&](auto N2) {
+            constexpr int n2 = decltype(N2)::value;
+            const c128 a = x[n2], b = x[4 + n2];
+            y[0][n2] = a + b;
+            y[1][n2] = mul_root<8, n2, DIR>(a - b);
+        });
+        // stage 2: DFT4 over n2, outputs k = k1 + 2 k2 wanted for k2 in {0, 3} only:  X0 = (a+c)+(b+d),  X3 = (a-c) - DIR i (b-d)
+        static_for<2>([&](auto K1) {
+            constexpr int k1 = decltype(K1)::value;
+            const c128 s02 = y[k1][0] + y[k1][2], d02 = y[k1][0] - y[k1][2];
+            const c128 s13 = y[k1][1] + y[k1][3], d13 = mul_i<DIR>(y[k1][1] - y[k1][3]);
+            x[k1] = s02 + s13;
+            x[k1 + 6] = d02 - d13;
+        });
+    }
+};
