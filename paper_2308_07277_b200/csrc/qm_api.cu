@@ -139,7 +139,7 @@ struct qm_gspace {
     int sm_count = 148;
     int max_smem = 0;
     int z_cta_per_sm = 2;           // resident z-kernel CTAs per SM the grid is sized for (QM_Z_CTA_PER_SM)
-    int plane_stagger_ns = 300;     // de-phasing delay between the plane kernel's groups (QM_PLANE_STAGGER_NS)
+    int plane_stagger_ns = 0;       // de-phasing delay between the plane kernel's groups (QM_PLANE_STAGGER_NS)
     ~qm_gspace() { for (auto *k : kpts) delete k; }
 };
 
