@@ -264,6 +264,16 @@ def run_ours(args):
     prof = qm.qm_profile_read(gs.handle)
     qm.qm_profile_enable(gs.handle, False)
 
+    # SURVEY A17 second figure: one qm_apply_h call with all bands of the config (the library sub-batches internally)
+    gs.apply_h(psi_dev[0], out_dev[0], k=0)
+    torch.cuda.synchronize()
+    a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a0.record()
+    gs.apply_h(psi_dev[0], out_dev[0], k=0)
+    a1.record()
+    torch.cuda.synchronize()
+    one_call_ms = a0.elapsed_time(a1)
+
     # next row of the scope table: subspace products <psi_i|H psi_j>, all bands x all bands and one
     # call batch x one call batch, device-timed outside the step timing above (own figure, not part of `value`)
     sub = {}
@@ -414,6 +424,7 @@ def run_ours(args):
                 "gpu_launches": int(launches),
                 "roofline": roofline, "fft_path": fft_path, "kernels": kernels,
                 "fp64_peaks_tflops": {"dmma_probe": dmma_peak, "dfma_probe": dfma_peak},
+                "one_call_all_bands": {"bands": nb, "ms": one_call_ms, "band_applies_per_s": nb / (one_call_ms * 1e-3)},
                 "taylor": {"order": 4, "bands": nb, "call_batch": cb, "ms": taylor_ms,
                            "band_steps_per_s": nb / (taylor_ms * 1e-3),
                            "h_applies_per_s": 4 * nb / (taylor_ms * 1e-3)},
