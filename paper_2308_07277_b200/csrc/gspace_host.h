@@ -44,8 +44,7 @@ struct QmKTables {
     int mmax[3] = {0, 0, 0};
     std::vector<int32_t> idx, miller;          // miller: ng*3
     std::vector<double> g2;
-    std::vector<int32_t> gstick, stickoff, stickapos;
-    std::vector<uint16_t> gzpos;
+    std::vector<int32_t> stickoff;             // [S+1] first G of each stick
     std::vector<int16_t> xrow;
     std::vector<short4> rowiv;                 // per plane row: occupied i2 intervals
     std::vector<int4> rowinfo;                 // packed (a1|b1<<16, a2|b2<<16, first stick of the row, 0)
@@ -97,7 +96,6 @@ static inline int qm_build_tables(const double *lattice, const double *recip, do
     const int ng = (int)ents.size();
     kp->ng = ng;
     kp->idx.resize(ng); kp->miller.resize((size_t)ng * 3); kp->g2.resize(ng);
-    kp->gstick.resize(ng); kp->gzpos.resize(ng);
     kp->stickoff.clear();
     std::vector<int32_t> stick_i1, stick_i2;
     int64_t cur = -1;
@@ -113,8 +111,6 @@ static inline int qm_build_tables(const double *lattice, const double *recip, do
             stick_i1.push_back((int)(line / n2));
             stick_i2.push_back((int)(line % n2));
         }
-        kp->gstick[i] = (int32_t)kp->stickoff.size() - 1;
-        kp->gzpos[i] = (uint16_t)qm_pos(ax[2], (int)(e.idx % n3));
     }
     const int S = (int)kp->stickoff.size();
     kp->stickoff.push_back(ng);
@@ -202,8 +198,5 @@ static inline int qm_build_tables(const double *lattice, const double *recip, do
             if (iv.z <= iv.w && iv.z < (ax[1].r1 - q) * ax[1].r2) kp->y_quarter = false;
         }
     }
-    kp->stickapos.resize(S);
-    for (int s = 0; s < S; ++s)
-        kp->stickapos[s] = kp->xrow[stick_i1[s]] * kp->rowpitch + qm_pos(ax[1], stick_i2[s]);
     return 0;
 }

@@ -49,9 +49,6 @@ template <class T> struct DevBuf {
 };
 
 struct KPoint : QmKTables {
-    DevBuf<int32_t> d_gstick, d_stickoff, d_stickapos;
-    DevBuf<uint16_t> d_gzpos;
-    DevBuf<int16_t> d_xrow;
     DevBuf<int4> d_rowinfo, d_stickinfo;
     DevBuf<double> d_g2;
     // non-local
@@ -63,8 +60,7 @@ struct KPoint : QmKTables {
     QmKPlanDev plan() const {
         QmKPlanDev p;
         p.ng = ng; p.nsticks = nsticks; p.nx = nx; p.rowpitch = rowpitch;
-        p.g_stick = d_gstick.p; p.g_zpos = d_gzpos.p; p.stick_off = d_stickoff.p;
-        p.stick_apos = d_stickapos.p; p.xrow = d_xrow.p; p.g2 = d_g2.p;
+        p.g2 = d_g2.p;
         p.row_info = d_rowinfo.p; p.x_iv = xiv; p.stick_info = d_stickinfo.p;
         return p;
     }
@@ -151,11 +147,6 @@ int build_kpoint(qm_gspace *g, KPoint *kp) {
     const int rc = qm_build_tables(g->lattice, g->recip, g->ecut, g->grid, g->ax, kp, &msg);
     if (rc == -1) return fail(QM_EGRID, msg);
     if (rc != 0) return fail(QM_EINVAL, msg);
-    CU_TRY(kp->d_gstick.upload(kp->gstick));
-    CU_TRY(kp->d_gzpos.upload(kp->gzpos));
-    CU_TRY(kp->d_stickoff.upload(kp->stickoff));
-    CU_TRY(kp->d_stickapos.upload(kp->stickapos));
-    CU_TRY(kp->d_xrow.upload(kp->xrow));
     CU_TRY(kp->d_rowinfo.upload(kp->rowinfo));
     CU_TRY(kp->d_stickinfo.upload(kp->stickinfo));
     CU_TRY(kp->d_g2.upload(kp->g2));

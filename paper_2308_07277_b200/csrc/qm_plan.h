@@ -14,11 +14,6 @@ struct QmKPlanDev {        // per k-point tables on the device
     int nsticks;           // S: (i1,i2) lines that intersect the sphere
     int nx;                // X: distinct i1 among the sticks
     int rowpitch;          // pitch of one plane row (odd, >= axis2.len)
-    const int32_t *g_stick;      // [ng]   stick of each G
-    const uint16_t *g_zpos;      // [ng]   padded position of its z index (LineCfg::pos(i3))
-    const int32_t *stick_off;    // [S+1]  first G of each stick
-    const int32_t *stick_apos;   // [S]    position in the plane array: row*rowpitch + pos(i2)
-    const int16_t *xrow;         // [n1]   compact row of box index i1, or -1
     short4 x_iv;                 //        occupied i1 intervals [x,y] -> rows 0.., [z,w] -> following rows
     const int4 *row_info;        // [X]    per plane row: (a1 | b1<<16, a2 | b2<<16, first stick, 0): occupied i2 intervals
     const int4 *stick_info;      // [S]    per stick: (a1 | b1<<16, a2 | b2<<16, first G, 0): occupied i3 intervals
@@ -28,7 +23,7 @@ struct QmKPlanDev {        // per k-point tables on the device
 struct QmGridDev {
     QmAxis ax[3];
     const c128 *tw[3];     // tw[a][j] = exp(-2 pi i j / n_a)
-    const double *vt;      // re-laid-out potential [p(z)][pcol(y)][x] * 1/(n1 n2 n3), or nullptr
+    const double *vt;      // re-laid-out potential (fft_phases.cuh VLayout) * 1/(n1 n2 n3), or nullptr
 };
 
 // transposed label p -> natural index (p / r2) + r1 * (p % r2)
