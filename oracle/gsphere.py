@@ -12,17 +12,10 @@ import numpy as np
 
 
 def reciprocal_lattice(lattice: np.ndarray) -> np.ndarray:
-    """Rows b_i with a_i . b_j = 2 pi delta_ij, by the textbook cross-product
-    definition b_1 = 2 pi (a_2 x a_3) / (a_1 . (a_2 x a_3)) and cyclic, in plain IEEE double scalars."""
-    a = [[float(x) for x in row] for row in np.asarray(lattice, dtype=np.float64).reshape(3, 3)]
-
-    def cross(u, v):
-        return [u[1] * v[2] - u[2] * v[1], u[2] * v[0] - u[0] * v[2], u[0] * v[1] - u[1] * v[0]]
-
-    c = [cross(a[1], a[2]), cross(a[2], a[0]), cross(a[0], a[1])]
-    det = a[0][0] * c[0][0] + a[0][1] * c[0][1] + a[0][2] * c[0][2]
-    f = 2.0 * math.pi / det
-    return np.array([[f * x for x in row] for row in c])
+    """Rows b_i with a_i . b_j = 2 pi delta_ij, i.e. B = 2 pi (A^-1)^T  (PAPER.md:625-631 prints the
+    three axes of the bcc example; the defining relation is the one above)."""
+    a = np.asarray(lattice, dtype=np.float64).reshape(3, 3)
+    return 2.0 * math.pi * np.linalg.inv(a).T
 
 
 def gsphere(lattice, ecut_ry: float, grid, k_cryst=(0.0, 0.0, 0.0)):
@@ -46,12 +39,8 @@ def gsphere(lattice, ecut_ry: float, grid, k_cryst=(0.0, 0.0, 0.0)):
     r3 = np.arange(-bound[2], bound[2] + 1)
     M1, M2, M3 = np.meshgrid(r1, r2, r3, indexing="ij")
     m = np.stack([M1.ravel(), M2.ravel(), M3.ravel()], axis=1)
-    f = m.astype(np.float64) + k[None, :]
-    # q = (m + k) . B written out per component (elementwise, fixed order; no BLAS call)
-    qx = f[:, 0] * b[0, 0] + f[:, 1] * b[1, 0] + f[:, 2] * b[2, 0]
-    qy = f[:, 0] * b[0, 1] + f[:, 1] * b[1, 1] + f[:, 2] * b[2, 1]
-    qz = f[:, 0] * b[0, 2] + f[:, 1] * b[1, 2] + f[:, 2] * b[2, 2]
-    g2 = qx * qx + qy * qy + qz * qz
+    q = (m.astype(np.float64) + k[None, :]) @ b          # Cartesian k + G_m, rows
+    g2 = q[:, 0] * q[:, 0] + q[:, 1] * q[:, 1] + q[:, 2] * q[:, 2]
     keep = g2 <= ecut_ry
     m = m[keep]
     g2 = g2[keep]

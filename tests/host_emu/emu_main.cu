@@ -4,7 +4,7 @@
 // index logic of the pipeline can be checked against numpy on a machine without a GPU.
 //
 // usage: emu_main <n> <lat9.bin> <ecut> <k1> <k2> <k3> <nb> <psi.bin> <v.bin> <out_prefix>
-// writes <out_prefix>.idx (int32), .hloc (T+L apply, c128 [nb][ng]), .g2r (c128 [nb][n^3]), .r2g
+// writes <out_prefix>.idx (int32), .g2 (the library's host |k+G|^2 table), .hloc (T+L apply, c128 [nb][ng]), .g2r (c128 [nb][n^3]), .r2g
 #include <cstdio>
 #include <cstdlib>
 #include <string>
@@ -180,7 +180,7 @@ template <class C> int run(int n, const double *lat, double ecut, const double *
         for (int p = 0; p < n; ++p) emu.template plane<2>(p, W.data(), nullptr, &g2r[b * n3], 1.0, ncol);
         emu.zfwd(W.data(), nullptr, &r2g[(size_t)b * kp.ng], false);
     }
-    dump(prefix + ".idx", kp.idx); dump(prefix + ".hloc", hloc); dump(prefix + ".g2r", g2r); dump(prefix + ".r2g", r2g);
+    dump(prefix + ".idx", kp.idx); dump(prefix + ".g2", kp.g2); dump(prefix + ".hloc", hloc); dump(prefix + ".g2r", g2r); dump(prefix + ".r2g", r2g);
     printf("ng %d sticks %d nx %d quarter x%d y%d z%d\n", kp.ng, kp.nsticks, kp.nx, (int)kp.x_quarter, (int)kp.y_quarter, (int)kp.z_quarter);
     return 0;
 }

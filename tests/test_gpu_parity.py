@@ -1,12 +1,13 @@
 """GPU parity: qm_apply_h (through the C ABI) vs the CPU oracle, element by element (-m gpu).
 
-Tolerance 1e-11 max relative error per band (north_star; A13); index maps bit exact; g2 <= 2 ulp (A14).
+Tolerance 1e-11 max relative error per band (north_star; A13); index maps bit exact; |k+G|^2 of BOTH sides within the
+derived rounding bound of an exact rational evaluation (A14; tests/common.py exact_g2).
 Each config is run three times (A19): full H, D = 0 (no projectors), V = 0.
 """
 import numpy as np
 import pytest
 
-from tests.common import TOL, band_errors, problem
+from tests.common import G2_TOL_U, TOL, UNIT_ROUNDOFF, band_errors, exact_g2, problem
 from oracle import hpsi as oh
 from oracle import hpsi_fft as of
 
@@ -61,8 +62,14 @@ def test_index_map_bit_exact(qm, name):
         assert gs.num_g(ik) == pk["idx"].size
         np.testing.assert_array_equal(gs.index_map(ik), pk["idx"])
         np.testing.assert_array_equal(gs.miller(ik), pk["miller"])
+        # A14: neither side mirrors the other; each is held to the exact value (rational arithmetic) within the
+        # rounding bound derived from the operation count.  Full sphere for the small configs, a fixed sample else.
         g2 = gs.g2(ik)
-        assert np.max(np.abs(g2 - pk["g2"]) / np.maximum(np.spacing(pk["g2"]), 1e-300)) <= 2.0
+        sel = np.arange(g2.size) if g2.size <= 3000 else np.unique(
+            np.concatenate([[0, 1, g2.size - 1], np.random.default_rng(ik).integers(0, g2.size, 3000)]))
+        ex, scale = exact_g2(pk["lat"], pk["k"], pk["miller"][sel])
+        assert np.all(np.abs(g2[sel] - ex) <= G2_TOL_U * UNIT_ROUNDOFF * scale)
+        assert np.all(np.abs(pk["g2"][sel] - ex) <= G2_TOL_U * UNIT_ROUNDOFF * scale)
         assert gs.alias_free(ik)
     gs.close()
 

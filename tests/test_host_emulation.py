@@ -13,6 +13,7 @@ import numpy as np
 import pytest
 
 from oracle import gsphere as og
+from tests.common import G2_TOL_U, UNIT_ROUNDOFF, exact_g2
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 SRC = os.path.join(ROOT, "tests", "host_emu", "emu_main.cu")
@@ -73,10 +74,15 @@ def test_emulated_fft_path_matches_numpy(emu_bin, n, lat, ecut, k):
                         str(nb), os.path.join(d, "psi.bin"), os.path.join(d, "v.bin"), pre], check=True,
                        capture_output=True)
         got_idx = np.fromfile(pre + ".idx", dtype=np.int32)
+        got_g2 = np.fromfile(pre + ".g2", dtype=np.float64)
         hloc = np.fromfile(pre + ".hloc", dtype=np.complex128).reshape(nb, ng)
         g2r = np.fromfile(pre + ".g2r", dtype=np.complex128).reshape(nb, n, n, n)
         r2g = np.fromfile(pre + ".r2g", dtype=np.complex128).reshape(nb, ng)
     np.testing.assert_array_equal(got_idx, idx)                 # host tables vs oracle: bit exact
+    # A14: the library's host |k+G|^2 table against the exact rational evaluation (not against the oracle's spelling)
+    sel = np.arange(ng) if ng <= 2000 else np.random.default_rng(1).integers(0, ng, 2000)
+    ex, sc = exact_g2(lat, k, miller[sel])
+    assert np.all(np.abs(got_g2[sel] - ex) <= G2_TOL_U * UNIT_ROUNDOFF * sc)
     box = np.zeros((nb, n ** 3), dtype=np.complex128)
     box[:, idx] = psi
     psi_r = np.fft.ifftn(box.reshape(nb, n, n, n), axes=(1, 2, 3))

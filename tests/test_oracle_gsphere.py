@@ -7,7 +7,8 @@ import numpy as np
 import pytest
 
 from oracle import gsphere as og
-from workloads import CONFIGS, cell_for
+from tests.common import G2_TOL_U, UNIT_ROUNDOFF, exact_g2
+from workloads import CONFIGS, cell_for, make_kpoints
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden", "bcc_fe_gspace.txt")
 
@@ -100,6 +101,24 @@ def test_brute_force_k_point_sphere():
     assert sorted(ref) == list(idx)
     q = (miller + k) @ b
     np.testing.assert_allclose(g2, np.sum(q * q, axis=1), rtol=1e-14)
+
+
+@pytest.mark.parametrize("name,ik", [("cfg1", 0), ("cfg2", 3), ("cfg3", 0), ("bcc", 0)])
+def test_g2_against_exact_rational_evaluation(name, ik):
+    """A14: the oracle's |k+G|^2 against an exact evaluation (rational arithmetic, one final rounding), within the
+    rounding bound derived from the operation count (tests/common.py G2_TOL_U).  A wrong reciprocal axis, a
+    transposed B or a dropped k fails this by many orders of magnitude."""
+    if name == "bcc":
+        _, lat = _bcc()
+        k, ecut, grid = np.zeros(3), 160.0, (18, 18, 18)
+    else:
+        cfg = CONFIGS[name]
+        lat, _ = cell_for(cfg)
+        k, ecut, grid = make_kpoints(cfg)[ik], cfg.ecutwfc_ry, cfg.grid
+    miller, idx, g2 = og.gsphere(lat, ecut, grid, k)
+    ex, scale = exact_g2(lat, k, miller)
+    assert np.all(np.abs(g2 - ex) <= G2_TOL_U * UNIT_ROUNDOFF * scale)
+    assert np.all(ex <= ecut * (1 + 1e-12))
 
 
 def test_grid_too_small_is_an_error():
