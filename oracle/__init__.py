@@ -13,7 +13,9 @@ Parts:
                       sum as explicit C loops in hpsi_direct.c for large N_G)
   O3  dft.py          naive DFT straight from the definition (8^3-size checks)
   O5  subspace.py     subspace products <psi_i|phi_j>
-  O7  propagate.py    Taylor-series exp(-i dt H) psi, eq. 52 (8(f) rank 3)
+  O7  propagate.py    Taylor-series exp(-i dt H) psi, eq. 52, and the split-operator form, eq. 53 (8(f) rank 3;
+                      PAPER.md:1131-1139)
+  O8  mtxel.py        GW plane-wave matrix elements M_nn'(k,q,G), eq. 56 (8(f) rank 4)
   O6  density.py      n(r) = sum_i f_i |psi_i(r)|^2 by direct synthesis (8(f) rank 2)
 
 Pins (tests/test_oracle_*.py, ``-m "not gpu"``): the paper's printed bcc

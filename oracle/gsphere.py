@@ -18,8 +18,9 @@ def reciprocal_lattice(lattice: np.ndarray) -> np.ndarray:
     return 2.0 * math.pi * np.linalg.inv(a).T
 
 
-def gsphere(lattice, ecut_ry: float, grid, k_cryst=(0.0, 0.0, 0.0)):
-    """All integer m with |k + G_m|^2 [bohr^-2] <= ecut [Ry]  (== q^2/2 <= E_cut Ha).
+def gsphere(lattice, ecut_ry: float, grid, k_cryst=(0.0, 0.0, 0.0), strict: bool = False):
+    """All integer m with |k + G_m|^2 [bohr^-2] <= ecut [Ry]  (== q^2/2 <= E_cut Ha); `strict` selects `<`
+    (the epsilon sphere of PAPER.md:1319-1321, eq. 56, is printed with a strict inequality).
 
     Returns (miller int32[ng,3], idx int32[ng], g2 float64[ng]) sorted by
     ascending C-order flat box index
@@ -41,7 +42,7 @@ def gsphere(lattice, ecut_ry: float, grid, k_cryst=(0.0, 0.0, 0.0)):
     m = np.stack([M1.ravel(), M2.ravel(), M3.ravel()], axis=1)
     q = (m.astype(np.float64) + k[None, :]) @ b          # Cartesian k + G_m, rows
     g2 = q[:, 0] * q[:, 0] + q[:, 1] * q[:, 1] + q[:, 2] * q[:, 2]
-    keep = g2 <= ecut_ry
+    keep = (g2 < ecut_ry) if strict else (g2 <= ecut_ry)
     m = m[keep]
     g2 = g2[keep]
     for i, n in enumerate((n1, n2, n3)):

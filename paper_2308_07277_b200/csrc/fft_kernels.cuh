@@ -5,7 +5,6 @@
 //   k_zfwd  : a4(z)+a5  forward z-FFT, gather to the sphere, + 1/2|k+G|^2 psi_in
 #pragma once
 #include <cuda_runtime.h>
-#include <cstdio>
 #include "fft_phases.cuh"
 #include "async_copy.cuh"
 #include "qm_plan.h"
@@ -151,9 +150,6 @@ template <int TT, int TPG> __host__ __device__ constexpr int qm_team_slot(int te
     return (TT == 12 && TPG == 8) ? ((team >> 1) + 4 * (team & 1)) : team;
 }
 template <int G> __device__ __forceinline__ void group_barrier(int grp) {
-#ifdef QM_ABLATE_GBAR     /* timing experiment only: results are wrong */
-    return;
-#endif
     if constexpr (G == 32) __syncwarp();
     else asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "r"(G) : "memory");
 }
@@ -327,12 +323,6 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
     cx.rowinfo_s = rowinfo_s;
     for (int i = threadIdx.x; i < cx.X; i += blockDim.x) rowinfo_s[i] = kp.row_info[i];
     __syncthreads();
-#ifdef QM_PLANE_TIMING
-    long long tacc[3] = {0, 0, 0}, t0 = clock64(), t1;
-#define QM_TICK(i) do { t1 = clock64(); tacc[i] += t1 - t0; t0 = t1; } while (0)
-#else
-#define QM_TICK(i) do {} while (0)
-#endif
     // per-thread twiddle rows, loaded once (u is fixed for the whole kernel)
     const int u_tw = (int)(threadIdx.x % G) % C::TT;
     TwRow<C::R1> twa;
@@ -362,19 +352,12 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
         plane_y_phase<C, MODE>(cx, W, pl, prev, have_cur, twa, twb);
         if (!have_cur) break;
         __syncthreads();
-        QM_TICK(0);
         const int p = pl % n3;
         const int z = (p / gd.ax[2].r2) + gd.ax[2].r1 * (p % gd.ax[2].r2);
         double sc = scale;
         if constexpr (MODE == 3) sc = scale * occ[pl / n3];
         plane_x_phase<C, MODE>(cx, kp.x_iv, gd.vt, box ? box + z : nullptr, pl, sc, stagger_ns, rhot, twa, twb);
         __syncthreads();
-        QM_TICK(1);
         prev = pl;
     }
-#ifdef QM_PLANE_TIMING
-    QM_TICK(2);
-    if (threadIdx.x == 0 && (blockIdx.x == 0 || blockIdx.x == 77 || blockIdx.x == 147))
-        printf("cta %d clk: y %lld x %lld tail %lld\n", blockIdx.x, tacc[0], tacc[1], tacc[2]);
-#endif
 }

@@ -337,10 +337,6 @@ template <int R> struct VRow { double v[R]; };
 template <class C> struct VLayout { static constexpr int R2E = C::R2 + (C::R2 & 1), COL = C::R1 * R2E; };
 template <class C> QM_HD void load_vrow(VRow<C::R2> &vr, const double *vcol, int u) {
     if (u >= C::R1) return;
-#ifdef QM_ABLATE_V        /* timing experiment only */
-    static_for<C::R2>([&](auto I) { vr.v[decltype(I)::value] = 1.0; });
-    return;
-#endif
     const double2 *q = reinterpret_cast<const double2 *>(vcol) + u;
     static_for<VLayout<C>::R2E / 2>([&](auto I) {
         constexpr int j = decltype(I)::value;

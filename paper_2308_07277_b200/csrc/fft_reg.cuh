@@ -130,9 +130,6 @@ template <int RA, int RB, int DIR> struct DftPFA {
     static constexpr int R = RA * RB;
     static constexpr int EA = RB * qm_modinv(RB % RA, RA), EB = RA * qm_modinv(RA % RB, RB);
     static QM_HD void run(c128 (&x)[R]) {
-#ifdef QM_ABLATE_DFT      /* timing experiment only: results are wrong */
-        return;
-#endif
         c128 y[R];
         static_for<RB>([&](auto N2) {
             constexpr int n2 = decltype(N2)::value;
