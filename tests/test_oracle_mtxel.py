@@ -100,9 +100,14 @@ def test_wrap_and_no_wrap_agree_on_a_large_enough_grid_and_fft_route_agrees():
     c = om.matrix_elements_fft(bra, ib, ket, ik, ie, grid)
     np.testing.assert_allclose(a, c, rtol=0, atol=1e-11)
     # on a grid that is too small the lookups wrap: the two readings differ, the grid route follows `wrap`
-    small = (13, 13, 13)
-    cfg, lat, _, (mb, ib), (mk, ik), (me, ie, _) = _spheres(grid=small)
-    bra, ket = bra[:, :ib.size], ket[:, :ik.size]
+    lat, small = 10.26 * np.eye(3), (11, 11, 11)
+    kb, kk = np.array([0.3, 0.0, -0.2]), np.zeros(3)
+    mb, ib, _ = og.gsphere(lat, 12.0, small, kb)
+    mk, ik, _ = og.gsphere(lat, 12.0, small, kk)
+    me, ie, _ = og.gsphere(lat, 6.0, small, kb - kk, strict=True)
+    assert small[0] < 2 * max(np.abs(mb).max(), np.abs(mk).max()) + np.abs(me).max() + 1
+    bra = rng.standard_normal((2, ib.size)) + 1j * rng.standard_normal((2, ib.size))
+    ket = rng.standard_normal((2, ik.size)) + 1j * rng.standard_normal((2, ik.size))
     a = om.matrix_elements(bra, mb, ket, mk, me, small, wrap=True)
     b = om.matrix_elements(bra, mb, ket, mk, me, small, wrap=False)
     assert np.max(np.abs(a - b)) > 1e-3
