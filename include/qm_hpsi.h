@@ -22,9 +22,20 @@
  * qm_status; qm_last_error() gives thread-local text for the last failure.
  * Hot-path calls (qm_apply_h) only enqueue work on `stream` (a cudaStream_t
  * passed as void*): no device synchronisation, no host<->device copy, no
- * allocation after the first call with a given nbands.
+ * allocation after the first call with a given nbands (none at all after
+ * qm_reserve).
  * There is no CPU fallback: without a CUDA device every compute call fails
  * with QM_ECUDA.
+ *
+ * Devices and streams.  A handle belongs to the CUDA device that was current in
+ * qm_gspace_create; every call that touches the device returns QM_EINVAL if
+ * another device is current.  Work spaces are owned per k-point: calls for
+ * DIFFERENT k-points of one handle may be in flight on different streams at the
+ * same time (e.g. the ten k-points of a band x k batch); calls for the SAME
+ * k-point, and qm_set_vloc / qm_split_operator_set / the density calls (shared
+ * tables), must be stream-ordered with respect to each other -- the library
+ * cannot detect a violation.  Host-side state (qm_last_error is thread-local;
+ * the handle is not locked) allows one calling thread per handle at a time.
  */
 #ifndef QM_HPSI_H
 #define QM_HPSI_H
@@ -94,11 +105,30 @@ QM_API int qm_set_vloc(qm_gspace *g, const double *V_r_dev, void *stream);
 QM_API int qm_set_nonlocal(qm_gspace *g, int k, const qm_c128 *beta_kG_dev, int nproj,
                     const double *D_dev, int d_block, void *stream);
 
+/* Grow every library-owned work space that qm_apply_h / qm_split_operator_propagate / the density and debug calls
+ * need for blocks of up to `nbands` wavefunctions at k-point k (projector work spaces are sized by qm_set_nonlocal), so
+ * that no later call allocates.  May synchronise the device (cudaMalloc); not a hot-path call. */
+QM_API int qm_reserve(qm_gspace *g, int k, int nbands);
+
 /* psi_out = H psi_in for a block of nbands wavefunctions at k-point k.
  *  psi_in_dev, psi_out_dev  DEVICE  [nbands][ng(k)] row-major complex128; must not overlap;
  *                           psi_out is overwritten. */
 QM_API int qm_apply_h(qm_gspace *g, const qm_c128 *psi_in_dev, qm_c128 *psi_out_dev,
                int nbands, int k, void *stream);
+
+/* A fixed batch of qm_apply_h calls as ONE submission (north_star: "batched over (band,k)"; the paper's band and
+ * k-point independence).  The items -- (k[i], psi_in_dev[i], psi_out_dev[i], nbands[i]), every pointer
+ * DEVICE and fixed for the life of the plan -- are captured once into a CUDA graph: items of different k-points sit on
+ * parallel branches (k-points own their work spaces), items of one k-point run in list order.  qm_batch_plan_launch
+ * enqueues the whole graph on `stream`; it replaces the per-call launch latency that dominates the small configs.
+ * qm_set_vloc / qm_set_nonlocal must have been called for every k used; creation reserves the work spaces
+ * (qm_reserve) and may synchronise.  A later qm_set_nonlocal with a different nproj for a k-point in the plan
+ * invalidates it.  The plan borrows the handle: destroy it before qm_gspace_destroy. */
+typedef struct qm_batch_plan qm_batch_plan;
+QM_API int qm_batch_plan_create(qm_gspace *g, int nitems, const int *k, const qm_c128 *const *psi_in_dev,
+                                qm_c128 *const *psi_out_dev, const int *nbands, qm_batch_plan **out);
+QM_API int qm_batch_plan_launch(qm_batch_plan *p, void *stream);
+QM_API int qm_batch_plan_destroy(qm_batch_plan *p);
 
 /* Electron density from Bloch states (eq. 2, 1008):  n(r_j) = sum_i f_i |psi_i(r_j)|^2 with
  * psi_i(r_j) = sum_{G in sphere(k)} psi_i(G) exp(+i G.r_j) (unnormalised synthesis, reading A5/A20; the Bloch phase
@@ -123,6 +153,45 @@ QM_API int qm_density_get(qm_gspace *g, double *rho_dev, double scale, void *str
  * psi_out is overwritten.  order == 0 copies.  Two library-owned blocks of the same size are grown on first use. */
 QM_API int qm_taylor_propagate(qm_gspace *g, int k, const qm_c128 *psi_in_dev, qm_c128 *psi_out_dev, int nbands, double dt,
                         int order, void *stream);
+
+/* Split-operator exponential of the TDKS propagator (eq. 53; the paper's second expoper form):
+ *   psi_out = exp(-i dt T/2) exp(-i dt V) exp(-i dt T/2) psi_in
+ * T(G) = 1/2 |k+G|^2 is diagonal on the sphere: its half-steps are the phases exp(-i dt |k+G|^2 / 4), applied as psi
+ * is scattered and as the result is gathered.  V is the LOCAL potential (reading A22 of DESIGN.md: the paper does not say
+ * what V holds when projectors are present; they are not part of this propagator -- use qm_taylor_propagate): the
+ * middle factor is the multiplication by exp(-i dt V(r_j)) on the FFT grid between the backward and the forward
+ * transform, i.e. on the sphere  sum_G' Ehat(G - G') psi(G'),  Ehat = (1/N) DFT[exp(-i dt V)].  One pass, three kernels.
+ *   qm_split_operator_set        builds exp(-i dt V(r)) / N and the kinetic phases of every k-point on `stream`
+ *                                V_r_dev DEVICE n1*n2*n3 doubles, C order, Hartree (copied); dt in atomic units of time
+ *   qm_split_operator_propagate  psi_in_dev, psi_out_dev DEVICE [nbands][ng(k)] complex128, must not overlap;
+ *                                QM_ENOTSET before qm_split_operator_set. */
+QM_API int qm_split_operator_set(qm_gspace *g, const double *V_r_dev, double dt, void *stream);
+QM_API int qm_split_operator_propagate(qm_gspace *g, int k, const qm_c128 *psi_in_dev, qm_c128 *psi_out_dev, int nbands,
+                                       void *stream);
+
+/* GW plane-wave matrix elements (eqs. 56-57; the paper's matrix_elements):
+ *   M_{nn'}(k, q, G) = < n k+q | exp(i (q+G).r) | n' k > = sum_G'' conj(c_{n,k+q}(G''+G)) c_{n'k}(G'')
+ * for the G of the epsilon sphere |q+G|^2 < ecut_eps (strict, as printed in eq. 56), q = kpts[k_bra] - kpts[k_ket]
+ * in crystal coordinates.  Reading A21 of DESIGN.md: eq. 56 is the definition (eq. 57 names the FFT directions the
+ * other way round from eq. 9); G''+G is looked up modulo the FFT box (reading A8), so on a box with
+ * n_i >= 2 m_wfn + m_eps + 1 nothing wraps.  No cell-volume factor.  Computed as the paper describes: both states are
+ * synthesised on the grid (scatter + pruned backward FFT), multiplied, and analysed (forward FFT pruned to the
+ * epsilon sphere); the ket boxes are synthesised once per call.
+ *   qm_mtxel_create     builds the epsilon sphere (sorted like the wavefunction spheres: ascending C-order box index) and
+ *                       its stick tables on the handle's FFT box; QM_EGRID if it does not fit (2|m_i|+1 > n_i).
+ *                       The qm_mtxel borrows the handle: destroy it before qm_gspace_destroy.
+ *   qm_mtxel_num_g / _get_miller / _get_index_map   HOST outputs, ng_eps / ng_eps*3 / ng_eps entries
+ *   qm_matrix_elements  bra_dev DEVICE [nbra][ng(k_bra)], ket_dev DEVICE [nket][ng(k_ket)] complex128;
+ *                       out_dev DEVICE [nbra][nket][ng_eps] complex128, overwritten.  Only enqueues on `stream`
+ *                       after its work spaces ((nket + a few) boxes of n1*n2*n3 complex128) exist. */
+typedef struct qm_mtxel qm_mtxel;
+QM_API int qm_mtxel_create(qm_gspace *g, int k_bra, int k_ket, double ecut_eps_ry, qm_mtxel **out);
+QM_API int qm_mtxel_destroy(qm_mtxel *m);
+QM_API int qm_mtxel_num_g(const qm_mtxel *m, int *ng);
+QM_API int qm_mtxel_get_miller(const qm_mtxel *m, int32_t *miller_host);
+QM_API int qm_mtxel_get_index_map(const qm_mtxel *m, int32_t *idx_host);
+QM_API int qm_matrix_elements(qm_mtxel *m, const qm_c128 *bra_dev, int nbra, const qm_c128 *ket_dev, int nket,
+                              qm_c128 *out_dev, void *stream);
 
 /* Subspace products S[i][j] = <a_i|b_j> = sum_G conj(a_i(G)) b_j(G) over the sphere of k-point k: the step right
  * after h_psi in the Davidson solver, the paper's WavefunG.vdot(psi, phi) = ZGEMM.

@@ -42,6 +42,18 @@ _SIGS = {
     "qm_set_vloc": [_vp, _vp, _vp],
     "qm_set_nonlocal": [_vp, _i, _vp, _i, _vp, _i, _vp],
     "qm_apply_h": [_vp, _vp, _vp, _i, _i, _vp],
+    "qm_reserve": [_vp, _i, _i],
+    "qm_batch_plan_create": [_vp, _i, _vp, _vp, _vp, _vp, ctypes.POINTER(_vp)],
+    "qm_batch_plan_launch": [_vp, _vp],
+    "qm_batch_plan_destroy": [_vp],
+    "qm_split_operator_set": [_vp, _vp, _d, _vp],
+    "qm_split_operator_propagate": [_vp, _i, _vp, _vp, _i, _vp],
+    "qm_mtxel_create": [_vp, _i, _i, _d, ctypes.POINTER(_vp)],
+    "qm_mtxel_destroy": [_vp],
+    "qm_mtxel_num_g": [_vp, ctypes.POINTER(_i)],
+    "qm_mtxel_get_miller": [_vp, _vp],
+    "qm_mtxel_get_index_map": [_vp, _vp],
+    "qm_matrix_elements": [_vp, _vp, _i, _vp, _i, _vp, _vp],
     "qm_subspace": [_vp, _i, _vp, _i, _vp, _i, _vp, _vp],
     "qm_taylor_propagate": [_vp, _i, _vp, _vp, _i, _d, _i, _vp],
     "qm_density_reset": [_vp, _vp],
@@ -211,6 +223,97 @@ def qm_apply_h(h, psi_in_dev, psi_out_dev, k=0, stream=None):
     return psi_out_dev
 
 
+def qm_batch_plan_create(h, items):
+    """items: list of (k, psi_in_dev, psi_out_dev) with [nbands][ng(k)] complex128 CUDA tensors (kept alive by the caller)."""
+    import torch
+    n = len(items)
+    ks = (ctypes.c_int * n)(*[int(it[0]) for it in items])
+    nbs = (ctypes.c_int * n)()
+    pin = (ctypes.c_void_p * n)()
+    pout = (ctypes.c_void_p * n)()
+    for i, (k, a, b) in enumerate(items):
+        nbs[i] = _check_block(h, k, a, "psi_in")
+        if tuple(b.shape) != tuple(a.shape):
+            raise TypeError("psi_out: shape differs from psi_in")
+        pin[i] = _dev_ptr(a, torch.complex128, "psi_in").value
+        pout[i] = _dev_ptr(b, torch.complex128, "psi_out").value
+    p = _vp()
+    _check(load_library().qm_batch_plan_create(h, n, ks, pin, pout, nbs, ctypes.byref(p)))
+    return p
+
+
+def qm_batch_plan_launch(p, stream=None):
+    _check(load_library().qm_batch_plan_launch(p, _stream_ptr(stream)))
+
+
+def qm_batch_plan_destroy(p):
+    _check(load_library().qm_batch_plan_destroy(p))
+
+
+def qm_reserve(h, k, nbands):
+    _check(load_library().qm_reserve(h, int(k), int(nbands)))
+
+
+def qm_split_operator_set(h, v_r_dev, dt, stream=None):
+    import torch
+    _check(load_library().qm_split_operator_set(h, _dev_ptr(v_r_dev, torch.float64, "V_r"), float(dt), _stream_ptr(stream)))
+
+
+def qm_split_operator_propagate(h, psi_in_dev, psi_out_dev, k=0, stream=None):
+    import torch
+    nb = _check_block(h, k, psi_in_dev, "psi_in")
+    if tuple(psi_out_dev.shape) != tuple(psi_in_dev.shape):
+        raise TypeError("psi_out: shape differs from psi_in")
+    _check(load_library().qm_split_operator_propagate(h, k, _dev_ptr(psi_in_dev, torch.complex128, "psi_in"),
+                                                      _dev_ptr(psi_out_dev, torch.complex128, "psi_out"), nb,
+                                                      _stream_ptr(stream)))
+    return psi_out_dev
+
+
+def qm_mtxel_create(h, k_bra, k_ket, ecut_eps_ry):
+    m = _vp()
+    _check(load_library().qm_mtxel_create(h, int(k_bra), int(k_ket), float(ecut_eps_ry), ctypes.byref(m)))
+    return m
+
+
+def qm_mtxel_destroy(m):
+    _check(load_library().qm_mtxel_destroy(m))
+
+
+def qm_mtxel_num_g(m) -> int:
+    n = _i()
+    _check(load_library().qm_mtxel_num_g(m, ctypes.byref(n)))
+    return n.value
+
+
+def qm_mtxel_get_miller(m) -> np.ndarray:
+    out = np.empty((qm_mtxel_num_g(m), 3), dtype=np.int32)
+    _check(load_library().qm_mtxel_get_miller(m, out.ctypes.data))
+    return out
+
+
+def qm_mtxel_get_index_map(m) -> np.ndarray:
+    out = np.empty(qm_mtxel_num_g(m), dtype=np.int32)
+    _check(load_library().qm_mtxel_get_index_map(m, out.ctypes.data))
+    return out
+
+
+def qm_matrix_elements(m, h, k_bra, k_ket, bra_dev, ket_dev, out_dev=None, stream=None):
+    """out [nbra][nket][ng_eps] = M_{nn'}(G) (include/qm_hpsi.h); h, k_bra, k_ket only check the operand shapes."""
+    import torch
+    nbra = _check_block(h, k_bra, bra_dev, "bra")
+    nket = _check_block(h, k_ket, ket_dev, "ket")
+    ng = qm_mtxel_num_g(m)
+    if out_dev is None:
+        out_dev = torch.empty((nbra, nket, ng), dtype=torch.complex128, device=bra_dev.device)
+    if tuple(out_dev.shape) != (nbra, nket, ng):
+        raise TypeError("out: expected shape [nbra][nket][ng_eps]")
+    _check(load_library().qm_matrix_elements(m, _dev_ptr(bra_dev, torch.complex128, "bra"), nbra,
+                                             _dev_ptr(ket_dev, torch.complex128, "ket"), nket,
+                                             _dev_ptr(out_dev, torch.complex128, "out"), _stream_ptr(stream)))
+    return out_dev
+
+
 def qm_subspace(h, a_dev, b_dev, s_dev=None, k=0, stream=None):
     """S[i][j] = <a_i|b_j> over the sphere of k-point k (include/qm_hpsi.h); returns the [na][nb] device tensor."""
     import torch
@@ -369,6 +472,17 @@ class GSpace:
         return qm_apply_h(self._h, psi_in, psi_out, k, stream)
 
     def subspace(self, a, b, s=None, k=0, stream=None): return qm_subspace(self._h, a, b, s, k, stream)
+    def reserve(self, nbands, k=0): qm_reserve(self._h, k, nbands)
+    def batch_plan(self, items): return BatchPlan(self, items)
+    def split_operator_set(self, v, dt, stream=None): qm_split_operator_set(self._h, v, dt, stream)
+
+    def split_operator_propagate(self, psi_in, psi_out=None, k=0, stream=None):
+        import torch
+        if psi_out is None:
+            psi_out = torch.empty_like(psi_in)
+        return qm_split_operator_propagate(self._h, psi_in, psi_out, k, stream)
+
+    def mtxel(self, k_bra, k_ket, ecut_eps_ry): return MatrixElements(self, k_bra, k_ket, ecut_eps_ry)
 
     def taylor_propagate(self, psi_in, dt, order, psi_out=None, k=0, stream=None):
         import torch
@@ -407,3 +521,42 @@ class GSpace:
         return qm_debug_r2g(self._h, box_r, out, k, stream)
 
     def launch_count(self): return qm_get_launch_count(self._h)
+
+
+class MatrixElements:
+    """Owning wrapper of a qm_mtxel (the paper's matrix_elements step of Epsilon)."""
+
+    def __init__(self, gs: GSpace, k_bra: int, k_ket: int, ecut_eps_ry: float):
+        self._gs, self.k_bra, self.k_ket = gs, k_bra, k_ket          # keeps the borrowed handle alive
+        self._m = qm_mtxel_create(gs.handle, k_bra, k_ket, ecut_eps_ry)
+
+    def close(self):
+        if getattr(self, "_m", None) is not None:
+            qm_mtxel_destroy(self._m)
+            self._m = None
+
+    __del__ = close
+
+    def num_g(self): return qm_mtxel_num_g(self._m)
+    def miller(self): return qm_mtxel_get_miller(self._m)
+    def index_map(self): return qm_mtxel_get_index_map(self._m)
+
+    def apply(self, bra, ket, out=None, stream=None):
+        return qm_matrix_elements(self._m, self._gs.handle, self.k_bra, self.k_ket, bra, ket, out, stream)
+
+
+class BatchPlan:
+    """Owning wrapper of a qm_batch_plan: a fixed list of (k, psi_in, psi_out) applies launched as one CUDA graph."""
+
+    def __init__(self, gs: GSpace, items):
+        self._gs, self._items = gs, list(items)                      # keep the handle and the tensors alive
+        self._p = qm_batch_plan_create(gs.handle, self._items)
+
+    def close(self):
+        if getattr(self, "_p", None) is not None:
+            qm_batch_plan_destroy(self._p)
+            self._p = None
+
+    __del__ = close
+
+    def launch(self, stream=None): qm_batch_plan_launch(self._p, stream)

@@ -19,10 +19,11 @@ template <class C> __host__ __device__ constexpr size_t qm_z_smem() {
     return ((size_t)QM_ZT * (C::L | 1) + (size_t)C::N * QM_ZT) * sizeof(c128) + 16;
 }
 
-template <class C>
+// PH: multiply psi(G) by the per-G factor phase[g] as it is loaded (split-operator half-step, eq. 53).
+template <class C, bool PH>
 __global__ void __launch_bounds__(QM_ZT * C::TT, 2)
-k_zinv(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ psi, c128 *__restrict__ W, int ntiles,
-       int quarter)
+k_zinv(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ psi, const c128 *__restrict__ phase,
+       c128 *__restrict__ W, int ntiles, int quarter)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int LP = C::L | 1;
@@ -35,7 +36,10 @@ k_zinv(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ psi,
     const int t2 = tid % QM_ZT, u2 = tid / QM_ZT;      // pass 2: stick fastest
     TwRow<C::R1> twa;
     load_twrow(twa, tw, u1, C::R2);
-    const c128 *psib = psi + (size_t)band * kp.ng;
+    const c128 *psib_raw = psi + (size_t)band * kp.ng;
+    const auto psib = [&]() {
+        if constexpr (PH) return PhasedPtr{psib_raw, phase}; else return psib_raw;
+    }();
     c128 *Wb = W + (size_t)band * ntiles * C::N * QM_ZT;
     auto info = [&](int tile) {
         const int s = tile * QM_ZT + t1;
@@ -69,10 +73,11 @@ k_zinv(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ psi,
     if (tid == 0) bulk_wait0();
 }
 
-template <class C>
+// GM: what the gather stores (fft_phases.cuh GM_*).  aux: GM_KINETIC psi_in [nb][ng]; GM_PHASE per-G factors [ng].
+template <class C, int GM>
 __global__ void __launch_bounds__(QM_ZT * C::TT, 2)
 k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
-       const c128 *__restrict__ psi_in, c128 *__restrict__ out, int ntiles, int kinetic, int quarter)
+       const c128 *__restrict__ aux, c128 *__restrict__ out, int ntiles, double scale, int quarter)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int LP = C::L | 1;
@@ -95,6 +100,7 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
     TwRow<C::R2> twb;
     load_twrow(twb, tw, u2, C::R1);
     const size_t boff = (size_t)band * kp.ng;
+    const c128 *auxb = GM == GM_KINETIC ? aux + boff : aux;
     __syncthreads();
     const SLine lines_s = qm_sline(lines), stage_s = qm_sline(stage);
     for (int tile = blockIdx.x, it = 0; tile < ntiles; tile += gridDim.x, ++it) {
@@ -104,7 +110,7 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
         if (t1 < ns) q = kp.stick_info[tile * QM_ZT + t1];
         const Pruned pr = make_pruned<C>((int)(short)(q.x & 0xffff), q.x >> 16, (int)(short)(q.y & 0xffff), q.y >> 16, u1, 1);
         c128 kin[NPRE];
-        if (quarter) prefetch_kin<C>(psi_in + boff + q.z, kp.g2 + q.z, pr, kinetic != 0 && t1 < ns, kin);
+        if (quarter) prefetch_kin<C, GM>(auxb + q.z, kp.g2 + q.z, pr, t1 < ns, kin);
         mbar_wait(wbar, (uint32_t)(it & 1));
         zfwd_step1_load<C>(stage_s + t2, QM_ZT, lines_s + t2 * LP, u2, twb);
         __syncthreads();                       // staging buffer consumed, lines complete
@@ -114,15 +120,15 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
             bulk_g2s(stage, Wb + (size_t)(tile + gridDim.x) * C::N * QM_ZT, TILE_BYTES, wbar);
         }
         if (t1 < ns) {
-            if (quarter) zfwd_step2_gather_pre<C>(lines_s + t1 * LP, out + boff + q.z, pr, u1, kin);
-            else zfwd_step2_gather<C>(lines_s + t1 * LP, out + boff + q.z, kinetic ? psi_in + boff + q.z : nullptr, kp.g2 + q.z,
-                                      pr, u1, kinetic != 0);
+            if (quarter) zfwd_step2_gather_pre<C, GM>(lines_s + t1 * LP, out + boff + q.z, pr, u1, kin, scale);
+            else zfwd_step2_gather<C, GM>(lines_s + t1 * LP, out + boff + q.z, auxb + q.z, kp.g2 + q.z, pr, u1, scale);
         }
         __syncthreads();
     }
 }
 
-// MODE 0 apply, 1 g2r (write natural-order box), 2 r2g (read natural-order box), 3 density (rho += w |psi(r)|^2)
+// MODE 0 apply, 1 g2r (write a transposed box), 2 r2g (read a transposed box, optionally times the conjugate of a second
+// one), 3 density (rho += w |psi(r)|^2), 4 apply with a complex field (split-operator middle factor); fft_phases.cuh
 //
 // One CTA per (band, z-plane).  The CTA is split into independent groups of G threads (G/TT teams of TT
 // threads, one team per line); a group walks its own rows / columns and only synchronises with itself
@@ -244,7 +250,8 @@ __device__ __forceinline__ void plane_y_phase(const PlaneCtx cx, c128 *__restric
 
 template <class C, int MODE>
 __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_iv, const double *__restrict__ vt,
-                                           c128 *__restrict__ box, int pl, double scale, int stagger_ns,
+                                           c128 *__restrict__ box, const c128 *__restrict__ box2, int npair2, int pl,
+                                           double scale, int stagger_ns,
                                            double *__restrict__ rhot, const TwRow<C::R1> &twa, const TwRow<C::R2> &twb)
 {
     constexpr int G = QM_GROUP, TPG = G / C::TT, RP = C::L | 1;
@@ -280,12 +287,18 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
             // scale = weight * occupation of this band; rhot = running density of this plane in the V layout
             if (ok) xcol_density<C>(myscr, u, rhot + ((size_t)p * C::N + col) * VLayout<C>::COL, scale);
         } else if (ok) {
+            // transposed boxes (fft_phases.cuh BoxT): column (p, col) of state `band`; with a second operand the plane
+            // index counts pairs: band = a * npair2 + b, first operand state a, second operand state b (MODE 2)
             c128 *bx = nullptr;
-            if constexpr (MODE != 0) {
-                const int y = (col / C::R2) + C::R1 * (col % C::R2);
-                bx = box + (size_t)band * C::N * C::N * n3 + (size_t)y * n3;     // + z added by the caller through `box`
+            const c128 *bx2 = nullptr;
+            const size_t coloff = ((size_t)p * C::N + col) * C::N, boxsz = (size_t)C::N * C::N * n3;
+            if constexpr (MODE == 1) bx = box + (size_t)band * boxsz + coloff;
+            if constexpr (MODE == 2) {
+                bx = box + (size_t)(npair2 > 0 ? band / npair2 : band) * boxsz + coloff;
+                if (npair2 > 0) bx2 = box2 + (size_t)(band % npair2) * boxsz + coloff;
             }
-            xcol_step2<C, MODE>(myscr, u, twb, vr, bx, (long)C::N * n3, scale);
+            if constexpr (MODE == 4) bx2 = box2 + coloff;
+            xcol_step2<C, MODE>(myscr, u, twb, vr, bx, bx2, scale);
         }
         if constexpr (MODE == 0) {   // prefetch V of this team's next column behind steps 3 and 1
             const int ncol = col + ngroups * TPG;
@@ -306,8 +319,9 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
 
 template <class C, int MODE>
 __global__ void __launch_bounds__(QM_PLANE_MAX_THREADS)
-k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ box, int ngroups, double scale,
-        int stagger_ns, int nplanes, int quarter, const double *__restrict__ occ, double *__restrict__ rhot)
+k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ box, const c128 *__restrict__ box2,
+        int npair2, int ngroups, double scale, int stagger_ns, int nplanes, int quarter, const double *__restrict__ occ,
+        double *__restrict__ rhot)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int G = QM_GROUP;
@@ -352,11 +366,9 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
         plane_y_phase<C, MODE>(cx, W, pl, prev, have_cur, twa, twb);
         if (!have_cur) break;
         __syncthreads();
-        const int p = pl % n3;
-        const int z = (p / gd.ax[2].r2) + gd.ax[2].r1 * (p % gd.ax[2].r2);
         double sc = scale;
         if constexpr (MODE == 3) sc = scale * occ[pl / n3];
-        plane_x_phase<C, MODE>(cx, kp.x_iv, gd.vt, box ? box + z : nullptr, pl, sc, stagger_ns, rhot, twa, twb);
+        plane_x_phase<C, MODE>(cx, kp.x_iv, gd.vt, box, box2, npair2, pl, sc, stagger_ns, rhot, twa, twb);
         __syncthreads();
         prev = pl;
     }

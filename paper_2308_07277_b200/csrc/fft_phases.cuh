@@ -104,6 +104,18 @@ QM_HD void st_pred(const SLine &l, c128 v, bool pred) {
 #endif
 }
 
+// A sphere-side operand that is multiplied by a per-G phase as it is loaded (split-operator propagator,
+// PAPER.md:1137-1139 eq. 53: psi(G) exp(-i dt |k+G|^2 / 4) on the way into the backward transform).  Pointer-like, so
+// the pruned passes below take it in place of a plain pointer; `ph` is indexed like the first band of `a`.
+struct PhasedPtr {
+    const c128 *a, *ph;
+    QM_HD PhasedPtr operator+(int e) const { return PhasedPtr{a + e, ph + e}; }
+};
+QM_HD c128 ld_pred(const PhasedPtr &p, bool pred) {
+    const c128 x = ld_pred(p.a, pred), w = ld_pred(p.ph, pred);
+    return cmul(x, w);
+}
+
 // ---- pruned passes with hoisted addressing ---------------------------------------------------------
 // A thread with fixed u touches the line elements i = n*R2 + u (n = 0..R1-1).  When only two index
 // intervals [a1,b1], [a2,b2] of the line exist (stored back to back with element stride `stride`), the
@@ -272,10 +284,32 @@ template <class C, class L, class TW> QM_HD void zfwd_step1_load(const L stageco
         line[u * C::R2P + d] = (d == 0) ? t[d] : cmul(t[d], tw.template get<d>());
     });
 }
-// zfwd pass 2: finishes the forward transform and gathers to the sphere with the kinetic term fused
-// (PAPER.md:668-674): out[g] = (V psi)(G) + 1/2 |k+G|^2 psi_in[g] for the G of this stick only.
-template <class C, class L> QM_HD void zfwd_step2_gather(const L line, c128 *out, const c128 *psi_in, const double *g2,
-                                                          const Pruned pr, int u, bool kinetic) {
+// zfwd pass 2: finishes the forward transform and gathers to the sphere.  What is stored for a G of this stick (GM):
+//   GM_PLAIN    out[g] = F(G)                                                   (debug r2g)
+//   GM_KINETIC  out[g] = F(G) + 1/2 |k+G|^2 psi_in[g]       kinetic term fused
+//   GM_PHASE    out[g] = F(G) * aux[g]                      split-operator half-step, PAPER.md:1137-1139 (eq. 53)
+//   GM_CONJ     out[g] = conj(F(G)) * scale                 GW matrix elements, PAPER.md:1319-1328 (eq. 56; A21)
+// The per-G operand is fetched ahead of the transform (`kin`: the term to add, or the factor to multiply by).
+enum { GM_PLAIN = 0, GM_KINETIC = 1, GM_PHASE = 2, GM_CONJ = 3 };
+template <int GM> QM_HD c128 gather_fetch(const c128 *aux, const double *g2, int off, bool pred) {
+    if constexpr (GM == GM_KINETIC) {
+        const c128 x = ld_pred(aux + off, pred);
+        const double h = pred ? 0.5 * g2[off] : 0.0;
+        return c128{h * x.x, h * x.y};
+    } else if constexpr (GM == GM_PHASE) {
+        return ld_pred(aux + off, pred);
+    } else {
+        return c128{0.0, 0.0};
+    }
+}
+template <int GM> QM_HD c128 gather_combine(c128 f, c128 kin, double scale) {
+    if constexpr (GM == GM_KINETIC) return f + kin;
+    else if constexpr (GM == GM_PHASE) return cmul(f, kin);
+    else if constexpr (GM == GM_CONJ) return c128{f.x * scale, -f.y * scale};
+    else return f;
+}
+template <class C, int GM, class L> QM_HD void zfwd_step2_gather(const L line, c128 *out, const c128 *aux, const double *g2,
+                                                                  const Pruned pr, int u, double scale) {
     if (u >= C::R2) return;
     c128 t[C::R1];
     static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = line[a * C::R2P + u]; });
@@ -284,30 +318,24 @@ template <class C, class L> QM_HD void zfwd_step2_gather(const L line, c128 *out
         constexpr int c = decltype(I)::value;
         const bool in2 = (pr.m2 >> c) & 1u, in1 = (pr.m1 >> c) & 1u;
         const int off = (in2 ? pr.c2 : pr.c1) + c * C::R2;
-        if (in1 || in2) {
-            c128 v = t[c];
-            if (kinetic) { const double h = 0.5 * g2[off]; const c128 x = psi_in[off]; v.x = fma(h, x.x, v.x); v.y = fma(h, x.y, v.y); }
-            out[off] = v;
-        }
+        if (in1 || in2) out[off] = gather_combine<GM>(t[c], gather_fetch<GM>(aux, g2, off, true), scale);
     });
 }
-// Quarter-rule forms of the gather (see Quarter): the 1/2|k+G|^2 psi_in terms of the <= 2Q outputs a thread can
-// own are fetched ahead of the transform (prefetch_kin) and added when the outputs are stored.
-template <class C> QM_HD void prefetch_kin(const c128 *psi_in, const double *g2, const Pruned pr, bool kinetic,
-                                            c128 (&kin)[2 * Quarter<C>::Q]) {
+// Quarter-rule forms of the gather (see Quarter): the per-G operands of the <= 2Q outputs a thread can own are
+// fetched ahead of the transform (prefetch_kin) and combined when the outputs are stored.
+template <class C, int GM> QM_HD void prefetch_kin(const c128 *aux, const double *g2, const Pruned pr, bool active,
+                                                    c128 (&kin)[2 * Quarter<C>::Q]) {
     constexpr int Q = Quarter<C>::Q;
     static_for<Q>([&](auto I) {
         constexpr int j = decltype(I)::value;
         const int o1 = pr.c1 + j * C::R2, o2 = pr.c2 + (C::R1 - Q + j) * C::R2;
-        const bool q1 = kinetic && ((pr.m1 >> j) & 1u), q2 = kinetic && ((pr.m2 >> (C::R1 - Q + j)) & 1u);
-        const c128 x1 = ld_pred(psi_in + o1, q1), x2 = ld_pred(psi_in + o2, q2);
-        const double h1 = q1 ? 0.5 * g2[o1] : 0.0, h2 = q2 ? 0.5 * g2[o2] : 0.0;
-        kin[j] = c128{h1 * x1.x, h1 * x1.y};
-        kin[Q + j] = c128{h2 * x2.x, h2 * x2.y};
+        const bool q1 = active && ((pr.m1 >> j) & 1u), q2 = active && ((pr.m2 >> (C::R1 - Q + j)) & 1u);
+        kin[j] = gather_fetch<GM>(aux, g2, o1, q1);
+        kin[Q + j] = gather_fetch<GM>(aux, g2, o2, q2);
     });
 }
-template <class C, class L> QM_HD void zfwd_step2_gather_pre(const L line, c128 *out, const Pruned pr, int u,
-                                                              const c128 (&kin)[2 * Quarter<C>::Q]) {
+template <class C, int GM, class L> QM_HD void zfwd_step2_gather_pre(const L line, c128 *out, const Pruned pr, int u,
+                                                                      const c128 (&kin)[2 * Quarter<C>::Q], double scale) {
     if (u >= C::R2) return;
     constexpr int Q = Quarter<C>::Q;
     c128 t[C::R1];
@@ -316,8 +344,8 @@ template <class C, class L> QM_HD void zfwd_step2_gather_pre(const L line, c128 
     static_for<Q>([&](auto I) {
         constexpr int j = decltype(I)::value;
         constexpr int c2 = C::R1 - Q + j;
-        st_pred(out + pr.c1 + j * C::R2, t[j] + kin[j], (pr.m1 >> j) & 1u);
-        st_pred(out + pr.c2 + c2 * C::R2, t[c2] + kin[Q + j], (pr.m2 >> c2) & 1u);
+        st_pred(out + pr.c1 + j * C::R2, gather_combine<GM>(t[j], kin[j], scale), (pr.m1 >> j) & 1u);
+        st_pred(out + pr.c2 + c2 * C::R2, gather_combine<GM>(t[c2], kin[Q + j], scale), (pr.m2 >> c2) & 1u);
     });
 }
 
@@ -326,10 +354,15 @@ template <class C, class L> QM_HD void zfwd_step2_gather_pre(const L line, c128 
 // [a2,b2] -> the following rows; everything else is not stored (zero).  Steps 1 and 3 of a column are
 // prunedA_step1 / prunedB_step2 on the plane array with stride = row pitch; step 2 works on the scratch line:
 // MODE 0: apply  (backward step 2, multiply by v[x], forward step 1)      PAPER.md:659-662 (eq. 47)
-// MODE 1: g2r    (backward step 2, write psi(r)*scale to box, stop)
-// MODE 2: r2g    (read box, forward step 1)
+// MODE 1: g2r    (backward step 2, write psi(r)*scale to the column of a transposed box, stop)
+// MODE 2: r2g    (read the column of a transposed box -- optionally times the conjugate of a second one: the pair
+//                 product phi_a(r) conj(phi_b(r)) of the GW matrix elements, PAPER.md:1319-1328 -- , forward step 1)
+// MODE 4: apply with a complex field (backward step 2, multiply by f[x], forward step 1): the middle factor
+//                 exp(-i dt V(r)) of the split-operator propagator, PAPER.md:1137-1139 (eq. 53)
 // v: this thread's R2 potential values V(x = u + R1*k2), already in registers (prefetched by the caller).
-// box: pointer to element x=0 of this column in a natural-order box, xstride = n2*n3.
+// Transposed box ("BoxT"): element (x, y, z) at [(p * N2 + col) * N1 + x], p / col = transposed z / y labels, x natural;
+// a thread's x = u + R1*k2 make the lanes of a team read contiguous 16-byte words.  box / box2 / the field point at
+// element x = 0 of this column.
 template <int R> struct VRow { double v[R]; };
 // V of one plane column is stored in pairs: vcol[(j * R1 + u) * 2 + e] = V(x = u + R1*(2j + e)), j < R2E/2
 // (R2E = R2 rounded up to even, the pad is zero), so a thread reads its R2 values with 16-byte loads and the
@@ -346,17 +379,22 @@ template <class C> QM_HD void load_vrow(VRow<C::R2> &vr, const double *vcol, int
     });
 }
 template <class C, int MODE, class L, class TW>
-QM_HD void xcol_step2(const L scr, int u, const TW &tw, const VRow<C::R2> &vr, c128 *box, long xstride, double scale) {
+QM_HD void xcol_step2(const L scr, int u, const TW &tw, const VRow<C::R2> &vr, c128 *box, const c128 *box2, double scale) {
     if (u >= C::R1) return;
     c128 t[C::R2];
     if constexpr (MODE == 2) {
-        static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; t[k2] = box[(long)(u + C::R1 * k2) * xstride]; });
+        static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; t[k2] = box[u + C::R1 * k2]; });
+        if (box2) static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; t[k2] = cmul_conj(t[k2], box2[u + C::R1 * k2]); });
     } else {
+        c128 f[MODE == 4 ? C::R2 : 1];
+        if constexpr (MODE == 4) static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; f[k2] = box2[u + C::R1 * k2]; });
         static_for<C::R2>([&](auto I) { constexpr int n2 = decltype(I)::value; t[n2] = scr[u * C::R2P + n2]; });
         Dft<C::R2, +1>::run(t);                      // t[k2] = psi(x = u + R1*k2)
         if constexpr (MODE == 1) {
-            static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; box[(long)(u + C::R1 * k2) * xstride] = cscale(t[k2], scale); });
+            static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; box[u + C::R1 * k2] = cscale(t[k2], scale); });
             return;
+        } else if constexpr (MODE == 4) {
+            static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; t[k2] = cmul(t[k2], f[k2]); });
         } else {
             static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; t[k2] = cscale(t[k2], vr.v[k2]); });
         }

@@ -57,8 +57,9 @@ struct QmKTables {
 };
 
 // returns 0, or -1 (sphere does not fit the grid) / -2 (empty sphere); msg gets the reason
+// strict: keep |k+G|^2 < ecut instead of <= (the epsilon sphere of the GW matrix elements, eq. 56)
 static inline int qm_build_tables(const double *lattice, const double *recip, double ecut, const int *grid,
-                                  const QmAxis *ax, QmKTables *kp, std::string *msg)
+                                  const QmAxis *ax, QmKTables *kp, std::string *msg, bool strict = false)
 {
     const double *b = recip, *a = lattice;
     const int n1 = grid[0], n2 = grid[1], n3 = grid[2];
@@ -78,7 +79,7 @@ static inline int qm_build_tables(const double *lattice, const double *recip, do
                 const double qy = f1 * b[1] + f2 * b[4] + f3 * b[7];
                 const double qz = f1 * b[2] + f2 * b[5] + f3 * b[8];
                 const double q2 = qx * qx + qy * qy + qz * qz;
-                if (q2 <= ecut) {
+                if (strict ? q2 < ecut : q2 <= ecut) {
                     Ent e; e.m[0] = m1; e.m[1] = m2; e.m[2] = m3; e.g2 = q2; e.idx = 0;
                     ents.push_back(e);
                     kp->mmax[0] = std::max(kp->mmax[0], std::abs(m1));

@@ -57,6 +57,12 @@ struct KPoint : QmKTables {
     int nmblk = 0, nkc = 0, ngt = 0, nic = 0;          // tile counts of the two beta copies
     DevBuf<c128> d_beta1, d_beta2;
     DevBuf<double> d_D;
+    // workspaces of this k-point (calls on different k-points may run on different streams)
+    DevBuf<c128> d_W, d_Ppart, d_P, d_part;
+    DevBuf<double> d_qt;
+    DevBuf<int> d_pdesc;
+    DevBuf<c128> d_sophase;                             // split-operator: exp(-i dt |k+G|^2 / 4)
+    double ecut_override = 0.0;                         // epsilon spheres (qm_mtxel) carry their own cut-off
     QmKPlanDev plan() const {
         QmKPlanDev p;
         p.ng = ng; p.nsticks = nsticks; p.nx = nx; p.rowpitch = rowpitch;
@@ -127,29 +133,63 @@ struct qm_gspace {
     DevBuf<double> d_vt, d_rhot;
     bool rho_open = false;
     bool v_set = false;
-    DevBuf<c128> d_W, d_Ppart, d_P;
-    DevBuf<double> d_qt;
-    DevBuf<c128> d_part, d_subpart, d_tay_h, d_tay_t;
-    DevBuf<int> d_pdesc;
+    DevBuf<c128> d_subpart, d_tay_h, d_tay_t;
+    DevBuf<c128> d_boxt;            // transposed boxes of the debug hooks
+    DevBuf<c128> d_sofield;         // split-operator: exp(-i dt V(r)) / N in the transposed-box layout
+    bool so_set = false;
+    double so_dt = 0.0;
     unsigned long long launches = 0;
+    int device = 0;                 // the CUDA device the handle was created on (every call checks it)
     int sm_count = 148;
     int max_smem = 0;
+    size_t l2_bytes = 0;
+    int fft_chunk = 0;              // bands per internal pass of the FFT path (0: derived from the L2 size; QM_FFT_CHUNK)
     int z_cta_per_sm = 2;           // resident z-kernel CTAs per SM the grid is sized for (QM_Z_CTA_PER_SM)
     int plane_stagger_ns = 0;       // de-phasing delay between the plane kernel's groups (QM_PLANE_STAGGER_NS)
     ~qm_gspace() { for (auto *k : kpts) delete k; }
 };
 
+// GW plane-wave matrix elements for one (k+q, k) pair of k-points: the epsilon sphere |q+G|^2 < ecut_eps on the
+// handle's FFT box, with its own stick tables, and the workspaces of qm_matrix_elements.
+struct qm_mtxel {
+    qm_gspace *g = nullptr;
+    int k_bra = 0, k_ket = 0;
+    KPoint sph;
+    DevBuf<c128> d_ketbox, d_brabox, d_Wp;
+};
+
+// A fixed list of qm_apply_h calls captured as one CUDA graph (qm_batch_plan_*).
+struct qm_batch_plan {
+    qm_gspace *g = nullptr;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    unsigned long long launches = 0;        // kernels per graph launch
+    ~qm_batch_plan() {
+        if (exec) cudaGraphExecDestroy(exec);
+        if (graph) cudaGraphDestroy(graph);
+    }
+};
+
 namespace {
 
-
-int build_kpoint(qm_gspace *g, KPoint *kp) {
+int build_kpoint(qm_gspace *g, KPoint *kp, bool strict = false) {
     std::string msg;
-    const int rc = qm_build_tables(g->lattice, g->recip, g->ecut, g->grid, g->ax, kp, &msg);
+    const int rc = qm_build_tables(g->lattice, g->recip, strict ? kp->ecut_override : g->ecut, g->grid, g->ax, kp, &msg, strict);
     if (rc == -1) return fail(QM_EGRID, msg);
     if (rc != 0) return fail(QM_EINVAL, msg);
     CU_TRY(kp->d_rowinfo.upload(kp->rowinfo));
     CU_TRY(kp->d_stickinfo.upload(kp->stickinfo));
     CU_TRY(kp->d_g2.upload(kp->g2));
+    return QM_OK;
+}
+
+// every entry point that touches the device: the handle belongs to one device, which must be current
+int check_device(const qm_gspace *g) {
+    int dev = -1;
+    CU_TRY(cudaGetDevice(&dev));
+    if (dev != g->device)
+        return fail(QM_EINVAL, "handle was created on CUDA device " + std::to_string(g->device) + ", current device is " +
+                                   std::to_string(dev));
     return QM_OK;
 }
 
@@ -162,7 +202,7 @@ size_t plane_smem(const qm_gspace *g, const KPoint *kp, int ngroups) {
     return (a_elems + (size_t)ngroups * tpg * sl) * sizeof(c128) + (size_t)kp->nx * sizeof(int4) + 16;
 }
 
-// number of independent 64-thread groups of the plane kernel: the fewest groups that reach the
+// number of independent groups of the plane kernel: the fewest groups that reach the
 // minimum number of column rounds within the shared-memory and thread limits
 int plane_groups(const qm_gspace *g, const KPoint *kp) {
     const QmAxis &ax = g->ax[0];
@@ -186,41 +226,43 @@ int z_grid_x(const qm_gspace *g, int ntiles, int nb, int cta_per_sm) {
     const int rounds = (ntiles + gx - 1) / gx;          // fewest CTAs that keep the same number of rounds
     return (ntiles + rounds - 1) / rounds;
 }
-template <class C> int launch_zinv(qm_gspace *g, KPoint *kp, const c128 *psi, int nb, cudaStream_t st) {
-    const size_t smem = qm_z_smem<C>();
-    static bool attr = false;
-    if (!attr) { CU_TRY(cudaFuncSetAttribute(k_zinv<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
+template <class C, bool PH> int launch_zinv(qm_gspace *g, KPoint *kp, const c128 *psi, const c128 *phase, c128 *W, int nb,
+                                            cudaStream_t st) {
     const int ntiles = (kp->nsticks + QM_ZT - 1) / QM_ZT;
     dim3 grid(z_grid_x(g, ntiles, nb, g->z_cta_per_sm), nb);
     g->prof.begin(QM_K_ZINV, st);
-    k_zinv<C><<<grid, QM_ZT * C::TT, smem, st>>>(kp->plan(), g->d_tw[2].p, psi, g->d_W.p, ntiles, kp->z_quarter ? 1 : 0);
+    k_zinv<C, PH><<<grid, QM_ZT * C::TT, qm_z_smem<C>(), st>>>(kp->plan(), g->d_tw[2].p, psi, phase, W, ntiles,
+                                                                kp->z_quarter ? 1 : 0);
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
     return QM_OK;
 }
-template <class C> int launch_zfwd(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb, int kinetic,
-                                   cudaStream_t st) {
-    const size_t smem = qm_z_smem<C>();
-    static bool attr = false;
-    if (!attr) { CU_TRY(cudaFuncSetAttribute(k_zfwd<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
+template <class C, int GM> int launch_zfwd(qm_gspace *g, KPoint *kp, const c128 *W, const c128 *aux, c128 *out, int nb,
+                                           double scale, cudaStream_t st) {
     const int ntiles = (kp->nsticks + QM_ZT - 1) / QM_ZT;
     dim3 grid(z_grid_x(g, ntiles, nb, g->z_cta_per_sm), nb);
     g->prof.begin(QM_K_ZFWD, st);
-    k_zfwd<C><<<grid, QM_ZT * C::TT, smem, st>>>(kp->plan(), g->d_tw[2].p, g->d_W.p, psi_in, out, ntiles, kinetic,
-                                                  kp->z_quarter ? 1 : 0);
+    k_zfwd<C, GM><<<grid, QM_ZT * C::TT, qm_z_smem<C>(), st>>>(kp->plan(), g->d_tw[2].p, W, aux, out, ntiles, scale,
+                                                                kp->z_quarter ? 1 : 0);
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
     return QM_OK;
 }
-template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *box, int nb, double scale,
-                                              cudaStream_t st, const double *occ = nullptr, double *rhot = nullptr) {
+struct PlaneArgs {          // operands of the plane kernel beyond the stick planes W
+    c128 *box = nullptr;            // MODE 1 output / MODE 2 first operand (transposed boxes, one per state)
+    const c128 *box2 = nullptr;     // MODE 2 second operand (conjugated) / MODE 4 complex field
+    int npair2 = 0;                 // MODE 2 with a second operand: states in box2 (plane index counts pairs a * npair2 + b)
+    double scale = 1.0;
+    const double *occ = nullptr;    // MODE 3
+    double *rhot = nullptr;
+};
+template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *W, int nb, const PlaneArgs &a, cudaStream_t st) {
     const int ngroups = plane_groups(g, kp);
     const size_t smem = plane_smem(g, kp, ngroups);
     if (smem > (size_t)g->max_smem)
         return fail(QM_EGRID, "plane kernel does not fit shared memory for this grid / sphere");
-    CU_TRY(cudaFuncSetAttribute(k_plane<C, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     QmGridDev gd;
     for (int i = 0; i < 3; ++i) { gd.ax[i] = g->ax[i]; gd.tw[i] = g->d_tw[i].p; }
     gd.vt = g->d_vt.p;
@@ -228,9 +270,9 @@ template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *bo
     // persistent: one CTA per SM walks the (band, z-plane) list; density mode: one CTA per z-plane, all bands
     const int grid = MODE == 3 ? std::min(g->grid[2], g->sm_count) : std::min(nplanes, g->sm_count);
     g->prof.begin(QM_K_PLANE, st);
-    k_plane<C, MODE><<<grid, ngroups * PLANE_GROUP, smem, st>>>(kp->plan(), gd, g->d_W.p, box, ngroups, scale,
+    k_plane<C, MODE><<<grid, ngroups * PLANE_GROUP, smem, st>>>(kp->plan(), gd, W, a.box, a.box2, a.npair2, ngroups, a.scale,
                                                                    g->plane_stagger_ns, nplanes,
-                                                                   (kp->y_quarter ? 1 : 0) | (kp->x_quarter ? 2 : 0), occ, rhot);
+                                                                   (kp->y_quarter ? 1 : 0) | (kp->x_quarter ? 2 : 0), a.occ, a.rhot);
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
@@ -247,30 +289,72 @@ template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *bo
     X(96, 8, 12) X(100, 10, 10) X(108, 9, 12) X(120, 10, 12) X(128, 8, 16) X(144, 12, 12)
 #endif
 
-int dispatch_zinv(qm_gspace *g, KPoint *kp, const c128 *psi, int nb, cudaStream_t st) {
+template <bool PH> int dispatch_zinv(qm_gspace *g, KPoint *kp, const c128 *psi, const c128 *phase, c128 *W, int nb,
+                                     cudaStream_t st) {
     switch (g->grid[2]) {
-#define X(N, A, B) case N: return launch_zinv<LineCfg<A, B>>(g, kp, psi, nb, st);
+#define X(N, A, B) case N: return launch_zinv<LineCfg<A, B>, PH>(g, kp, psi, phase, W, nb, st);
         QM_FOR_SIZES(X)
 #undef X
     }
     return fail(QM_EGRID, "unsupported FFT length (axis 3)");
 }
-int dispatch_zfwd(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb, int kinetic, cudaStream_t st) {
+template <int GM> int dispatch_zfwd(qm_gspace *g, KPoint *kp, const c128 *W, const c128 *aux, c128 *out, int nb, double scale,
+                                    cudaStream_t st) {
     switch (g->grid[2]) {
-#define X(N, A, B) case N: return launch_zfwd<LineCfg<A, B>>(g, kp, psi_in, out, nb, kinetic, st);
+#define X(N, A, B) case N: return launch_zfwd<LineCfg<A, B>, GM>(g, kp, W, aux, out, nb, scale, st);
         QM_FOR_SIZES(X)
 #undef X
     }
     return fail(QM_EGRID, "unsupported FFT length (axis 3)");
 }
-template <int MODE> int dispatch_plane(qm_gspace *g, KPoint *kp, c128 *box, int nb, double scale, cudaStream_t st,
-                                       const double *occ = nullptr, double *rhot = nullptr) {
+template <int MODE> int dispatch_plane(qm_gspace *g, KPoint *kp, c128 *W, int nb, const PlaneArgs &a, cudaStream_t st) {
     switch (g->grid[0]) {
-#define X(N, A, B) case N: return launch_plane<LineCfg<A, B>, MODE>(g, kp, box, nb, scale, st, occ, rhot);
+#define X(N, A, B) case N: return launch_plane<LineCfg<A, B>, MODE>(g, kp, W, nb, a, st);
         QM_FOR_SIZES(X)
 #undef X
     }
     return fail(QM_EGRID, "unsupported FFT length (axes 1,2)");
+}
+
+// Opt every kernel this handle can launch into its dynamic shared memory ONCE, at handle creation, on the handle's
+// device (function attributes are per device; nothing of this kind is left on the hot path).
+template <class C> int prep_z_kernels() {
+    const int smem = (int)qm_z_smem<C>();
+    CU_TRY(cudaFuncSetAttribute(k_zinv<C, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    CU_TRY(cudaFuncSetAttribute(k_zinv<C, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    CU_TRY(cudaFuncSetAttribute(k_zfwd<C, GM_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    CU_TRY(cudaFuncSetAttribute(k_zfwd<C, GM_KINETIC>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    CU_TRY(cudaFuncSetAttribute(k_zfwd<C, GM_PHASE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    CU_TRY(cudaFuncSetAttribute(k_zfwd<C, GM_CONJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    return QM_OK;
+}
+template <class C> int prep_plane_kernels(int max_smem) {
+    CU_TRY(cudaFuncSetAttribute(k_plane<C, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+    CU_TRY(cudaFuncSetAttribute(k_plane<C, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+    CU_TRY(cudaFuncSetAttribute(k_plane<C, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+    CU_TRY(cudaFuncSetAttribute(k_plane<C, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+    CU_TRY(cudaFuncSetAttribute(k_plane<C, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+    return QM_OK;
+}
+int prepare_kernels(qm_gspace *g) {
+    int rc = QM_EGRID;
+    switch (g->grid[2]) {
+#define X(N, A, B) case N: rc = prep_z_kernels<LineCfg<A, B>>(); break;
+        QM_FOR_SIZES(X)
+#undef X
+    }
+    if (rc) return rc;
+    rc = QM_EGRID;
+    switch (g->grid[0]) {
+#define X(N, A, B) case N: rc = prep_plane_kernels<LineCfg<A, B>>(g->max_smem); break;
+        QM_FOR_SIZES(X)
+#undef X
+    }
+    if (rc) return rc;
+    CU_TRY(cudaFuncSetAttribute(k_proj1_pipe, cudaFuncAttributeMaxDynamicSharedMemorySize, P1_SMEM));
+    CU_TRY(cudaFuncSetAttribute(k_proj2_sk, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM));
+    CU_TRY(cudaFuncSetAttribute(k_sub_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, SG_SMEM));
+    return QM_OK;
 }
 
 // rho[x][y][z] = scale * rhot[p][col][j][u][e]   (inverse of k_relayout_v's index map; fft_phases.cuh VLayout)
@@ -310,66 +394,147 @@ __global__ void k_relayout_v(const double *__restrict__ v, double *__restrict__ 
     }
 }
 
+// Transposed box <-> natural C-order box (fft_phases.cuh BoxT): boxt[b][(p * n2 + col) * n1 + x] <-> box[b][(x * n2 + y) * n3 + z],
+// p / col the transposed labels of z / y.  TO_T: natural -> transposed, else transposed -> natural.  nb boxes.
+template <bool TO_T>
+__global__ void k_box_relayout(const c128 *__restrict__ src, c128 *__restrict__ dst, QmAxis a1, QmAxis a2, QmAxis a3, int nb)
+{
+    const size_t boxsz = (size_t)a1.n * a2.n * a3.n, total = boxsz * nb;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t b = i / boxsz, e = i % boxsz;                 // e indexes the transposed box
+        const int x = (int)(e % a1.n), col = (int)((e / a1.n) % a2.n), p = (int)(e / ((size_t)a1.n * a2.n));
+        const int y = (col / a2.r2) + a2.r1 * (col % a2.r2);
+        const int z = (p / a3.r2) + a3.r1 * (p % a3.r2);
+        const size_t nat = b * boxsz + ((size_t)x * a2.n + y) * a3.n + z;
+        if (TO_T) dst[i] = src[nat]; else dst[nat] = src[i];
+    }
+}
+
+// split-operator tables (eq. 53; reading A22)
+//   field[(p * n2 + col) * n1 + x] = exp(-i dt V(x, y, z)) / N      (transposed-box layout; 1/N of the FFT pair folded in)
+//   phase[g] = exp(-i dt |k+G|^2 / 4)                               (exp(-i (dt/2) T), T = 1/2 |k+G|^2)
+__global__ void k_so_field(const double *__restrict__ v, c128 *__restrict__ field, QmAxis a1, QmAxis a2, QmAxis a3, double dt)
+{
+    const size_t boxsz = (size_t)a1.n * a2.n * a3.n;
+    const double inv = 1.0 / (double)boxsz;
+    for (size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x; e < boxsz; e += (size_t)gridDim.x * blockDim.x) {
+        const int x = (int)(e % a1.n), col = (int)((e / a1.n) % a2.n), p = (int)(e / ((size_t)a1.n * a2.n));
+        const int y = (col / a2.r2) + a2.r1 * (col % a2.r2);
+        const int z = (p / a3.r2) + a3.r1 * (p % a3.r2);
+        double sn, cs;
+        sincos(-dt * v[((size_t)x * a2.n + y) * a3.n + z], &sn, &cs);
+        field[e] = c128{cs * inv, sn * inv};
+    }
+}
+__global__ void k_so_phase(const double *__restrict__ g2, c128 *__restrict__ phase, int ng, double dt)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= ng) return;
+    double sn, cs;
+    sincos(-dt * (0.5 * g2[i]) / 2.0, &sn, &cs);
+    phase[i] = c128{cs, sn};
+}
+
 int check_handle(const qm_gspace *g, int k) {
     if (!g) return fail(QM_EINVAL, "null handle");
     if (k < 0 || k >= (int)g->kpts.size()) return fail(QM_EINVAL, "k-point index out of range");
-    return QM_OK;
+    return check_device(g);
 }
 
-int ensure_workspace(qm_gspace *g, const KPoint *kp, int nb) {
-    const size_t ntiles = ((size_t)kp->nsticks + QM_ZT - 1) / QM_ZT;      // W is blocked by stick tile (WView)
-    CU_TRY(g->d_W.resize((size_t)nb * ntiles * QM_ZT * g->grid[2]));
+size_t w_elems_per_band(const qm_gspace *g, const KPoint *kp) {        // W is blocked by stick tile (WView)
+    return ((size_t)kp->nsticks + QM_ZT - 1) / QM_ZT * QM_ZT * g->grid[2];
+}
+// bands per internal pass of the FFT path: the stick planes of one pass stay inside the L2 cache, so that what
+// k_zinv writes is still there when the plane kernel and k_zfwd read it
+int fft_chunk_bands(const qm_gspace *g, const KPoint *kp) {
+    if (g->fft_chunk > 0) return g->fft_chunk;
+    const size_t per_band = w_elems_per_band(g, kp) * sizeof(c128);
+    const size_t budget = g->l2_bytes ? g->l2_bytes / 4 * 3 : (size_t)64 << 20;
+    return (int)std::min<size_t>(64, std::max<size_t>(16, budget / std::max<size_t>(per_band, 1)));
+}
+int ensure_workspace(qm_gspace *g, KPoint *kp, int nb) {
+    CU_TRY(kp->d_W.resize((size_t)std::min(nb, fft_chunk_bands(g, kp)) * w_elems_per_band(g, kp)));
+    return QM_OK;
+}
+struct NlPlan { int nsplit, nrows_pad, ncta2; size_t pcount; };
+NlPlan nl_plan(const qm_gspace *g, const KPoint *kp) {
+    NlPlan p;
+    p.nsplit = std::max(1, std::min(kp->nkc, g->sm_count * P1_OCC / std::max(1, kp->nmblk)));
+    p.nrows_pad = kp->nmblk * P1_ROWS;
+    p.pcount = (size_t)p.nrows_pad * P_NB;
+    p.ncta2 = (int)std::min<long long>((long long)kp->ngt * kp->nic, 2LL * g->sm_count);
+    return p;
+}
+int ensure_nonlocal_workspace(qm_gspace *g, KPoint *kp) {
+    if (kp->nproj == 0) return QM_OK;
+    const NlPlan p = nl_plan(g, kp);
+    CU_TRY(kp->d_Ppart.resize(p.pcount * p.nsplit));
+    CU_TRY(kp->d_P.resize(p.pcount));
+    CU_TRY(kp->d_qt.resize((size_t)kp->nic * P2_Q_DOUBLES));
+    CU_TRY(kp->d_part.resize((size_t)2 * p.ncta2 * P2_PART));
+    CU_TRY(kp->d_pdesc.resize((size_t)2 * p.ncta2));
     return QM_OK;
 }
 
 int run_nonlocal(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb, cudaStream_t st) {
     if (kp->nproj == 0) return QM_OK;
-    static bool attr = false;
-    if (!attr) {
-        CU_TRY(cudaFuncSetAttribute(k_proj1_pipe, cudaFuncAttributeMaxDynamicSharedMemorySize, P1_SMEM));
-        CU_TRY(cudaFuncSetAttribute(k_proj2_sk, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM));
-        attr = true;
-    }
-    const int nsplit = std::max(1, std::min(kp->nkc, g->sm_count * P1_OCC / kp->nmblk));
-    const int nrows_pad = kp->nmblk * P1_ROWS;
-    const size_t pcount = (size_t)nrows_pad * P_NB;
-    CU_TRY(g->d_Ppart.resize(pcount * nsplit));
-    CU_TRY(g->d_P.resize(pcount));
-    CU_TRY(g->d_qt.resize((size_t)kp->nic * P2_Q_DOUBLES));
-    const long long stages2 = (long long)kp->ngt * kp->nic;
-    const int ncta2 = (int)std::min<long long>(stages2, 2LL * g->sm_count);
-    CU_TRY(g->d_part.resize((size_t)2 * ncta2 * P2_PART));
-    CU_TRY(g->d_pdesc.resize((size_t)2 * ncta2));
+    const NlPlan p = nl_plan(g, kp);
+    const int nsplit = p.nsplit, nrows_pad = p.nrows_pad, ncta2 = p.ncta2;
+    const size_t pcount = p.pcount;
     for (int band0 = 0; band0 < nb; band0 += P_NB) {
         g->prof.begin(QM_K_PROJ1, st);
         k_proj1_pipe<<<dim3(kp->nmblk, nsplit), (P1_CW + 1) * 32, P1_SMEM, st>>>(
-            kp->d_beta1.p, kp->nkc, psi_in, kp->ng, nb, band0, g->d_Ppart.p, nrows_pad, nsplit);
+            kp->d_beta1.p, kp->nkc, psi_in, kp->ng, nb, band0, kp->d_Ppart.p, nrows_pad, nsplit);
         g->prof.end(st);
         const int qcount = kp->nic * P2_KS * P_NB;
         if (16 % kp->dblock == 0 && kp->nic * P2_KS <= nrows_pad) {
             g->prof.begin(QM_K_PREDUCE, st);      // fused split-K reduction + D multiply
-            k_reduce_dmul<<<(kp->nic * P2_KS) / 16, 256, 0, st>>>(g->d_Ppart.p, nsplit, nrows_pad, kp->d_D.p, kp->dblock,
-                                                                   kp->nproj, g->d_qt.p);
+            k_reduce_dmul<<<(kp->nic * P2_KS) / 16, 256, 0, st>>>(kp->d_Ppart.p, nsplit, nrows_pad, kp->d_D.p, kp->dblock,
+                                                                   kp->nproj, kp->d_qt.p);
             g->prof.end(st);
             g->launches += 1;
         } else {
             g->prof.begin(QM_K_PREDUCE, st);
-            k_reduce_p2<<<(unsigned)((pcount + 255) / 256), 256, 0, st>>>(g->d_Ppart.p, nsplit, (int)pcount, g->d_P.p);
+            k_reduce_p2<<<(unsigned)((pcount + 255) / 256), 256, 0, st>>>(kp->d_Ppart.p, nsplit, (int)pcount, kp->d_P.p);
             g->prof.end(st);
             g->prof.begin(QM_K_DMUL, st);
-            k_dmul_tiles<<<(qcount + 255) / 256, 256, 0, st>>>(kp->d_D.p, kp->dblock, kp->nproj, kp->nic, g->d_P.p,
-                                                              g->d_qt.p);
+            k_dmul_tiles<<<(qcount + 255) / 256, 256, 0, st>>>(kp->d_D.p, kp->dblock, kp->nproj, kp->nic, kp->d_P.p,
+                                                              kp->d_qt.p);
             g->prof.end(st);
             g->launches += 2;
         }
         g->prof.begin(QM_K_PROJ2, st);
-        k_proj2_sk<<<ncta2, (P2_CW + 1) * 32, P2_SMEM, st>>>(kp->d_beta2.p, kp->nic, kp->ngt, g->d_qt.p, kp->ng, nb,
-                                                             band0, out, g->d_part.p, g->d_pdesc.p);
-        k_proj2_fixup<<<2 * ncta2, 256, 0, st>>>(g->d_part.p, g->d_pdesc.p, 2 * ncta2, kp->ng, nb, band0, out);
+        k_proj2_sk<<<ncta2, (P2_CW + 1) * 32, P2_SMEM, st>>>(kp->d_beta2.p, kp->nic, kp->ngt, kp->d_qt.p, kp->ng, nb,
+                                                             band0, out, kp->d_part.p, kp->d_pdesc.p);
+        k_proj2_fixup<<<2 * ncta2, 256, 0, st>>>(kp->d_part.p, kp->d_pdesc.p, 2 * ncta2, kp->ng, nb, band0, out);
         g->prof.end(st);
         g->launches += 3;
     }
     CU_TRY(cudaGetLastError());
+    return QM_OK;
+}
+
+// the local part of the path for nb bands, in passes of fft_chunk_bands (stick planes stay L2 resident)
+//   kind 0: H apply (V real, kinetic gather)   kind 1: split-operator step (phases + complex field)
+int run_local(qm_gspace *g, KPoint *kp, const c128 *in, c128 *out, int nb, int kind, cudaStream_t st) {
+    const int chunk = fft_chunk_bands(g, kp);
+    for (int b0 = 0; b0 < nb; b0 += chunk) {
+        const int n = std::min(chunk, nb - b0);
+        const c128 *pin = in + (size_t)b0 * kp->ng;
+        c128 *pout = out + (size_t)b0 * kp->ng;
+        int rc;
+        PlaneArgs a;
+        if (kind == 0) {
+            rc = dispatch_zinv<false>(g, kp, pin, nullptr, kp->d_W.p, n, st); if (rc) return rc;
+            rc = dispatch_plane<0>(g, kp, kp->d_W.p, n, a, st); if (rc) return rc;
+            rc = dispatch_zfwd<GM_KINETIC>(g, kp, kp->d_W.p, pin, pout, n, 1.0, st); if (rc) return rc;
+        } else {
+            a.box2 = g->d_sofield.p;
+            rc = dispatch_zinv<true>(g, kp, pin, kp->d_sophase.p, kp->d_W.p, n, st); if (rc) return rc;
+            rc = dispatch_plane<4>(g, kp, kp->d_W.p, n, a, st); if (rc) return rc;
+            rc = dispatch_zfwd<GM_PHASE>(g, kp, kp->d_W.p, kp->d_sophase.p, pout, n, 1.0, st); if (rc) return rc;
+        }
+    }
     return QM_OK;
 }
 
@@ -378,7 +543,7 @@ int run_nonlocal(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb
 extern "C" {
 
 QM_API const char *qm_last_error(void) { return g_err.c_str(); }
-QM_API const char *qm_version(void) { return "qm_hpsi 0.1 (sm_100a)"; }
+QM_API const char *qm_version(void) { return "qm_hpsi 0.2 (sm_100a)"; }
 
 QM_API int qm_fft_size_supported(int n) { return qm_find_size(n) ? 1 : 0; }
 
@@ -404,11 +569,17 @@ QM_API int qm_gspace_create(const double *lattice_bohr, double ecutwfc_ry, const
     int rc = QM_OK;
     auto bail = [&](int code) { delete g; return code; };
     {
+        int l2 = 0;
         cudaError_t e = cudaGetDevice(&dev);
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&g->sm_count, cudaDevAttrMultiProcessorCount, dev);
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&g->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev);
         if (e != cudaSuccess) { fail(QM_ECUDA, cudaGetErrorString(e)); return bail(QM_ECUDA); }
+        g->device = dev;
+        g->l2_bytes = (size_t)std::max(l2, 0);
     }
+    rc = prepare_kernels(g);
+    if (rc != QM_OK) return bail(rc);
     for (int a = 0; a < 3; ++a) {
         const int n = g->grid[a];
         std::vector<c128> tw(n);
@@ -440,6 +611,7 @@ QM_API int qm_gspace_create(const double *lattice_bohr, double ecutwfc_ry, const
     }
     if (const char *e = getenv("QM_PLANE_STAGGER_NS")) g->plane_stagger_ns = atoi(e);
     if (const char *e = getenv("QM_Z_CTA_PER_SM")) g->z_cta_per_sm = std::max(1, atoi(e));
+    if (const char *e = getenv("QM_FFT_CHUNK")) g->fft_chunk = std::max(0, atoi(e));
     *out = g;
     return QM_OK;
 }
@@ -450,34 +622,39 @@ QM_API int qm_gspace_num_k(const qm_gspace *g, int *nk) {
     if (!g || !nk) return fail(QM_EINVAL, "null argument");
     *nk = (int)g->kpts.size(); return QM_OK;
 }
+static int check_k(const qm_gspace *g, int k) {
+    if (!g) return fail(QM_EINVAL, "null handle");
+    if (k < 0 || k >= (int)g->kpts.size()) return fail(QM_EINVAL, "k-point index out of range");
+    return QM_OK;
+}
 QM_API int qm_gspace_num_g(const qm_gspace *g, int k, int *ng) {
-    int rc = check_handle(g, k); if (rc) return rc;
+    int rc = check_k(g, k); if (rc) return rc;
     if (!ng) return fail(QM_EINVAL, "null argument");
     *ng = g->kpts[k]->ng; return QM_OK;
 }
 QM_API int qm_gspace_num_sticks(const qm_gspace *g, int k, int *nsticks, int *nxcols) {
-    int rc = check_handle(g, k); if (rc) return rc;
+    int rc = check_k(g, k); if (rc) return rc;
     if (nsticks) *nsticks = g->kpts[k]->nsticks;
     if (nxcols) *nxcols = g->kpts[k]->nx;
     return QM_OK;
 }
 QM_API int qm_gspace_get_index_map(const qm_gspace *g, int k, int32_t *idx_host) {
-    int rc = check_handle(g, k); if (rc) return rc;
+    int rc = check_k(g, k); if (rc) return rc;
     if (!idx_host) return fail(QM_EINVAL, "null argument");
     std::memcpy(idx_host, g->kpts[k]->idx.data(), g->kpts[k]->idx.size() * sizeof(int32_t)); return QM_OK;
 }
 QM_API int qm_gspace_get_miller(const qm_gspace *g, int k, int32_t *m_host) {
-    int rc = check_handle(g, k); if (rc) return rc;
+    int rc = check_k(g, k); if (rc) return rc;
     if (!m_host) return fail(QM_EINVAL, "null argument");
     std::memcpy(m_host, g->kpts[k]->miller.data(), g->kpts[k]->miller.size() * sizeof(int32_t)); return QM_OK;
 }
 QM_API int qm_gspace_get_g2(const qm_gspace *g, int k, double *g2_host) {
-    int rc = check_handle(g, k); if (rc) return rc;
+    int rc = check_k(g, k); if (rc) return rc;
     if (!g2_host) return fail(QM_EINVAL, "null argument");
     std::memcpy(g2_host, g->kpts[k]->g2.data(), g->kpts[k]->g2.size() * sizeof(double)); return QM_OK;
 }
 QM_API int qm_gspace_alias_free(const qm_gspace *g, int k, int *flag) {
-    int rc = check_handle(g, k); if (rc) return rc;
+    int rc = check_k(g, k); if (rc) return rc;
     if (!flag) return fail(QM_EINVAL, "null argument");
     *flag = 1;
     for (int i = 0; i < 3; ++i) if (4 * g->kpts[k]->mmax[i] + 1 > g->grid[i]) *flag = 0;
@@ -486,6 +663,7 @@ QM_API int qm_gspace_alias_free(const qm_gspace *g, int k, int *flag) {
 
 QM_API int qm_set_vloc(qm_gspace *g, const double *V_r_dev, void *stream) {
     if (!g || !V_r_dev) return fail(QM_EINVAL, "qm_set_vloc: null argument");
+    int rc = check_device(g); if (rc) return rc;
     const size_t n = (size_t)g->grid[0] * g->grid[1] * g->grid[2];
     const size_t r2e = (size_t)g->ax[0].r2 + (g->ax[0].r2 & 1);
     CU_TRY(g->d_vt.resize((size_t)g->grid[2] * g->grid[1] * g->ax[0].r1 * r2e));
@@ -520,7 +698,15 @@ QM_API int qm_set_nonlocal(qm_gspace *g, int k, const qm_c128 *beta_kG_dev, int 
     CU_TRY(cudaMemcpyAsync(kp->d_D.p, D_dev, dcount * sizeof(double), cudaMemcpyDeviceToDevice, st));
     kp->nproj = nproj; kp->dblock = d_block; kp->nl_set = true;
     kp->nmblk = nmblk; kp->nkc = nkc; kp->ngt = ngt; kp->nic = nic;
-    return QM_OK;
+    return ensure_nonlocal_workspace(g, kp);        // projector workspaces do not depend on nbands: sized here, once
+}
+
+QM_API int qm_reserve(qm_gspace *g, int k, int nbands) {
+    int rc = check_handle(g, k); if (rc) return rc;
+    if (nbands <= 0) return fail(QM_EINVAL, "qm_reserve: nbands <= 0");
+    KPoint *kp = g->kpts[k];
+    rc = ensure_workspace(g, kp, nbands); if (rc) return rc;
+    return ensure_nonlocal_workspace(g, kp);
 }
 
 QM_API int qm_apply_h(qm_gspace *g, const qm_c128 *psi_in_dev, qm_c128 *psi_out_dev, int nbands, int k, void *stream) {
@@ -536,11 +722,188 @@ QM_API int qm_apply_h(qm_gspace *g, const qm_c128 *psi_in_dev, qm_c128 *psi_out_
     if (a < b + bytes && b < a + bytes) return fail(QM_EINVAL, "qm_apply_h: psi_in and psi_out overlap");
     cudaStream_t st = (cudaStream_t)stream;
     rc = ensure_workspace(g, kp, nbands); if (rc) return rc;
-    rc = dispatch_zinv(g, kp, in, nbands, st); if (rc) return rc;
-    rc = dispatch_plane<0>(g, kp, nullptr, nbands, 1.0, st); if (rc) return rc;
-    rc = dispatch_zfwd(g, kp, in, out, nbands, 1, st); if (rc) return rc;
+    rc = run_local(g, kp, in, out, nbands, 0, st); if (rc) return rc;
     return run_nonlocal(g, kp, in, out, nbands, st);
 }
+
+QM_API int qm_split_operator_set(qm_gspace *g, const double *V_r_dev, double dt, void *stream) {
+    if (!g || !V_r_dev) return fail(QM_EINVAL, "qm_split_operator_set: null argument");
+    int rc = check_device(g); if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n = (size_t)g->grid[0] * g->grid[1] * g->grid[2];
+    CU_TRY(g->d_sofield.resize(n));
+    k_so_field<<<g->sm_count * 4, 256, 0, st>>>(V_r_dev, g->d_sofield.p, g->ax[0], g->ax[1], g->ax[2], dt);
+    g->launches++;
+    for (KPoint *kp : g->kpts) {
+        CU_TRY(kp->d_sophase.resize((size_t)kp->ng));
+        k_so_phase<<<(kp->ng + 255) / 256, 256, 0, st>>>(kp->d_g2.p, kp->d_sophase.p, kp->ng, dt);
+        g->launches++;
+    }
+    CU_TRY(cudaGetLastError());
+    g->so_set = true; g->so_dt = dt;
+    return QM_OK;
+}
+
+QM_API int qm_split_operator_propagate(qm_gspace *g, int k, const qm_c128 *psi_in_dev, qm_c128 *psi_out_dev, int nbands,
+                                       void *stream) {
+    int rc = check_handle(g, k); if (rc) return rc;
+    if (!psi_in_dev || !psi_out_dev || nbands <= 0) return fail(QM_EINVAL, "qm_split_operator_propagate: bad argument");
+    if (!g->so_set) return fail(QM_ENOTSET, "qm_split_operator_propagate before qm_split_operator_set");
+    KPoint *kp = g->kpts[k];
+    const c128 *in = reinterpret_cast<const c128 *>(psi_in_dev);
+    c128 *out = reinterpret_cast<c128 *>(psi_out_dev);
+    const size_t bytes = (size_t)nbands * kp->ng * sizeof(c128);
+    const char *a = (const char *)in, *b = (const char *)out;
+    if (a < b + bytes && b < a + bytes) return fail(QM_EINVAL, "qm_split_operator_propagate: psi_in and psi_out overlap");
+    rc = ensure_workspace(g, kp, nbands); if (rc) return rc;
+    return run_local(g, kp, in, out, nbands, 1, (cudaStream_t)stream);
+}
+
+QM_API int qm_mtxel_create(qm_gspace *g, int k_bra, int k_ket, double ecut_eps_ry, qm_mtxel **out) {
+    int rc = check_handle(g, k_bra); if (rc) return rc;
+    rc = check_handle(g, k_ket); if (rc) return rc;
+    if (!out || !(ecut_eps_ry > 0.0)) return fail(QM_EINVAL, "qm_mtxel_create: bad argument");
+    *out = nullptr;
+    qm_mtxel *m = new (std::nothrow) qm_mtxel();
+    if (!m) return fail(QM_ENOMEM, "host allocation failed");
+    m->g = g; m->k_bra = k_bra; m->k_ket = k_ket;
+    for (int i = 0; i < 3; ++i) m->sph.k[i] = g->kpts[k_bra]->k[i] - g->kpts[k_ket]->k[i];      // q = (k+q) - k
+    m->sph.ecut_override = ecut_eps_ry;
+    rc = build_kpoint(g, &m->sph, true);
+    if (rc == QM_OK && plane_smem(g, &m->sph, 1) > (size_t)g->max_smem)
+        rc = fail(QM_EGRID, "plane working set of the epsilon sphere exceeds shared memory");
+    if (rc != QM_OK) { delete m; return rc; }
+    *out = m;
+    return QM_OK;
+}
+QM_API int qm_mtxel_destroy(qm_mtxel *m) { delete m; return QM_OK; }
+QM_API int qm_mtxel_num_g(const qm_mtxel *m, int *ng) {
+    if (!m || !ng) return fail(QM_EINVAL, "null argument");
+    *ng = m->sph.ng; return QM_OK;
+}
+QM_API int qm_mtxel_get_miller(const qm_mtxel *m, int32_t *miller_host) {
+    if (!m || !miller_host) return fail(QM_EINVAL, "null argument");
+    std::memcpy(miller_host, m->sph.miller.data(), m->sph.miller.size() * sizeof(int32_t)); return QM_OK;
+}
+QM_API int qm_mtxel_get_index_map(const qm_mtxel *m, int32_t *idx_host) {
+    if (!m || !idx_host) return fail(QM_EINVAL, "null argument");
+    std::memcpy(idx_host, m->sph.idx.data(), m->sph.idx.size() * sizeof(int32_t)); return QM_OK;
+}
+
+// scatter + backward FFT of `n` states of k-point kp into transposed boxes (unnormalised synthesis, reading A5/A20)
+static int synth_boxes(qm_gspace *g, KPoint *kp, const c128 *psi, int n, c128 *boxes, cudaStream_t st) {
+    const size_t boxsz = (size_t)g->grid[0] * g->grid[1] * g->grid[2];
+    int rc = ensure_workspace(g, kp, n); if (rc) return rc;
+    const int chunk = fft_chunk_bands(g, kp);
+    for (int b0 = 0; b0 < n; b0 += chunk) {
+        const int c = std::min(chunk, n - b0);
+        rc = dispatch_zinv<false>(g, kp, psi + (size_t)b0 * kp->ng, nullptr, kp->d_W.p, c, st); if (rc) return rc;
+        PlaneArgs a; a.box = boxes + (size_t)b0 * boxsz; a.scale = 1.0;
+        rc = dispatch_plane<1>(g, kp, kp->d_W.p, c, a, st); if (rc) return rc;
+    }
+    return QM_OK;
+}
+
+QM_API int qm_matrix_elements(qm_mtxel *m, const qm_c128 *bra_dev, int nbra, const qm_c128 *ket_dev, int nket,
+                              qm_c128 *out_dev, void *stream) {
+    if (!m || !bra_dev || !ket_dev || !out_dev || nbra <= 0 || nket <= 0) return fail(QM_EINVAL, "qm_matrix_elements: bad argument");
+    qm_gspace *g = m->g;
+    int rc = check_device(g); if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    KPoint *kb = g->kpts[m->k_bra], *kk = g->kpts[m->k_ket];
+    const size_t boxsz = (size_t)g->grid[0] * g->grid[1] * g->grid[2];
+    const size_t wpair = w_elems_per_band(g, &m->sph);
+    // bras per pass: the stick planes of (bras x nket) pairs within ~512 MB
+    const size_t cap = ((size_t)512 << 20) / sizeof(c128);
+    const int bpass = (int)std::max<size_t>(1, std::min<size_t>((size_t)nbra, cap / std::max<size_t>(1, wpair * nket)));
+    CU_TRY(m->d_ketbox.resize(boxsz * nket));
+    CU_TRY(m->d_brabox.resize(boxsz * bpass));
+    CU_TRY(m->d_Wp.resize(wpair * bpass * nket));
+    rc = synth_boxes(g, kk, reinterpret_cast<const c128 *>(ket_dev), nket, m->d_ketbox.p, st); if (rc) return rc;
+    c128 *out = reinterpret_cast<c128 *>(out_dev);
+    for (int a0 = 0; a0 < nbra; a0 += bpass) {
+        const int na = std::min(bpass, nbra - a0);
+        rc = synth_boxes(g, kb, reinterpret_cast<const c128 *>(bra_dev) + (size_t)a0 * kb->ng, na, m->d_brabox.p, st);
+        if (rc) return rc;
+        // pair (a, b): forward transform of phi_a(r) conj(phi_b(r)) pruned to the epsilon sphere, then
+        // M_ab(G) = conj(F(G)) / N  = (1/N) sum_r conj(phi_a) phi_b exp(+i G.r)          (eq. 56, reading A21)
+        PlaneArgs pa; pa.box = m->d_brabox.p; pa.box2 = m->d_ketbox.p; pa.npair2 = nket;
+        rc = dispatch_plane<2>(g, &m->sph, m->d_Wp.p, na * nket, pa, st); if (rc) return rc;
+        rc = dispatch_zfwd<GM_CONJ>(g, &m->sph, m->d_Wp.p, nullptr, out + (size_t)a0 * nket * m->sph.ng, na * nket,
+                                    1.0 / (double)boxsz, st);
+        if (rc) return rc;
+    }
+    return QM_OK;
+}
+
+QM_API int qm_batch_plan_create(qm_gspace *g, int nitems, const int *k, const qm_c128 *const *psi_in_dev,
+                                qm_c128 *const *psi_out_dev, const int *nbands, qm_batch_plan **out) {
+    if (!g || !k || !psi_in_dev || !psi_out_dev || !nbands || !out || nitems <= 0)
+        return fail(QM_EINVAL, "qm_batch_plan_create: bad argument");
+    *out = nullptr;
+    int rc = check_device(g); if (rc) return rc;
+    if (g->prof.on) return fail(QM_EINVAL, "qm_batch_plan_create: switch the per-kernel profiler off first");
+    for (int i = 0; i < nitems; ++i) {              // nothing may allocate while the graph is being captured
+        rc = check_handle(g, k[i]); if (rc) return rc;
+        if (nbands[i] <= 0 || !psi_in_dev[i] || !psi_out_dev[i]) return fail(QM_EINVAL, "qm_batch_plan_create: bad item");
+        rc = qm_reserve(g, k[i], nbands[i]); if (rc) return rc;
+    }
+    constexpr int MAXB = 16;
+    const int nbranch = std::min<int>(MAXB, (int)g->kpts.size());
+    cudaStream_t s0 = nullptr, sb[MAXB] = {nullptr};
+    cudaEvent_t fork = nullptr, join[MAXB] = {nullptr};
+    bool used[MAXB] = {false};
+    qm_batch_plan *p = new (std::nothrow) qm_batch_plan();
+    if (!p) return fail(QM_ENOMEM, "host allocation failed");
+    p->g = g;
+    auto cleanup = [&]() {
+        if (fork) cudaEventDestroy(fork);
+        for (int b = 0; b < nbranch; ++b) { if (join[b]) cudaEventDestroy(join[b]); if (sb[b]) cudaStreamDestroy(sb[b]); }
+        if (s0) cudaStreamDestroy(s0);
+    };
+    cudaError_t e = cudaStreamCreateWithFlags(&s0, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&fork, cudaEventDisableTiming);
+    for (int b = 0; b < nbranch && e == cudaSuccess; ++b) {
+        e = cudaStreamCreateWithFlags(&sb[b], cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&join[b], cudaEventDisableTiming);
+    }
+    if (e != cudaSuccess) { cleanup(); delete p; return fail(QM_ECUDA, cudaGetErrorString(e)); }
+    const unsigned long long l0 = g->launches;
+    e = cudaStreamBeginCapture(s0, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) { cleanup(); delete p; return fail(QM_ECUDA, cudaGetErrorString(e)); }
+    // k-points have their own work spaces: one branch per k-point (modulo MAXB), items of a branch in list order
+    rc = QM_OK;
+    e = cudaEventRecord(fork, s0);
+    for (int i = 0; i < nitems && rc == QM_OK && e == cudaSuccess; ++i) {
+        const int b = k[i] % nbranch;
+        if (!used[b]) { e = cudaStreamWaitEvent(sb[b], fork, 0); used[b] = true; if (e != cudaSuccess) break; }
+        rc = qm_apply_h(g, psi_in_dev[i], psi_out_dev[i], nbands[i], k[i], sb[b]);
+    }
+    for (int b = 0; b < nbranch && e == cudaSuccess; ++b)
+        if (used[b]) { e = cudaEventRecord(join[b], sb[b]); if (e == cudaSuccess) e = cudaStreamWaitEvent(s0, join[b], 0); }
+    cudaGraph_t graph = nullptr;
+    const cudaError_t e2 = cudaStreamEndCapture(s0, &graph);
+    p->launches = g->launches - l0;
+    g->launches = l0;                               // capturing launched nothing
+    if (rc == QM_OK && (e != cudaSuccess || e2 != cudaSuccess)) rc = fail(QM_ECUDA, cudaGetErrorString(e != cudaSuccess ? e : e2));
+    if (rc == QM_OK) {
+        p->graph = graph;
+        const cudaError_t e3 = cudaGraphInstantiate(&p->exec, graph, 0);
+        if (e3 != cudaSuccess) rc = fail(QM_ECUDA, cudaGetErrorString(e3));
+    } else if (graph) cudaGraphDestroy(graph);
+    cleanup();
+    if (rc != QM_OK) { delete p; return rc; }
+    *out = p;
+    return QM_OK;
+}
+QM_API int qm_batch_plan_launch(qm_batch_plan *p, void *stream) {
+    if (!p || !p->exec) return fail(QM_EINVAL, "qm_batch_plan_launch: null plan");
+    int rc = check_device(p->g); if (rc) return rc;
+    CU_TRY(cudaGraphLaunch(p->exec, (cudaStream_t)stream));
+    p->g->launches += p->launches;
+    return QM_OK;
+}
+QM_API int qm_batch_plan_destroy(qm_batch_plan *p) { delete p; return QM_OK; }
 
 QM_API int qm_host_synchronize(qm_gspace *g) {
     if (!g) return fail(QM_EINVAL, "null handle");
@@ -599,8 +962,6 @@ QM_API int qm_subspace(qm_gspace *g, int k, const qm_c128 *a_dev, int na, const 
     if (!a_dev || !b_dev || !s_dev || na <= 0 || nb <= 0) return fail(QM_EINVAL, "qm_subspace: bad argument");
     KPoint *kp = g->kpts[k];
     cudaStream_t st = (cudaStream_t)stream;
-    static bool attr = false;
-    if (!attr) { CU_TRY(cudaFuncSetAttribute(k_sub_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, SG_SMEM)); attr = true; }
     const int ntm = (na + SG_T - 1) / SG_T, ntn = (nb + SG_T - 1) / SG_T;
     const int nkc = (kp->ng + SG_KS - 1) / SG_KS;
     const int nsplit = std::max(1, std::min(nkc, g->sm_count / (ntm * ntn)));
@@ -678,8 +1039,15 @@ QM_API int qm_density_accumulate(qm_gspace *g, int k, const qm_c128 *psi_dev, in
     KPoint *kp = g->kpts[k];
     cudaStream_t st = (cudaStream_t)stream;
     rc = ensure_workspace(g, kp, nbands); if (rc) return rc;
-    rc = dispatch_zinv(g, kp, reinterpret_cast<const c128 *>(psi_dev), nbands, st); if (rc) return rc;
-    return dispatch_plane<3>(g, kp, nullptr, nbands, weight, st, occ_dev, g->d_rhot.p);
+    const int chunk = fft_chunk_bands(g, kp);
+    for (int b0 = 0; b0 < nbands; b0 += chunk) {        // band order is kept: the running sum stays deterministic
+        const int n = std::min(chunk, nbands - b0);
+        rc = dispatch_zinv<false>(g, kp, reinterpret_cast<const c128 *>(psi_dev) + (size_t)b0 * kp->ng, nullptr, kp->d_W.p, n, st);
+        if (rc) return rc;
+        PlaneArgs a; a.scale = weight; a.occ = occ_dev + b0; a.rhot = g->d_rhot.p;
+        rc = dispatch_plane<3>(g, kp, kp->d_W.p, n, a, st); if (rc) return rc;
+    }
+    return QM_OK;
 }
 QM_API int qm_density_get(qm_gspace *g, double *rho_dev, double scale, void *stream) {
     if (!g || !rho_dev) return fail(QM_EINVAL, "qm_density_get: null argument");
@@ -702,10 +1070,22 @@ QM_API int qm_debug_g2r(qm_gspace *g, const qm_c128 *psi_g_dev, qm_c128 *box_r_d
     if (!psi_g_dev || !box_r_dev || nbands <= 0) return fail(QM_EINVAL, "qm_debug_g2r: bad argument");
     KPoint *kp = g->kpts[k];
     cudaStream_t st = (cudaStream_t)stream;
+    const size_t boxsz = (size_t)g->grid[0] * g->grid[1] * g->grid[2];
     rc = ensure_workspace(g, kp, nbands); if (rc) return rc;
-    rc = dispatch_zinv(g, kp, reinterpret_cast<const c128 *>(psi_g_dev), nbands, st); if (rc) return rc;
-    const double scale = 1.0 / ((double)g->grid[0] * g->grid[1] * g->grid[2]);
-    return dispatch_plane<1>(g, kp, reinterpret_cast<c128 *>(box_r_dev), nbands, scale, st);
+    const int chunk = fft_chunk_bands(g, kp);
+    CU_TRY(g->d_boxt.resize(boxsz * std::min(chunk, nbands)));
+    for (int b0 = 0; b0 < nbands; b0 += chunk) {
+        const int n = std::min(chunk, nbands - b0);
+        rc = dispatch_zinv<false>(g, kp, reinterpret_cast<const c128 *>(psi_g_dev) + (size_t)b0 * kp->ng, nullptr, kp->d_W.p, n, st);
+        if (rc) return rc;
+        PlaneArgs a; a.box = g->d_boxt.p; a.scale = 1.0 / (double)boxsz;
+        rc = dispatch_plane<1>(g, kp, kp->d_W.p, n, a, st); if (rc) return rc;
+        k_box_relayout<false><<<g->sm_count * 8, 256, 0, st>>>(g->d_boxt.p, reinterpret_cast<c128 *>(box_r_dev) + (size_t)b0 * boxsz,
+                                                              g->ax[0], g->ax[1], g->ax[2], n);
+        g->launches++;
+    }
+    CU_TRY(cudaGetLastError());
+    return QM_OK;
 }
 
 QM_API int qm_debug_r2g(qm_gspace *g, const qm_c128 *box_r_dev, qm_c128 *psi_g_dev, int nbands, int k, void *stream) {
@@ -713,10 +1093,22 @@ QM_API int qm_debug_r2g(qm_gspace *g, const qm_c128 *box_r_dev, qm_c128 *psi_g_d
     if (!psi_g_dev || !box_r_dev || nbands <= 0) return fail(QM_EINVAL, "qm_debug_r2g: bad argument");
     KPoint *kp = g->kpts[k];
     cudaStream_t st = (cudaStream_t)stream;
+    const size_t boxsz = (size_t)g->grid[0] * g->grid[1] * g->grid[2];
     rc = ensure_workspace(g, kp, nbands); if (rc) return rc;
-    rc = dispatch_plane<2>(g, kp, const_cast<c128 *>(reinterpret_cast<const c128 *>(box_r_dev)), nbands, 1.0, st);
-    if (rc) return rc;
-    return dispatch_zfwd(g, kp, nullptr, reinterpret_cast<c128 *>(psi_g_dev), nbands, 0, st);
+    const int chunk = fft_chunk_bands(g, kp);
+    CU_TRY(g->d_boxt.resize(boxsz * std::min(chunk, nbands)));
+    for (int b0 = 0; b0 < nbands; b0 += chunk) {
+        const int n = std::min(chunk, nbands - b0);
+        k_box_relayout<true><<<g->sm_count * 8, 256, 0, st>>>(reinterpret_cast<const c128 *>(box_r_dev) + (size_t)b0 * boxsz, g->d_boxt.p,
+                                                             g->ax[0], g->ax[1], g->ax[2], n);
+        g->launches++;
+        PlaneArgs a; a.box = g->d_boxt.p;
+        rc = dispatch_plane<2>(g, kp, kp->d_W.p, n, a, st); if (rc) return rc;
+        rc = dispatch_zfwd<GM_PLAIN>(g, kp, kp->d_W.p, nullptr, reinterpret_cast<c128 *>(psi_g_dev) + (size_t)b0 * kp->ng, n, 1.0, st);
+        if (rc) return rc;
+    }
+    CU_TRY(cudaGetLastError());
+    return QM_OK;
 }
 
 QM_API int qm_get_launch_count(const qm_gspace *g, unsigned long long *count) {

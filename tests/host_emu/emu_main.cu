@@ -78,14 +78,20 @@ template <class C> struct Emu {
                     const int4 q = kp.stickinfo[s0 + t];
                     if (kp.z_quarter) {
                         c128 kin[2 * Quarter<C>::Q];
-                        prefetch_kin<C>(psi_in + q.z, kp.g2.data() + q.z, stick_pruned(q, u), kinetic, kin);
-                        zfwd_step2_gather_pre<C>(qm_sline(&lines[t * LP]), out + q.z, stick_pruned(q, u), u, kin);
-                    } else zfwd_step2_gather<C>(qm_sline(&lines[t * LP]), out + q.z, kinetic ? psi_in + q.z : nullptr, kp.g2.data() + q.z, stick_pruned(q, u), u, kinetic);
+                        if (kinetic) {
+                            prefetch_kin<C, GM_KINETIC>(psi_in + q.z, kp.g2.data() + q.z, stick_pruned(q, u), true, kin);
+                            zfwd_step2_gather_pre<C, GM_KINETIC>(qm_sline(&lines[t * LP]), out + q.z, stick_pruned(q, u), u, kin, 1.0);
+                        } else {
+                            prefetch_kin<C, GM_PLAIN>(nullptr, nullptr, stick_pruned(q, u), true, kin);
+                            zfwd_step2_gather_pre<C, GM_PLAIN>(qm_sline(&lines[t * LP]), out + q.z, stick_pruned(q, u), u, kin, 1.0);
+                        }
+                    } else if (kinetic) zfwd_step2_gather<C, GM_KINETIC>(qm_sline(&lines[t * LP]), out + q.z, psi_in + q.z, kp.g2.data() + q.z, stick_pruned(q, u), u, 1.0);
+                    else zfwd_step2_gather<C, GM_PLAIN>(qm_sline(&lines[t * LP]), out + q.z, nullptr, nullptr, stick_pruned(q, u), u, 1.0);
                 }
             }
         }
     }
-    // k_plane for one (band, p).  vt: relaid potential; box: natural-order box of this band
+    // k_plane for one (band, p).  vt: relaid potential; box: transposed box (fft_phases.cuh BoxT) of this band
     template <int MODE> void plane(int p, c128 *W, const double *vt, c128 *box, double scale, int ncol) {
         const int X = kp.nx, rp = kp.rowpitch, S = kp.nsticks, n3 = ax.n, nthr = ncol * C::TT;
         // A is deliberately filled with garbage: every position must be written before it is read
@@ -105,7 +111,6 @@ template <class C> struct Emu {
             }
             for (int task = 0; task < X * C::TT; ++task) lineA_step2<C>(qm_sline(&A[(task / C::TT) * rp]), task % C::TT);
         }
-        const int z = (p / ax.r2) + ax.r1 * (p % ax.r2);
         const XRows xr{kp.xiv.x, kp.xiv.y, kp.xiv.z, kp.xiv.w};
         for (int cbase = 0; cbase < C::N; cbase += ncol) {
             if (MODE != 2)
@@ -119,11 +124,10 @@ template <class C> struct Emu {
             for (int tid = 0; tid < nthr; ++tid) {
                 int c = tid / C::TT, u = tid % C::TT, col = cbase + c;
                 if (col >= C::N) continue;
-                int y = (col / C::R2) + C::R1 * (col % C::R2);
                 VRow<C::R2> vr;
                 if (MODE == 0) load_vrow<C>(vr, vt + ((size_t)p * C::N + col) * VLayout<C>::COL, u);
-                c128 *bx = MODE == 0 ? nullptr : box + (size_t)y * n3 + z;
-                xcol_step2<C, MODE>(qm_sline(&scr[(size_t)c * SL]), u, rowB(u), vr, bx, (long)C::N * n3, scale);
+                c128 *bx = MODE == 0 ? nullptr : box + ((size_t)p * C::N + col) * C::N;
+                xcol_step2<C, MODE>(qm_sline(&scr[(size_t)c * SL]), u, rowB(u), vr, bx, nullptr, scale);
             }
             if (MODE != 1)
                 for (int tid = 0; tid < nthr; ++tid) {
@@ -179,6 +183,17 @@ template <class C> int run(int n, const double *lat, double ecut, const double *
         for (int p = 0; p < n; ++p) emu.template plane<1>(p, W.data(), nullptr, &g2r[b * n3], 1.0 / (double)n3, ncol);
         for (int p = 0; p < n; ++p) emu.template plane<2>(p, W.data(), nullptr, &g2r[b * n3], 1.0, ncol);
         emu.zfwd(W.data(), nullptr, &r2g[(size_t)b * kp.ng], false);
+    }
+    {   // the emulated planes wrote / read transposed boxes: bring g2r back to natural C order for the comparison
+        std::vector<c128> nat(g2r.size());
+        for (int b = 0; b < nb; ++b)
+            for (int p = 0; p < n; ++p)
+                for (int col = 0; col < n; ++col)
+                    for (int x = 0; x < n; ++x) {
+                        const int y = (col / ax[1].r2) + ax[1].r1 * (col % ax[1].r2), z = (p / ax[2].r2) + ax[2].r1 * (p % ax[2].r2);
+                        nat[b * n3 + ((size_t)x * n + y) * n + z] = g2r[b * n3 + ((size_t)p * n + col) * n + x];
+                    }
+        g2r.swap(nat);
     }
     dump(prefix + ".idx", kp.idx); dump(prefix + ".g2", kp.g2); dump(prefix + ".hloc", hloc); dump(prefix + ".g2r", g2r); dump(prefix + ".r2g", r2g);
     printf("ng %d sticks %d nx %d quarter x%d y%d z%d\n", kp.ng, kp.nsticks, kp.nx, (int)kp.x_quarter, (int)kp.y_quarter, (int)kp.z_quarter);
