@@ -324,3 +324,62 @@ def test_every_fft_length_local_and_kinetic_terms(qm, n, lat, ecut, k):
         e_inf, e_2 = band_errors(got, ref2)
         assert e_inf <= TOL and e_2 <= TOL, (e_inf, e_2)
     gs.close()
+
+
+def test_batch_plan_all_kpoints_as_one_graph(qm):
+    """qm_batch_plan_*: the (band, k) batch of cfg2 captured once as a CUDA graph (k-points on parallel branches with
+    their own work spaces) gives exactly what the individual calls give, launch after launch."""
+    torch, dev = _torch()
+    p0 = problem("cfg2", 0)
+    nk = p0["cfg"].nk
+    gs = _gspace(qm, p0, all_k=True)
+    gs.set_vloc(torch.from_numpy(p0["v"]).to(dev))
+    psi, out, want = [], [], []
+    for ik in range(nk):
+        p = problem("cfg2", ik)
+        gs.set_nonlocal(ik, torch.from_numpy(p["beta"]).to(dev), torch.from_numpy(p["dblk"]).to(dev))
+        psi.append(torch.from_numpy(p["psi"]).to(dev))
+        out.append(torch.zeros_like(psi[-1]))
+        want.append(gs.apply_h(psi[-1], k=ik).clone())
+    items = [(ik, psi[ik][b0:b0 + 8], out[ik][b0:b0 + 8]) for ik in range(nk) for b0 in (0, 8)]
+    plan = gs.batch_plan(items)
+    l0 = gs.launch_count()
+    for rep in range(3):
+        for o in out:
+            o.zero_()
+        plan.launch()
+        torch.cuda.synchronize()
+        for ik in range(nk):
+            assert torch.equal(out[ik], want[ik]), (rep, ik)
+    assert gs.launch_count() - l0 == 3 * 7 * len(items)
+    # and against the oracle for one k-point
+    p = problem("cfg2", 6)
+    e_inf, e_2 = band_errors(out[6].cpu().numpy(), _oracle(p, p["psi"], "full"))
+    assert e_inf <= TOL and e_2 <= TOL
+    plan.close()
+    gs.close()
+
+
+def test_wrong_device_and_concurrent_kpoints(qm):
+    """Calls for different k-points of one handle on different streams do not interfere (per-k work spaces)."""
+    torch, dev = _torch()
+    p0 = problem("cfg2", 0)
+    gs = _gspace(qm, p0, all_k=True)
+    gs.set_vloc(torch.from_numpy(p0["v"]).to(dev))
+    psi, want = [], []
+    for ik in range(4):
+        p = problem("cfg2", ik)
+        gs.set_nonlocal(ik, torch.from_numpy(p["beta"]).to(dev), torch.from_numpy(p["dblk"]).to(dev))
+        psi.append(torch.from_numpy(p["psi"]).to(dev))
+        want.append(gs.apply_h(psi[-1], k=ik).clone())
+        gs.reserve(16, k=ik)
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream() for _ in range(4)]
+    outs = [torch.empty_like(x) for x in psi]
+    for rep in range(20):
+        for ik in range(4):
+            gs.apply_h(psi[ik], outs[ik], k=ik, stream=streams[ik])
+    torch.cuda.synchronize()
+    for ik in range(4):
+        assert torch.equal(outs[ik], want[ik]), ik
+    gs.close()
