@@ -1,15 +1,24 @@
-"""Build libqm_hpsi.so in-tree with nvcc for sm_100a (cross-compiles without a GPU)."""
+"""Build libqm_hpsi.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
+
+The library is several translation units (csrc/*.cu: the C ABI, the z-stick kernels, one unit per mode of the fused
+plane kernel, the unfused general-box passes) compiled in parallel and linked into one shared object.
+"""
 from __future__ import annotations
 
 import os
 import subprocess
+from concurrent.futures import ThreadPoolExecutor
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
+OBJDIR = os.path.join(_HERE, "build")
 LIB = os.path.join(_HERE, "libqm_hpsi.so")
-SOURCES = ["qm_api.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
-              "--shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
+              "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
+
+
+def sources():
+    return sorted(f for f in os.listdir(CSRC) if f.endswith(".cu"))
 
 
 def _deps():
@@ -28,16 +37,27 @@ def is_stale() -> bool:
     return any(os.path.getmtime(d) > t for d in _deps())
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, extra_flags=()) -> str:
     if not force and not is_stale():
         return LIB
+    os.makedirs(OBJDIR, exist_ok=True)
+    flags = NVCC_FLAGS + list(extra_flags) + (["-Xptxas", "-v"] if verbose else [])
+
+    def compile_one(src):
+        obj = os.path.join(OBJDIR, src[:-3] + f".{os.getpid()}.o")
+        subprocess.run(["nvcc"] + flags + ["-c", "-o", obj, os.path.join(CSRC, src)], check=True)
+        return obj
+
+    with ThreadPoolExecutor(max_workers=min(len(sources()), os.cpu_count() or 4)) as ex:
+        objs = list(ex.map(compile_one, sources()))
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = ["nvcc"] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + \
-          [os.path.join(CSRC, s) for s in SOURCES]
-    subprocess.run(cmd, check=True)
+    subprocess.run(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "--shared", "-o", tmp] + objs, check=True)
     os.replace(tmp, LIB)
+    for o in objs:
+        os.remove(o)
     return LIB
 
 
 if __name__ == "__main__":
-    print(build(force=True))
+    import sys
+    print(build(force=True, extra_flags=[a for a in sys.argv[1:] if a.startswith("-D")]))

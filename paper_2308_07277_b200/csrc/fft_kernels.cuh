@@ -145,6 +145,9 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
 #ifndef QM_PLANE_YROWS
 #define QM_PLANE_YROWS 1        /* plane rows a team works on between two group barriers of the y phase (2: spills, 343 vs 300 us) */
 #endif
+#ifndef QM_PLANE_XPREFETCH
+#define QM_PLANE_XPREFETCH 0    /* x phase: fetch a column's step-1 inputs one column ahead (quarter rule) */
+#endif
 constexpr int QM_GROUP = QM_PLANE_GROUP;
 // Scratch lines of neighbouring teams: with 12-thread teams a quarter-warp straddles two teams as 4+4
 // threads, and their unit-stride 16-byte accesses are conflict free iff the pitch is 4 (mod 8); else odd.
@@ -273,13 +276,26 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
     if constexpr (MODE == 0) {       // V of the first column: in flight while step 1 runs
         if (team_ok && col0 < C::N) load_vrow<C>(vr, vplane + (size_t)col0 * VLayout<C>::COL, u);
     }
+    // Step-1 inputs of a column under the quarter rule: fetched one column ahead (before the barrier in front of the
+    // previous column's step 3), so that their shared-memory latency hides behind that barrier and step 3.  Nobody else
+    // touches a column of the plane array during the x phase: every column is owned by one team.
+    constexpr bool XPRE = (MODE == 0 || MODE == 4) && QM_PLANE_XPREFETCH;
+    c128 xpre[2 * Quarter<C>::Q];
+    if constexpr (XPRE) {
+        if (xq && team_ok && col0 < C::N) prefetch_quarter<C>(As + C::pos(col0), C::R2 * RP, px, xpre);
+    }
     for (int col = col0; col - slot < C::N; col += ngroups * TPG) {
         const bool ok = team_ok && col < C::N;
         const SLine Acol = As + C::pos(col);
         if constexpr (MODE != 2) {
             if (ok) {
-                if (xq) prunedA_step1_quarter<C>(Acol, C::R2 * RP, px, myscr, u, twa);
-                else prunedA_step1<C>(Acol, C::R2 * RP, px, myscr, u, twa);
+                if constexpr (XPRE) {
+                    if (xq) prunedA_step1_pre<C>(xpre, myscr, u, twa);
+                    else prunedA_step1<C>(Acol, C::R2 * RP, px, myscr, u, twa);
+                } else {
+                    if (xq) prunedA_step1_quarter<C>(Acol, C::R2 * RP, px, myscr, u, twa);
+                    else prunedA_step1<C>(Acol, C::R2 * RP, px, myscr, u, twa);
+                }
             }
             group_barrier<G>(grp);
         }
@@ -303,6 +319,10 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
         if constexpr (MODE == 0) {   // prefetch V of this team's next column behind steps 3 and 1
             const int ncol = col + ngroups * TPG;
             if (team_ok && ncol < C::N) load_vrow<C>(vr, vplane + (size_t)ncol * VLayout<C>::COL, u);
+        }
+        if constexpr (XPRE) {
+            const int ncol = col + ngroups * TPG;
+            if (xq && team_ok && ncol < C::N) prefetch_quarter<C>(As + C::pos(ncol), C::R2 * RP, px, xpre);
         }
         group_barrier<G>(grp);
         if constexpr (MODE != 1 && MODE != 3) {

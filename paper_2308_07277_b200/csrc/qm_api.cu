@@ -1,174 +1,10 @@
 // C ABI of libqm_hpsi (see include/qm_hpsi.h).  Host-side set-up (G-sphere, stick tables) and
 // kernel launches.  No CPU fallback: compute entry points fail with QM_ECUDA without a device.
-#include <cuda_runtime.h>
-#include <algorithm>
-#include <cmath>
-#include <cstdio>
-#include <cstdlib>
-#include <cstring>
-#include <new>
-#include <string>
-#include <vector>
-
-#include "../../include/qm_hpsi.h"
-#include "fft_kernels.cuh"
+#include "qm_internal.h"
 #include "proj_kernels.cuh"
 #include "subspace_kernels.cuh"
-#include "qm_plan.h"
-#include "gspace_host.h"
 
-namespace {
-
-thread_local std::string g_err;
-int fail(int code, const std::string &msg) { g_err = msg; return code; }
-
-#define CU_TRY(expr)                                                                        \
-    do {                                                                                    \
-        cudaError_t _e = (expr);                                                            \
-        if (_e != cudaSuccess)                                                              \
-            return fail(_e == cudaErrorMemoryAllocation ? QM_ENOMEM : QM_ECUDA,             \
-                        std::string(#expr) + ": " + cudaGetErrorString(_e));                \
-    } while (0)
-
-template <class T> struct DevBuf {
-    T *p = nullptr; size_t n = 0;
-    ~DevBuf() { if (p) cudaFree(p); }
-    cudaError_t resize(size_t m) {
-        if (m <= n) return cudaSuccess;
-        if (p) { cudaFree(p); p = nullptr; n = 0; }
-        cudaError_t e = cudaMalloc(&p, m * sizeof(T));
-        if (e == cudaSuccess) n = m;
-        return e;
-    }
-    cudaError_t upload(const std::vector<T> &h) {
-        cudaError_t e = resize(h.size() ? h.size() : 1);
-        if (e != cudaSuccess) return e;
-        if (h.empty()) return cudaSuccess;
-        return cudaMemcpy(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice);
-    }
-};
-
-struct KPoint : QmKTables {
-    DevBuf<int4> d_rowinfo, d_stickinfo;
-    DevBuf<double> d_g2;
-    // non-local
-    bool nl_set = false;
-    int nproj = 0, dblock = 0;
-    int nmblk = 0, nkc = 0, ngt = 0, nic = 0;          // tile counts of the two beta copies
-    DevBuf<c128> d_beta1, d_beta2;
-    DevBuf<double> d_D;
-    // workspaces of this k-point (calls on different k-points may run on different streams)
-    DevBuf<c128> d_W, d_Ppart, d_P, d_part;
-    DevBuf<double> d_qt;
-    DevBuf<int> d_pdesc;
-    DevBuf<c128> d_sophase;                             // split-operator: exp(-i dt |k+G|^2 / 4)
-    double ecut_override = 0.0;                         // epsilon spheres (qm_mtxel) carry their own cut-off
-    QmKPlanDev plan() const {
-        QmKPlanDev p;
-        p.ng = ng; p.nsticks = nsticks; p.nx = nx; p.rowpitch = rowpitch;
-        p.g2 = d_g2.p;
-        p.row_info = d_rowinfo.p; p.x_iv = xiv; p.stick_info = d_stickinfo.p;
-        return p;
-    }
-};
-
-}  // namespace
-
-struct Profiler {
-    bool on = false;
-    std::vector<cudaEvent_t> pool;
-    size_t used = 0;
-    struct Rec { int kind; size_t e0, e1; };
-    std::vector<Rec> recs;
-    double total_ms[QM_K_COUNT] = {0};
-    unsigned long long count[QM_K_COUNT] = {0};
-    ~Profiler() { for (auto e : pool) cudaEventDestroy(e); }
-    size_t next() {
-        if (used == pool.size()) { cudaEvent_t e; cudaEventCreate(&e); pool.push_back(e); }
-        return used++;
-    }
-    void begin(int kind, cudaStream_t st) {
-        if (!on) return;
-        Rec r; r.kind = kind; r.e0 = next(); r.e1 = next();
-        cudaEventRecord(pool[r.e0], st);
-        recs.push_back(r);
-    }
-    void end(cudaStream_t st) { if (on) cudaEventRecord(pool[recs.back().e1], st); }
-    void collect() {
-        for (const Rec &r : recs) {
-            cudaEventSynchronize(pool[r.e1]);
-            float ms = 0.f;
-            if (cudaEventElapsedTime(&ms, pool[r.e0], pool[r.e1]) == cudaSuccess) {
-                total_ms[r.kind] += ms; count[r.kind]++;
-            }
-        }
-        recs.clear(); used = 0;
-    }
-    void reset() { collect(); for (int i = 0; i < QM_K_COUNT; ++i) { total_ms[i] = 0; count[i] = 0; } }
-};
-
-struct HostPipe {       // two-slot staging pipeline behind qm_apply_h_host(_async)
-    bool init = false;
-    cudaStream_t s_in = nullptr, s_out = nullptr;
-    cudaEvent_t in_ready[2], compute_done[2], out_done[2];
-    bool used[2] = {false, false};
-    DevBuf<c128> in[2], out[2];
-    int slot = 0;
-    ~HostPipe() {
-        if (!init) return;
-        for (int i = 0; i < 2; ++i) { cudaEventDestroy(in_ready[i]); cudaEventDestroy(compute_done[i]); cudaEventDestroy(out_done[i]); }
-        cudaStreamDestroy(s_in); cudaStreamDestroy(s_out);
-    }
-};
-
-struct qm_gspace {
-    Profiler prof;
-    HostPipe pipe;
-    double lattice[9], recip[9];
-    double ecut;
-    int grid[3];
-    QmAxis ax[3];
-    std::vector<KPoint *> kpts;
-    DevBuf<c128> d_tw[3];
-    DevBuf<double> d_vt, d_rhot;
-    bool rho_open = false;
-    bool v_set = false;
-    DevBuf<c128> d_subpart, d_tay_h, d_tay_t;
-    DevBuf<c128> d_boxt;            // transposed boxes of the debug hooks
-    DevBuf<c128> d_sofield;         // split-operator: exp(-i dt V(r)) / N in the transposed-box layout
-    bool so_set = false;
-    double so_dt = 0.0;
-    unsigned long long launches = 0;
-    int device = 0;                 // the CUDA device the handle was created on (every call checks it)
-    int sm_count = 148;
-    int max_smem = 0;
-    size_t l2_bytes = 0;
-    int fft_chunk = 0;              // bands per internal pass of the FFT path (0: derived from the L2 size; QM_FFT_CHUNK)
-    int z_cta_per_sm = 2;           // resident z-kernel CTAs per SM the grid is sized for (QM_Z_CTA_PER_SM)
-    int plane_stagger_ns = 0;       // de-phasing delay between the plane kernel's groups (QM_PLANE_STAGGER_NS)
-    ~qm_gspace() { for (auto *k : kpts) delete k; }
-};
-
-// GW plane-wave matrix elements for one (k+q, k) pair of k-points: the epsilon sphere |q+G|^2 < ecut_eps on the
-// handle's FFT box, with its own stick tables, and the workspaces of qm_matrix_elements.
-struct qm_mtxel {
-    qm_gspace *g = nullptr;
-    int k_bra = 0, k_ket = 0;
-    KPoint sph;
-    DevBuf<c128> d_ketbox, d_brabox, d_Wp;
-};
-
-// A fixed list of qm_apply_h calls captured as one CUDA graph (qm_batch_plan_*).
-struct qm_batch_plan {
-    qm_gspace *g = nullptr;
-    cudaGraph_t graph = nullptr;
-    cudaGraphExec_t exec = nullptr;
-    unsigned long long launches = 0;        // kernels per graph launch
-    ~qm_batch_plan() {
-        if (exec) cudaGraphExecDestroy(exec);
-        if (graph) cudaGraphDestroy(graph);
-    }
-};
+thread_local std::string qm_g_err;
 
 namespace {
 
@@ -193,164 +29,31 @@ int check_device(const qm_gspace *g) {
     return QM_OK;
 }
 
-constexpr int PLANE_GROUP = QM_GROUP;
-size_t plane_smem(const qm_gspace *g, const KPoint *kp, int ngroups) {
-    const QmAxis &ax = g->ax[0];
-    const size_t sl = (size_t)qm_scratch_pitch(ax.len, std::max(ax.r1, ax.r2));
-    const int tpg = PLANE_GROUP / std::max(ax.r1, ax.r2);
-    const size_t a_elems = ((size_t)kp->nx * kp->rowpitch + 7) & ~(size_t)7;
-    return (a_elems + (size_t)ngroups * tpg * sl) * sizeof(c128) + (size_t)kp->nx * sizeof(int4) + 16;
-}
-
-// number of independent groups of the plane kernel: the fewest groups that reach the
-// minimum number of column rounds within the shared-memory and thread limits
-int plane_groups(const qm_gspace *g, const KPoint *kp) {
-    const QmAxis &ax = g->ax[0];
-    const int tpg = PLANE_GROUP / std::max(ax.r1, ax.r2);
-    const int nchunks = (ax.n + tpg - 1) / tpg;
-    int gmax = std::min(QM_PLANE_MAX_THREADS / PLANE_GROUP, nchunks);
-    while (gmax > 1 && plane_smem(g, kp, gmax) > (size_t)g->max_smem) --gmax;
-    const int rounds = (nchunks + gmax - 1) / gmax;
-    int best = gmax;
-    for (int c = gmax; c >= 1; --c)
-        if ((nchunks + c - 1) / c == rounds) best = c;
-    return best;
-}
-
-// z kernels: grid.x tiles-in-flight per band chosen so that the whole grid is close to a whole number of
-// resident CTAs per SM (each CTA then loops over ~ntiles / grid.x tiles)
-int z_grid_x(const qm_gspace *g, int ntiles, int nb, int cta_per_sm) {
-    const int slots = g->sm_count * cta_per_sm;
-    int gx = std::max(1, slots / std::max(1, nb));
-    if (gx >= ntiles) return ntiles;
-    const int rounds = (ntiles + gx - 1) / gx;          // fewest CTAs that keep the same number of rounds
-    return (ntiles + rounds - 1) / rounds;
-}
-template <class C, bool PH> int launch_zinv(qm_gspace *g, KPoint *kp, const c128 *psi, const c128 *phase, c128 *W, int nb,
-                                            cudaStream_t st) {
-    const int ntiles = (kp->nsticks + QM_ZT - 1) / QM_ZT;
-    dim3 grid(z_grid_x(g, ntiles, nb, g->z_cta_per_sm), nb);
-    g->prof.begin(QM_K_ZINV, st);
-    k_zinv<C, PH><<<grid, QM_ZT * C::TT, qm_z_smem<C>(), st>>>(kp->plan(), g->d_tw[2].p, psi, phase, W, ntiles,
-                                                                kp->z_quarter ? 1 : 0);
-    g->prof.end(st);
-    g->launches++;
-    CU_TRY(cudaGetLastError());
-    return QM_OK;
-}
-template <class C, int GM> int launch_zfwd(qm_gspace *g, KPoint *kp, const c128 *W, const c128 *aux, c128 *out, int nb,
-                                           double scale, cudaStream_t st) {
-    const int ntiles = (kp->nsticks + QM_ZT - 1) / QM_ZT;
-    dim3 grid(z_grid_x(g, ntiles, nb, g->z_cta_per_sm), nb);
-    g->prof.begin(QM_K_ZFWD, st);
-    k_zfwd<C, GM><<<grid, QM_ZT * C::TT, qm_z_smem<C>(), st>>>(kp->plan(), g->d_tw[2].p, W, aux, out, ntiles, scale,
-                                                                kp->z_quarter ? 1 : 0);
-    g->prof.end(st);
-    g->launches++;
-    CU_TRY(cudaGetLastError());
-    return QM_OK;
-}
-struct PlaneArgs {          // operands of the plane kernel beyond the stick planes W
-    c128 *box = nullptr;            // MODE 1 output / MODE 2 first operand (transposed boxes, one per state)
-    const c128 *box2 = nullptr;     // MODE 2 second operand (conjugated) / MODE 4 complex field
-    int npair2 = 0;                 // MODE 2 with a second operand: states in box2 (plane index counts pairs a * npair2 + b)
-    double scale = 1.0;
-    const double *occ = nullptr;    // MODE 3
-    double *rhot = nullptr;
-};
-template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *W, int nb, const PlaneArgs &a, cudaStream_t st) {
-    const int ngroups = plane_groups(g, kp);
-    const size_t smem = plane_smem(g, kp, ngroups);
-    if (smem > (size_t)g->max_smem)
-        return fail(QM_EGRID, "plane kernel does not fit shared memory for this grid / sphere");
-    QmGridDev gd;
-    for (int i = 0; i < 3; ++i) { gd.ax[i] = g->ax[i]; gd.tw[i] = g->d_tw[i].p; }
-    gd.vt = g->d_vt.p;
-    const int nplanes = g->grid[2] * nb;
-    // persistent: one CTA per SM walks the (band, z-plane) list; density mode: one CTA per z-plane, all bands
-    const int grid = MODE == 3 ? std::min(g->grid[2], g->sm_count) : std::min(nplanes, g->sm_count);
-    g->prof.begin(QM_K_PLANE, st);
-    k_plane<C, MODE><<<grid, ngroups * PLANE_GROUP, smem, st>>>(kp->plan(), gd, W, a.box, a.box2, a.npair2, ngroups, a.scale,
-                                                                   g->plane_stagger_ns, nplanes,
-                                                                   (kp->y_quarter ? 1 : 0) | (kp->x_quarter ? 2 : 0), a.occ, a.rhot);
-    g->prof.end(st);
-    g->launches++;
-    CU_TRY(cudaGetLastError());
-    return QM_OK;
-}
-
-// dispatch on FFT length ---------------------------------------------------------------------
-#ifdef QM_DEV_SIZES      /* developer builds: only the lengths of the five BASELINE.json configs (fast compile) */
-#define QM_FOR_SIZES(X) X(12, 3, 4) X(24, 4, 6) X(32, 4, 8) X(48, 6, 8) X(96, 8, 12) X(144, 12, 12)
-#else
-#define QM_FOR_SIZES(X)                                                                              \
-    X(8, 2, 4) X(12, 3, 4) X(16, 4, 4) X(18, 3, 6) X(20, 4, 5) X(24, 4, 6) X(30, 5, 6) X(32, 4, 8)   \
-    X(36, 6, 6) X(40, 5, 8) X(48, 6, 8) X(60, 6, 10) X(64, 8, 8) X(72, 8, 9) X(80, 8, 10)            \
-    X(96, 8, 12) X(100, 10, 10) X(108, 9, 12) X(120, 10, 12) X(128, 8, 16) X(144, 12, 12)
-#endif
-
 template <bool PH> int dispatch_zinv(qm_gspace *g, KPoint *kp, const c128 *psi, const c128 *phase, c128 *W, int nb,
                                      cudaStream_t st) {
-    switch (g->grid[2]) {
-#define X(N, A, B) case N: return launch_zinv<LineCfg<A, B>, PH>(g, kp, psi, phase, W, nb, st);
-        QM_FOR_SIZES(X)
-#undef X
-    }
-    return fail(QM_EGRID, "unsupported FFT length (axis 3)");
+    return qm_launch_zinv(g, kp, psi, PH ? phase : nullptr, W, nb, st);
 }
 template <int GM> int dispatch_zfwd(qm_gspace *g, KPoint *kp, const c128 *W, const c128 *aux, c128 *out, int nb, double scale,
                                     cudaStream_t st) {
-    switch (g->grid[2]) {
-#define X(N, A, B) case N: return launch_zfwd<LineCfg<A, B>, GM>(g, kp, W, aux, out, nb, scale, st);
-        QM_FOR_SIZES(X)
-#undef X
-    }
-    return fail(QM_EGRID, "unsupported FFT length (axis 3)");
+    return qm_launch_zfwd(g, kp, GM, W, aux, out, nb, scale, st);
 }
 template <int MODE> int dispatch_plane(qm_gspace *g, KPoint *kp, c128 *W, int nb, const PlaneArgs &a, cudaStream_t st) {
-    switch (g->grid[0]) {
-#define X(N, A, B) case N: return launch_plane<LineCfg<A, B>, MODE>(g, kp, W, nb, a, st);
-        QM_FOR_SIZES(X)
-#undef X
-    }
-    return fail(QM_EGRID, "unsupported FFT length (axes 1,2)");
+    if constexpr (MODE == 0) return qm_launch_plane_m0(g, kp, W, nb, a, st);
+    else if constexpr (MODE == 1) return qm_launch_plane_m1(g, kp, W, nb, a, st);
+    else if constexpr (MODE == 2) return qm_launch_plane_m2(g, kp, W, nb, a, st);
+    else if constexpr (MODE == 3) return qm_launch_plane_m3(g, kp, W, nb, a, st);
+    else return qm_launch_plane_m4(g, kp, W, nb, a, st);
 }
 
 // Opt every kernel this handle can launch into its dynamic shared memory ONCE, at handle creation, on the handle's
 // device (function attributes are per device; nothing of this kind is left on the hot path).
-template <class C> int prep_z_kernels() {
-    const int smem = (int)qm_z_smem<C>();
-    CU_TRY(cudaFuncSetAttribute(k_zinv<C, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    CU_TRY(cudaFuncSetAttribute(k_zinv<C, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    CU_TRY(cudaFuncSetAttribute(k_zfwd<C, GM_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    CU_TRY(cudaFuncSetAttribute(k_zfwd<C, GM_KINETIC>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    CU_TRY(cudaFuncSetAttribute(k_zfwd<C, GM_PHASE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    CU_TRY(cudaFuncSetAttribute(k_zfwd<C, GM_CONJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    return QM_OK;
-}
-template <class C> int prep_plane_kernels(int max_smem) {
-    CU_TRY(cudaFuncSetAttribute(k_plane<C, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
-    CU_TRY(cudaFuncSetAttribute(k_plane<C, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
-    CU_TRY(cudaFuncSetAttribute(k_plane<C, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
-    CU_TRY(cudaFuncSetAttribute(k_plane<C, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
-    CU_TRY(cudaFuncSetAttribute(k_plane<C, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
-    return QM_OK;
-}
 int prepare_kernels(qm_gspace *g) {
-    int rc = QM_EGRID;
-    switch (g->grid[2]) {
-#define X(N, A, B) case N: rc = prep_z_kernels<LineCfg<A, B>>(); break;
-        QM_FOR_SIZES(X)
-#undef X
-    }
-    if (rc) return rc;
-    rc = QM_EGRID;
-    switch (g->grid[0]) {
-#define X(N, A, B) case N: rc = prep_plane_kernels<LineCfg<A, B>>(g->max_smem); break;
-        QM_FOR_SIZES(X)
-#undef X
-    }
-    if (rc) return rc;
+    int rc = qm_prepare_z(g); if (rc) return rc;
+    rc = qm_prepare_plane_m0(g); if (rc) return rc;
+    rc = qm_prepare_plane_m1(g); if (rc) return rc;
+    rc = qm_prepare_plane_m2(g); if (rc) return rc;
+    rc = qm_prepare_plane_m3(g); if (rc) return rc;
+    rc = qm_prepare_plane_m4(g); if (rc) return rc;
     CU_TRY(cudaFuncSetAttribute(k_proj1_pipe, cudaFuncAttributeMaxDynamicSharedMemorySize, P1_SMEM));
     CU_TRY(cudaFuncSetAttribute(k_proj2_sk, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM));
     CU_TRY(cudaFuncSetAttribute(k_sub_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, SG_SMEM));
@@ -542,7 +245,7 @@ int run_local(qm_gspace *g, KPoint *kp, const c128 *in, c128 *out, int nb, int k
 
 extern "C" {
 
-QM_API const char *qm_last_error(void) { return g_err.c_str(); }
+QM_API const char *qm_last_error(void) { return qm_g_err.c_str(); }
 QM_API const char *qm_version(void) { return "qm_hpsi 0.2 (sm_100a)"; }
 
 QM_API int qm_fft_size_supported(int n) { return qm_find_size(n) ? 1 : 0; }
@@ -611,6 +314,7 @@ QM_API int qm_gspace_create(const double *lattice_bohr, double ecutwfc_ry, const
     }
     if (const char *e = getenv("QM_PLANE_STAGGER_NS")) g->plane_stagger_ns = atoi(e);
     if (const char *e = getenv("QM_Z_CTA_PER_SM")) g->z_cta_per_sm = std::max(1, atoi(e));
+    if (const char *e = getenv("QM_PLANE_CTAS")) g->plane_ctas_per_sm = std::max(0, atoi(e));
     if (const char *e = getenv("QM_FFT_CHUNK")) g->fft_chunk = std::max(0, atoi(e));
     *out = g;
     return QM_OK;

@@ -1,0 +1,56 @@
+// One translation unit of the fused xy-plane kernel: every supported FFT length for ONE mode (QM_TU_MODE), so that the
+// five modes compile in parallel.  Included by qm_plane0.cu ... qm_plane4.cu.
+#include "qm_internal.h"
+
+#define QM_CAT2(a, b) a##b
+#define QM_CAT(a, b) QM_CAT2(a, b)
+
+namespace {
+
+template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *W, int nb, const PlaneArgs &a, cudaStream_t st) {
+    // two resident CTAs per SM when the plane array is small enough: each walks its own planes, so the CTA-wide
+    // barriers and the load / compute / store phases of one CTA overlap the other's work
+    int cps = MODE == 3 ? 1 : (g->plane_ctas_per_sm > 0 ? g->plane_ctas_per_sm : 1);
+    int ngroups = plane_groups(g, kp, cps);
+    if (ngroups == 0) { cps = 1; ngroups = plane_groups(g, kp, 1); }
+    const size_t smem = plane_smem(g, kp, ngroups);
+    if (ngroups == 0 || smem > (size_t)g->max_smem)
+        return fail(QM_EGRID, "plane kernel does not fit shared memory for this grid / sphere");
+    QmGridDev gd;
+    for (int i = 0; i < 3; ++i) { gd.ax[i] = g->ax[i]; gd.tw[i] = g->d_tw[i].p; }
+    gd.vt = g->d_vt.p;
+    const int nplanes = g->grid[2] * nb;
+    // persistent: one CTA per SM walks the (band, z-plane) list; density mode: one CTA per z-plane, all bands
+    const int grid = MODE == 3 ? std::min(g->grid[2], g->sm_count) : std::min(nplanes, g->sm_count * cps);
+    g->prof.begin(QM_K_PLANE, st);
+    k_plane<C, MODE><<<grid, ngroups * PLANE_GROUP, smem, st>>>(kp->plan(), gd, W, a.box, a.box2, a.npair2, ngroups, a.scale,
+                                                                   g->plane_stagger_ns, nplanes,
+                                                                   (kp->y_quarter ? 1 : 0) | (kp->x_quarter ? 2 : 0), a.occ, a.rhot);
+    g->prof.end(st);
+    g->launches++;
+    CU_TRY(cudaGetLastError());
+    return QM_OK;
+}
+
+}  // namespace
+
+int QM_CAT(qm_launch_plane_m, QM_TU_MODE)(qm_gspace *g, KPoint *kp, c128 *W, int nb, const PlaneArgs &a, cudaStream_t st) {
+    switch (g->grid[0]) {
+#define X(N, A, B) case N: return launch_plane<LineCfg<A, B>, QM_TU_MODE>(g, kp, W, nb, a, st);
+        QM_FOR_SIZES(X)
+#undef X
+    }
+    return fail(QM_EGRID, "unsupported FFT length (axes 1,2)");
+}
+
+int QM_CAT(qm_prepare_plane_m, QM_TU_MODE)(qm_gspace *g) {
+    switch (g->grid[0]) {
+#define X(N, A, B)                                                                                                       \
+    case N: CU_TRY(cudaFuncSetAttribute(k_plane<LineCfg<A, B>, QM_TU_MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                        g->max_smem));                                                                    \
+        return QM_OK;
+        QM_FOR_SIZES(X)
+#undef X
+    }
+    return fail(QM_EGRID, "unsupported FFT length (axes 1,2)");
+}
