@@ -7,6 +7,7 @@
 #include <cuda_runtime.h>
 #include "fft_phases.cuh"
 #include "async_copy.cuh"
+#include "tmem_rows.cuh"
 #include "qm_plan.h"
 
 // z kernels.  A CTA owns tiles of QM_ZT adjacent sticks of one band (looping over tiles gridDim.x apart, so the
@@ -148,6 +149,9 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
 #ifndef QM_PLANE_XPREFETCH
 #define QM_PLANE_XPREFETCH 0    /* x phase: fetch a column's step-1 inputs one column ahead (quarter rule) */
 #endif
+#ifndef QM_PLANE_TW_TMEM
+#define QM_PLANE_TW_TMEM 1      /* per-thread twiddle rows live in tensor memory (tmem_rows.cuh) instead of registers */
+#endif
 constexpr int QM_GROUP = QM_PLANE_GROUP;
 // Scratch lines of neighbouring teams: with 12-thread teams a quarter-warp straddles two teams as 4+4
 // threads, and their unit-stride 16-byte accesses are conflict free iff the pitch is 4 (mod 8); else odd.
@@ -173,17 +177,68 @@ template <int G> __device__ __forceinline__ void group_barrier(int grp) {
 struct PlaneCtx {
     c128 *A, *scr;
     const int4 *rowinfo_s;
+    const int4 *rowtab_s;       // [X][TT] hoisted addressing of every (row, u): Pruned with the row's first stick folded in, or nullptr
     int X, ngroups, n3, quarter;
     size_t wband;
+    uint32_t tw_a, tw_b;        // TMEM addresses of this thread's twiddle rows (QM_PLANE_TW_TMEM)
+};
+// Branch-free lines.  The plane kernel never branches on "does this thread have a line": a thread without one (a team
+// beyond the last row / column, a lane beyond the last team, a lane u >= R of a pass with fewer than TT butterflies) is
+// pointed at a line nobody reads -- its team's scratch line while that is idle, else the group's sink line -- and its
+// global accesses are masked off.  Idle lanes cost the same issue slots either way, and the warp stays convergent, which
+// tcgen05.ld (below) needs; ptxas also spills the transform's registers around a tcgen05.ld that sits between two
+// divergent regions (measured: 600-800 B of spills per thread), and not around one in straight-line code.
+//
+// The tail of a first pass (twiddle multiply + store).  With the rows in tensor memory the factors are brought in
+// QM_TW_CHUNK at a time.  DIRB: false = backward first pass (stepA1_tail), true = forward (stepB1_tail).
+#ifndef QM_TW_CHUNK
+#define QM_TW_CHUNK 4
+#endif
+template <class C, bool DIRB, int NR, int R, class L>
+__device__ __forceinline__ void plane_tail(const c128 (&t)[NR][R], const L (&dst)[NR], int u, const TwRow<R> &in_regs, uint32_t taddr)
+{
+#if QM_PLANE_TW_TMEM
+    static_for<(R + QM_TW_CHUNK - 1) / QM_TW_CHUNK>([&](auto I) {
+        constexpr int j0 = decltype(I)::value * QM_TW_CHUNK, j1 = j0 + QM_TW_CHUNK < R ? j0 + QM_TW_CHUNK : R;
+        constexpr int l0 = j0 == 0 ? 1 : j0;            // factor 0 is 1 and is not stored
+        TwChunk<l0, (l0 < j1 ? j1 : l0 + 1)> ch;
+        if constexpr (l0 < j1) tmem_load_chunk(ch, taddr);
+        static_for<NR>([&](auto II) {
+            constexpr int i = decltype(II)::value;
+            if constexpr (DIRB) stepB1_tail_range<C, j0, j1, false>(t[i], dst[i], u, ch);
+            else stepA1_tail_range<C, j0, j1, false>(t[i], dst[i], u, ch);
+        });
+    });
+#else
+    static_for<NR>([&](auto II) {
+        constexpr int i = decltype(II)::value;
+        if constexpr (DIRB) stepB1_tail_range<C, 0, R, false>(t[i], dst[i], u, in_regs);
+        else stepA1_tail_range<C, 0, R, false>(t[i], dst[i], u, in_regs);
+    });
+#endif
+}
+// Scratch lines: one per team, plus one sink line per group (behind the group's team lines) when some lane of a group
+// can be without work in a pass (R1 != R2, or G not a multiple of TT).
+template <class C> struct PlaneGeom {
+    static constexpr int G = QM_GROUP, TPG = G / C::TT;
+    static constexpr bool SINK = (C::R1 != C::R2) || (G % C::TT != 0);
+    static constexpr int LPG = TPG + (SINK ? 1 : 0);     // scratch lines per group
 };
 template <class C> struct PlaneIds {
     static constexpr int G = QM_GROUP, TPG = G / C::TT;
     int grp, team, u, slot; bool team_ok;
+    int u1, u2;           // u clamped for passes with R1 / R2 butterflies per line
+    bool a1, a2;          // this lane has a butterfly in such a pass
+    int scr_line, sink_line;
     __device__ PlaneIds() {
         const int tid = threadIdx.x, gl = tid % G;
         grp = tid / G; team = gl / C::TT; u = gl % C::TT;
         team_ok = team < TPG;
         slot = qm_team_slot<C::TT, TPG>(team);
+        a1 = team_ok && u < C::R1; a2 = team_ok && u < C::R2;
+        u1 = u < C::R1 ? u : 0; u2 = u < C::R2 ? u : 0;
+        sink_line = grp * PlaneGeom<C>::LPG + (PlaneGeom<C>::SINK ? TPG : 0);
+        scr_line = grp * PlaneGeom<C>::LPG + (team_ok ? team : TPG);
     }
 };
 
@@ -192,12 +247,15 @@ __device__ __forceinline__ void plane_y_phase(const PlaneCtx cx, c128 *__restric
                                               const TwRow<C::R1> &twa, const TwRow<C::R2> &twb)
 {
     constexpr int G = QM_GROUP, TPG = G / C::TT, RP = C::L | 1, NPRE = 2 * Quarter<C>::Q;
+    constexpr int SL = qm_scratch_pitch(C::L, C::TT);
     constexpr bool HAS_BACK = MODE != 2, HAS_FWD = MODE != 1 && MODE != 3;
     const PlaneIds<C> id;
-    const int u = id.u, grp = id.grp, slot = id.slot, X = cx.X, n3 = cx.n3, quarter = cx.quarter & 1;
+    const int grp = id.grp, slot = id.slot, X = cx.X, n3 = cx.n3, quarter = cx.quarter & 1;
     const bool do_back = HAS_BACK && have_cur, do_fwd = HAS_FWD && prev >= 0;
     if (!(do_back || do_fwd)) return;
     const SLine As = qm_sline(cx.A);
+    // where a lane without work reads and writes: the scratch lines are idle during the y phase
+    const SLine junk = qm_sline(cx.scr + (size_t)id.scr_line * SL);
     const int pc = have_cur ? pl : 0, pp = prev >= 0 ? prev : 0;
     const WView Wcur = qm_wview(W + (size_t)(pc / n3) * cx.wband, pc % n3, n3);
     const WView Wprev = qm_wview(W + (size_t)(pp / n3) * cx.wband, pp % n3, n3);
@@ -205,48 +263,54 @@ __device__ __forceinline__ void plane_y_phase(const PlaneCtx cx, c128 *__restric
     // group barriers and NR independent load -> transform -> store chains between two barriers.
     constexpr int NR = QM_PLANE_YROWS;
     const int rstride = cx.ngroups * TPG;
-    for (int r0 = grp * TPG + slot; r0 - slot < X; r0 += NR * rstride) {
-        bool ok[NR];
+    for (int r0 = grp * TPG + slot; r0 - slot < X; r0 += NR * rstride) {      // same trip count for a whole group
         int sbase[NR];
         Pruned pr[NR];
         c128 pre[NR][NPRE];
+        SLine row1[NR], row2[NR];          // the row as seen by passes with R1 / R2 butterflies
 #pragma unroll
         for (int i = 0; i < NR; ++i) {
             const int r = r0 + i * rstride;
-            ok[i] = id.team_ok && r < X;
-            sbase[i] = 0;
-            pr[i] = Pruned{0u, 0u, 0, 0};
-            if (ok[i]) {
-                const int4 q = cx.rowinfo_s[r];
+            const bool ok = id.team_ok && r < X;
+            if (cx.rowtab_s) {
+                const int4 e = cx.rowtab_s[(ok ? r : 0) * C::TT + id.u];
+                sbase[i] = 0;
+                pr[i] = Pruned{(unsigned)e.x, (unsigned)e.y, e.z, e.w};
+                if (!ok) pr[i].m1 = pr[i].m2 = 0u;
+            } else {
+                const int4 q = cx.rowinfo_s[ok ? r : 0];
                 sbase[i] = q.z;
-                pr[i] = make_pruned_packed<C>(q.x, q.y, u, 1);
+                pr[i] = make_pruned_packed<C>(q.x, q.y, id.u2, 1);
+                if (!(ok && id.a2)) pr[i].m1 = pr[i].m2 = 0u;          // no global access at all
             }
-            if (do_back && quarter && ok[i]) prefetch_quarter<C>(Wcur + sbase[i], C::R2, pr[i], pre[i]);
+            row1[i] = (ok && id.a1) ? As + r * RP : junk;
+            row2[i] = (ok && id.a2) ? As + r * RP : junk;
+            if (do_back && quarter) prefetch_quarter<C>(Wcur + sbase[i], C::R2, pr[i], pre[i]);
         }
         if (do_fwd) {
+            c128 t[NR][C::R2];
 #pragma unroll
-            for (int i = 0; i < NR; ++i)
-                if (ok[i]) lineB_step1<C>(As + (r0 + i * rstride) * RP, u, twb);
+            for (int i = 0; i < NR; ++i) lineB_step1_head<C, false>(row1[i], id.u1, t[i]);
+            plane_tail<C, true>(t, row1, id.u1, twb, cx.tw_b);
             group_barrier<G>(grp);
-        }
 #pragma unroll
-        for (int i = 0; i < NR; ++i) {
-            const SLine Arow = As + (r0 + i * rstride) * RP;
-            if (do_fwd && ok[i]) {
-                if (quarter) prunedB_step2_quarter<C>(Arow, Wprev + sbase[i], C::R2, pr[i], u);
-                else prunedB_step2<C>(Arow, Wprev + sbase[i], C::R2, pr[i], u);
-            }
-            // the team that read the row in the step above is the one that refills it: no barrier needed
-            if (do_back && ok[i]) {
-                if (quarter) prunedA_step1_pre<C>(pre[i], Arow, u, twa);
-                else prunedA_step1<C>(Wcur + sbase[i], C::R2, pr[i], Arow, u, twa);
+            for (int i = 0; i < NR; ++i) {
+                if (quarter) prunedB_step2_quarter<C, false>(row2[i], Wprev + sbase[i], C::R2, pr[i], id.u2);
+                else prunedB_step2<C, false>(row2[i], Wprev + sbase[i], C::R2, pr[i], id.u2);
             }
         }
+        // the team that read the row in the step above is the one that refills it: no barrier needed
         if (do_back) {
+            c128 t[NR][C::R1];
+#pragma unroll
+            for (int i = 0; i < NR; ++i) {
+                if (quarter) prunedA_step1_pre_head<C, false>(pre[i], t[i], id.u2);
+                else prunedA_step1_head<C, false>(Wcur + sbase[i], C::R2, pr[i], t[i], id.u2);
+            }
+            plane_tail<C, false>(t, row2, id.u2, twa, cx.tw_a);
             group_barrier<G>(grp);
 #pragma unroll
-            for (int i = 0; i < NR; ++i)
-                if (ok[i]) lineA_step2<C>(As + (r0 + i * rstride) * RP, u);
+            for (int i = 0; i < NR; ++i) lineA_step2<C, false>(row1[i], id.u1);
         }
     }
 }
@@ -260,78 +324,83 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
     constexpr int G = QM_GROUP, TPG = G / C::TT, RP = C::L | 1;
     constexpr int SL = qm_scratch_pitch(C::L, C::TT);    // scratch line pitch
     const PlaneIds<C> id;
-    const int u = id.u, grp = id.grp, slot = id.slot, n3 = cx.n3, ngroups = cx.ngroups;
-    const bool team_ok = id.team_ok;
+    const int grp = id.grp, slot = id.slot, n3 = cx.n3, nteams = cx.ngroups * TPG;
     const bool xq = (cx.quarter & 2) != 0;               // quarter rule holds for the x rows: 2Q loads / stores per column
     const SLine As = qm_sline(cx.A);
-    const Pruned px = make_pruned<C>(x_iv.x, x_iv.y, x_iv.z, x_iv.w, u, RP);
+    const Pruned px = make_pruned<C>(x_iv.x, x_iv.y, x_iv.z, x_iv.w, id.u2, RP);
+    const Pruned pnone = Pruned{0u, 0u, 0, 0};
     const int band = pl / n3, p = pl - band * n3;
-    const SLine myscr = qm_sline(cx.scr + (size_t)(grp * TPG + id.team) * SL);
+    // a team's scratch line; lanes beyond the last team and lanes without a butterfly in a pass use the group's sink line
+    const SLine sink = qm_sline(cx.scr + (size_t)id.sink_line * SL);
+    const SLine teamscr = qm_sline(cx.scr + (size_t)id.scr_line * SL);
+    const SLine scrA[1] = {id.a2 ? teamscr : sink}, scrB[1] = {id.a1 ? teamscr : sink};
     const double *vplane = vt + (size_t)p * C::N * VLayout<C>::COL;
     VRow<C::R2> vr;
     // De-phase the groups: they all do identical load -> FP64 -> store bursts, and when they run in
     // lock step the shared-memory pipe and the FP64 pipe are used alternately instead of together.
     if (stagger_ns > 0) __nanosleep((unsigned)(grp * stagger_ns));
     const int col0 = grp * TPG + slot;
-    if constexpr (MODE == 0) {       // V of the first column: in flight while step 1 runs
-        if (team_ok && col0 < C::N) load_vrow<C>(vr, vplane + (size_t)col0 * VLayout<C>::COL, u);
-    }
+    auto vcol = [&](int c) { return vplane + (size_t)(c < C::N ? c : C::N - 1) * VLayout<C>::COL; };
+    if constexpr (MODE == 0) load_vrow<C>(vr, vcol(col0), id.u1);       // V of the first column: in flight while step 1 runs
     // Step-1 inputs of a column under the quarter rule: fetched one column ahead (before the barrier in front of the
     // previous column's step 3), so that their shared-memory latency hides behind that barrier and step 3.  Nobody else
     // touches a column of the plane array during the x phase: every column is owned by one team.
     constexpr bool XPRE = (MODE == 0 || MODE == 4) && QM_PLANE_XPREFETCH;
     c128 xpre[2 * Quarter<C>::Q];
     if constexpr (XPRE) {
-        if (xq && team_ok && col0 < C::N) prefetch_quarter<C>(As + C::pos(col0), C::R2 * RP, px, xpre);
+        if (xq) prefetch_quarter<C>(As + C::pos(col0), C::R2 * RP, (id.a2 && col0 < C::N) ? px : pnone, xpre);
     }
-    for (int col = col0; col - slot < C::N; col += ngroups * TPG) {
-        const bool ok = team_ok && col < C::N;
+    for (int col = col0; col - slot < C::N; col += nteams) {      // same trip count for a whole group
+        const bool ok = id.team_ok && col < C::N;
+        const int colc = col < C::N ? col : C::N - 1;    // a column that exists, for the addresses of lanes without one
         const SLine Acol = As + C::pos(col);
+        const Pruned pxc = (ok && id.a2) ? px : pnone;   // plane-array accesses of a lane without work are masked off
         if constexpr (MODE != 2) {
-            if (ok) {
-                if constexpr (XPRE) {
-                    if (xq) prunedA_step1_pre<C>(xpre, myscr, u, twa);
-                    else prunedA_step1<C>(Acol, C::R2 * RP, px, myscr, u, twa);
-                } else {
-                    if (xq) prunedA_step1_quarter<C>(Acol, C::R2 * RP, px, myscr, u, twa);
-                    else prunedA_step1<C>(Acol, C::R2 * RP, px, myscr, u, twa);
-                }
+            c128 t[1][C::R1];
+            if constexpr (XPRE) {
+                if (xq) prunedA_step1_pre_head<C, false>(xpre, t[0], id.u2);
+                else prunedA_step1_head<C, false>(Acol, C::R2 * RP, pxc, t[0], id.u2);
+            } else {
+                if (xq) {
+                    c128 pre[2 * Quarter<C>::Q];
+                    prefetch_quarter<C>(Acol, C::R2 * RP, pxc, pre);
+                    prunedA_step1_pre_head<C, false>(pre, t[0], id.u2);
+                } else prunedA_step1_head<C, false>(Acol, C::R2 * RP, pxc, t[0], id.u2);
             }
+            plane_tail<C, false>(t, scrA, id.u2, twa, cx.tw_a);
             group_barrier<G>(grp);
         }
         if constexpr (MODE == 3) {
             // scale = weight * occupation of this band; rhot = running density of this plane in the V layout
-            if (ok) xcol_density<C>(myscr, u, rhot + ((size_t)p * C::N + col) * VLayout<C>::COL, scale);
-        } else if (ok) {
+            if (ok) xcol_density<C>(teamscr, id.u, rhot + ((size_t)p * C::N + col) * VLayout<C>::COL, scale);
+        } else {
             // transposed boxes (fft_phases.cuh BoxT): column (p, col) of state `band`; with a second operand the plane
             // index counts pairs: band = a * npair2 + b, first operand state a, second operand state b (MODE 2)
             c128 *bx = nullptr;
             const c128 *bx2 = nullptr;
-            const size_t coloff = ((size_t)p * C::N + col) * C::N, boxsz = (size_t)C::N * C::N * n3;
+            const size_t coloff = ((size_t)p * C::N + colc) * C::N, boxsz = (size_t)C::N * C::N * n3;
             if constexpr (MODE == 1) bx = box + (size_t)band * boxsz + coloff;
             if constexpr (MODE == 2) {
                 bx = box + (size_t)(npair2 > 0 ? band / npair2 : band) * boxsz + coloff;
                 if (npair2 > 0) bx2 = box2 + (size_t)(band % npair2) * boxsz + coloff;
             }
             if constexpr (MODE == 4) bx2 = box2 + coloff;
-            xcol_step2<C, MODE>(myscr, u, twb, vr, bx, bx2, scale);
+            c128 t[1][C::R2];
+            xcol_step2_head<C, MODE, false>(scrB[0], id.u1, vr, bx, bx2, scale, t[0], ok && id.a1);
+            if constexpr (MODE != 1) plane_tail<C, true>(t, scrB, id.u1, twb, cx.tw_b);
         }
-        if constexpr (MODE == 0) {   // prefetch V of this team's next column behind steps 3 and 1
-            const int ncol = col + ngroups * TPG;
-            if (team_ok && ncol < C::N) load_vrow<C>(vr, vplane + (size_t)ncol * VLayout<C>::COL, u);
-        }
+        if constexpr (MODE == 0)     // prefetch V of this team's next column behind steps 3 and 1
+            load_vrow<C>(vr, vcol(col + nteams), id.u1);
         if constexpr (XPRE) {
-            const int ncol = col + ngroups * TPG;
-            if (xq && team_ok && ncol < C::N) prefetch_quarter<C>(As + C::pos(ncol), C::R2 * RP, px, xpre);
+            const int ncol = col + nteams;
+            if (xq) prefetch_quarter<C>(As + C::pos(ncol), C::R2 * RP, (id.a2 && ncol < C::N) ? px : pnone, xpre);
         }
         group_barrier<G>(grp);
         if constexpr (MODE != 1 && MODE != 3) {
             // no barrier after step 3: the scratch column a thread reads here is exactly the one it
             // overwrites in the next iteration's step 1 (MODE 2 has no step 1 and writes rows: barrier).
-            if (ok) {
-                if (xq) prunedB_step2_quarter<C>(myscr, Acol, C::R2 * RP, px, u);
-                else prunedB_step2<C>(myscr, Acol, C::R2 * RP, px, u);
-            }
+            if (xq) prunedB_step2_quarter<C, false>(scrA[0], Acol, C::R2 * RP, pxc, id.u2);
+            else prunedB_step2<C, false>(scrA[0], Acol, C::R2 * RP, pxc, id.u2);
             if constexpr (MODE == 2) group_barrier<G>(grp);
         }
     }
@@ -353,9 +422,21 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
     cx.wband = (size_t)((kp.nsticks + QM_ZT - 1) / QM_ZT) * QM_ZT * gd.ax[2].n;   // W elements per band
     cx.A = reinterpret_cast<c128 *>(smem_raw);
     cx.scr = cx.A + (((size_t)cx.X * RP + 7) & ~(size_t)7);
-    int4 *rowinfo_s = reinterpret_cast<int4 *>(cx.scr + (size_t)ngroups * TPG * SL);
+    int4 *rowinfo_s = reinterpret_cast<int4 *>(cx.scr + (size_t)ngroups * PlaneGeom<C>::LPG * SL);
     cx.rowinfo_s = rowinfo_s;
     for (int i = threadIdx.x; i < cx.X; i += blockDim.x) rowinfo_s[i] = kp.row_info[i];
+    // (quarter & 4): room for the hoisted y addressing of every (row, u), worked out once per kernel
+    int4 *rowtab_s = rowinfo_s + cx.X + 1;                 // one int4 in between holds the tensor-memory base address
+    cx.rowtab_s = (quarter & 4) ? rowtab_s : nullptr;
+    if (quarter & 4) {
+        for (int i = threadIdx.x; i < cx.X * C::TT; i += blockDim.x) {
+            const int r = i / C::TT, uu = i % C::TT;
+            const int4 q = kp.row_info[r];
+            Pruned pr = make_pruned_packed<C>(q.x, q.y, uu < C::R2 ? uu : 0, 1);
+            if (uu >= C::R2) pr.m1 = pr.m2 = 0u;
+            rowtab_s[i] = int4{(int)pr.m1, (int)pr.m2, pr.c1 + q.z, pr.c2 + q.z};
+        }
+    }
     __syncthreads();
     // per-thread twiddle rows, loaded once (u is fixed for the whole kernel)
     const int u_tw = (int)(threadIdx.x % G) % C::TT;
@@ -366,6 +447,24 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
     const auto &twb = [&]() -> const TwRow<C::R2> & {
         if constexpr (C::R1 == C::R2) return twa; else return twb_store;
     }();
+    cx.tw_a = cx.tw_b = 0;
+#if QM_PLANE_TW_TMEM
+    // ... and parked in tensor memory: 4 columns per factor in the warp's lane window, one column range per warp of an
+    // SM sub-partition (warps w, w+4, w+8, ... share a lane window)
+    constexpr int ROWCOLS = 4 * C::R1 + (C::R1 != C::R2 ? 4 * C::R2 : 0);
+    uint32_t &tmem_base_s = *reinterpret_cast<uint32_t *>(rowinfo_s + cx.X);      // the 16 bytes behind the row table
+    const uint32_t tmem_cols = (uint32_t)qm_tmem_cols_pow2(ROWCOLS * (int)((blockDim.x / 32 + 3) / 4));
+    if (threadIdx.x < 32) tmem_alloc(&tmem_base_s, tmem_cols);
+    tmem_fence_before_sync();
+    __syncthreads();
+    tmem_fence_after_sync();
+    const uint32_t tmem_base = tmem_base_s;
+    cx.tw_a = tmem_warp_addr(tmem_base, 0, ROWCOLS);
+    cx.tw_b = C::R1 != C::R2 ? cx.tw_a + 4 * C::R1 : cx.tw_a;
+    tmem_store_row(cx.tw_a, twa);
+    if constexpr (C::R1 != C::R2) tmem_store_row(cx.tw_b, twb_store);
+    tmem_wait_st();
+#endif
     const int n3 = cx.n3;
     // plane sequence of this CTA.  Apply / debug modes: pl = blockIdx.x, + gridDim.x, ... (pl = band * n3 + p).
     // Density mode: the CTA owns z-planes p = blockIdx.x, + gridDim.x, ... and walks ALL bands of a plane before
@@ -392,4 +491,9 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
         __syncthreads();
         prev = pl;
     }
+#if QM_PLANE_TW_TMEM
+    tmem_fence_before_sync();
+    __syncthreads();
+    if (threadIdx.x < 32) tmem_dealloc(tmem_base, tmem_cols);
+#endif
 }

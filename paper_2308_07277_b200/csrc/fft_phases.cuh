@@ -147,10 +147,39 @@ template <class C> QM_HD Pruned make_pruned_packed(int x, int y, int u, int stri
 // of the line, estride = R2*stride (elements between n and n+1); writes the full padded line `dst`.
 // Interval 1 lies below N/2 and interval 2 at or above it (host tables), so for most n the interval is known at
 // compile time and the access is base + immediate under one mask-bit test.
-template <class C, class P, class L, class TW>
-QM_HD void prunedA_step1(const P src, int estride, const Pruned pr, const L dst, int u, const TW &tw) {
-    if (u >= C::R2) return;
-    c128 t[C::R1];
+// Every first pass is written as a head (loads + radix-R butterflies into t[]) and a tail (twiddle multiply + store), so
+// that a caller may fetch the twiddle row between the two (tmem_rows.cuh); the one-call forms below do both.
+// The tails take the factors j in [J0, J1) of the row at a time (TwChunk: a window of a row), so that a row that is not
+// held in registers can be brought in piecewise.
+template <int J0, int J1> struct TwChunk {
+    c128 w[J1 - J0];
+    template <int J> QM_HD c128 get() const { static_assert(J >= J0 && J < J1, "factor outside the chunk"); return w[J - J0]; }
+};
+template <class C, int J0, int J1, bool GUARD = true, class L, class TW>
+QM_HD void stepA1_tail_range(const c128 (&t)[C::R1], const L dst, int u, const TW &tw) {
+    if constexpr (GUARD) if (u >= C::R2) return;
+    static_for<J1 - J0>([&](auto I) {
+        constexpr int k1 = J0 + decltype(I)::value;
+        if constexpr (k1 == 0) dst[u] = t[0];
+        else dst[k1 * C::R2P + u] = cmul_conj(t[k1], tw.template get<k1>());
+    });
+}
+template <class C, int J0, int J1, bool GUARD = true, class L, class TW>
+QM_HD void stepB1_tail_range(const c128 (&t)[C::R2], const L line, int u, const TW &tw) {
+    if constexpr (GUARD) if (u >= C::R1) return;
+    static_for<J1 - J0>([&](auto I) {
+        constexpr int d = J0 + decltype(I)::value;
+        if constexpr (d == 0) line[u * C::R2P] = t[0];
+        else line[u * C::R2P + d] = cmul(t[d], tw.template get<d>());
+    });
+}
+template <class C, class L, class TW>
+QM_HD void stepA1_tail(const c128 (&t)[C::R1], const L dst, int u, const TW &tw) { stepA1_tail_range<C, 0, C::R1>(t, dst, u, tw); }
+template <class C, class L, class TW>
+QM_HD void stepB1_tail(const c128 (&t)[C::R2], const L line, int u, const TW &tw) { stepB1_tail_range<C, 0, C::R2>(t, line, u, tw); }
+template <class C, bool GUARD = true, class P>
+QM_HD void prunedA_step1_head(const P src, int estride, const Pruned pr, c128 (&t)[C::R1], int u) {
+    if constexpr (GUARD) if (u >= C::R2) return;
     const P p1 = src + pr.c1, p2 = src + pr.c2;
     const unsigned mm = pr.m1 | pr.m2;
     static_for<C::R1>([&](auto I) {
@@ -163,10 +192,12 @@ QM_HD void prunedA_step1(const P src, int estride, const Pruned pr, const L dst,
         }
     });
     Dft<C::R1, +1>::run(t);
-    static_for<C::R1>([&](auto I) {
-        constexpr int k1 = decltype(I)::value;
-        dst[k1 * C::R2P + u] = (k1 == 0) ? t[k1] : cmul_conj(t[k1], tw.template get<k1>());
-    });
+}
+template <class C, class P, class L, class TW>
+QM_HD void prunedA_step1(const P src, int estride, const Pruned pr, const L dst, int u, const TW &tw) {
+    c128 t[C::R1];
+    prunedA_step1_head<C>(src, estride, pr, t, u);
+    stepA1_tail<C>(t, dst, u, tw);
 }
 // "Quarter" form of the pruned backward step 1: when every occupied index lies below N/4 or at/above 3N/4
 // (true for every alias-free grid, 4 m + 1 <= n), only the first Q and the last Q first-pass inputs of a thread
@@ -183,11 +214,10 @@ QM_HD void prefetch_quarter(const P src, int estride, const Pruned pr, c128 (&pr
         pre[Q + j] = ld_pred(p2 + (C::R1 - Q + j) * estride, (pr.m2 >> (C::R1 - Q + j)) & 1u);
     });
 }
-template <class C, class L, class TW>
-QM_HD void prunedA_step1_pre(const c128 (&pre)[2 * Quarter<C>::Q], const L dst, int u, const TW &tw) {
-    if (u >= C::R2) return;
+template <class C, bool GUARD = true>
+QM_HD void prunedA_step1_pre_head(const c128 (&pre)[2 * Quarter<C>::Q], c128 (&t)[C::R1], int u) {
+    if constexpr (GUARD) if (u >= C::R2) return;
     constexpr int Q = Quarter<C>::Q;
-    c128 t[C::R1];
     static_for<C::R1>([&](auto I) {
         constexpr int n1 = decltype(I)::value;
         if constexpr (n1 < Q) t[n1] = pre[n1];
@@ -195,10 +225,12 @@ QM_HD void prunedA_step1_pre(const c128 (&pre)[2 * Quarter<C>::Q], const L dst, 
         else t[n1] = c128{0.0, 0.0};
     });
     DftQuarterIn<C::R1, +1>::run(t);
-    static_for<C::R1>([&](auto I) {
-        constexpr int k1 = decltype(I)::value;
-        dst[k1 * C::R2P + u] = (k1 == 0) ? t[k1] : cmul_conj(t[k1], tw.template get<k1>());
-    });
+}
+template <class C, class L, class TW>
+QM_HD void prunedA_step1_pre(const c128 (&pre)[2 * Quarter<C>::Q], const L dst, int u, const TW &tw) {
+    c128 t[C::R1];
+    prunedA_step1_pre_head<C>(pre, t, u);
+    stepA1_tail<C>(t, dst, u, tw);
 }
 template <class C, class P, class L, class TW>
 QM_HD void prunedA_step1_quarter(const P src, int estride, const Pruned pr, const L dst, int u, const TW &tw) {
@@ -208,9 +240,9 @@ QM_HD void prunedA_step1_quarter(const P src, int estride, const Pruned pr, cons
     prunedA_step1_pre<C>(pre, dst, u, tw);
 }
 // Forward step 2 with pruned output: reads the full padded line `srcline`, stores only what exists.
-template <class C, class L, class P>
+template <class C, bool GUARD = true, class L, class P>
 QM_HD void prunedB_step2(const L srcline, const P dst, int estride, const Pruned pr, int u) {
-    if (u >= C::R2) return;
+    if constexpr (GUARD) if (u >= C::R2) return;
     c128 t[C::R1];
     static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = srcline[a * C::R2P + u]; });
     Dft<C::R1, -1>::run(t);
@@ -227,9 +259,9 @@ QM_HD void prunedB_step2(const L srcline, const P dst, int estride, const Pruned
     });
 }
 // Quarter-rule form of the pruned forward step 2: only the first Q and last Q outputs of a thread can exist.
-template <class C, class L, class P>
+template <class C, bool GUARD = true, class L, class P>
 QM_HD void prunedB_step2_quarter(const L srcline, const P dst, int estride, const Pruned pr, int u) {
-    if (u >= C::R2) return;
+    if constexpr (GUARD) if (u >= C::R2) return;
     constexpr int Q = Quarter<C>::Q;
     c128 t[C::R1];
     static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = srcline[a * C::R2P + u]; });
@@ -244,22 +276,22 @@ QM_HD void prunedB_step2_quarter(const L srcline, const P dst, int estride, cons
 }
 
 // ---- full (unpruned) in-place passes ---------------------------------------------------------------------
-template <class C, class L> QM_HD void lineA_step2(const L line, int u) {
-    if (u >= C::R1) return;
+template <class C, bool GUARD = true, class L> QM_HD void lineA_step2(const L line, int u) {
+    if constexpr (GUARD) if (u >= C::R1) return;
     c128 t[C::R2];
     static_for<C::R2>([&](auto I) { constexpr int n2 = decltype(I)::value; t[n2] = line[u * C::R2P + n2]; });
     Dft<C::R2, +1>::run(t);
     static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; line[u * C::R2P + k2] = t[k2]; });
 }
-template <class C, class L, class TW> QM_HD void lineB_step1(const L line, int u, const TW &tw) {
-    if (u >= C::R1) return;
-    c128 t[C::R2];
+template <class C, bool GUARD = true, class L> QM_HD void lineB_step1_head(const L line, int u, c128 (&t)[C::R2]) {
+    if constexpr (GUARD) if (u >= C::R1) return;
     static_for<C::R2>([&](auto I) { constexpr int b = decltype(I)::value; t[b] = line[u * C::R2P + b]; });
     Dft<C::R2, -1>::run(t);
-    static_for<C::R2>([&](auto I) {
-        constexpr int d = decltype(I)::value;
-        line[u * C::R2P + d] = (d == 0) ? t[d] : cmul(t[d], tw.template get<d>());
-    });
+}
+template <class C, class L, class TW> QM_HD void lineB_step1(const L line, int u, const TW &tw) {
+    c128 t[C::R2];
+    lineB_step1_head<C>(line, u, t);
+    stepB1_tail<C>(t, line, u, tw);
 }
 
 // ---- z kernels: one shared-memory round trip per stick ------------------------------------------------
@@ -378,10 +410,14 @@ template <class C> QM_HD void load_vrow(VRow<C::R2> &vr, const double *vcol, int
         if constexpr (2 * j + 1 < C::R2) vr.v[2 * j + 1] = d.y;
     });
 }
-template <class C, int MODE, class L, class TW>
-QM_HD void xcol_step2(const L scr, int u, const TW &tw, const VRow<C::R2> &vr, c128 *box, const c128 *box2, double scale) {
-    if (u >= C::R1) return;
-    c128 t[C::R2];
+// head: everything up to the forward radix pass (returns false in MODE 1, which stops after the backward transform);
+// tail: stepB1_tail on the scratch line.
+// `act` = false: a lane that stands in for nothing (GUARD = false callers): it computes on whatever it was pointed at and
+// must not store to global memory.
+template <class C, int MODE, bool GUARD = true, class L>
+QM_HD void xcol_step2_head(const L scr, int u, const VRow<C::R2> &vr, c128 *box, const c128 *box2, double scale, c128 (&t)[C::R2],
+                           bool act = true) {
+    if constexpr (GUARD) if (u >= C::R1) return;
     if constexpr (MODE == 2) {
         static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; t[k2] = box[u + C::R1 * k2]; });
         if (box2) static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; t[k2] = cmul_conj(t[k2], box2[u + C::R1 * k2]); });
@@ -391,7 +427,7 @@ QM_HD void xcol_step2(const L scr, int u, const TW &tw, const VRow<C::R2> &vr, c
         static_for<C::R2>([&](auto I) { constexpr int n2 = decltype(I)::value; t[n2] = scr[u * C::R2P + n2]; });
         Dft<C::R2, +1>::run(t);                      // t[k2] = psi(x = u + R1*k2)
         if constexpr (MODE == 1) {
-            static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; box[u + C::R1 * k2] = cscale(t[k2], scale); });
+            if (act) static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; box[u + C::R1 * k2] = cscale(t[k2], scale); });
             return;
         } else if constexpr (MODE == 4) {
             static_for<C::R2>([&](auto I) { constexpr int k2 = decltype(I)::value; t[k2] = cmul(t[k2], f[k2]); });
@@ -400,10 +436,12 @@ QM_HD void xcol_step2(const L scr, int u, const TW &tw, const VRow<C::R2> &vr, c
         }
     }
     Dft<C::R2, -1>::run(t);
-    static_for<C::R2>([&](auto I) {
-        constexpr int d = decltype(I)::value;
-        scr[u * C::R2P + d] = (d == 0) ? t[d] : cmul(t[d], tw.template get<d>());
-    });
+}
+template <class C, int MODE, class L, class TW>
+QM_HD void xcol_step2(const L scr, int u, const TW &tw, const VRow<C::R2> &vr, c128 *box, const c128 *box2, double scale) {
+    c128 t[C::R2];
+    xcol_step2_head<C, MODE>(scr, u, vr, box, box2, scale, t);
+    if constexpr (MODE != 1) stepB1_tail<C>(t, scr, u, tw);
 }
 // MODE 3 of the plane kernel (density, eq. 2): backward step 2, then rho(x) += w |psi(x)|^2 on this
 // thread's R2 points.  The running density of a plane column is kept in the V layout (VLayout), so the read-modify-

@@ -170,12 +170,18 @@ struct qm_batch_plan {
 };
 
 constexpr int PLANE_GROUP = QM_GROUP;
+inline size_t plane_rowtab_bytes(const qm_gspace *g, const KPoint *kp) {
+    return (size_t)kp->nx * std::max(g->ax[0].r1, g->ax[0].r2) * sizeof(int4);
+}
 inline size_t plane_smem(const qm_gspace *g, const KPoint *kp, int ngroups) {
     const QmAxis &ax = g->ax[0];
-    const size_t sl = (size_t)qm_scratch_pitch(ax.len, std::max(ax.r1, ax.r2));
-    const int tpg = PLANE_GROUP / std::max(ax.r1, ax.r2);
+    const int tt = std::max(ax.r1, ax.r2);
+    const size_t sl = (size_t)qm_scratch_pitch(ax.len, tt);
+    // scratch lines per group: one per team, plus a sink line when some lanes of a group have no butterfly in a pass
+    // (fft_kernels.cuh PlaneGeom)
+    const int lpg = PLANE_GROUP / tt + ((ax.r1 != ax.r2 || PLANE_GROUP % tt != 0) ? 1 : 0);
     const size_t a_elems = ((size_t)kp->nx * kp->rowpitch + 7) & ~(size_t)7;
-    return (a_elems + (size_t)ngroups * tpg * sl) * sizeof(c128) + (size_t)kp->nx * sizeof(int4) + 16;
+    return (a_elems + (size_t)ngroups * lpg * sl) * sizeof(c128) + (size_t)kp->nx * sizeof(int4) + 16;
 }
 
 // number of independent groups of the plane kernel: the fewest groups that reach the

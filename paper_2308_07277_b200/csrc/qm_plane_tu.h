@@ -12,10 +12,21 @@ template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *W,
     // barriers and the load / compute / store phases of one CTA overlap the other's work
     int cps = MODE == 3 ? 1 : (g->plane_ctas_per_sm > 0 ? g->plane_ctas_per_sm : 1);
     int ngroups = plane_groups(g, kp, cps);
+#if QM_PLANE_TW_TMEM
+    // every resident CTA allocates its own tensor-memory columns (512 per SM): one CTA per SM if two do not fit
+    if (cps > 1 && ngroups > 0) {
+        const int rowcols = 4 * C::R1 + (C::R1 != C::R2 ? 4 * C::R2 : 0);
+        if (cps * qm_tmem_cols_pow2(rowcols * ((ngroups * PLANE_GROUP / 32 + 3) / 4)) > 512) ngroups = 0;
+    }
+#endif
     if (ngroups == 0) { cps = 1; ngroups = plane_groups(g, kp, 1); }
-    const size_t smem = plane_smem(g, kp, ngroups);
+    size_t smem = plane_smem(g, kp, ngroups);
     if (ngroups == 0 || smem > (size_t)g->max_smem)
         return fail(QM_EGRID, "plane kernel does not fit shared memory for this grid / sphere");
+    // the per-(row, u) addressing table of the y phase, when there is room for it beside the plane array
+    const size_t budget = cps == 1 ? (size_t)g->max_smem : ((size_t)g->max_smem + 1024) / cps - 1024;
+    const bool rowtab = smem + plane_rowtab_bytes(g, kp) <= budget;
+    if (rowtab) smem += plane_rowtab_bytes(g, kp);
     QmGridDev gd;
     for (int i = 0; i < 3; ++i) { gd.ax[i] = g->ax[i]; gd.tw[i] = g->d_tw[i].p; }
     gd.vt = g->d_vt.p;
@@ -25,7 +36,7 @@ template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *W,
     g->prof.begin(QM_K_PLANE, st);
     k_plane<C, MODE><<<grid, ngroups * PLANE_GROUP, smem, st>>>(kp->plan(), gd, W, a.box, a.box2, a.npair2, ngroups, a.scale,
                                                                    g->plane_stagger_ns, nplanes,
-                                                                   (kp->y_quarter ? 1 : 0) | (kp->x_quarter ? 2 : 0), a.occ, a.rhot);
+                                                                   (kp->y_quarter ? 1 : 0) | (kp->x_quarter ? 2 : 0) | (rowtab ? 4 : 0), a.occ, a.rhot);
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
