@@ -37,18 +37,27 @@ __device__ __forceinline__ double2 ldg_c128(const c128 *p) {
 #ifndef QM_P1_KS
 #define QM_P1_KS 16         /* K slice per stage of GEMM 1 */
 #endif
+// NB = bands per GEMM call (the N of both GEMMs): 16 at the configs' call batch of 16; 32 when the caller hands over
+// more bands at once (beta is then streamed once per 32 bands and both GEMMs become tensor-pipe bound).
 constexpr int P1_ROWS = QM_P1_ROWS, P1_KS = QM_P1_KS, P1_CW = P1_ROWS / 16, P1_ST = QM_P1_STAGES, P1_OCC = QM_P1_OCC,
-              P1_PSI_PITCH = P1_KS + 4, P_NB = 16;
+              P1_PSI_PITCH = P1_KS + 4, P_NB = 16, P_NB_MAX = 32;
 constexpr int P1_BETA_BYTES = P1_ROWS * P1_KS * 16;                 // 32768
-constexpr int P1_PSI_BYTES = P_NB * P1_PSI_PITCH * 16;              // 5120
-constexpr int P1_STAGE_BYTES = P1_BETA_BYTES + P1_PSI_BYTES;
-constexpr int P1_SMEM = P1_ST * P1_STAGE_BYTES + 2 * P1_ST * 8 + 16;
-constexpr int P2_G = 64, P2_KS = 16, P2_CW = 4, P2_ST = 4, P2_Q_PITCH = 20;
+template <int NB> struct P1Cfg {
+    static constexpr int PSI_BYTES = NB * P1_PSI_PITCH * 16;       // 5120 (NB = 16)
+    static constexpr int STAGE_BYTES = P1_BETA_BYTES + PSI_BYTES;
+    static constexpr int SMEM = P1_ST * STAGE_BYTES + 2 * P1_ST * 8 + 16;
+};
+constexpr int P2_G = 64, P2_KS = 16, P2_CW = 4;
 constexpr int P2_BETA_BYTES = P2_KS * P2_G * 16;                    // 16384
-constexpr int P2_Q_DOUBLES = 3 * P2_KS * P2_Q_PITCH;                // 960
-constexpr int P2_Q_BYTES = P2_Q_DOUBLES * 8;                        // 7680
-constexpr int P2_STAGE_BYTES = P2_BETA_BYTES + P2_Q_BYTES;
-constexpr int P2_SMEM = P2_ST * P2_STAGE_BYTES + 2 * P2_ST * 8 + 16;
+template <int NB> struct P2Cfg {
+    static constexpr int ST = NB <= 16 ? 4 : 3;                     // ring stages (two CTAs per SM must fit)
+    static constexpr int Q_PITCH = NB + 4;                          // doubles per projector row of a Q plane
+    static constexpr int Q_DOUBLES = 3 * P2_KS * Q_PITCH;           // planes (Qr, Qi, Qr+Qi): 960 (NB = 16)
+    static constexpr int Q_BYTES = Q_DOUBLES * 8;
+    static constexpr int STAGE_BYTES = P2_BETA_BYTES + Q_BYTES;
+    static constexpr int SMEM = ST * STAGE_BYTES + 2 * ST * 8 + 16;
+    static constexpr int PART = NB * P2_G;                          // c128 per partial tile
+};
 
 __device__ __forceinline__ double2 lds_c128(const unsigned char *base, int byte_off) {
     return *reinterpret_cast<const double2 *>(base + byte_off);
@@ -82,27 +91,29 @@ __global__ void k_tile_beta2(const c128 *__restrict__ src, int ng, int nproj, c1
     }
 }
 
-// GEMM 1:  Ppart[split][row][n] = sum_{k in split} conj(beta[row][k]) psi[band0+n][k]
+// GEMM 1:  Ppart[split][row][n] = sum_{k in split} conj(beta[row][k]) psi[band0+n][k],  n < NB
+template <int NB>
 __global__ void __launch_bounds__((P1_CW + 1) * 32, P1_OCC)
 k_proj1_pipe(const c128 *__restrict__ beta1, int nkc, const c128 *__restrict__ psi, int ng, int nb, int band0,
              c128 *__restrict__ Ppart, int nrows_pad, int nsplit)
 {
     extern __shared__ __align__(128) unsigned char smem[];
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem + P1_ST * P1_STAGE_BYTES);
+    constexpr int STAGE = P1Cfg<NB>::STAGE_BYTES, PSI_BYTES = P1Cfg<NB>::PSI_BYTES, NJ = NB / 8;
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + P1_ST * STAGE);
     uint64_t *empty = full + P1_ST;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int mb = blockIdx.x, split = blockIdx.y;
     const int kc0 = (int)((long long)split * nkc / nsplit), kc1 = (int)((long long)(split + 1) * nkc / nsplit);
     const int nit = kc1 - kc0;
-    const int nvalid = min(P_NB, nb - band0);
+    const int nvalid = min(NB, nb - band0);
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < P1_ST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], P1_CW); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int s = 0; s < P1_ST; ++s) {       // rows of bands that do not exist stay zero for the whole kernel
-        double2 *pz = reinterpret_cast<double2 *>(smem + s * P1_STAGE_BYTES + P1_BETA_BYTES);
-        for (int i = threadIdx.x; i < P1_PSI_BYTES / 16; i += blockDim.x) pz[i] = make_double2(0.0, 0.0);
+        double2 *pz = reinterpret_cast<double2 *>(smem + s * STAGE + P1_BETA_BYTES);
+        for (int i = threadIdx.x; i < PSI_BYTES / 16; i += blockDim.x) pz[i] = make_double2(0.0, 0.0);
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
@@ -112,7 +123,7 @@ k_proj1_pipe(const c128 *__restrict__ beta1, int nkc, const c128 *__restrict__ p
         for (int it = 0; it < nit; ++it) {
             const int s = it % P1_ST;
             if (it >= P1_ST) mbar_wait(&empty[s], ((it / P1_ST) - 1) & 1);
-            unsigned char *stage = smem + s * P1_STAGE_BYTES;
+            unsigned char *stage = smem + s * STAGE;
             const int kc = kc0 + it;
             const int nk = min(P1_KS, ng - kc * P1_KS);
             if (nk < P1_KS && lane < nvalid) {          // ragged K tail: clear what the short copy will not write
@@ -131,41 +142,42 @@ k_proj1_pipe(const c128 *__restrict__ beta1, int nkc, const c128 *__restrict__ p
                          psi + (size_t)(band0 + lane) * ng + (size_t)kc * P1_KS, (uint32_t)(nk * 16), &full[s]);
         }
     } else {
-        // ---- consumer warps: rows 16*warp .. 16*warp+15, all 16 bands ----
+        // ---- consumer warps: rows 16*warp .. 16*warp+15, all NB bands ----
         const int r8 = lane >> 2, c = lane & 3;
-        double t1[2][2][2], t2[2][2][2], t3[2][2][2];
+        double t1[2][NJ][2], t2[2][NJ][2], t3[2][NJ][2];
 #pragma unroll
         for (int i = 0; i < 2; ++i)
 #pragma unroll
-            for (int j = 0; j < 2; ++j)
+            for (int j = 0; j < NJ; ++j)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) { t1[i][j][e] = 0.0; t2[i][j][e] = 0.0; t3[i][j][e] = 0.0; }
-        int aoff[2], boff[2];
+        int aoff[2];
 #pragma unroll
         for (int i = 0; i < 2; ++i) aoff[i] = ((warp * 16 + i * 8 + r8) * P1_KS) * 16;
-#pragma unroll
-        for (int j = 0; j < 2; ++j) boff[j] = P1_BETA_BYTES + ((j * 8 + r8) * P1_PSI_PITCH + c) * 16;
+        const int boff = P1_BETA_BYTES + (r8 * P1_PSI_PITCH + c) * 16;
         const int sw = (r8 & 1) << 2;
         for (int it = 0; it < nit; ++it) {
             const int s = it % P1_ST;
             mbar_wait(&full[s], (it / P1_ST) & 1);
-            const unsigned char *stage = smem + s * P1_STAGE_BYTES;
+            const unsigned char *stage = smem + s * STAGE;
 #pragma unroll
             for (int kk = 0; kk < P1_KS / 4; ++kk) {
-                double2 a[2], b[2];
+                double2 a[2], b[NJ];
 #pragma unroll
                 for (int i = 0; i < 2; ++i) a[i] = lds_c128(stage, aoff[i] + (((4 * kk) ^ sw) + c) * 16);
 #pragma unroll
-                for (int j = 0; j < 2; ++j) b[j] = lds_c128(stage, boff[j] + 4 * kk * 16);
+                for (int j = 0; j < NJ; ++j) b[j] = lds_c128(stage, boff + (j * 8 * P1_PSI_PITCH + 4 * kk) * 16);
+                double bs[NJ];
+#pragma unroll
+                for (int j = 0; j < NJ; ++j) bs[j] = b[j].x + b[j].y;
 #pragma unroll
                 for (int i = 0; i < 2; ++i) {
                     const double as = a[i].x - a[i].y;
 #pragma unroll
-                    for (int j = 0; j < 2; ++j) {
-                        const double bs = b[j].x + b[j].y;
+                    for (int j = 0; j < NJ; ++j) {
                         dmma884(t1[i][j][0], t1[i][j][1], a[i].x, b[j].x);
                         dmma884(t2[i][j][0], t2[i][j][1], a[i].y, b[j].y);
-                        dmma884(t3[i][j][0], t3[i][j][1], as, bs);
+                        dmma884(t3[i][j][0], t3[i][j][1], as, bs[j]);
                     }
                 }
             }
@@ -173,21 +185,21 @@ k_proj1_pipe(const c128 *__restrict__ beta1, int nkc, const c128 *__restrict__ p
             if (lane == 0) mbar_arrive(&empty[s]);
         }
         // conj(a) b:  re = T1 + T2,  im = T3 - T1 + T2
-        c128 *P = Ppart + (size_t)split * nrows_pad * P_NB;
+        c128 *P = Ppart + (size_t)split * nrows_pad * NB;
 #pragma unroll
         for (int i = 0; i < 2; ++i)
 #pragma unroll
-            for (int j = 0; j < 2; ++j) {
+            for (int j = 0; j < NJ; ++j) {
                 const int row = mb * P1_ROWS + warp * 16 + i * 8 + r8, col = j * 8 + 2 * c;
 #pragma unroll
                 for (int e = 0; e < 2; ++e)
-                    P[(size_t)row * P_NB + col + e] =
+                    P[(size_t)row * NB + col + e] =
                         c128{t1[i][j][e] + t2[i][j][e], t3[i][j][e] - t1[i][j][e] + t2[i][j][e]};
             }
     }
 }
 
-// Q tiles for GEMM 2: qt[ic][plane][16][20], planes (Qr, Qi, Qr+Qi);  Q = D * (sum of the split partials)
+// Q tiles for GEMM 2: qt[ic][plane][16][NB + 4], planes (Qr, Qi, Qr+Qi);  Q = D * (sum of the split partials)
 __global__ void k_reduce_p2(const c128 *__restrict__ Ppart, int nsplit, int count, c128 *__restrict__ P)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -199,37 +211,41 @@ __global__ void k_reduce_p2(const c128 *__restrict__ Ppart, int nsplit, int coun
     }
     P[i] = c128{sr, si};
 }
+template <int NB>
 __global__ void k_dmul_tiles(const double *__restrict__ D, int db, int nproj, int nic, const c128 *__restrict__ P,
                              double *__restrict__ qt)
 {
+    constexpr int QP = P2Cfg<NB>::Q_PITCH;
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= nic * P2_KS * P_NB) return;
-    const int i = idx / P_NB, n = idx % P_NB;
+    if (idx >= nic * P2_KS * NB) return;
+    const int i = idx / NB, n = idx % NB;
     double sr = 0.0, si = 0.0;
     if (i < nproj) {
         const int blk = i / db, ii = i % db;
         const double *d = D + ((size_t)blk * db + ii) * db;
         for (int j = 0; j < db; ++j) {
-            const double2 v = ldg_c128(P + (size_t)(blk * db + j) * P_NB + n);
+            const double2 v = ldg_c128(P + (size_t)(blk * db + j) * NB + n);
             sr += d[j] * v.x; si += d[j] * v.y;
         }
     }
-    double *t = qt + (size_t)(i / P2_KS) * P2_Q_DOUBLES + (i % P2_KS) * P2_Q_PITCH + n;
-    t[0] = sr; t[P2_KS * P2_Q_PITCH] = si; t[2 * P2_KS * P2_Q_PITCH] = sr + si;
+    double *t = qt + (size_t)(i / P2_KS) * P2Cfg<NB>::Q_DOUBLES + (i % P2_KS) * QP + n;
+    t[0] = sr; t[P2_KS * QP] = si; t[2 * P2_KS * QP] = sr + si;
 }
 
 // Fused split-K reduction + D multiply for block sizes that divide 16 (every BASELINE.json config has 4x4 blocks):
-// a CTA owns 16 projector rows x 16 bands, sums the split partials in a fixed order (deterministic), keeps P in
+// a CTA owns 16 projector rows x NB bands, sums the split partials in a fixed order (deterministic), keeps P in
 // shared memory and writes the Q tiles (Qr, Qi, Qr+Qi) GEMM 2 consumes.
-__global__ void __launch_bounds__(256)
+template <int NB>
+__global__ void __launch_bounds__(16 * NB)
 k_reduce_dmul(const c128 *__restrict__ Ppart, int nsplit, int nrows_pad, const double *__restrict__ D, int db, int nproj,
               double *__restrict__ qt)
 {
-    __shared__ double2 Ps[16][P_NB + 1];
-    const int n = threadIdx.x % P_NB, rl = threadIdx.x / P_NB;
+    constexpr int QP = P2Cfg<NB>::Q_PITCH;
+    __shared__ double2 Ps[16][NB + 1];
+    const int n = threadIdx.x % NB, rl = threadIdx.x / NB;
     const int row = blockIdx.x * 16 + rl;
-    const size_t count = (size_t)nrows_pad * P_NB;
-    const c128 *src = Ppart + (size_t)row * P_NB + n;
+    const size_t count = (size_t)nrows_pad * NB;
+    const c128 *src = Ppart + (size_t)row * NB + n;
     double sr[4] = {0.0, 0.0, 0.0, 0.0}, si[4] = {0.0, 0.0, 0.0, 0.0};
     int s = 0;
     for (; s + 4 <= nsplit; s += 4) {
@@ -245,8 +261,8 @@ k_reduce_dmul(const c128 *__restrict__ Ppart, int nsplit, int nrows_pad, const d
         const double *d = D + ((size_t)blk * db + ii) * db;
         for (int j = 0; j < db; ++j) { const double2 v = Ps[r0 + j][n]; const double dj = __ldg(d + j); qr += dj * v.x; qi += dj * v.y; }
     }
-    double *t = qt + (size_t)(row / P2_KS) * P2_Q_DOUBLES + (row % P2_KS) * P2_Q_PITCH + n;
-    t[0] = qr; t[P2_KS * P2_Q_PITCH] = qi; t[2 * P2_KS * P2_Q_PITCH] = qr + qi;
+    double *t = qt + (size_t)(row / P2_KS) * P2Cfg<NB>::Q_DOUBLES + (row % P2_KS) * QP + n;
+    t[0] = qr; t[P2_KS * QP] = qi; t[2 * P2_KS * QP] = qr + qi;
 }
 
 // GEMM 2:  out[band0+n][g] += sum_i beta[i][g] Q[i][n]
@@ -254,19 +270,21 @@ k_reduce_dmul(const c128 *__restrict__ Ppart, int nsplit, int nrows_pad, const d
 // per CTA (two CTAs per SM), so every SM gets the same amount of work whatever N_G is.  A CTA whose range
 // starts or ends inside a G tile writes that tile's partial sum to a side buffer; k_proj2_fixup adds the
 // partials of each split tile to `out` in a fixed order (deterministic, no atomics).
-constexpr int P2_PART = P_NB * P2_G;      // c128 per partial tile
+template <int NB>
 __global__ void __launch_bounds__((P2_CW + 1) * 32, 2)
 k_proj2_sk(const c128 *__restrict__ beta2, int nic, int ngt, const double *__restrict__ qt, int ng, int nb, int band0,
            c128 *__restrict__ out, c128 *__restrict__ part, int *__restrict__ pdesc)
 {
     extern __shared__ __align__(128) unsigned char smem[];
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem + P2_ST * P2_STAGE_BYTES);
-    uint64_t *empty = full + P2_ST;
+    using Q = P2Cfg<NB>;
+    constexpr int ST = Q::ST, STAGE = Q::STAGE_BYTES, QP = Q::Q_PITCH, NJ = NB / 8;
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + ST * STAGE);
+    uint64_t *empty = full + ST;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long total = (long long)ngt * nic;
     const int s_begin = (int)(total * blockIdx.x / gridDim.x), s_end = (int)(total * (blockIdx.x + 1) / gridDim.x);
     if (threadIdx.x == 0) {
-        for (int s = 0; s < P2_ST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], P2_CW); }
+        for (int s = 0; s < ST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], P2_CW); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         pdesc[2 * blockIdx.x] = -1; pdesc[2 * blockIdx.x + 1] = -1;
     }
@@ -274,53 +292,52 @@ k_proj2_sk(const c128 *__restrict__ beta2, int nic, int ngt, const double *__res
     if (warp == P2_CW) {
         if (lane == 0) {
             for (int st = s_begin; st < s_end; ++st) {
-                const int it = st - s_begin, s = it % P2_ST;
-                if (it >= P2_ST) mbar_wait(&empty[s], ((it / P2_ST) - 1) & 1);
-                unsigned char *stage = smem + s * P2_STAGE_BYTES;
-                mbar_expect_tx(&full[s], P2_STAGE_BYTES);
+                const int it = st - s_begin, s = it % ST;
+                if (it >= ST) mbar_wait(&empty[s], ((it / ST) - 1) & 1);
+                unsigned char *stage = smem + s * STAGE;
+                mbar_expect_tx(&full[s], STAGE);
                 bulk_g2s(stage, beta2 + (size_t)st * (P2_KS * P2_G), P2_BETA_BYTES, &full[s]);    // layout [gt][ic] == st
-                bulk_g2s(stage + P2_BETA_BYTES, qt + (size_t)(st % nic) * P2_Q_DOUBLES, P2_Q_BYTES, &full[s]);
+                bulk_g2s(stage + P2_BETA_BYTES, qt + (size_t)(st % nic) * Q::Q_DOUBLES, Q::Q_BYTES, &full[s]);
             }
         }
     } else {
         const int r8 = lane >> 2, c = lane & 3;
-        int aoff[2], qoff[2];
+        int aoff[2];
 #pragma unroll
         for (int i = 0; i < 2; ++i) aoff[i] = (c * P2_G + 8 * (2 * warp + i) + (r8 ^ (2 * c))) * 16;
-#pragma unroll
-        for (int j = 0; j < 2; ++j) qoff[j] = P2_BETA_BYTES + (c * P2_Q_PITCH + 8 * j + r8) * 8;
+        const int qoff = P2_BETA_BYTES + (c * QP + r8) * 8;
         int st = s_begin;
         bool first_seg = true;
         while (st < s_end) {
             const int gt = st / nic, ic0 = st % nic;
             const int ic1 = min(nic, ic0 + (s_end - st));
-            double t1[2][2][2], t2[2][2][2], t3[2][2][2];
+            double t1[2][NJ][2], t2[2][NJ][2], t3[2][NJ][2];
 #pragma unroll
             for (int i = 0; i < 2; ++i)
 #pragma unroll
-                for (int j = 0; j < 2; ++j)
+                for (int j = 0; j < NJ; ++j)
 #pragma unroll
                     for (int e = 0; e < 2; ++e) { t1[i][j][e] = 0.0; t2[i][j][e] = 0.0; t3[i][j][e] = 0.0; }
             for (int ic = ic0; ic < ic1; ++ic, ++st) {
-                const int it = st - s_begin, s = it % P2_ST;
-                mbar_wait(&full[s], (it / P2_ST) & 1);
-                const unsigned char *stage = smem + s * P2_STAGE_BYTES;
+                const int it = st - s_begin, s = it % ST;
+                mbar_wait(&full[s], (it / ST) & 1);
+                const unsigned char *stage = smem + s * STAGE;
 #pragma unroll
                 for (int kk = 0; kk < P2_KS / 4; ++kk) {
                     double2 a[2];
-                    double qr[2], qi[2], qs[2];
+                    double qr[NJ], qi[NJ], qs[NJ];
 #pragma unroll
                     for (int i = 0; i < 2; ++i) a[i] = lds_c128(stage, aoff[i] + 4 * kk * P2_G * 16);
 #pragma unroll
-                    for (int j = 0; j < 2; ++j) {
-                        const double *q = reinterpret_cast<const double *>(stage + qoff[j] + 4 * kk * P2_Q_PITCH * 8);
-                        qr[j] = q[0]; qi[j] = q[P2_KS * P2_Q_PITCH]; qs[j] = q[2 * P2_KS * P2_Q_PITCH];
+                    for (int j = 0; j < NJ; ++j) {
+                        const double *q = reinterpret_cast<const double *>(stage + qoff + (4 * kk * QP + 8 * j) * 8);
+                        qr[j] = q[0]; qi[j] = q[P2_KS * QP]; qs[j] = q[2 * P2_KS * QP];
                     }
 #pragma unroll
                     for (int i = 0; i < 2; ++i) {
                         const double as = a[i].x + a[i].y;
 #pragma unroll
-                        for (int j = 0; j < 2; ++j) {
+                        for (int j = 0; j < NJ; ++j) {
                             dmma884(t1[i][j][0], t1[i][j][1], a[i].x, qr[j]);
                             dmma884(t2[i][j][0], t2[i][j][1], a[i].y, qi[j]);
                             dmma884(t3[i][j][0], t3[i][j][1], as, qs[j]);
@@ -335,14 +352,14 @@ k_proj2_sk(const c128 *__restrict__ beta2, int nic, int ngt, const double *__res
             c128 *pslot = nullptr;
             if (!whole) {
                 const int slot = 2 * blockIdx.x + (first_seg ? 0 : 1);
-                pslot = part + (size_t)slot * P2_PART;
+                pslot = part + (size_t)slot * Q::PART;
                 if (warp == 0 && lane == 0) pdesc[slot] = gt;
             }
 #pragma unroll
             for (int i = 0; i < 2; ++i) {
                 const int gl = 8 * (2 * warp + i) + r8, g = gt * P2_G + gl;
 #pragma unroll
-                for (int j = 0; j < 2; ++j)
+                for (int j = 0; j < NJ; ++j)
 #pragma unroll
                     for (int e = 0; e < 2; ++e) {
                         const int nl = j * 8 + 2 * c + e, n = band0 + nl;
@@ -363,21 +380,23 @@ k_proj2_sk(const c128 *__restrict__ beta2, int nic, int ngt, const double *__res
 }
 
 // One block per partial slot; the first slot of a split tile sums all that tile's partials into `out`.
+template <int NB>
 __global__ void k_proj2_fixup(const c128 *__restrict__ part, const int *__restrict__ pdesc, int nslots, int ng, int nb,
                               int band0, c128 *__restrict__ out)
 {
+    constexpr int PART = P2Cfg<NB>::PART;
     const int b = blockIdx.x;
     const int gt = pdesc[b];
     if (gt < 0) return;
     for (int j = b - 1; j >= 0 && j >= b - 4; --j) if (pdesc[j] == gt) return;     // not the first slot of this tile
-    for (int e = threadIdx.x; e < P2_PART; e += blockDim.x) {
+    for (int e = threadIdx.x; e < PART; e += blockDim.x) {
         const int nl = e / P2_G, gl = e % P2_G;
         const int g = gt * P2_G + gl, n = band0 + nl;
         if (g >= ng || n >= nb) continue;
         double sr = 0.0, si = 0.0;
         for (int j = b; j < nslots; ++j) {
             const int d = pdesc[j];
-            if (d == gt) { const double2 v = ldg_c128(part + (size_t)j * P2_PART + e); sr += v.x; si += v.y; }
+            if (d == gt) { const double2 v = ldg_c128(part + (size_t)j * PART + e); sr += v.x; si += v.y; }
             else if (d >= 0) break;
         }
         c128 *o = out + (size_t)n * ng + g;

@@ -54,8 +54,10 @@ int prepare_kernels(qm_gspace *g) {
     rc = qm_prepare_plane_m2(g); if (rc) return rc;
     rc = qm_prepare_plane_m3(g); if (rc) return rc;
     rc = qm_prepare_plane_m4(g); if (rc) return rc;
-    CU_TRY(cudaFuncSetAttribute(k_proj1_pipe, cudaFuncAttributeMaxDynamicSharedMemorySize, P1_SMEM));
-    CU_TRY(cudaFuncSetAttribute(k_proj2_sk, cudaFuncAttributeMaxDynamicSharedMemorySize, P2_SMEM));
+    CU_TRY(cudaFuncSetAttribute(k_proj1_pipe<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, P1Cfg<16>::SMEM));
+    CU_TRY(cudaFuncSetAttribute(k_proj2_sk<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, P2Cfg<16>::SMEM));
+    CU_TRY(cudaFuncSetAttribute(k_proj1_pipe<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, P1Cfg<32>::SMEM));
+    CU_TRY(cudaFuncSetAttribute(k_proj2_sk<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, P2Cfg<32>::SMEM));
     CU_TRY(cudaFuncSetAttribute(k_sub_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, SG_SMEM));
     return QM_OK;
 }
@@ -164,7 +166,7 @@ NlPlan nl_plan(const qm_gspace *g, const KPoint *kp) {
     NlPlan p;
     p.nsplit = std::max(1, std::min(kp->nkc, g->sm_count * P1_OCC / std::max(1, kp->nmblk)));
     p.nrows_pad = kp->nmblk * P1_ROWS;
-    p.pcount = (size_t)p.nrows_pad * P_NB;
+    p.pcount = (size_t)p.nrows_pad * P_NB_MAX;       // sized for the widest band tile
     p.ncta2 = (int)std::min<long long>((long long)kp->ngt * kp->nic, 2LL * g->sm_count);
     return p;
 }
@@ -173,46 +175,53 @@ int ensure_nonlocal_workspace(qm_gspace *g, KPoint *kp) {
     const NlPlan p = nl_plan(g, kp);
     CU_TRY(kp->d_Ppart.resize(p.pcount * p.nsplit));
     CU_TRY(kp->d_P.resize(p.pcount));
-    CU_TRY(kp->d_qt.resize((size_t)kp->nic * P2_Q_DOUBLES));
-    CU_TRY(kp->d_part.resize((size_t)2 * p.ncta2 * P2_PART));
+    CU_TRY(kp->d_qt.resize((size_t)kp->nic * P2Cfg<P_NB_MAX>::Q_DOUBLES));
+    CU_TRY(kp->d_part.resize((size_t)2 * p.ncta2 * P2Cfg<P_NB_MAX>::PART));
     CU_TRY(kp->d_pdesc.resize((size_t)2 * p.ncta2));
     return QM_OK;
+}
+
+// One pass of the projector pair over NB bands starting at band0.
+template <int NB>
+void nonlocal_pass(qm_gspace *g, KPoint *kp, const NlPlan &p, const c128 *psi_in, c128 *out, int nb, int band0, cudaStream_t st) {
+    const int nsplit = p.nsplit, nrows_pad = p.nrows_pad, ncta2 = p.ncta2;
+    const size_t pcount = (size_t)nrows_pad * NB;
+    g->prof.begin(QM_K_PROJ1, st);
+    k_proj1_pipe<NB><<<dim3(kp->nmblk, nsplit), (P1_CW + 1) * 32, P1Cfg<NB>::SMEM, st>>>(
+        kp->d_beta1.p, kp->nkc, psi_in, kp->ng, nb, band0, kp->d_Ppart.p, nrows_pad, nsplit);
+    g->prof.end(st);
+    const int qcount = kp->nic * P2_KS * NB;
+    if (16 % kp->dblock == 0 && kp->nic * P2_KS <= nrows_pad) {
+        g->prof.begin(QM_K_PREDUCE, st);      // fused split-K reduction + D multiply
+        k_reduce_dmul<NB><<<(kp->nic * P2_KS) / 16, 16 * NB, 0, st>>>(kp->d_Ppart.p, nsplit, nrows_pad, kp->d_D.p, kp->dblock,
+                                                                      kp->nproj, kp->d_qt.p);
+        g->prof.end(st);
+        g->launches += 1;
+    } else {
+        g->prof.begin(QM_K_PREDUCE, st);
+        k_reduce_p2<<<(unsigned)((pcount + 255) / 256), 256, 0, st>>>(kp->d_Ppart.p, nsplit, (int)pcount, kp->d_P.p);
+        g->prof.end(st);
+        g->prof.begin(QM_K_DMUL, st);
+        k_dmul_tiles<NB><<<(qcount + 255) / 256, 256, 0, st>>>(kp->d_D.p, kp->dblock, kp->nproj, kp->nic, kp->d_P.p,
+                                                               kp->d_qt.p);
+        g->prof.end(st);
+        g->launches += 2;
+    }
+    g->prof.begin(QM_K_PROJ2, st);
+    k_proj2_sk<NB><<<ncta2, (P2_CW + 1) * 32, P2Cfg<NB>::SMEM, st>>>(kp->d_beta2.p, kp->nic, kp->ngt, kp->d_qt.p, kp->ng, nb,
+                                                                     band0, out, kp->d_part.p, kp->d_pdesc.p);
+    k_proj2_fixup<NB><<<2 * ncta2, 256, 0, st>>>(kp->d_part.p, kp->d_pdesc.p, 2 * ncta2, kp->ng, nb, band0, out);
+    g->prof.end(st);
+    g->launches += 3;
 }
 
 int run_nonlocal(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb, cudaStream_t st) {
     if (kp->nproj == 0) return QM_OK;
     const NlPlan p = nl_plan(g, kp);
-    const int nsplit = p.nsplit, nrows_pad = p.nrows_pad, ncta2 = p.ncta2;
-    const size_t pcount = p.pcount;
-    for (int band0 = 0; band0 < nb; band0 += P_NB) {
-        g->prof.begin(QM_K_PROJ1, st);
-        k_proj1_pipe<<<dim3(kp->nmblk, nsplit), (P1_CW + 1) * 32, P1_SMEM, st>>>(
-            kp->d_beta1.p, kp->nkc, psi_in, kp->ng, nb, band0, kp->d_Ppart.p, nrows_pad, nsplit);
-        g->prof.end(st);
-        const int qcount = kp->nic * P2_KS * P_NB;
-        if (16 % kp->dblock == 0 && kp->nic * P2_KS <= nrows_pad) {
-            g->prof.begin(QM_K_PREDUCE, st);      // fused split-K reduction + D multiply
-            k_reduce_dmul<<<(kp->nic * P2_KS) / 16, 256, 0, st>>>(kp->d_Ppart.p, nsplit, nrows_pad, kp->d_D.p, kp->dblock,
-                                                                   kp->nproj, kp->d_qt.p);
-            g->prof.end(st);
-            g->launches += 1;
-        } else {
-            g->prof.begin(QM_K_PREDUCE, st);
-            k_reduce_p2<<<(unsigned)((pcount + 255) / 256), 256, 0, st>>>(kp->d_Ppart.p, nsplit, (int)pcount, kp->d_P.p);
-            g->prof.end(st);
-            g->prof.begin(QM_K_DMUL, st);
-            k_dmul_tiles<<<(qcount + 255) / 256, 256, 0, st>>>(kp->d_D.p, kp->dblock, kp->nproj, kp->nic, kp->d_P.p,
-                                                              kp->d_qt.p);
-            g->prof.end(st);
-            g->launches += 2;
-        }
-        g->prof.begin(QM_K_PROJ2, st);
-        k_proj2_sk<<<ncta2, (P2_CW + 1) * 32, P2_SMEM, st>>>(kp->d_beta2.p, kp->nic, kp->ngt, kp->d_qt.p, kp->ng, nb,
-                                                             band0, out, kp->d_part.p, kp->d_pdesc.p);
-        k_proj2_fixup<<<2 * ncta2, 256, 0, st>>>(kp->d_part.p, kp->d_pdesc.p, 2 * ncta2, kp->ng, nb, band0, out);
-        g->prof.end(st);
-        g->launches += 3;
-    }
+    // 32-band passes while more than 16 bands remain (beta is streamed once per pass), then one 16-band pass
+    int band0 = 0;
+    for (; nb - band0 > P_NB; band0 += 32) nonlocal_pass<32>(g, kp, p, psi_in, out, nb, band0, st);
+    if (band0 < nb) nonlocal_pass<16>(g, kp, p, psi_in, out, nb, band0, st);
     CU_TRY(cudaGetLastError());
     return QM_OK;
 }
