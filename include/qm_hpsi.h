@@ -68,9 +68,12 @@ typedef enum {
  * (GSpace(recilat, ecut) and the per-k gkspc.)
  *  lattice_bohr  HOST  9 doubles, rows a1,a2,a3
  *  ecutwfc_ry          cut-off in Rydberg
- *  fft_grid      HOST  3 ints n1,n2,n3; each must be a supported FFT length (see qm_fft_size_supported)
- *                      and n1 == n2 (the fused xy-plane kernel uses one line factorisation for both axes; n3 is free).
- *                      Anything else returns QM_EGRID.
+ *  fft_grid      HOST  3 ints n1,n2,n3; each must be a supported FFT length (see qm_fft_size_supported: products of two
+ *                      radices <= 16 with factors 2, 3, 5, from 8 to 256) and hold the sphere (2|m_i|+1 <= n_i), else
+ *                      QM_EGRID.  The three lengths are independent.  Boxes with n1 == n2 <= 144 whose xy-plane working set
+ *                      fits one SM's shared memory (up to the 216-atom cell at 30 Ry) run the fused xy-plane kernel; every
+ *                      other legal box (n1 != n2, longer axes, larger planes: PAPER.md:689-712, 1490, 1666) runs the same
+ *                      transforms as separate y | x | y passes through HBM -- same results, same entry points.
  *  kpts_cryst    HOST  nk*3 doubles (may be NULL iff nk==1 => Gamma)
  *  out                 receives the handle; destroy with qm_gspace_destroy.
  * Uploads the tables to the current CUDA device (synchronously; this is set-up, not hot path). */

@@ -37,7 +37,36 @@ template <int GM> int dispatch_zfwd(qm_gspace *g, KPoint *kp, const c128 *W, con
                                     cudaStream_t st) {
     return qm_launch_zfwd(g, kp, GM, W, aux, out, nb, scale, st);
 }
+// Unfused path: bands per slab pass (the slab of half-transformed planes is bounded, not proportional to the call)
+size_t gen_slab_per_band(const qm_gspace *g, const KPoint *kp) { return (size_t)g->grid[2] * kp->nx * g->grid[1]; }
+int gen_sub_bands(const qm_gspace *g, const KPoint *kp, int nb) {
+    const size_t budget = (size_t)1 << 25;          // c128 elements: 512 MB
+    return (int)std::max<size_t>(1, std::min<size_t>((size_t)nb, budget / std::max<size_t>(1, gen_slab_per_band(g, kp))));
+}
+template <int MODE> int launch_gen_x(qm_gspace *g, KPoint *kp, c128 *slab, int bp0, int nbp, const PlaneArgs &a, cudaStream_t st) {
+    if constexpr (MODE == 0) return qm_launch_gen_x_m0(g, kp, slab, bp0, nbp, a, st);
+    else if constexpr (MODE == 1) return qm_launch_gen_x_m1(g, kp, slab, bp0, nbp, a, st);
+    else if constexpr (MODE == 2) return qm_launch_gen_x_m2(g, kp, slab, bp0, nbp, a, st);
+    else if constexpr (MODE == 3) return qm_launch_gen_x_m3(g, kp, slab, bp0, nbp, a, st);
+    else return qm_launch_gen_x_m4(g, kp, slab, bp0, nbp, a, st);
+}
+// y backward | x round trip of MODE | y forward, a bounded number of bands at a time (gen_kernels.cuh)
+template <int MODE> int run_general(qm_gspace *g, KPoint *kp, c128 *W, int nb, const PlaneArgs &a, cudaStream_t st) {
+    const int n3 = g->grid[2], sub = gen_sub_bands(g, kp, nb);
+    CU_TRY(kp->d_slab.resize((size_t)sub * gen_slab_per_band(g, kp)));
+    for (int b0 = 0; b0 < nb; b0 += sub) {
+        const int n = std::min(sub, nb - b0), bp0 = b0 * n3, nbp = n * n3;
+        int rc;
+        if constexpr (MODE != 2) { rc = qm_launch_gen_y(g, kp, true, W, kp->d_slab.p, bp0, nbp, st); if (rc) return rc; }
+        rc = launch_gen_x<MODE>(g, kp, kp->d_slab.p, bp0, nbp, a, st); if (rc) return rc;
+        if constexpr (MODE == 0 || MODE == 2 || MODE == 4) {
+            rc = qm_launch_gen_y(g, kp, false, W, kp->d_slab.p, bp0, nbp, st); if (rc) return rc;
+        }
+    }
+    return QM_OK;
+}
 template <int MODE> int dispatch_plane(qm_gspace *g, KPoint *kp, c128 *W, int nb, const PlaneArgs &a, cudaStream_t st) {
+    if (!g->fused) return run_general<MODE>(g, kp, W, nb, a, st);
     if constexpr (MODE == 0) return qm_launch_plane_m0(g, kp, W, nb, a, st);
     else if constexpr (MODE == 1) return qm_launch_plane_m1(g, kp, W, nb, a, st);
     else if constexpr (MODE == 2) return qm_launch_plane_m2(g, kp, W, nb, a, st);
@@ -49,11 +78,20 @@ template <int MODE> int dispatch_plane(qm_gspace *g, KPoint *kp, c128 *W, int nb
 // device (function attributes are per device; nothing of this kind is left on the hot path).
 int prepare_kernels(qm_gspace *g) {
     int rc = qm_prepare_z(g); if (rc) return rc;
-    rc = qm_prepare_plane_m0(g); if (rc) return rc;
-    rc = qm_prepare_plane_m1(g); if (rc) return rc;
-    rc = qm_prepare_plane_m2(g); if (rc) return rc;
-    rc = qm_prepare_plane_m3(g); if (rc) return rc;
-    rc = qm_prepare_plane_m4(g); if (rc) return rc;
+    if (g->fused) {
+        rc = qm_prepare_plane_m0(g); if (rc) return rc;
+        rc = qm_prepare_plane_m1(g); if (rc) return rc;
+        rc = qm_prepare_plane_m2(g); if (rc) return rc;
+        rc = qm_prepare_plane_m3(g); if (rc) return rc;
+        rc = qm_prepare_plane_m4(g); if (rc) return rc;
+    } else {
+        rc = qm_prepare_gen_y(g); if (rc) return rc;
+        rc = qm_prepare_gen_x_m0(g); if (rc) return rc;
+        rc = qm_prepare_gen_x_m1(g); if (rc) return rc;
+        rc = qm_prepare_gen_x_m2(g); if (rc) return rc;
+        rc = qm_prepare_gen_x_m3(g); if (rc) return rc;
+        rc = qm_prepare_gen_x_m4(g); if (rc) return rc;
+    }
     CU_TRY(cudaFuncSetAttribute(k_proj1_pipe<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, P1Cfg<16>::SMEM));
     CU_TRY(cudaFuncSetAttribute(k_proj2_sk<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, P2Cfg<16>::SMEM));
     CU_TRY(cudaFuncSetAttribute(k_proj1_pipe<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, P1Cfg<32>::SMEM));
@@ -159,6 +197,10 @@ int fft_chunk_bands(const qm_gspace *g, const KPoint *kp) {
 }
 int ensure_workspace(qm_gspace *g, KPoint *kp, int nb) {
     CU_TRY(kp->d_W.resize((size_t)std::min(nb, fft_chunk_bands(g, kp)) * w_elems_per_band(g, kp)));
+    if (!g->fused) {
+        const int n = std::min(nb, fft_chunk_bands(g, kp));
+        CU_TRY(kp->d_slab.resize((size_t)gen_sub_bands(g, kp, n) * gen_slab_per_band(g, kp)));
+    }
     return QM_OK;
 }
 struct NlPlan { int nsplit, nrows_pad, ncta2; size_t pcount; };
@@ -268,7 +310,6 @@ QM_API int qm_gspace_create(const double *lattice_bohr, double ecutwfc_ry, const
     *out = nullptr;
     for (int i = 0; i < 3; ++i)
         if (!qm_find_size(fft_grid[i])) return fail(QM_EGRID, "unsupported FFT length " + std::to_string(fft_grid[i]));
-    if (fft_grid[0] != fft_grid[1]) return fail(QM_EGRID, "this version needs n1 == n2");
     int dev = 0, count = 0;
     if (cudaGetDeviceCount(&count) != cudaSuccess || count == 0)
         return fail(QM_ECUDA, "no CUDA device (there is no CPU fallback)");
@@ -290,8 +331,6 @@ QM_API int qm_gspace_create(const double *lattice_bohr, double ecutwfc_ry, const
         g->device = dev;
         g->l2_bytes = (size_t)std::max(l2, 0);
     }
-    rc = prepare_kernels(g);
-    if (rc != QM_OK) return bail(rc);
     for (int a = 0; a < 3; ++a) {
         const int n = g->grid[a];
         std::vector<c128> tw(n);
@@ -316,11 +355,16 @@ QM_API int qm_gspace_create(const double *lattice_bohr, double ecutwfc_ry, const
         for (int i = 0; i < 3; ++i) kp->k[i] = kpts_cryst ? kpts_cryst[3 * ik + i] : 0.0;
         rc = build_kpoint(g, kp);
         if (rc != QM_OK) return bail(rc);
-        if (plane_smem(g, kp, 1) > (size_t)g->max_smem) {
-            fail(QM_EGRID, "plane working set exceeds shared memory for this grid / sphere");
-            return bail(QM_EGRID);
-        }
     }
+    // The fused plane kernel takes the box when x and y share one line factorisation (n1 == n2 <= 144) and the plane
+    // array of every k-point fits one SM's shared memory; every other legal box goes through the unfused passes.
+    g->fused = g->grid[0] == g->grid[1] && g->grid[0] <= kQmFusedMax;
+    if (g->fused)
+        for (const KPoint *kp : g->kpts)
+            if (plane_smem(g, kp, 1) > (size_t)g->max_smem) g->fused = false;
+    if (const char *e = getenv("QM_FORCE_UNFUSED")) if (atoi(e) > 0) g->fused = false;
+    rc = prepare_kernels(g);
+    if (rc != QM_OK) return bail(rc);
     if (const char *e = getenv("QM_PLANE_STAGGER_NS")) g->plane_stagger_ns = atoi(e);
     if (const char *e = getenv("QM_Z_CTA_PER_SM")) g->z_cta_per_sm = std::max(1, atoi(e));
     if (const char *e = getenv("QM_PLANE_CTAS")) g->plane_ctas_per_sm = std::max(0, atoi(e));
@@ -483,7 +527,7 @@ QM_API int qm_mtxel_create(qm_gspace *g, int k_bra, int k_ket, double ecut_eps_r
     for (int i = 0; i < 3; ++i) m->sph.k[i] = g->kpts[k_bra]->k[i] - g->kpts[k_ket]->k[i];      // q = (k+q) - k
     m->sph.ecut_override = ecut_eps_ry;
     rc = build_kpoint(g, &m->sph, true);
-    if (rc == QM_OK && plane_smem(g, &m->sph, 1) > (size_t)g->max_smem)
+    if (rc == QM_OK && g->fused && plane_smem(g, &m->sph, 1) > (size_t)g->max_smem)
         rc = fail(QM_EGRID, "plane working set of the epsilon sphere exceeds shared memory");
     if (rc != QM_OK) { delete m; return rc; }
     *out = m;

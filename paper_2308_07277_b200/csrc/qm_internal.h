@@ -59,6 +59,7 @@ struct KPoint : QmKTables {
     DevBuf<double> d_D;
     // workspaces of this k-point (calls on different k-points may run on different streams)
     DevBuf<c128> d_W, d_Ppart, d_P, d_part;
+    DevBuf<c128> d_slab;                                // unfused path: half-transformed planes (gen_kernels.cuh)
     DevBuf<double> d_qt;
     DevBuf<int> d_pdesc;
     DevBuf<c128> d_sophase;                             // split-operator: exp(-i dt |k+G|^2 / 4)
@@ -137,6 +138,7 @@ struct qm_gspace {
     bool so_set = false;
     double so_dt = 0.0;
     unsigned long long launches = 0;
+    bool fused = true;              // the fused plane kernel takes this box (else: the unfused passes, gen_kernels.cuh)
     int device = 0;                 // the CUDA device the handle was created on (every call checks it)
     int sm_count = 148;
     int max_smem = 0;
@@ -223,15 +225,18 @@ struct PlaneArgs {          // operands of the plane kernel beyond the stick pla
 };
 
 // dispatch on FFT length ---------------------------------------------------------------------
+// QM_FOR_SIZES: the lengths the fused plane kernel is compiled for; QM_FOR_SIZES_ALL adds the lengths above 144 that only the
+// z kernels and the unfused passes take (gspace_host.h kQmSizes lists them all).
 #ifdef QM_DEV_SIZES      /* developer builds: only the lengths of the five BASELINE.json configs (fast compile) */
 #define QM_FOR_SIZES(X) X(12, 3, 4) X(24, 4, 6) X(32, 4, 8) X(48, 6, 8) X(96, 8, 12) X(144, 12, 12)
+#define QM_FOR_SIZES_ALL(X) QM_FOR_SIZES(X) X(36, 6, 6) X(192, 12, 16)
 #else
 #define QM_FOR_SIZES(X)                                                                              \
     X(8, 2, 4) X(12, 3, 4) X(16, 4, 4) X(18, 3, 6) X(20, 4, 5) X(24, 4, 6) X(30, 5, 6) X(32, 4, 8)   \
     X(36, 6, 6) X(40, 5, 8) X(48, 6, 8) X(60, 6, 10) X(64, 8, 8) X(72, 8, 9) X(80, 8, 10)            \
     X(96, 8, 12) X(100, 10, 10) X(108, 9, 12) X(120, 10, 12) X(128, 8, 16) X(144, 12, 12)
+#define QM_FOR_SIZES_ALL(X) QM_FOR_SIZES(X) X(160, 10, 16) X(180, 12, 15) X(192, 12, 16) X(225, 15, 15) X(240, 15, 16) X(256, 16, 16)
 #endif
-
 
 // ---- launches implemented in the other translation units ------------------------------------------------------
 // phase == nullptr: plain scatter; else psi(G) * phase[g] on the way in (split-operator half-step)
@@ -251,3 +256,16 @@ int qm_prepare_plane_m1(qm_gspace *g);
 int qm_prepare_plane_m2(qm_gspace *g);
 int qm_prepare_plane_m3(qm_gspace *g);
 int qm_prepare_plane_m4(qm_gspace *g);
+// unfused passes (qm_geny.cu, qm_genx<M>.cu): one slab pass over the planes [bp0, bp0 + nbp) of a launch
+int qm_launch_gen_y(qm_gspace *g, KPoint *kp, bool back, c128 *W, c128 *slab, int bp0, int nbp, cudaStream_t st);
+int qm_launch_gen_x_m0(qm_gspace *g, KPoint *kp, c128 *slab, int bp0, int nbp, const PlaneArgs &a, cudaStream_t st);
+int qm_launch_gen_x_m1(qm_gspace *g, KPoint *kp, c128 *slab, int bp0, int nbp, const PlaneArgs &a, cudaStream_t st);
+int qm_launch_gen_x_m2(qm_gspace *g, KPoint *kp, c128 *slab, int bp0, int nbp, const PlaneArgs &a, cudaStream_t st);
+int qm_launch_gen_x_m3(qm_gspace *g, KPoint *kp, c128 *slab, int bp0, int nbp, const PlaneArgs &a, cudaStream_t st);
+int qm_launch_gen_x_m4(qm_gspace *g, KPoint *kp, c128 *slab, int bp0, int nbp, const PlaneArgs &a, cudaStream_t st);
+int qm_prepare_gen_y(qm_gspace *g);
+int qm_prepare_gen_x_m0(qm_gspace *g);
+int qm_prepare_gen_x_m1(qm_gspace *g);
+int qm_prepare_gen_x_m2(qm_gspace *g);
+int qm_prepare_gen_x_m3(qm_gspace *g);
+int qm_prepare_gen_x_m4(qm_gspace *g);

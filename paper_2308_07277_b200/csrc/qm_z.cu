@@ -45,7 +45,7 @@ int qm_launch_zinv(qm_gspace *g, KPoint *kp, const c128 *psi, const c128 *phase,
 #define X(N, A, B)                                                                               \
     case N: return phase ? launch_zinv<LineCfg<A, B>, true>(g, kp, psi, phase, W, nb, st)         \
                          : launch_zinv<LineCfg<A, B>, false>(g, kp, psi, nullptr, W, nb, st);
-        QM_FOR_SIZES(X)
+        QM_FOR_SIZES_ALL(X)
 #undef X
     }
     return fail(QM_EGRID, "unsupported FFT length (axis 3)");
@@ -65,7 +65,7 @@ int qm_launch_zfwd(qm_gspace *g, KPoint *kp, int gm, const c128 *W, const c128 *
                    cudaStream_t st) {
     switch (g->grid[2]) {
 #define X(N, A, B) case N: return zfwd_by_mode<LineCfg<A, B>>(g, kp, gm, W, aux, out, nb, scale, st);
-        QM_FOR_SIZES(X)
+        QM_FOR_SIZES_ALL(X)
 #undef X
     }
     return fail(QM_EGRID, "unsupported FFT length (axis 3)");
@@ -74,7 +74,7 @@ int qm_launch_zfwd(qm_gspace *g, KPoint *kp, int gm, const c128 *W, const c128 *
 int qm_prepare_z(qm_gspace *g) {
     switch (g->grid[2]) {
 #define X(N, A, B) case N: return prep_z_kernels<LineCfg<A, B>>();
-        QM_FOR_SIZES(X)
+        QM_FOR_SIZES_ALL(X)
 #undef X
     }
     return fail(QM_EGRID, "unsupported FFT length (axis 3)");

@@ -199,8 +199,10 @@ def test_parity_other_d_block_sizes(qm, name, db):
     gs.close()
 
 
-@pytest.mark.parametrize("nb", [1, 3, 17])
+@pytest.mark.parametrize("nb", [1, 3, 17, 24, 33, 40, 48, 64])
 def test_ragged_band_counts(qm, nb):
+    """Band counts around the projector GEMMs' band tiles: 32-band passes while more than 16 bands remain, then one
+    16-band pass (ragged tiles are zero padded on the way in and masked on the way out)."""
     p = problem("cfg3")
     gs = _gspace(qm, p)
     psi = np.ascontiguousarray(p["psi"][:nb])
