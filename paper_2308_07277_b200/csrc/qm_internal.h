@@ -146,7 +146,7 @@ struct qm_gspace {
     int fft_chunk = 0;              // bands per internal pass of the FFT path (0: derived from the L2 size; QM_FFT_CHUNK)
     int z_cta_per_sm = 2;           // resident z-kernel CTAs per SM the grid is sized for (QM_Z_CTA_PER_SM)
     int plane_stagger_ns = 0;       // de-phasing delay between the plane kernel's groups (QM_PLANE_STAGGER_NS)
-    int plane_ctas_per_sm = 0;      // resident plane-kernel CTAs per SM (0: chosen from the shared-memory footprint; QM_PLANE_CTAS)
+    int plane_ctas_per_sm = 0;      // resident plane-kernel CTAs per SM (0: two when two plane arrays fit, else one; QM_PLANE_CTAS)
     ~qm_gspace() { for (auto *k : kpts) delete k; }
 };
 

@@ -8,9 +8,10 @@
 namespace {
 
 template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *W, int nb, const PlaneArgs &a, cudaStream_t st) {
-    // two resident CTAs per SM when the plane array is small enough: each walks its own planes, so the CTA-wide
-    // barriers and the load / compute / store phases of one CTA overlap the other's work
-    int cps = MODE == 3 ? 1 : (g->plane_ctas_per_sm > 0 ? g->plane_ctas_per_sm : 1);
+    // two resident CTAs per SM (half the groups each) when two plane arrays fit: each walks its own planes, so the
+    // CTA-wide barriers and the load / compute / store phases of one CTA overlap the other's work (measured with the
+    // twiddle rows in tensor memory: cfg4 -5 %, cfg3 -15 %, cfg2 -11 % plane-kernel time; cfg5's plane array allows one)
+    int cps = MODE == 3 ? 1 : (g->plane_ctas_per_sm > 0 ? g->plane_ctas_per_sm : 2);
     int ngroups = plane_groups(g, kp, cps);
 #if QM_PLANE_TW_TMEM
     // every resident CTA allocates its own tensor-memory columns (512 per SM): one CTA per SM if two do not fit

@@ -53,6 +53,13 @@ CASES = [
     (120, 24.0 * np.eye(3), 30.0, (0.0, 0.0, 0.0)),
     (128, 26.0 * np.eye(3), 30.0, (0.0, 0.0, 0.0)),
     (144, 30.78 * np.eye(3), 30.0, (0.0, 0.0, 0.0)),
+    # lengths above 144 (z kernels and the unfused passes on the GPU; the same line factorisations here)
+    (160, 12.0 * np.eye(3), 16.0, (0.0, 0.0, 0.0)),
+    (180, 12.0 * np.eye(3), 16.0, (0.1, 0.0, -0.2)),
+    (192, 12.0 * np.eye(3), 16.0, (0.0, 0.0, 0.0)),
+    (225, 12.0 * np.eye(3), 16.0, (0.0, 0.0, 0.0)),
+    (240, 12.0 * np.eye(3), 16.0, (0.0, 0.0, 0.0)),
+    (256, 12.0 * np.eye(3), 16.0, (0.0, 0.0, 0.0)),
 ]
 
 
