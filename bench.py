@@ -500,6 +500,18 @@ def run_ours(args):
                 if ent["frac"] > 1.0:
                     ent["invalid"] = "frac > 1: the work model or the peak is wrong"
             kernels[name] = ent
+        if "k_plane" in kernels:
+            # second roof of the fused plane kernel: the shared-memory pipe.  Algorithmic 16-byte accesses per z-plane (one
+            # store + one load per element and exchange stage): y passes 6 N X, x passes N (4 N + 2 X);
+            # peak = 128 B/clk/SM (B300_MICROARCH.md "smem crossbar BW") x SMs x the SM clock sampled during the run.
+            n1 = cfg.grid[0]
+            acc = cb * N3 * (8.0 * n1 * nx + 4.0 * n1 * n1)
+            clk = (sampler.summary().get("sm_mhz") or 1965.0) * 1e6
+            smem_peak = 128.0 * torch.cuda.get_device_properties(dev).multi_processor_count * clk / 1e12
+            a = acc * 16.0 / (kernels["k_plane"]["avg_ms"] * 1e-3) / 1e12
+            kernels["k_plane"]["co_bound"] = {"bound": "smem", "achieved": a, "peak": smem_peak, "unit": "TB/s",
+                                              "frac": a / smem_peak,
+                                              "note": "algorithmic shared-memory bytes of the six exchange stages per plane"}
         dom = max((k for k in kernels if "bound" in kernels[k]), key=lambda k: kernels[k]["share"])
         d = kernels[dom]
         roofline = {"kernel": dom, "bound": d["bound"], "achieved": d["achieved"], "peak": d["peak"],
@@ -552,6 +564,9 @@ def run_ours(args):
                 "all_configs": all_cfg,
                 "roofline": roofline, "fft_path": fft_path, "kernels": kernels,
                 "fp64_peaks_tflops": {"dmma_probe": dmma_peak, "dfma_probe": dfma_peak},
+                "exchange_probe": dict(zip(("smem_ns", "shfl_ns", "tmem_read_ns"), qm.qm_probe_exchange()),
+                                       note="SM time per warp-wide hand-over of one complex128 per lane, 12 warps per SM "
+                                            "(csrc/probe_kernels.cuh)"),
                 "one_call_all_bands": {"bands": nb, "ms": one_call_ms, "band_applies_per_s": nb / (one_call_ms * 1e-3)},
                 "taylor": {"order": 4, "bands": nb, "call_batch": cb, "ms": taylor_ms,
                            "band_steps_per_s": nb / (taylor_ms * 1e-3),

@@ -258,6 +258,13 @@ QM_API const char *qm_kernel_name(int kind);
  * projector GEMMs (MEASURED_PEAKS.json has no FP64 entry). Synchronous. */
 QM_API int qm_probe_fp64_tensor_peak(double *tflops_dmma, double *tflops_dfma);
 
+/* Exchange probe (csrc/probe_kernels.cuh): SM time, in ns, of one warp-wide hand-over of a complex128 per lane with 12
+ * warps per SM running the same loop -- through shared memory (STS.128 + LDS.128), through warp shuffles (4 x SHFL.32),
+ * and the read of a thread-private element from tensor memory (tcgen05.ld).  HOST outputs.  Reported by bench.py beside
+ * the plane kernel's figures (why the transposes go through shared memory and the twiddle rows through
+ * tensor memory).  Synchronous. */
+QM_API int qm_probe_exchange(double *ns_smem, double *ns_shfl, double *ns_tmem);
+
 QM_API const char *qm_last_error(void);                    /* thread-local text */
 QM_API const char *qm_version(void);
 

@@ -3,6 +3,7 @@
 #include "qm_internal.h"
 #include "proj_kernels.cuh"
 #include "subspace_kernels.cuh"
+#include "probe_kernels.cuh"
 
 thread_local std::string qm_g_err;
 
@@ -927,6 +928,36 @@ QM_API int qm_probe_fp64_tensor_peak(double *tflops_dmma, double *tflops_dfma) {
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
     if (tflops_dmma) *tflops_dmma = best_mma;
     if (tflops_dfma) *tflops_dfma = best_fma;
+    return QM_OK;
+}
+
+QM_API int qm_probe_exchange(double *ns_smem, double *ns_shfl, double *ns_tmem) {
+    int dev = 0, sms = 0, count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || count == 0) return fail(QM_ECUDA, "no CUDA device");
+    CU_TRY(cudaGetDevice(&dev));
+    CU_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    double *sink = nullptr;
+    CU_TRY(cudaMalloc(&sink, sizeof(double)));
+    cudaEvent_t e0, e1;
+    CU_TRY(cudaEventCreate(&e0)); CU_TRY(cudaEventCreate(&e1));
+    const int iters = 1 << 14, threads = 384, blocks = sms;       // 12 warps per SM, like the plane kernel
+    double best[3] = {1e30, 1e30, 1e30};
+    for (int rep = 0; rep < 3; ++rep)
+        for (int mode = 0; mode < 3; ++mode) {
+            float ms = 0.f;
+            CU_TRY(cudaEventRecord(e0));
+            if (mode == 0) k_probe_exchange<0><<<blocks, threads>>>(sink, iters);
+            else if (mode == 1) k_probe_exchange<1><<<blocks, threads>>>(sink, iters);
+            else k_probe_exchange<2><<<blocks, threads>>>(sink, iters);
+            CU_TRY(cudaEventRecord(e1)); CU_TRY(cudaEventSynchronize(e1));
+            CU_TRY(cudaEventElapsedTime(&ms, e0, e1));
+            // SM-time per warp-wide exchange of one complex128 per lane: 12 warps share the SM
+            best[mode] = std::min(best[mode], (double)ms * 1e6 / ((double)iters * (threads / 32)));
+        }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    if (ns_smem) *ns_smem = best[0];
+    if (ns_shfl) *ns_shfl = best[1];
+    if (ns_tmem) *ns_tmem = best[2];
     return QM_OK;
 }
 
