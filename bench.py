@@ -214,6 +214,51 @@ def _verify_timed_output(cfg, lat, kpts, v, dblk, per_k, out_dev, nrows=48):
             "against": "oracle/hpsi_direct.c (direct G-space sum), output of the timed steps"}
 
 
+def _unfused_figure(qm, torch, dev, hbm_peak):
+    """The 512-atom cell (4 x 4 x 4 cubic diamond-structure supercell, a = 41.04 bohr, 30 Ry, 192^3; PAPER.md:1490, 1666 name
+    432- and 1024-atom runs): its xy-plane working set exceeds one SM's shared memory, so the library runs the unfused
+    y | x | y passes.  Kinetic + local terms of a 16-band batch (the projectors are the same GEMMs as
+    everywhere), seeded random psi and V, device-timed; the three slab passes against the HBM roof."""
+    lat, ecut, grid, nbb = np.eye(3) * 41.04, 30.0, (192, 192, 192), 16
+    gs = qm.GSpace(lat, ecut, grid)
+    ng, (nst, nxr) = gs.num_g(0), gs.num_sticks(0)
+    gen = torch.Generator(device="cpu")
+    gen.manual_seed(512)
+    gs.set_vloc(torch.randn(grid, dtype=torch.float64, generator=gen).to(dev))
+    gs.set_nonlocal(0, None, None)
+    psi = torch.view_as_complex(torch.randn(nbb, ng, 2, dtype=torch.float64, generator=gen)).to(dev)
+    out = torch.empty_like(psi)
+    for _ in range(3):
+        gs.apply_h(psi, out)
+    torch.cuda.synchronize()
+    qm.qm_profile_enable(gs.handle, True)
+    qm.qm_profile_reset(gs.handle)
+    reps = 5
+    for _ in range(reps):
+        gs.apply_h(psi, out)
+    torch.cuda.synchronize()
+    prof = qm.qm_profile_read(gs.handle)
+    qm.qm_profile_enable(gs.handle, False)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        gs.apply_h(psi, out)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    gs.close()
+    slab = nbb * nxr * grid[1] * grid[2] * 16            # one copy of the half-transformed planes of the batch
+    pass_ms = sum(prof[k][0] for k in ("k_gen_y", "k_gen_x")) / reps
+    return {"workload": "512-atom cubic Si-like cell, ecutwfc 30 Ry, FFT grid 192x192x192, kinetic + local terms, "
+                        "16-band batch, seeded random psi and V", "ng": ng, "sticks": nst, "x_columns": nxr,
+            "ms_per_call": ms, "band_applies_per_s": nbb / (ms * 1e-3),
+            "kernel_ms_per_call": {k: v[0] / reps for k, v in prof.items() if v[1]},
+            "slab_passes": {"bound": "hbm", "alg_bytes": 4 * slab, "ms": pass_ms, "unit": "GB/s",
+                            "achieved": 4 * slab / (pass_ms * 1e-3) / 1e9, "peak": hbm_peak,
+                            "frac": 4 * slab / (pass_ms * 1e-3) / 1e9 / hbm_peak,
+                            "note": "y backward writes the slab, x reads and writes it, y forward reads it"}}
+
+
 def _small_config_figure(qm, torch, dev, name, steps):
     """Device-timed applies/s of one of the other BASELINE.json configs (no roofline claim for cfg1-3: launch bound,
     SURVEY 8(d)); same step definition as the headline: all bands x all k at the config's call batch."""
@@ -562,6 +607,8 @@ def run_ours(args):
                 "gpu_launches": int(launches),
                 "verified": verify,
                 "all_configs": all_cfg,
+                "unfused_512_atoms": (_unfused_figure(qm, torch, dev, hbm_peak)
+                                      if world == 1 and args.config == "cfg5" and not args.no_all_configs else None),
                 "roofline": roofline, "fft_path": fft_path, "kernels": kernels,
                 "fp64_peaks_tflops": {"dmma_probe": dmma_peak, "dfma_probe": dfma_peak},
                 "exchange_probe": dict(zip(("smem_ns", "shfl_ns", "tmem_read_ns"), qm.qm_probe_exchange()),

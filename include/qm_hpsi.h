@@ -246,7 +246,9 @@ typedef enum {
     QM_K_PROJ2 = 6,     /* out += beta Q    (DMMA)                      (a8) */
     QM_K_SUBGEMM = 7,   /* S = A^H B (DMMA, split-K)                     (8(f) rank 1) */
     QM_K_SUBREDUCE = 8, /* split-K reduction of S */
-    QM_K_COUNT = 9
+    QM_K_GENY = 9,      /* unfused y pass (backward or forward) of boxes the fused plane kernel does not take */
+    QM_K_GENX = 10,     /* unfused x round trip incl. V_loc multiply of such boxes */
+    QM_K_COUNT = 11
 } qm_kernel_kind;
 QM_API int qm_profile_enable(qm_gspace *g, int on);
 QM_API int qm_profile_reset(qm_gspace *g);

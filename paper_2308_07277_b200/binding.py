@@ -72,7 +72,7 @@ _SIGS = {
     "qm_profile_read": [_vp, _i, ctypes.POINTER(_d), ctypes.POINTER(ctypes.c_ulonglong)],
 }
 EXPORTS = sorted(list(_SIGS) + ["qm_last_error", "qm_version", "qm_kernel_name"])
-QM_K_COUNT = 9
+QM_K_COUNT = 11
 
 
 def load_library():

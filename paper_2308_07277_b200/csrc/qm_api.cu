@@ -894,7 +894,7 @@ QM_API int qm_profile_read(qm_gspace *g, int kind, double *total_ms, unsigned lo
 }
 QM_API const char *qm_kernel_name(int kind) {
     static const char *names[QM_K_COUNT] = {"k_zinv", "k_plane", "k_zfwd", "k_proj1", "k_reduce_p", "k_dmul",
-                                            "k_proj2", "k_sub_gemm", "k_sub_reduce"};
+                                            "k_proj2", "k_sub_gemm", "k_sub_reduce", "k_gen_y", "k_gen_x"};
     return (kind >= 0 && kind < QM_K_COUNT) ? names[kind] : "?";
 }
 

@@ -12,9 +12,14 @@ namespace {
 template <class C, bool BACK> int launch_gen_y(qm_gspace *g, KPoint *kp, c128 *W, c128 *slab, int bp0, int nbp, cudaStream_t st) {
     using GG = GenGeom<C>;
     const long long items = (long long)nbp * kp->nx;
-    const unsigned grid = (unsigned)((items + GG::TPG - 1) / GG::TPG);
+    if (items * GG::TPG >= (1LL << 31)) return fail(QM_EINVAL, "unfused y pass: too many rows in one launch");
+    // persistent: a CTA walks row chunks gridDim.x apart (twiddle rows loaded once); several CTAs per SM hide latency
+    const long long nchunks = (items + GG::TPG - 1) / GG::TPG;
+    int per_sm = 1;
+    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_gen_y<C, BACK>, GEN_GROUP, GG::y_smem()));
+    const unsigned grid = (unsigned)std::min<long long>(nchunks, (long long)g->sm_count * std::max(1, per_sm));
     const size_t wband = (size_t)((kp->nsticks + QM_ZT - 1) / QM_ZT) * QM_ZT * g->grid[2];
-    g->prof.begin(QM_K_PLANE, st);
+    g->prof.begin(QM_K_GENY, st);
     k_gen_y<C, BACK><<<grid, GEN_GROUP, GG::y_smem(), st>>>(kp->plan(), g->d_tw[1].p, W, slab, g->grid[2], bp0, nbp,
                                                              kp->y_quarter ? 1 : 0, wband);
     g->prof.end(st);
@@ -30,8 +35,12 @@ template <class C, int MODE> int launch_gen_x(qm_gspace *g, KPoint *kp, c128 *sl
     if (smem > (size_t)g->max_smem) return fail(QM_EGRID, "x tile of the unfused path does not fit shared memory");
     const int n2 = g->grid[1], n3 = g->grid[2];
     const int nchunk = (n2 + GG::TC - 1) / GG::TC;
-    const unsigned grid = (unsigned)((MODE == 3 ? n3 : nbp) * nchunk);
-    g->prof.begin(QM_K_PLANE, st);
+    const long long tiles = (long long)(MODE == 3 ? n3 : nbp) * nchunk;
+    // persistent: a CTA walks tiles gridDim.x apart; as many CTAs as are resident
+    int per_sm = 1;
+    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_gen_x<C, MODE>, GG::XG * GEN_GROUP, smem));
+    const unsigned grid = (unsigned)std::min<long long>(tiles, (long long)g->sm_count * std::max(1, per_sm));
+    g->prof.begin(QM_K_GENX, st);
     k_gen_x<C, MODE><<<grid, GG::XG * GEN_GROUP, smem, st>>>(kp->plan(), g->d_tw[0].p, g->d_vt.p, slab, a.box, a.box2, a.npair2,
                                                              a.scale, n2, n3, bp0, nbp,
                                                              (kp->y_quarter ? 1 : 0) | (kp->x_quarter ? 2 : 0), a.occ, a.rhot);
