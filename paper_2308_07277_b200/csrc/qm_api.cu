@@ -224,10 +224,11 @@ int ensure_nonlocal_workspace(qm_gspace *g, KPoint *kp) {
     return QM_OK;
 }
 
-// One pass of the projector pair over NB bands starting at band0.
+// One pass of the projector pair over NB bands starting at band0, in two halves: project (P = beta^H psi, split-K
+// reduction, Q = D P; needs psi_in only) and expand (out += beta Q; needs the local part of out to be there).
 template <int NB>
-void nonlocal_pass(qm_gspace *g, KPoint *kp, const NlPlan &p, const c128 *psi_in, c128 *out, int nb, int band0, cudaStream_t st) {
-    const int nsplit = p.nsplit, nrows_pad = p.nrows_pad, ncta2 = p.ncta2;
+void nonlocal_project(qm_gspace *g, KPoint *kp, const NlPlan &p, const c128 *psi_in, int nb, int band0, cudaStream_t st) {
+    const int nsplit = p.nsplit, nrows_pad = p.nrows_pad;
     const size_t pcount = (size_t)nrows_pad * NB;
     g->prof.begin(QM_K_PROJ1, st);
     k_proj1_pipe<NB><<<dim3(kp->nmblk, nsplit), (P1_CW + 1) * 32, P1Cfg<NB>::SMEM, st>>>(
@@ -239,7 +240,7 @@ void nonlocal_pass(qm_gspace *g, KPoint *kp, const NlPlan &p, const c128 *psi_in
         k_reduce_dmul<NB><<<(kp->nic * P2_KS) / 16, 16 * NB, 0, st>>>(kp->d_Ppart.p, nsplit, nrows_pad, kp->d_D.p, kp->dblock,
                                                                       kp->nproj, kp->d_qt.p);
         g->prof.end(st);
-        g->launches += 1;
+        g->launches += 2;
     } else {
         g->prof.begin(QM_K_PREDUCE, st);
         k_reduce_p2<<<(unsigned)((pcount + 255) / 256), 256, 0, st>>>(kp->d_Ppart.p, nsplit, (int)pcount, kp->d_P.p);
@@ -248,23 +249,53 @@ void nonlocal_pass(qm_gspace *g, KPoint *kp, const NlPlan &p, const c128 *psi_in
         k_dmul_tiles<NB><<<(qcount + 255) / 256, 256, 0, st>>>(kp->d_D.p, kp->dblock, kp->nproj, kp->nic, kp->d_P.p,
                                                                kp->d_qt.p);
         g->prof.end(st);
-        g->launches += 2;
+        g->launches += 3;
     }
+}
+template <int NB>
+void nonlocal_expand(qm_gspace *g, KPoint *kp, const NlPlan &p, c128 *out, int nb, int band0, cudaStream_t st) {
+    const int ncta2 = p.ncta2;
     g->prof.begin(QM_K_PROJ2, st);
     k_proj2_sk<NB><<<ncta2, (P2_CW + 1) * 32, P2Cfg<NB>::SMEM, st>>>(kp->d_beta2.p, kp->nic, kp->ngt, kp->d_qt.p, kp->ng, nb,
                                                                      band0, out, kp->d_part.p, kp->d_pdesc.p);
     k_proj2_fixup<NB><<<2 * ncta2, 256, 0, st>>>(kp->d_part.p, kp->d_pdesc.p, 2 * ncta2, kp->ng, nb, band0, out);
     g->prof.end(st);
-    g->launches += 3;
+    g->launches += 2;
+}
+// 32-band passes while more than 16 bands remain (beta is streamed once per pass), then one 16-band pass
+inline bool pass_is_32(int nb, int band0) { return nb - band0 > P_NB; }
+void nl_project(qm_gspace *g, KPoint *kp, const NlPlan &p, const c128 *psi_in, int nb, int band0, cudaStream_t st) {
+    if (pass_is_32(nb, band0)) nonlocal_project<32>(g, kp, p, psi_in, nb, band0, st);
+    else nonlocal_project<16>(g, kp, p, psi_in, nb, band0, st);
+}
+void nl_expand(qm_gspace *g, KPoint *kp, const NlPlan &p, c128 *out, int nb, int band0, cudaStream_t st) {
+    if (pass_is_32(nb, band0)) nonlocal_expand<32>(g, kp, p, out, nb, band0, st);
+    else nonlocal_expand<16>(g, kp, p, out, nb, band0, st);
 }
 
-int run_nonlocal(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb, cudaStream_t st) {
-    if (kp->nproj == 0) return QM_OK;
+// The whole apply: local part (FFT path) and projectors.  The first pass's projection needs psi_in only, so it runs on
+// the k-point's side stream beside the FFT path (fork / join by events: the tails of the FFT kernels and of GEMM 1 fill each
+// other's idle SMs; also valid under stream capture); everything else is ordered on `st`.
+int run_local(qm_gspace *g, KPoint *kp, const c128 *in, c128 *out, int nb, int kind, cudaStream_t st);
+int run_apply(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb, cudaStream_t st) {
+    if (kp->nproj == 0) return run_local(g, kp, psi_in, out, nb, 0, st);
     const NlPlan p = nl_plan(g, kp);
-    // 32-band passes while more than 16 bands remain (beta is streamed once per pass), then one 16-band pass
-    int band0 = 0;
-    for (; nb - band0 > P_NB; band0 += 32) nonlocal_pass<32>(g, kp, p, psi_in, out, nb, band0, st);
-    if (band0 < nb) nonlocal_pass<16>(g, kp, p, psi_in, out, nb, band0, st);
+    // (not while the per-kernel profiler is on: its event pairs would time kernels that share the device)
+    const bool overlap = g->nl_overlap && kp->side_stream != nullptr && !g->prof.on;
+    if (overlap) {
+        CU_TRY(cudaEventRecord(kp->ev_fork, st));
+        CU_TRY(cudaStreamWaitEvent(kp->side_stream, kp->ev_fork, 0));
+        nl_project(g, kp, p, psi_in, nb, 0, kp->side_stream);
+        CU_TRY(cudaEventRecord(kp->ev_join, kp->side_stream));
+    }
+    int rc = run_local(g, kp, psi_in, out, nb, 0, st); if (rc) return rc;
+    if (overlap) CU_TRY(cudaStreamWaitEvent(st, kp->ev_join, 0));
+    else nl_project(g, kp, p, psi_in, nb, 0, st);
+    nl_expand(g, kp, p, out, nb, 0, st);
+    for (int band0 = pass_is_32(nb, 0) ? 32 : 16; band0 < nb; band0 += pass_is_32(nb, band0) ? 32 : 16) {
+        nl_project(g, kp, p, psi_in, nb, band0, st);
+        nl_expand(g, kp, p, out, nb, band0, st);
+    }
     CU_TRY(cudaGetLastError());
     return QM_OK;
 }
@@ -364,6 +395,7 @@ QM_API int qm_gspace_create(const double *lattice_bohr, double ecutwfc_ry, const
         for (const KPoint *kp : g->kpts)
             if (plane_smem(g, kp, 1) > (size_t)g->max_smem) g->fused = false;
     if (const char *e = getenv("QM_FORCE_UNFUSED")) if (atoi(e) > 0) g->fused = false;
+    if (const char *e = getenv("QM_NL_OVERLAP")) g->nl_overlap = atoi(e) != 0;
     rc = prepare_kernels(g);
     if (rc != QM_OK) return bail(rc);
     if (const char *e = getenv("QM_PLANE_STAGGER_NS")) g->plane_stagger_ns = atoi(e);
@@ -454,6 +486,11 @@ QM_API int qm_set_nonlocal(qm_gspace *g, int k, const qm_c128 *beta_kG_dev, int 
     g->launches += 2;
     CU_TRY(cudaGetLastError());
     CU_TRY(cudaMemcpyAsync(kp->d_D.p, D_dev, dcount * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    if (!kp->side_stream) {
+        CU_TRY(cudaStreamCreateWithFlags(&kp->side_stream, cudaStreamNonBlocking));
+        CU_TRY(cudaEventCreateWithFlags(&kp->ev_fork, cudaEventDisableTiming));
+        CU_TRY(cudaEventCreateWithFlags(&kp->ev_join, cudaEventDisableTiming));
+    }
     kp->nproj = nproj; kp->dblock = d_block; kp->nl_set = true;
     kp->nmblk = nmblk; kp->nkc = nkc; kp->ngt = ngt; kp->nic = nic;
     return ensure_nonlocal_workspace(g, kp);        // projector workspaces do not depend on nbands: sized here, once
@@ -480,8 +517,7 @@ QM_API int qm_apply_h(qm_gspace *g, const qm_c128 *psi_in_dev, qm_c128 *psi_out_
     if (a < b + bytes && b < a + bytes) return fail(QM_EINVAL, "qm_apply_h: psi_in and psi_out overlap");
     cudaStream_t st = (cudaStream_t)stream;
     rc = ensure_workspace(g, kp, nbands); if (rc) return rc;
-    rc = run_local(g, kp, in, out, nbands, 0, st); if (rc) return rc;
-    return run_nonlocal(g, kp, in, out, nbands, st);
+    return run_apply(g, kp, in, out, nbands, st);
 }
 
 QM_API int qm_split_operator_set(qm_gspace *g, const double *V_r_dev, double dt, void *stream) {

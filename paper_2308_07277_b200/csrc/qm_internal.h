@@ -63,6 +63,13 @@ struct KPoint : QmKTables {
     DevBuf<double> d_qt;
     DevBuf<int> d_pdesc;
     DevBuf<c128> d_sophase;                             // split-operator: exp(-i dt |k+G|^2 / 4)
+    cudaStream_t side_stream = nullptr;                 // GEMM 1 of an apply runs here, beside the FFT path (qm_api.cu run_apply)
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    ~KPoint() {
+        if (ev_fork) cudaEventDestroy(ev_fork);
+        if (ev_join) cudaEventDestroy(ev_join);
+        if (side_stream) cudaStreamDestroy(side_stream);
+    }
     double ecut_override = 0.0;                         // epsilon spheres (qm_mtxel) carry their own cut-off
     QmKPlanDev plan() const {
         QmKPlanDev p;
@@ -138,6 +145,7 @@ struct qm_gspace {
     bool so_set = false;
     double so_dt = 0.0;
     unsigned long long launches = 0;
+    bool nl_overlap = true;         // projection GEMM of an apply on a side stream beside the FFT path (QM_NL_OVERLAP=0: off)
     bool fused = true;              // the fused plane kernel takes this box (else: the unfused passes, gen_kernels.cuh)
     int device = 0;                 // the CUDA device the handle was created on (every call checks it)
     int sm_count = 148;
