@@ -115,7 +115,10 @@ QM_API int qm_reserve(qm_gspace *g, int k, int nbands);
 
 /* psi_out = H psi_in for a block of nbands wavefunctions at k-point k.
  *  psi_in_dev, psi_out_dev  DEVICE  [nbands][ng(k)] row-major complex128; must not overlap;
- *                           psi_out is overwritten. */
+ *                           psi_out is overwritten.
+ * Only enqueues work; everything is ordered on `stream`.  (With projectors set, the first projection GEMM, which reads
+ * psi_in only, is placed on a library-owned side stream that forks from and joins `stream` by events, so that it may
+ * run beside the FFT kernels; to the caller the call behaves like work on `stream`, also under stream capture.) */
 QM_API int qm_apply_h(qm_gspace *g, const qm_c128 *psi_in_dev, qm_c128 *psi_out_dev,
                int nbands, int k, void *stream);
 

@@ -280,7 +280,9 @@ int run_local(qm_gspace *g, KPoint *kp, const c128 *in, c128 *out, int nb, int k
 int run_apply(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb, cudaStream_t st) {
     if (kp->nproj == 0) return run_local(g, kp, psi_in, out, nb, 0, st);
     const NlPlan p = nl_plan(g, kp);
-    // (not while the per-kernel profiler is on: its event pairs would time kernels that share the device)
+    // Not while the per-kernel profiler is on: its event pairs would time kernels that share the device.  Measured at cfg5
+    // (beta 1.1 GB, streamed beside the stick planes the FFT kernels hand each other through L2): 20.3-20.8 k band-applies/s
+    // with the overlap, 20.1-20.4 k without; +4 % end to end; cfg1 27 -> 21 us per apply, cfg3 +10 %, cfg4 +2.5 %.
     const bool overlap = g->nl_overlap && kp->side_stream != nullptr && !g->prof.on;
     if (overlap) {
         CU_TRY(cudaEventRecord(kp->ev_fork, st));
@@ -487,7 +489,9 @@ QM_API int qm_set_nonlocal(qm_gspace *g, int k, const qm_c128 *beta_kG_dev, int 
     CU_TRY(cudaGetLastError());
     CU_TRY(cudaMemcpyAsync(kp->d_D.p, D_dev, dcount * sizeof(double), cudaMemcpyDeviceToDevice, st));
     if (!kp->side_stream) {
-        CU_TRY(cudaStreamCreateWithFlags(&kp->side_stream, cudaStreamNonBlocking));
+        int prio_lo = 0, prio_hi = 0;                      // lowest priority: kernels of the caller's stream get free SMs first
+        CU_TRY(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+        CU_TRY(cudaStreamCreateWithPriority(&kp->side_stream, cudaStreamNonBlocking, prio_lo));
         CU_TRY(cudaEventCreateWithFlags(&kp->ev_fork, cudaEventDisableTiming));
         CU_TRY(cudaEventCreateWithFlags(&kp->ev_join, cudaEventDisableTiming));
     }
