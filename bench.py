@@ -259,7 +259,7 @@ def _unfused_figure(qm, torch, dev, hbm_peak):
                             "note": "y backward writes the slab, x reads and writes it, y forward reads it"}}
 
 
-def _small_config_figure(qm, torch, dev, name, steps):
+def _small_config_figure(qm, torch, dev, name, steps, peaks=None):
     """Device-timed applies/s of one of the other BASELINE.json configs (no roofline claim for cfg1-3: launch bound,
     SURVEY 8(d)); same step definition as the headline: all bands x all k at the config's call batch."""
     from workloads import CONFIGS, cell_for, make_kpoints
@@ -299,6 +299,25 @@ def _small_config_figure(qm, torch, dev, name, steps):
         res[tag] = (ms, (gs.launch_count() - l0) / reps)
     ver = _verify_timed_output(cfg, lat, kpts, v, dblk, per_k, out_dev, nrows=32)
     ng = gs.num_g(0)
+    # per-kernel device time of one step of plain calls (events around every launch; the side stream is off meanwhile)
+    qm.qm_profile_enable(gs.handle, True)
+    qm.qm_profile_reset(gs.handle)
+    step_calls()
+    torch.cuda.synchronize()
+    prof = qm.qm_profile_read(gs.handle)
+    qm.qm_profile_enable(gs.handle, False)
+    kern = {k: {"avg_ms": t / n, "launches_per_step": n} for k, (t, n) in prof.items() if n}
+    if peaks is not None and "k_plane" in kern:
+        # the same two roofs as the headline's plane kernel, per launch of `cb` bands
+        dmma_peak, smem_peak = peaks
+        n1, n3 = cfg.grid[0], cfg.grid[2]
+        nxr = gs.num_sticks(0)[1]
+        t = kern["k_plane"]["avg_ms"] * 1e-3
+        fl = cb * n3 * ((2 * nxr + 2 * n1) * 5.0 * n1 * np.log2(n1) + 2.0 * n1 * cfg.grid[1])
+        by = cb * n3 * (8.0 * n1 * nxr + 4.0 * n1 * n1) * 16.0
+        kern["k_plane"].update(bound="alu", achieved=fl / t / 1e12, peak=dmma_peak, unit="TFLOP/s", frac=fl / t / 1e12 / dmma_peak,
+                               co_bound={"bound": "smem", "achieved": by / t / 1e12, "peak": smem_peak, "unit": "TB/s",
+                                         "frac": by / t / 1e12 / smem_peak})
     plan.close()
     gs.close()
     best = min(res, key=lambda t: res[t][0])
@@ -307,7 +326,8 @@ def _small_config_figure(qm, torch, dev, name, steps):
     return {"workload": _config_dict(cfg, ng, 0, 0)["workload"], "call_batch": cb, "band_applies_per_s": nb * cfg.nk / (ms * 1e-3),
             "ms_per_full_band_apply": ms, "us_per_call": ms * 1e3 / ncalls, "calls_per_step": ncalls,
             "launch_mode": best, "ms_by_mode": {t: r[0] for t, r in res.items()},
-            "launches_per_call": res["calls"][1] / ncalls, "verified": ver["verified"], "max_rel_err": ver["max_rel_err"]}
+            "launches_per_call": res["calls"][1] / ncalls, "kernels": kern,
+            "verified": ver["verified"], "max_rel_err": ver["max_rel_err"]}
 
 
 def run_ours(args):
@@ -585,7 +605,10 @@ def run_ours(args):
                                 "frac": d1_bytes / (fft_ms * 1e-3) / 1e9 / hbm_peak if fft_ms else None}
         all_cfg = None
         if world == 1 and args.config == "cfg5" and not args.no_all_configs:
-            all_cfg = {n: _small_config_figure(qm, torch, dev, n, args.steps) for n in ("cfg1", "cfg2", "cfg3", "cfg4")}
+            sm_clk = (sampler.summary().get("sm_mhz") or 1965.0) * 1e6
+            pk = (dmma_peak, 128.0 * torch.cuda.get_device_properties(dev).multi_processor_count * sm_clk / 1e12)
+            all_cfg = {n: _small_config_figure(qm, torch, dev, n, args.steps, peaks=pk if n in ("cfg3", "cfg4") else None)
+                       for n in ("cfg1", "cfg2", "cfg3", "cfg4")}
             all_cfg["cfg5"] = {"workload": _config_dict(cfg, ng, nsticks, nx)["workload"], "call_batch": cb,
                                "band_applies_per_s": value, "ms_per_full_band_apply": ms / args.steps,
                                "us_per_call": ms / args.steps * 1e3 / (cfg.nk * ((nb + cb - 1) // cb)),

@@ -207,7 +207,9 @@ int ensure_workspace(qm_gspace *g, KPoint *kp, int nb) {
 struct NlPlan { int nsplit, nrows_pad, ncta2; size_t pcount; };
 NlPlan nl_plan(const qm_gspace *g, const KPoint *kp) {
     NlPlan p;
-    p.nsplit = std::max(1, std::min(kp->nkc, g->sm_count * P1_OCC / std::max(1, kp->nmblk)));
+    // split-K: one CTA per SM, but at least 8 K slices per split -- the reduction kernel sums the splits of an entry one
+    // after the other, and on small spheres 148 two-slice splits cost more there than they save in GEMM 1
+    p.nsplit = std::max(1, std::min({kp->nkc, g->sm_count * P1_OCC / std::max(1, kp->nmblk), std::max(1, kp->nkc / 8)}));
     p.nrows_pad = kp->nmblk * P1_ROWS;
     p.pcount = (size_t)p.nrows_pad * P_NB_MAX;       // sized for the widest band tile
     p.ncta2 = (int)std::min<long long>((long long)kp->ngt * kp->nic, 2LL * g->sm_count);
