@@ -292,9 +292,10 @@ int run_apply(qm_gspace *g, KPoint *kp, const c128 *psi_in, c128 *out, int nb, c
         nl_project(g, kp, p, psi_in, nb, 0, kp->side_stream);
         CU_TRY(cudaEventRecord(kp->ev_join, kp->side_stream));
     }
-    int rc = run_local(g, kp, psi_in, out, nb, 0, st); if (rc) return rc;
-    if (overlap) CU_TRY(cudaStreamWaitEvent(st, kp->ev_join, 0));
-    else nl_project(g, kp, p, psi_in, nb, 0, st);
+    const int rc = run_local(g, kp, psi_in, out, nb, 0, st);
+    if (overlap) CU_TRY(cudaStreamWaitEvent(st, kp->ev_join, 0));       // join even if the local part failed (stream capture)
+    if (rc) return rc;
+    if (!overlap) nl_project(g, kp, p, psi_in, nb, 0, st);
     nl_expand(g, kp, p, out, nb, 0, st);
     for (int band0 = pass_is_32(nb, 0) ? 32 : 16; band0 < nb; band0 += pass_is_32(nb, band0) ? 32 : 16) {
         nl_project(g, kp, p, psi_in, nb, band0, st);

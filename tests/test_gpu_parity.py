@@ -385,3 +385,39 @@ def test_wrong_device_and_concurrent_kpoints(qm):
     for ik in range(4):
         assert torch.equal(outs[ik], want[ik]), ik
     gs.close()
+
+
+def test_side_stream_projection_is_bitwise_neutral(qm):
+    """GEMM 1 on the side stream (default) and everything on the caller's stream (QM_NL_OVERLAP=0) give the same bits,
+    call after call on a non-default stream (the fork / join events order the shared work spaces)."""
+    import os
+    torch, dev = _torch()
+    p = problem("cfg3")
+    res = {}
+    for mode in ("1", "0"):
+        os.environ["QM_NL_OVERLAP"] = mode
+        try:
+            gs = _gspace(qm, p)
+        finally:
+            os.environ.pop("QM_NL_OVERLAP", None)
+        gs.set_vloc(torch.from_numpy(p["v"]).to(dev))
+        gs.set_nonlocal(0, torch.from_numpy(p["beta"]).to(dev), torch.from_numpy(p["dblk"]).to(dev))
+        psi = torch.from_numpy(p["psi"]).to(dev)
+        s = torch.cuda.Stream()
+        outs = [torch.empty_like(psi) for _ in range(6)]
+        torch.cuda.synchronize()
+        for o in outs:                                   # back-to-back calls reuse P / Q: any missing ordering shows up here
+            gs.apply_h(psi, o, stream=s)
+        torch.cuda.synchronize()
+        for o in outs[1:]:
+            assert torch.equal(o, outs[0])
+        res[mode] = outs[0].clone()
+        gs.close()
+    assert torch.equal(res["1"], res["0"])
+
+
+def test_exchange_probe_orders_the_three_mechanisms(qm):
+    """qm_probe_exchange: a tensor-memory read is cheaper than a shuffle hand-over, which is cheaper than the shared-memory
+    round trip; all three are positive and of nanosecond order."""
+    smem, shfl, tmem = qm.qm_probe_exchange()
+    assert 0.1 < tmem < shfl < smem < 100.0, (smem, shfl, tmem)
