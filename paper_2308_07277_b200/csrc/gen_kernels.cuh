@@ -14,6 +14,10 @@
 #include "fft_phases.cuh"
 #include "qm_plan.h"
 
+#ifndef QM_GEN_X_MINB
+#define QM_GEN_X_MINB 4      /* resident CTAs per SM the x pass is compiled for (168 registers: 4 x 3 warps per SM; measured
+                               -23 % x-pass time against the uncapped 176-254 registers and 2 CTAs) */
+#endif
 #ifndef QM_GEN_XG
 #define QM_GEN_XG 1          /* 96-thread groups per CTA of the x pass: 1 = independent groups, several resident CTAs per SM */
 #endif
@@ -127,7 +131,7 @@ k_gen_y(QmKPlanDev kp, const c128 *__restrict__ tw, c128 *__restrict__ W, c128 *
 // times the conjugate of a second one), 3 density, 4 apply with a complex field.  In MODE 3 a CTA owns its tile for ALL
 // bands of the launch and walks them in order, so every point of rho is summed by one thread in band order.
 template <class C, int MODE>
-__global__ void __launch_bounds__(GenGeom<C>::XG * GEN_GROUP)
+__global__ void __launch_bounds__(GenGeom<C>::XG * GEN_GROUP, QM_GEN_X_MINB)
 k_gen_x(QmKPlanDev kp, const c128 *__restrict__ tw, const double *__restrict__ vt, c128 *__restrict__ slab,
         c128 *__restrict__ box, const c128 *__restrict__ box2, int npair2, double scale, int n2, int n3, int bp0, int nbp,
         int quarter, const double *__restrict__ occ, double *__restrict__ rhot)
