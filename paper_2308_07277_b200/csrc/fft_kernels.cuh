@@ -149,6 +149,9 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
 #ifndef QM_PLANE_XPREFETCH
 #define QM_PLANE_XPREFETCH 0    /* x phase: fetch a column's step-1 inputs one column ahead (quarter rule) */
 #endif
+#ifndef QM_PLANE_XTW_LATE
+#define QM_PLANE_XTW_LATE 0     /* x phase: forward inter-pass twiddles applied in step 3 (on the way in) instead of step 2: measured +2 % at cfg5 */
+#endif
 #ifndef QM_PLANE_TW_TMEM
 #define QM_PLANE_TW_TMEM 1      /* per-thread twiddle rows live in tensor memory (tmem_rows.cuh) instead of registers */
 #endif
@@ -387,7 +390,10 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
             if constexpr (MODE == 4) bx2 = box2 + coloff;
             c128 t[1][C::R2];
             xcol_step2_head<C, MODE, false>(scrB[0], id.u1, vr, bx, bx2, scale, t[0], ok && id.a1);
-            if constexpr (MODE != 1) plane_tail<C, true>(t, scrB, id.u1, twb, cx.tw_b);
+            if constexpr (MODE != 1) {
+                if constexpr (QM_PLANE_XTW_LATE) stepB1_store<C>(t[0], scrB[0], id.u1);
+                else plane_tail<C, true>(t, scrB, id.u1, twb, cx.tw_b);
+            }
         }
         if constexpr (MODE == 0)     // prefetch V of this team's next column behind steps 3 and 1
             load_vrow<C>(vr, vcol(col + nteams), id.u1);
@@ -399,8 +405,24 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
         if constexpr (MODE != 1 && MODE != 3) {
             // no barrier after step 3: the scratch column a thread reads here is exactly the one it
             // overwrites in the next iteration's step 1 (MODE 2 has no step 1 and writes rows: barrier).
-            if (xq) prunedB_step2_quarter<C, false>(scrA[0], Acol, C::R2 * RP, pxc, id.u2);
-            else prunedB_step2<C, false>(scrA[0], Acol, C::R2 * RP, pxc, id.u2);
+            if constexpr (QM_PLANE_XTW_LATE) {
+                c128 t[C::R1];
+                stepB2_load<C>(scrA[0], id.u2, t);
+#if QM_PLANE_TW_TMEM
+                static_for<(C::R1 + QM_TW_CHUNK - 1) / QM_TW_CHUNK>([&](auto I) {
+                    constexpr int j0 = decltype(I)::value * QM_TW_CHUNK, j1 = j0 + QM_TW_CHUNK < C::R1 ? j0 + QM_TW_CHUNK : C::R1;
+                    constexpr int l0 = j0 == 0 ? 1 : j0;
+                    TwChunk<l0, (l0 < j1 ? j1 : l0 + 1)> ch;
+                    if constexpr (l0 < j1) { tmem_load_chunk(ch, cx.tw_a); stepB2_twiddle_range<C, l0, j1>(t, ch); }
+                });
+#else
+                stepB2_twiddle_range<C, 0, C::R1>(t, twa);
+#endif
+                stepB2_finish<C>(t, Acol, C::R2 * RP, pxc, xq);
+            } else {
+                if (xq) prunedB_step2_quarter<C, false>(scrA[0], Acol, C::R2 * RP, pxc, id.u2);
+                else prunedB_step2<C, false>(scrA[0], Acol, C::R2 * RP, pxc, id.u2);
+            }
             if constexpr (MODE == 2) group_barrier<G>(grp);
         }
     }
