@@ -38,3 +38,11 @@ __device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.
 __device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 // order this thread's generic-proxy shared-memory accesses before later async-proxy (bulk copy) accesses
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// Programmatic dependent launch (griddepcontrol): a kernel launched with the programmatic-serialisation attribute may
+// start while its predecessor in the stream is still running; pdl_wait() blocks until the predecessor has completed and
+// its writes are visible, pdl_launch_dependents() lets the successor's CTAs be scheduled as SM resources free up.  Both
+// are no-ops in a kernel launched the ordinary way.  Everything before pdl_wait() must touch only shared / tensor memory
+// and constant tables.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }

@@ -52,6 +52,8 @@ k_zinv(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ psi,
     int4 q = info(blockIdx.x), qn = info(blockIdx.x + gridDim.x);
     Pruned pr = pruned_of(q);
     c128 pre[NPRE];
+    pdl_launch_dependents();
+    pdl_wait();                 // psi may come from the previous kernel; W is still read by it
     if (quarter) prefetch_quarter<C>(psib + q.z, C::R2, pr, pre);
     const SLine lines_s = qm_sline(lines), stage_s = qm_sline(stage);
     for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
@@ -92,14 +94,17 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
     const int t1 = tid / C::TT, u1 = tid % C::TT;      // pass 2 (gather side): u fastest
     const int t2 = tid % QM_ZT, u2 = tid / QM_ZT;      // pass 1 (staging side): stick fastest
     const c128 *Wb = W + (size_t)band * ntiles * C::N * QM_ZT;
+    pdl_launch_dependents();
     if (tid == 0) {
         mbar_init(wbar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        pdl_wait();             // W comes from the previous kernel
         mbar_expect_tx(wbar, TILE_BYTES);
         bulk_g2s(stage, Wb + (size_t)blockIdx.x * C::N * QM_ZT, TILE_BYTES, wbar);
     }
     TwRow<C::R2> twb;
     load_twrow(twb, tw, u2, C::R1);
+    pdl_wait();
     const size_t boff = (size_t)band * kp.ng;
     const c128 *auxb = GM == GM_KINETIC ? aux + boff : aux;
     __syncthreads();
@@ -487,6 +492,8 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
     if constexpr (C::R1 != C::R2) tmem_store_row(cx.tw_b, twb_store);
     tmem_wait_st();
 #endif
+    pdl_launch_dependents();
+    pdl_wait();                 // the stick planes (and boxes) come from the previous kernel
     const int n3 = cx.n3;
     // plane sequence of this CTA.  Apply / debug modes: pl = blockIdx.x, + gridDim.x, ... (pl = band * n3 + p).
     // Density mode: the CTA owns z-planes p = blockIdx.x, + gridDim.x, ... and walks ALL bands of a plane before

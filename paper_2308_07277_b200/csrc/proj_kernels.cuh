@@ -116,6 +116,8 @@ k_proj1_pipe(const c128 *__restrict__ beta1, int nkc, const c128 *__restrict__ p
         for (int i = threadIdx.x; i < PSI_BYTES / 16; i += blockDim.x) pz[i] = make_double2(0.0, 0.0);
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    pdl_launch_dependents();
+    pdl_wait();
     __syncthreads();
 
     if (warp == P1_CW) {
@@ -242,6 +244,8 @@ k_reduce_dmul(const c128 *__restrict__ Ppart, int nsplit, int nrows_pad, const d
 {
     constexpr int QP = P2Cfg<NB>::Q_PITCH;
     __shared__ double2 Ps[16][NB + 1];
+    pdl_launch_dependents();
+    pdl_wait();
     const int n = threadIdx.x % NB, rl = threadIdx.x / NB;
     const int row = blockIdx.x * 16 + rl;
     const size_t count = (size_t)nrows_pad * NB;
@@ -283,11 +287,13 @@ k_proj2_sk(const c128 *__restrict__ beta2, int nic, int ngt, const double *__res
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long total = (long long)ngt * nic;
     const int s_begin = (int)(total * blockIdx.x / gridDim.x), s_end = (int)(total * (blockIdx.x + 1) / gridDim.x);
+    pdl_launch_dependents();
     if (threadIdx.x == 0) {
         for (int s = 0; s < ST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], P2_CW); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        pdesc[2 * blockIdx.x] = -1; pdesc[2 * blockIdx.x + 1] = -1;
     }
+    pdl_wait();                 // Q, out and the partial-tile table belong to the previous kernels until here
+    if (threadIdx.x == 0) { pdesc[2 * blockIdx.x] = -1; pdesc[2 * blockIdx.x + 1] = -1; }
     __syncthreads();
     if (warp == P2_CW) {
         if (lane == 0) {
@@ -386,6 +392,8 @@ __global__ void k_proj2_fixup(const c128 *__restrict__ part, const int *__restri
 {
     constexpr int PART = P2Cfg<NB>::PART;
     const int b = blockIdx.x;
+    pdl_launch_dependents();
+    pdl_wait();
     const int gt = pdesc[b];
     if (gt < 0) return;
     for (int j = b - 1; j >= 0 && j >= b - 4; --j) if (pdesc[j] == gt) return;     // not the first slot of this tile

@@ -233,14 +233,14 @@ void nonlocal_project(qm_gspace *g, KPoint *kp, const NlPlan &p, const c128 *psi
     const int nsplit = p.nsplit, nrows_pad = p.nrows_pad;
     const size_t pcount = (size_t)nrows_pad * NB;
     g->prof.begin(QM_K_PROJ1, st);
-    k_proj1_pipe<NB><<<dim3(kp->nmblk, nsplit), (P1_CW + 1) * 32, P1Cfg<NB>::SMEM, st>>>(
-        kp->d_beta1.p, kp->nkc, psi_in, kp->ng, nb, band0, kp->d_Ppart.p, nrows_pad, nsplit);
+    qm_launch_pdl(k_proj1_pipe<NB>, dim3(kp->nmblk, nsplit), dim3((P1_CW + 1) * 32), P1Cfg<NB>::SMEM, st, g->pdl,
+                  (const c128 *)kp->d_beta1.p, kp->nkc, psi_in, kp->ng, nb, band0, kp->d_Ppart.p, nrows_pad, nsplit);
     g->prof.end(st);
     const int qcount = kp->nic * P2_KS * NB;
     if (16 % kp->dblock == 0 && kp->nic * P2_KS <= nrows_pad) {
         g->prof.begin(QM_K_PREDUCE, st);      // fused split-K reduction + D multiply
-        k_reduce_dmul<NB><<<(kp->nic * P2_KS) / 16, 16 * NB, 0, st>>>(kp->d_Ppart.p, nsplit, nrows_pad, kp->d_D.p, kp->dblock,
-                                                                      kp->nproj, kp->d_qt.p);
+        qm_launch_pdl(k_reduce_dmul<NB>, dim3((kp->nic * P2_KS) / 16), dim3(16 * NB), 0, st, g->pdl, (const c128 *)kp->d_Ppart.p, nsplit,
+                      nrows_pad, (const double *)kp->d_D.p, kp->dblock, kp->nproj, kp->d_qt.p);
         g->prof.end(st);
         g->launches += 2;
     } else {
@@ -258,9 +258,10 @@ template <int NB>
 void nonlocal_expand(qm_gspace *g, KPoint *kp, const NlPlan &p, c128 *out, int nb, int band0, cudaStream_t st) {
     const int ncta2 = p.ncta2;
     g->prof.begin(QM_K_PROJ2, st);
-    k_proj2_sk<NB><<<ncta2, (P2_CW + 1) * 32, P2Cfg<NB>::SMEM, st>>>(kp->d_beta2.p, kp->nic, kp->ngt, kp->d_qt.p, kp->ng, nb,
-                                                                     band0, out, kp->d_part.p, kp->d_pdesc.p);
-    k_proj2_fixup<NB><<<2 * ncta2, 256, 0, st>>>(kp->d_part.p, kp->d_pdesc.p, 2 * ncta2, kp->ng, nb, band0, out);
+    qm_launch_pdl(k_proj2_sk<NB>, dim3(ncta2), dim3((P2_CW + 1) * 32), P2Cfg<NB>::SMEM, st, g->pdl, (const c128 *)kp->d_beta2.p, kp->nic,
+                  kp->ngt, (const double *)kp->d_qt.p, kp->ng, nb, band0, out, kp->d_part.p, kp->d_pdesc.p);
+    qm_launch_pdl(k_proj2_fixup<NB>, dim3(2 * ncta2), dim3(256), 0, st, g->pdl, (const c128 *)kp->d_part.p, (const int *)kp->d_pdesc.p,
+                  2 * ncta2, kp->ng, nb, band0, out);
     g->prof.end(st);
     g->launches += 2;
 }
@@ -401,6 +402,7 @@ QM_API int qm_gspace_create(const double *lattice_bohr, double ecutwfc_ry, const
             if (plane_smem(g, kp, 1) > (size_t)g->max_smem) g->fused = false;
     if (const char *e = getenv("QM_FORCE_UNFUSED")) if (atoi(e) > 0) g->fused = false;
     if (const char *e = getenv("QM_NL_OVERLAP")) g->nl_overlap = atoi(e) != 0;
+    if (const char *e = getenv("QM_PDL")) g->pdl = atoi(e) != 0;
     rc = prepare_kernels(g);
     if (rc != QM_OK) return bail(rc);
     if (const char *e = getenv("QM_PLANE_STAGGER_NS")) g->plane_stagger_ns = atoi(e);

@@ -145,6 +145,7 @@ struct qm_gspace {
     bool so_set = false;
     double so_dt = 0.0;
     unsigned long long launches = 0;
+    bool pdl = true;                // programmatic dependent launch between the kernels of an apply (QM_PDL=0: off)
     bool nl_overlap = true;         // projection GEMM of an apply on a side stream beside the FFT path (QM_NL_OVERLAP=0: off)
     bool fused = true;              // the fused plane kernel takes this box (else: the unfused passes, gen_kernels.cuh)
     int device = 0;                 // the CUDA device the handle was created on (every call checks it)
@@ -221,6 +222,20 @@ inline int z_grid_x(const qm_gspace *g, int ntiles, int nb, int cta_per_sm) {
     if (gx >= ntiles) return ntiles;
     const int rounds = (ntiles + gx - 1) / gx;          // fewest CTAs that keep the same number of rounds
     return (ntiles + rounds - 1) / rounds;
+}
+
+// Kernel launch with the programmatic-serialisation attribute (async_copy.cuh pdl_wait): only for kernels that call
+// pdl_wait() before they touch global memory.
+template <class... KArgs, class... Args>
+inline cudaError_t qm_launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl,
+                                 Args &&...args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(std::forward<Args>(args))...);
 }
 
 struct PlaneArgs {          // operands of the plane kernel beyond the stick planes W

@@ -35,9 +35,9 @@ template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *W,
     // persistent: one CTA per SM walks the (band, z-plane) list; density mode: one CTA per z-plane, all bands
     const int grid = MODE == 3 ? std::min(g->grid[2], g->sm_count) : std::min(nplanes, g->sm_count * cps);
     g->prof.begin(QM_K_PLANE, st);
-    k_plane<C, MODE><<<grid, ngroups * PLANE_GROUP, smem, st>>>(kp->plan(), gd, W, a.box, a.box2, a.npair2, ngroups, a.scale,
-                                                                   g->plane_stagger_ns, nplanes,
-                                                                   (kp->y_quarter ? 1 : 0) | (kp->x_quarter ? 2 : 0) | (rowtab ? 4 : 0), a.occ, a.rhot);
+    CU_TRY(qm_launch_pdl(k_plane<C, MODE>, dim3(grid), dim3(ngroups * PLANE_GROUP), smem, st, g->pdl, kp->plan(), gd, W, a.box, a.box2,
+                         a.npair2, ngroups, a.scale, g->plane_stagger_ns, nplanes,
+                         (kp->y_quarter ? 1 : 0) | (kp->x_quarter ? 2 : 0) | (rowtab ? 4 : 0), a.occ, a.rhot));
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());

@@ -9,8 +9,8 @@ template <class C, bool PH> int launch_zinv(qm_gspace *g, KPoint *kp, const c128
     const int ntiles = (kp->nsticks + QM_ZT - 1) / QM_ZT;
     dim3 grid(z_grid_x(g, ntiles, nb, g->z_cta_per_sm), nb);
     g->prof.begin(QM_K_ZINV, st);
-    k_zinv<C, PH><<<grid, QM_ZT * C::TT, qm_z_smem<C>(), st>>>(kp->plan(), g->d_tw[2].p, psi, phase, W, ntiles,
-                                                                kp->z_quarter ? 1 : 0);
+    CU_TRY(qm_launch_pdl(k_zinv<C, PH>, grid, dim3(QM_ZT * C::TT), qm_z_smem<C>(), st, g->pdl, kp->plan(), g->d_tw[2].p, psi, phase, W,
+                         ntiles, kp->z_quarter ? 1 : 0));
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
@@ -21,8 +21,8 @@ template <class C, int GM> int launch_zfwd(qm_gspace *g, KPoint *kp, const c128 
     const int ntiles = (kp->nsticks + QM_ZT - 1) / QM_ZT;
     dim3 grid(z_grid_x(g, ntiles, nb, g->z_cta_per_sm), nb);
     g->prof.begin(QM_K_ZFWD, st);
-    k_zfwd<C, GM><<<grid, QM_ZT * C::TT, qm_z_smem<C>(), st>>>(kp->plan(), g->d_tw[2].p, W, aux, out, ntiles, scale,
-                                                                kp->z_quarter ? 1 : 0);
+    CU_TRY(qm_launch_pdl(k_zfwd<C, GM>, grid, dim3(QM_ZT * C::TT), qm_z_smem<C>(), st, g->pdl, kp->plan(), g->d_tw[2].p, W, aux, out,
+                         ntiles, scale, kp->z_quarter ? 1 : 0));
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
