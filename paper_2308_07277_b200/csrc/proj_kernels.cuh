@@ -25,6 +25,9 @@ __device__ __forceinline__ double2 ldg_c128(const c128 *p) {
 //   beta1[mblk][kc][128 rows][16 k]  element (r,k) at r*16 + (k ^ ((r&1)<<2))      (GEMM 1, one 32 KB copy/stage)
 //   beta2[gt][ic][16 i][64 G]        element (i,g) at i*64 + (g ^ ((i&3)<<1))      (GEMM 2, one 16 KB copy/stage)
 // The XOR swizzles make every DMMA fragment load (one 16-byte LDS per thread) bank-conflict free.
+#ifndef QM_BETA_EVICT_FIRST
+#define QM_BETA_EVICT_FIRST 1   /* beta tiles are loaded with the L2 evict-first policy (read once per GEMM) */
+#endif
 #ifndef QM_P1_ROWS
 #define QM_P1_ROWS 128      /* projector rows per CTA of GEMM 1 (16 per consumer warp) */
 #endif
@@ -122,6 +125,9 @@ k_proj1_pipe(const c128 *__restrict__ beta1, int nkc, const c128 *__restrict__ p
 
     if (warp == P1_CW) {
         // ---- producer warp: one 32 KB bulk copy of the beta tile + one row copy per band ----
+#if QM_BETA_EVICT_FIRST
+        const uint64_t pol = l2_policy_evict_first();
+#endif
         for (int it = 0; it < nit; ++it) {
             const int s = it % P1_ST;
             if (it >= P1_ST) mbar_wait(&empty[s], ((it / P1_ST) - 1) & 1);
@@ -136,7 +142,11 @@ k_proj1_pipe(const c128 *__restrict__ beta1, int nkc, const c128 *__restrict__ p
             __syncwarp();
             if (lane == 0) {
                 mbar_expect_tx(&full[s], (uint32_t)(P1_BETA_BYTES + nvalid * nk * 16));
+#if QM_BETA_EVICT_FIRST
+                bulk_g2s_hint(stage, beta1 + ((size_t)mb * nkc + kc) * (P1_ROWS * P1_KS), P1_BETA_BYTES, &full[s], pol);
+#else
                 bulk_g2s(stage, beta1 + ((size_t)mb * nkc + kc) * (P1_ROWS * P1_KS), P1_BETA_BYTES, &full[s]);
+#endif
             }
             __syncwarp();
             if (lane < nvalid)
@@ -297,12 +307,19 @@ k_proj2_sk(const c128 *__restrict__ beta2, int nic, int ngt, const double *__res
     __syncthreads();
     if (warp == P2_CW) {
         if (lane == 0) {
+#if QM_BETA_EVICT_FIRST
+            const uint64_t pol = l2_policy_evict_first();
+#endif
             for (int st = s_begin; st < s_end; ++st) {
                 const int it = st - s_begin, s = it % ST;
                 if (it >= ST) mbar_wait(&empty[s], ((it / ST) - 1) & 1);
                 unsigned char *stage = smem + s * STAGE;
                 mbar_expect_tx(&full[s], STAGE);
+#if QM_BETA_EVICT_FIRST
+                bulk_g2s_hint(stage, beta2 + (size_t)st * (P2_KS * P2_G), P2_BETA_BYTES, &full[s], pol);    // layout [gt][ic] == st
+#else
                 bulk_g2s(stage, beta2 + (size_t)st * (P2_KS * P2_G), P2_BETA_BYTES, &full[s]);    // layout [gt][ic] == st
+#endif
                 bulk_g2s(stage + P2_BETA_BYTES, qt + (size_t)(st % nic) * Q::Q_DOUBLES, Q::Q_BYTES, &full[s]);
             }
         }
