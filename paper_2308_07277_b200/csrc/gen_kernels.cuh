@@ -12,6 +12,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include "fft_phases.cuh"
+#include "async_copy.cuh"
 #include "qm_plan.h"
 
 #ifndef QM_GEN_X_MINB
@@ -56,6 +57,8 @@ k_gen_y(QmKPlanDev kp, const c128 *__restrict__ tw, c128 *__restrict__ W, c128 *
     c128 *lines = reinterpret_cast<c128 *>(gen_smem);                  // [TPG][LP] (forward: two sets)
     TwRow<BACK ? C::R1 : C::R2> twr;
     load_twrow(twr, tw, u, BACK ? C::R2 : C::R1);
+    pdl_launch_dependents();
+    pdl_wait();                 // W and the slab come from the previous kernels
     const int items = nbp * X, nchunks = (items + TPG - 1) / TPG;            // 32-bit: a launch holds < 2^31 rows (host checks)
     // rows of a chunk are consecutive slab rows: row (chunk * TPG + t) of the launch at slab + that * N
     auto rows_in = [&](int chunk) { return max(0, min(TPG, items - chunk * TPG)); };
@@ -169,6 +172,8 @@ k_gen_x(QmKPlanDev kp, const c128 *__restrict__ tw, const double *__restrict__ v
             gen_cp_async16(buf + r * TCP + cc, plane + (size_t)r * n2 + (in ? c0 + cc : 0), in ? 16 : 0);
         }
     };
+    pdl_launch_dependents();
+    pdl_wait();                 // the slab (and the boxes) come from the previous kernels
     int cur = 0;
     if constexpr (LOADS) {
         if ((long long)blockIdx.x < ntiles) stage(blockIdx.x, 0, tiles);

@@ -20,8 +20,8 @@ template <class C, bool BACK> int launch_gen_y(qm_gspace *g, KPoint *kp, c128 *W
     const unsigned grid = (unsigned)std::min<long long>(nchunks, (long long)g->sm_count * std::max(1, per_sm));
     const size_t wband = (size_t)((kp->nsticks + QM_ZT - 1) / QM_ZT) * QM_ZT * g->grid[2];
     g->prof.begin(QM_K_GENY, st);
-    k_gen_y<C, BACK><<<grid, GEN_GROUP, GG::y_smem(), st>>>(kp->plan(), g->d_tw[1].p, W, slab, g->grid[2], bp0, nbp,
-                                                             kp->y_quarter ? 1 : 0, wband);
+    CU_TRY(qm_launch_pdl(k_gen_y<C, BACK>, dim3(grid), dim3(GEN_GROUP), GG::y_smem(), st, g->pdl, kp->plan(), (const c128 *)g->d_tw[1].p,
+                         W, slab, g->grid[2], bp0, nbp, kp->y_quarter ? 1 : 0, wband));
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
@@ -41,9 +41,9 @@ template <class C, int MODE> int launch_gen_x(qm_gspace *g, KPoint *kp, c128 *sl
     CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_gen_x<C, MODE>, GG::XG * GEN_GROUP, smem));
     const unsigned grid = (unsigned)std::min<long long>(tiles, (long long)g->sm_count * std::max(1, per_sm));
     g->prof.begin(QM_K_GENX, st);
-    k_gen_x<C, MODE><<<grid, GG::XG * GEN_GROUP, smem, st>>>(kp->plan(), g->d_tw[0].p, g->d_vt.p, slab, a.box, a.box2, a.npair2,
-                                                             a.scale, n2, n3, bp0, nbp,
-                                                             (kp->y_quarter ? 1 : 0) | (kp->x_quarter ? 2 : 0), a.occ, a.rhot);
+    CU_TRY(qm_launch_pdl(k_gen_x<C, MODE>, dim3(grid), dim3(GG::XG * GEN_GROUP), smem, st, g->pdl, kp->plan(), (const c128 *)g->d_tw[0].p,
+                         (const double *)g->d_vt.p, slab, a.box, a.box2, a.npair2, a.scale, n2, n3, bp0, nbp,
+                         (kp->y_quarter ? 1 : 0) | (kp->x_quarter ? 2 : 0), a.occ, a.rhot));
     g->prof.end(st);
     g->launches++;
     CU_TRY(cudaGetLastError());
