@@ -45,7 +45,7 @@ template <int N> __device__ __forceinline__ void gen_cp_async_wait() { asm volat
 // apart: one wavefront per lane, measured 2.4 x slower): backward, the finished lines are copied out of shared memory;
 // forward, the rows of the NEXT chunk land asynchronously in a second set of lines while this chunk is transformed.
 template <class C, bool BACK>
-__global__ void __launch_bounds__(GEN_GROUP)
+__global__ void __launch_bounds__(GEN_GROUP, QM_GEN_X_MINB)
 k_gen_y(QmKPlanDev kp, const c128 *__restrict__ tw, c128 *__restrict__ W, c128 *__restrict__ slab, int n3, int bp0, int nbp,
         int quarter, size_t wband)
 {
