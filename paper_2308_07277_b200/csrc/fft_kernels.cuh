@@ -202,16 +202,37 @@ struct PlaneCtx {
 #ifndef QM_TW_CHUNK
 #define QM_TW_CHUNK 4
 #endif
+#ifndef QM_TW_PIPELINE
+#define QM_TW_PIPELINE 1        /* read chunk c + 1 from tensor memory while chunk c is multiplied */
+#endif
 template <class C, bool DIRB, int NR, int R, class L>
 __device__ __forceinline__ void plane_tail(const c128 (&t)[NR][R], const L (&dst)[NR], int u, const TwRow<R> &in_regs, uint32_t taddr)
 {
-#if QM_PLANE_TW_TMEM
+#if QM_PLANE_TW_TMEM && QM_TW_PIPELINE
+    // chunk c + 1 is read while chunk c is multiplied: two raw register sets, used alternately
+    constexpr int NCH = (R + QM_TW_CHUNK - 1) / QM_TW_CHUNK;
+    int raw[2][4][4];
+    auto lo = [](int c) constexpr { return c == 0 ? 1 : c * QM_TW_CHUNK; };
+    auto hi = [](int c) constexpr { return (c + 1) * QM_TW_CHUNK < R ? (c + 1) * QM_TW_CHUNK : R; };
+    if constexpr (lo(0) < hi(0)) tmem_issue<hi(0) - lo(0)>(raw[0], taddr + 4 * lo(0));
+    static_for<NCH>([&](auto I) {
+        constexpr int c = decltype(I)::value;
+        constexpr int j0 = c * QM_TW_CHUNK, j1 = hi(c), l0 = lo(c);
+        TwChunk<l0, (l0 < j1 ? j1 : l0 + 1)> ch;
+        if constexpr (l0 < j1) tmem_land(ch, raw[c & 1]);
+        if constexpr (c + 1 < NCH) tmem_issue<hi(c + 1) - lo(c + 1)>(raw[(c + 1) & 1], taddr + 4 * lo(c + 1));
+        static_for<NR>([&](auto II) {
+            constexpr int i = decltype(II)::value;
+            if constexpr (DIRB) stepB1_tail_range<C, j0, j1, false>(t[i], dst[i], u, ch);
+            else stepA1_tail_range<C, j0, j1, false>(t[i], dst[i], u, ch);
+        });
+    });
+#elif QM_PLANE_TW_TMEM
     static_for<(R + QM_TW_CHUNK - 1) / QM_TW_CHUNK>([&](auto I) {
         constexpr int j0 = decltype(I)::value * QM_TW_CHUNK, j1 = j0 + QM_TW_CHUNK < R ? j0 + QM_TW_CHUNK : R;
         constexpr int l0 = j0 == 0 ? 1 : j0;            // factor 0 is 1 and is not stored
         TwChunk<l0, (l0 < j1 ? j1 : l0 + 1)> ch;
-        if constexpr (l0 < j1) tmem_load_chunk(ch, taddr);
-        static_for<NR>([&](auto II) {
+        if constexpr (l0 < j1) tmem_load_chunk(ch, taddr);        static_for<NR>([&](auto II) {
             constexpr int i = decltype(II)::value;
             if constexpr (DIRB) stepB1_tail_range<C, j0, j1, false>(t[i], dst[i], u, ch);
             else stepA1_tail_range<C, j0, j1, false>(t[i], dst[i], u, ch);

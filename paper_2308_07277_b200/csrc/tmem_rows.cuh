@@ -81,3 +81,37 @@ template <int J0, int J1> __device__ __forceinline__ void tmem_load_chunk(TwChun
         t.w[i] = c128{__hiloint2double(r[i][1], r[i][0]), __hiloint2double(r[i][3], r[i][2])};
     });
 }
+
+// The same in two halves, so that the next chunk's read is in flight while the current chunk is used: issue (tcgen05.ld
+// only) and land (tcgen05.wait::ld, then the raw registers pass through an empty asm statement so that no use can be
+// scheduled ahead of the wait).  tcgen05.wait::ld covers every read issued before it.
+template <int K> __device__ __forceinline__ void tmem_issue(int (&r)[4][4], uint32_t a) {
+    static_assert(K >= 1 && K <= 4, "chunk of 1..4 factors");
+    if constexpr (K == 4)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                     : "=r"(r[0][0]), "=r"(r[0][1]), "=r"(r[0][2]), "=r"(r[0][3]), "=r"(r[1][0]), "=r"(r[1][1]), "=r"(r[1][2]), "=r"(r[1][3]),
+                       "=r"(r[2][0]), "=r"(r[2][1]), "=r"(r[2][2]), "=r"(r[2][3]), "=r"(r[3][0]), "=r"(r[3][1]), "=r"(r[3][2]), "=r"(r[3][3])
+                     : "r"(a) : "memory");
+    else if constexpr (K == 3)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%12];\n"
+                     "tcgen05.ld.sync.aligned.32x32b.x4.b32 {%8, %9, %10, %11}, [%13];"
+                     : "=r"(r[0][0]), "=r"(r[0][1]), "=r"(r[0][2]), "=r"(r[0][3]), "=r"(r[1][0]), "=r"(r[1][1]), "=r"(r[1][2]), "=r"(r[1][3]),
+                       "=r"(r[2][0]), "=r"(r[2][1]), "=r"(r[2][2]), "=r"(r[2][3])
+                     : "r"(a), "r"(a + 8) : "memory");
+    else if constexpr (K == 2)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                     : "=r"(r[0][0]), "=r"(r[0][1]), "=r"(r[0][2]), "=r"(r[0][3]), "=r"(r[1][0]), "=r"(r[1][1]), "=r"(r[1][2]), "=r"(r[1][3])
+                     : "r"(a) : "memory");
+    else
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+                     : "=r"(r[0][0]), "=r"(r[0][1]), "=r"(r[0][2]), "=r"(r[0][3]) : "r"(a) : "memory");
+}
+template <int J0, int J1> __device__ __forceinline__ void tmem_land(TwChunk<J0, J1> &t, int (&r)[4][4]) {
+    constexpr int K = J1 - J0;
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+    static_for<K>([&](auto I) {
+        constexpr int i = decltype(I)::value;
+        asm volatile("" : "+r"(r[i][0]), "+r"(r[i][1]), "+r"(r[i][2]), "+r"(r[i][3]));
+        t.w[i] = c128{__hiloint2double(r[i][1], r[i][0]), __hiloint2double(r[i][3], r[i][2])};
+    });
+}
