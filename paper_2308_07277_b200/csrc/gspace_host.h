@@ -16,7 +16,7 @@ struct FftSize { int n, r1, r2; };
 static const FftSize kQmSizes[] = {
     {8, 2, 4},   {12, 3, 4},  {16, 4, 4},  {18, 3, 6},  {20, 4, 5},   {24, 4, 6},   {30, 5, 6},
     {32, 4, 8},  {36, 6, 6},  {40, 5, 8},  {48, 6, 8},  {60, 6, 10},  {64, 8, 8},   {72, 8, 9},
-    {80, 8, 10}, {96, 8, 12}, {100, 10, 10}, {108, 9, 12}, {120, 10, 12}, {128, 8, 16}, {144, 12, 12},
+    {80, 8, 10}, {96, 12, 8}, {100, 10, 10}, {108, 9, 12}, {120, 10, 12}, {128, 8, 16}, {144, 12, 12},
     // above 144: z kernels and the unfused xy passes only (the fused plane kernel is not compiled for them)
     {160, 10, 16}, {180, 12, 15}, {192, 12, 16}, {225, 15, 15}, {240, 15, 16}, {256, 16, 16},
 };

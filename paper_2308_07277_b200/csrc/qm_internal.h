@@ -251,13 +251,13 @@ struct PlaneArgs {          // operands of the plane kernel beyond the stick pla
 // QM_FOR_SIZES: the lengths the fused plane kernel is compiled for; QM_FOR_SIZES_ALL adds the lengths above 144 that only the
 // z kernels and the unfused passes take (gspace_host.h kQmSizes lists them all).
 #ifdef QM_DEV_SIZES      /* developer builds: only the lengths of the five BASELINE.json configs (fast compile) */
-#define QM_FOR_SIZES(X) X(12, 3, 4) X(24, 4, 6) X(32, 4, 8) X(48, 6, 8) X(96, 8, 12) X(144, 12, 12)
+#define QM_FOR_SIZES(X) X(12, 3, 4) X(24, 4, 6) X(32, 4, 8) X(48, 6, 8) X(96, 12, 8) X(144, 12, 12)
 #define QM_FOR_SIZES_ALL(X) QM_FOR_SIZES(X) X(36, 6, 6) X(192, 12, 16)
 #else
 #define QM_FOR_SIZES(X)                                                                              \
     X(8, 2, 4) X(12, 3, 4) X(16, 4, 4) X(18, 3, 6) X(20, 4, 5) X(24, 4, 6) X(30, 5, 6) X(32, 4, 8)   \
     X(36, 6, 6) X(40, 5, 8) X(48, 6, 8) X(60, 6, 10) X(64, 8, 8) X(72, 8, 9) X(80, 8, 10)            \
-    X(96, 8, 12) X(100, 10, 10) X(108, 9, 12) X(120, 10, 12) X(128, 8, 16) X(144, 12, 12)
+    X(96, 12, 8) X(100, 10, 10) X(108, 9, 12) X(120, 10, 12) X(128, 8, 16) X(144, 12, 12)
 #define QM_FOR_SIZES_ALL(X) QM_FOR_SIZES(X) X(160, 10, 16) X(180, 12, 15) X(192, 12, 16) X(225, 15, 15) X(240, 15, 16) X(256, 16, 16)
 #endif
 

@@ -211,7 +211,7 @@ int main(int argc, char **argv) {
 #define X(N, A, B) case N: return run<LineCfg<A, B>>(n, lat.data(), ecut, k, nb, argv[8], argv[9], argv[10]);
         X(8, 2, 4) X(12, 3, 4) X(16, 4, 4) X(18, 3, 6) X(20, 4, 5) X(24, 4, 6) X(30, 5, 6) X(32, 4, 8)
         X(36, 6, 6) X(40, 5, 8) X(48, 6, 8) X(60, 6, 10) X(64, 8, 8) X(72, 8, 9) X(80, 8, 10)
-        X(96, 8, 12) X(100, 10, 10) X(108, 9, 12) X(120, 10, 12) X(128, 8, 16) X(144, 12, 12)
+        X(96, 12, 8) X(100, 10, 10) X(108, 9, 12) X(120, 10, 12) X(128, 8, 16) X(144, 12, 12)
         X(160, 10, 16) X(180, 12, 15) X(192, 12, 16) X(225, 15, 15) X(240, 15, 16) X(256, 16, 16)
 #undef X
     }
