@@ -205,10 +205,19 @@ struct PlaneCtx {
 #ifndef QM_TW_PIPELINE
 #define QM_TW_PIPELINE 1        /* read chunk c + 1 from tensor memory while chunk c is multiplied */
 #endif
+// Which line factorisations park their rows in tensor memory: those whose rows would take 44 registers or more (12 x 12: 44,
+// 12 x 8: 72).  Measured per size, tensor memory against registers: 96 = 12 x 8 -20 %, 144 = 12 x 12 -5 %, 48 = 6 x 8 (48
+// registers) equal, 32 = 4 x 8 (40 registers) +12 %: short rows are cheaper to keep than to fetch.
+#ifndef QM_TW_TMEM_MIN_REGS
+#define QM_TW_TMEM_MIN_REGS 44
+#endif
+template <class C> constexpr bool plane_tw_tmem =
+    (QM_PLANE_TW_TMEM != 0) && (4 * (C::R1 - 1) + (C::R1 != C::R2 ? 4 * (C::R2 - 1) : 0) >= QM_TW_TMEM_MIN_REGS);
+
 template <class C, bool DIRB, int NR, int R, class L>
 __device__ __forceinline__ void plane_tail(const c128 (&t)[NR][R], const L (&dst)[NR], int u, const TwRow<R> &in_regs, uint32_t taddr)
 {
-#if QM_PLANE_TW_TMEM && QM_TW_PIPELINE
+  if constexpr (plane_tw_tmem<C> && QM_TW_PIPELINE) {
     // chunk c + 1 is read while chunk c is multiplied: two raw register sets, used alternately
     constexpr int NCH = (R + QM_TW_CHUNK - 1) / QM_TW_CHUNK;
     int raw[2][4][4];
@@ -227,7 +236,7 @@ __device__ __forceinline__ void plane_tail(const c128 (&t)[NR][R], const L (&dst
             else stepA1_tail_range<C, j0, j1, false>(t[i], dst[i], u, ch);
         });
     });
-#elif QM_PLANE_TW_TMEM
+  } else if constexpr (plane_tw_tmem<C>) {
     static_for<(R + QM_TW_CHUNK - 1) / QM_TW_CHUNK>([&](auto I) {
         constexpr int j0 = decltype(I)::value * QM_TW_CHUNK, j1 = j0 + QM_TW_CHUNK < R ? j0 + QM_TW_CHUNK : R;
         constexpr int l0 = j0 == 0 ? 1 : j0;            // factor 0 is 1 and is not stored
@@ -238,13 +247,13 @@ __device__ __forceinline__ void plane_tail(const c128 (&t)[NR][R], const L (&dst
             else stepA1_tail_range<C, j0, j1, false>(t[i], dst[i], u, ch);
         });
     });
-#else
+  } else {
     static_for<NR>([&](auto II) {
         constexpr int i = decltype(II)::value;
         if constexpr (DIRB) stepB1_tail_range<C, 0, R, false>(t[i], dst[i], u, in_regs);
         else stepA1_tail_range<C, 0, R, false>(t[i], dst[i], u, in_regs);
     });
-#endif
+  }
 }
 // Scratch lines: one per team, plus one sink line per group (behind the group's team lines) when some lane of a group
 // can be without work in a pass (R1 != R2, or G not a multiple of TT).
@@ -434,16 +443,16 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
             if constexpr (QM_PLANE_XTW_LATE) {
                 c128 t[C::R1];
                 stepB2_load<C>(scrA[0], id.u2, t);
-#if QM_PLANE_TW_TMEM
-                static_for<(C::R1 + QM_TW_CHUNK - 1) / QM_TW_CHUNK>([&](auto I) {
-                    constexpr int j0 = decltype(I)::value * QM_TW_CHUNK, j1 = j0 + QM_TW_CHUNK < C::R1 ? j0 + QM_TW_CHUNK : C::R1;
-                    constexpr int l0 = j0 == 0 ? 1 : j0;
-                    TwChunk<l0, (l0 < j1 ? j1 : l0 + 1)> ch;
-                    if constexpr (l0 < j1) { tmem_load_chunk(ch, cx.tw_a); stepB2_twiddle_range<C, l0, j1>(t, ch); }
-                });
-#else
-                stepB2_twiddle_range<C, 0, C::R1>(t, twa);
-#endif
+                if constexpr (plane_tw_tmem<C>) {
+                    static_for<(C::R1 + QM_TW_CHUNK - 1) / QM_TW_CHUNK>([&](auto I) {
+                        constexpr int j0 = decltype(I)::value * QM_TW_CHUNK, j1 = j0 + QM_TW_CHUNK < C::R1 ? j0 + QM_TW_CHUNK : C::R1;
+                        constexpr int l0 = j0 == 0 ? 1 : j0;
+                        TwChunk<l0, (l0 < j1 ? j1 : l0 + 1)> ch;
+                        if constexpr (l0 < j1) { tmem_load_chunk(ch, cx.tw_a); stepB2_twiddle_range<C, l0, j1>(t, ch); }
+                    });
+                } else {
+                    stepB2_twiddle_range<C, 0, C::R1>(t, twa);
+                }
                 stepB2_finish<C>(t, Acol, C::R2 * RP, pxc, xq);
             } else {
                 if (xq) prunedB_step2_quarter<C, false>(scrA[0], Acol, C::R2 * RP, pxc, id.u2);
@@ -496,23 +505,24 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
         if constexpr (C::R1 == C::R2) return twa; else return twb_store;
     }();
     cx.tw_a = cx.tw_b = 0;
-#if QM_PLANE_TW_TMEM
-    // ... and parked in tensor memory: 4 columns per factor in the warp's lane window, one column range per warp of an
-    // SM sub-partition (warps w, w+4, w+8, ... share a lane window)
-    constexpr int ROWCOLS = 4 * C::R1 + (C::R1 != C::R2 ? 4 * C::R2 : 0);
-    uint32_t &tmem_base_s = *reinterpret_cast<uint32_t *>(rowinfo_s + cx.X);      // the 16 bytes behind the row table
-    const uint32_t tmem_cols = (uint32_t)qm_tmem_cols_pow2(ROWCOLS * (int)((blockDim.x / 32 + 3) / 4));
-    if (threadIdx.x < 32) tmem_alloc(&tmem_base_s, tmem_cols);
-    tmem_fence_before_sync();
-    __syncthreads();
-    tmem_fence_after_sync();
-    const uint32_t tmem_base = tmem_base_s;
-    cx.tw_a = tmem_warp_addr(tmem_base, 0, ROWCOLS);
-    cx.tw_b = C::R1 != C::R2 ? cx.tw_a + 4 * C::R1 : cx.tw_a;
-    tmem_store_row(cx.tw_a, twa);
-    if constexpr (C::R1 != C::R2) tmem_store_row(cx.tw_b, twb_store);
-    tmem_wait_st();
-#endif
+    uint32_t tmem_base = 0, tmem_cols = 0;
+    if constexpr (plane_tw_tmem<C>) {
+        // ... and parked in tensor memory: 4 columns per factor in the warp's lane window, one column range per warp of an
+        // SM sub-partition (warps w, w+4, w+8, ... share a lane window)
+        constexpr int ROWCOLS = 4 * C::R1 + (C::R1 != C::R2 ? 4 * C::R2 : 0);
+        uint32_t &tmem_base_s = *reinterpret_cast<uint32_t *>(rowinfo_s + cx.X);      // the 16 bytes behind the row table
+        tmem_cols = (uint32_t)qm_tmem_cols_pow2(ROWCOLS * (int)((blockDim.x / 32 + 3) / 4));
+        if (threadIdx.x < 32) tmem_alloc(&tmem_base_s, tmem_cols);
+        tmem_fence_before_sync();
+        __syncthreads();
+        tmem_fence_after_sync();
+        tmem_base = tmem_base_s;
+        cx.tw_a = tmem_warp_addr(tmem_base, 0, ROWCOLS);
+        cx.tw_b = C::R1 != C::R2 ? cx.tw_a + 4 * C::R1 : cx.tw_a;
+        tmem_store_row(cx.tw_a, twa);
+        if constexpr (C::R1 != C::R2) tmem_store_row(cx.tw_b, twb_store);
+        tmem_wait_st();
+    }
     pdl_launch_dependents();
     pdl_wait();                 // the stick planes (and boxes) come from the previous kernel
     const int n3 = cx.n3;
@@ -541,9 +551,9 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
         __syncthreads();
         prev = pl;
     }
-#if QM_PLANE_TW_TMEM
-    tmem_fence_before_sync();
-    __syncthreads();
-    if (threadIdx.x < 32) tmem_dealloc(tmem_base, tmem_cols);
-#endif
+    if constexpr (plane_tw_tmem<C>) {
+        tmem_fence_before_sync();
+        __syncthreads();
+        if (threadIdx.x < 32) tmem_dealloc(tmem_base, tmem_cols);
+    }
 }

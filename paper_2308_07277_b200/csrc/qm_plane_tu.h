@@ -13,13 +13,11 @@ template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *W,
     // twiddle rows in tensor memory: cfg4 -5 %, cfg3 -15 %, cfg2 -11 % plane-kernel time; cfg5's plane array allows one)
     int cps = MODE == 3 ? 1 : (g->plane_ctas_per_sm > 0 ? g->plane_ctas_per_sm : 2);
     int ngroups = plane_groups(g, kp, cps);
-#if QM_PLANE_TW_TMEM
     // every resident CTA allocates its own tensor-memory columns (512 per SM): one CTA per SM if two do not fit
-    if (cps > 1 && ngroups > 0) {
+    if (plane_tw_tmem<C> && cps > 1 && ngroups > 0) {
         const int rowcols = 4 * C::R1 + (C::R1 != C::R2 ? 4 * C::R2 : 0);
         if (cps * qm_tmem_cols_pow2(rowcols * ((ngroups * PLANE_GROUP / 32 + 3) / 4)) > 512) ngroups = 0;
     }
-#endif
     if (ngroups == 0) { cps = 1; ngroups = plane_groups(g, kp, 1); }
     size_t smem = plane_smem(g, kp, ngroups);
     if (ngroups == 0 || smem > (size_t)g->max_smem)
