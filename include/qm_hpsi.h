@@ -209,6 +209,43 @@ QM_API int qm_matrix_elements(qm_mtxel *m, const qm_c128 *bra_dev, int nbra, con
 QM_API int qm_subspace(qm_gspace *g, int k, const qm_c128 *a_dev, int na, const qm_c128 *b_dev, int nb,
                 qm_c128 *s_dev, void *stream);
 
+/* qm_subspace for callers that are not allowed to allocate device memory: the same product, the same kernels, the same
+ * summation order (hence the same bits as qm_subspace on the same device), but no handle and no cudaMalloc anywhere.
+ *
+ * Who needs this.  qm_subspace keeps its split-K partial sums in a buffer it cudaMallocs on first use.  That is not
+ * possible for (1) a host application whose own memory pool (a framework's caching allocator, a DFT code's arena) has
+ * already claimed almost the whole device, so a cudaMalloc from inside this library fails with out-of-memory although
+ * the caller has buffers to hand out; (2) a solver iteration that keeps several streams busy: cudaMalloc and cudaFree
+ * synchronise the whole device, so one growing work space stalls every stream, not just the caller's; (3) a job that
+ * runs under a fixed memory budget and must know the footprint of this library when it is loaded, not when a larger
+ * block first arrives.  For them the partial sums live in ONE fixed array that is part of the library image
+ * (static __device__, QM_SUBSPACE_STATIC_MAX_ELEMS complex128 = 16 MiB): every GPU on which the library's kernels are
+ * loaded carries these 16 MiB until the process exits, whether or not this function is ever called.
+ *
+ *  a_dev  DEVICE  [na][ng] row-major complex128     b_dev  DEVICE  [nb][ng] row-major complex128     (16-byte aligned)
+ *  s_dev  DEVICE  [na][nb] row-major complex128, overwritten; must not overlap a or b.  a == b is allowed.
+ *  ng             row length = number of plane waves of the sphere (what qm_gspace_num_g reports); no handle is needed.
+ * The caller owns all three buffers; the call allocates no device memory (no cudaMalloc, cudaMallocAsync, cudaFree,
+ * and no library routine that would) -- not on the first call either.  It runs on the current device.
+ *
+ * Limit.  The partial sums of one call need  ceil(na/64)*64 * ceil(nb/64)*64  elements per K split and must fit the
+ * array: blocks up to 1024 x 1024 states (or 512 x 2048, ...) are taken; beyond that the call returns QM_EINVAL and
+ * touches nothing -- use qm_subspace there.  Inside the limit the split count is the one qm_subspace would choose.
+ *
+ * First call on a device.  It looks up the device address of the array (cudaGetSymbolAddress), reads the SM count and
+ * opts the GEMM kernel into its shared-memory size; these are synchronous set-up calls, remembered per device.  Make
+ * that first call during start-up, outside any stream capture; later calls on that device only enqueue two kernels on
+ * `stream`.
+ *
+ * Sharing.  There is one array per device and every call uses it.  Nothing in it has to start at zero: each call
+ * writes every partial sum it later reads, so whatever the previous call left behind is ignored.  But two calls whose
+ * kernels can run at the same time on one GPU (different streams without an ordering between them, or two host
+ * threads) overwrite each other's partial sums and both results are garbage -- the library cannot see this.  Order such
+ * calls on one stream or with events.  Different GPUs have different copies and do not interfere. */
+#define QM_SUBSPACE_STATIC_MAX_ELEMS (1u << 20)
+QM_API int qm_subspace_static(const qm_c128 *a_dev, int na, const qm_c128 *b_dev, int nb, int ng, qm_c128 *s_dev,
+                              void *stream);
+
 /* Same operation with HOST buffers (pinned memory recommended): the library copies psi_in to
  * a library-owned device buffer, applies H, copies the result back, all on `stream`, then
  * synchronises the stream.  This is the end-to-end entry bench.py times. */

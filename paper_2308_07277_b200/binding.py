@@ -55,6 +55,7 @@ _SIGS = {
     "qm_mtxel_get_index_map": [_vp, _vp],
     "qm_matrix_elements": [_vp, _vp, _i, _vp, _i, _vp, _vp],
     "qm_subspace": [_vp, _i, _vp, _i, _vp, _i, _vp, _vp],
+    "qm_subspace_static": [_vp, _i, _vp, _i, _i, _vp, _vp],
     "qm_taylor_propagate": [_vp, _i, _vp, _vp, _i, _d, _i, _vp],
     "qm_density_reset": [_vp, _vp],
     "qm_density_accumulate": [_vp, _i, _vp, _i, _vp, _d, _vp],
@@ -327,6 +328,26 @@ def qm_subspace(h, a_dev, b_dev, s_dev=None, k=0, stream=None):
     _check(load_library().qm_subspace(h, k, _dev_ptr(a_dev, torch.complex128, "a"), na,
                                       _dev_ptr(b_dev, torch.complex128, "b"), nb,
                                       _dev_ptr(s_dev, torch.complex128, "s"), _stream_ptr(stream)))
+    return s_dev
+
+
+def qm_subspace_static(a_dev, b_dev, s_dev, stream=None):
+    """S[i][j] = <a_i|b_j> written into the caller's s_dev [na][nb], for callers that may not allocate device memory
+    (their pool owns the GPU, or a cudaMalloc would stall their other streams): no handle, and the split-K partial sums
+    sit in a fixed 16 MiB array inside the library instead of a cudaMalloc'ed buffer (include/qm_hpsi.h).  All three
+    tensors are the caller's -- unlike qm_subspace, this wrapper does not create the output either.  Blocks beyond
+    1024 x 1024 states (padded to 64) raise QM_EINVAL.  Calls that can overlap on one GPU race on the shared array."""
+    import torch
+    for t, what in ((a_dev, "a"), (b_dev, "b"), (s_dev, "s")):
+        if not isinstance(t, torch.Tensor) or t.dim() != 2:
+            raise TypeError(f"{what}: expected a 2-D CUDA torch.Tensor")
+    na, ng = a_dev.shape
+    nb = b_dev.shape[0]
+    if b_dev.shape[1] != ng or tuple(s_dev.shape) != (na, nb):
+        raise TypeError("expected a [na][ng], b [nb][ng], s [na][nb]")
+    _check(load_library().qm_subspace_static(_dev_ptr(a_dev, torch.complex128, "a"), na,
+                                             _dev_ptr(b_dev, torch.complex128, "b"), nb, ng,
+                                             _dev_ptr(s_dev, torch.complex128, "s"), _stream_ptr(stream)))
     return s_dev
 
 

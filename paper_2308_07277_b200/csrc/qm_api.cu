@@ -4,6 +4,8 @@
 #include "proj_kernels.cuh"
 #include "subspace_kernels.cuh"
 #include "probe_kernels.cuh"
+#include <cstdint>
+#include <mutex>
 
 thread_local std::string qm_g_err;
 
@@ -781,6 +783,95 @@ QM_API int qm_subspace(qm_gspace *g, int k, const qm_c128 *a_dev, int na, const 
                                                        reinterpret_cast<c128 *>(s_dev));
     g->prof.end(st);
     g->launches += 2;
+    CU_TRY(cudaGetLastError());
+    return QM_OK;
+}
+
+// ---- qm_subspace_static: the subspace product without any device allocation (include/qm_hpsi.h) -----------------------
+// For callers that cannot cudaMalloc (their own pool owns the device, a cudaMalloc would stall their other streams, or
+// their memory budget is fixed when the library is loaded), the split-K partial sums of S = A^H B live in the array
+// below, which is part of the library image: 2^20 complex128 = 16 MiB on every GPU that loads the library, until exit.
+//
+// `qm_substat_part` means two different things.  In DEVICE code (k_sub_reduce_static) it is the array.  In HOST code it
+// is only a handle that stands for the array: it is NOT a device address, and a kernel that is handed
+// `qm_substat_part` as a pointer argument from the host would write to a host address (a fault, or on machines where
+// the GPU can reach host memory, silent corruption).  The host gets the real address with cudaGetSymbolAddress, once
+// per device and with that device current (substat_setup), and passes THAT to k_sub_gemm.
+static __device__ __align__(256) c128 qm_substat_part[QM_SUBSPACE_STATIC_MAX_ELEMS];
+
+// k_sub_reduce with the partial sums read from the static array (named directly: this is device code).  Same
+// summation order as k_sub_reduce, so both entry points return the same bits.
+__global__ void k_sub_reduce_static(int nsplit, size_t plane, int ldp, int na, int nb, c128 *__restrict__ s_out)
+{
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= na * nb) return;
+    const int i = idx / nb, j = idx % nb;
+    const c128 *src = qm_substat_part + (size_t)i * ldp + j;
+    double sr[4] = {0.0, 0.0, 0.0, 0.0}, si[4] = {0.0, 0.0, 0.0, 0.0};
+    int s = 0;
+    for (; s + 4 <= nsplit; s += 4) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { const double2 v = ldg_c128(src + (size_t)(s + q) * plane); sr[q] += v.x; si[q] += v.y; }
+    }
+    for (; s < nsplit; ++s) { const double2 v = ldg_c128(src + (size_t)s * plane); sr[0] += v.x; si[0] += v.y; }
+    s_out[idx] = c128{(sr[0] + sr[1]) + (sr[2] + sr[3]), (si[0] + si[1]) + (si[2] + si[3])};
+}
+
+namespace {
+constexpr int SUBSTAT_MAX_DEVICES = 64;
+struct SubStatDev { bool ready = false; c128 *part = nullptr; int sm_count = 0; };
+SubStatDev substat_dev[SUBSTAT_MAX_DEVICES];
+std::mutex substat_mu;
+
+// First call on a device: the array's address ON THAT DEVICE, its SM count, and the shared-memory opt-in of the GEMM
+// (function attributes are per device; no handle was necessarily created here).  None of these allocates.
+int substat_setup(const SubStatDev **out) {
+    int dev = -1;
+    CU_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= SUBSTAT_MAX_DEVICES) return fail(QM_EINVAL, "qm_subspace_static: device ordinal beyond 63");
+    std::lock_guard<std::mutex> lock(substat_mu);
+    SubStatDev &d = substat_dev[dev];
+    if (!d.ready) {
+        c128 *ptr = nullptr;
+        CU_TRY(cudaGetSymbolAddress((void **)&ptr, qm_substat_part));
+        if (!ptr) return fail(QM_ECUDA, "qm_subspace_static: cudaGetSymbolAddress returned a null address");
+        CU_TRY(cudaDeviceGetAttribute(&d.sm_count, cudaDevAttrMultiProcessorCount, dev));
+        CU_TRY(cudaFuncSetAttribute(k_sub_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, SG_SMEM));
+        d.part = ptr;
+        d.ready = true;
+    }
+    *out = &d;
+    return QM_OK;
+}
+}  // namespace
+
+QM_API int qm_subspace_static(const qm_c128 *a_dev, int na, const qm_c128 *b_dev, int nb, int ng, qm_c128 *s_dev,
+                              void *stream)
+{
+    if (!a_dev || !b_dev || !s_dev || na <= 0 || nb <= 0 || ng <= 0)
+        return fail(QM_EINVAL, "qm_subspace_static: bad argument");
+    if (((uintptr_t)a_dev | (uintptr_t)b_dev | (uintptr_t)s_dev) & 15)
+        return fail(QM_EINVAL, "qm_subspace_static: a, b and s must be 16-byte aligned");
+    const long long ntm = ((long long)na + SG_T - 1) / SG_T, ntn = ((long long)nb + SG_T - 1) / SG_T;
+    const long long plane_ll = ntm * SG_T * ntn * SG_T;
+    if (plane_ll > (long long)QM_SUBSPACE_STATIC_MAX_ELEMS)
+        return fail(QM_EINVAL, "qm_subspace_static: a block of " + std::to_string(na) + " x " + std::to_string(nb) +
+                                   " states needs " + std::to_string(plane_ll) + " partial sums per K split, the static "
+                                   "work space holds " + std::to_string(QM_SUBSPACE_STATIC_MAX_ELEMS) +
+                                   " (e.g. 1024 x 1024); use qm_subspace for larger blocks");
+    const SubStatDev *d = nullptr;
+    int rc = substat_setup(&d); if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int tiles = (int)(ntm * ntn), ldp = (int)ntn * SG_T;
+    const size_t plane = (size_t)plane_ll;
+    const int nkc = (ng + SG_KS - 1) / SG_KS;
+    int nsplit = std::max(1, std::min(nkc, d->sm_count / tiles));                  // qm_subspace's choice ...
+    nsplit = (int)std::min<size_t>((size_t)nsplit, QM_SUBSPACE_STATIC_MAX_ELEMS / plane);   // ... as far as the array holds it
+    // k_sub_gemm writes every element of every [split] plane that k_sub_reduce_static reads: nothing to clear
+    k_sub_gemm<<<dim3(tiles, nsplit), (SG_CW + 1) * 32, SG_SMEM, st>>>(
+        reinterpret_cast<const c128 *>(a_dev), na, reinterpret_cast<const c128 *>(b_dev), nb, ng, (int)ntn, nsplit,
+        d->part, ldp);
+    k_sub_reduce_static<<<(na * nb + 255) / 256, 256, 0, st>>>(nsplit, plane, ldp, na, nb, reinterpret_cast<c128 *>(s_dev));
     CU_TRY(cudaGetLastError());
     return QM_OK;
 }
