@@ -634,9 +634,6 @@ def run_ours(args):
                                       if world == 1 and args.config == "cfg5" and not args.no_all_configs else None),
                 "roofline": roofline, "fft_path": fft_path, "kernels": kernels,
                 "fp64_peaks_tflops": {"dmma_probe": dmma_peak, "dfma_probe": dfma_peak},
-                "exchange_probe": dict(zip(("smem_ns", "shfl_ns", "tmem_read_ns"), qm.qm_probe_exchange()),
-                                       note="SM time per warp-wide hand-over of one complex128 per lane, 12 warps per SM "
-                                            "(csrc/probe_kernels.cuh)"),
                 "one_call_all_bands": {"bands": nb, "ms": one_call_ms, "band_applies_per_s": nb / (one_call_ms * 1e-3)},
                 "taylor": {"order": 4, "bands": nb, "call_batch": cb, "ms": taylor_ms,
                            "band_steps_per_s": nb / (taylor_ms * 1e-3),

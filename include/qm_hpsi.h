@@ -108,9 +108,12 @@ QM_API int qm_set_vloc(qm_gspace *g, const double *V_r_dev, void *stream);
 QM_API int qm_set_nonlocal(qm_gspace *g, int k, const qm_c128 *beta_kG_dev, int nproj,
                     const double *D_dev, int d_block, void *stream);
 
-/* Grow every library-owned work space that qm_apply_h / qm_split_operator_propagate / the density and debug calls
- * need for blocks of up to `nbands` wavefunctions at k-point k (projector work spaces are sized by qm_set_nonlocal), so
- * that no later call allocates.  May synchronise the device (cudaMalloc); not a hot-path call. */
+/* Grow the per-k-point work spaces (stick planes, unfused slabs, projector partials) that qm_apply_h,
+ * qm_split_operator_propagate and qm_density_accumulate need for blocks of up to `nbands` wavefunctions at k-point k, so
+ * that none of those calls allocates later (projector work spaces are sized by qm_set_nonlocal as well).  NOT covered, and
+ * still grown on first use by their own calls: the density running sum (qm_density_reset), the two Taylor blocks
+ * (qm_taylor_propagate), the box of the debug hooks (qm_debug_g2r / r2g), the split-K partials of qm_subspace and the
+ * work spaces of a qm_mtxel handle.  May synchronise the device (cudaMalloc); not a hot-path call. */
 QM_API int qm_reserve(qm_gspace *g, int k, int nbands);
 
 /* psi_out = H psi_in for a block of nbands wavefunctions at k-point k.
@@ -128,8 +131,13 @@ QM_API int qm_apply_h(qm_gspace *g, const qm_c128 *psi_in_dev, qm_c128 *psi_out_
  * parallel branches (k-points own their work spaces), items of one k-point run in list order.  qm_batch_plan_launch
  * enqueues the whole graph on `stream`; it replaces the per-call launch latency that dominates the small configs.
  * qm_set_vloc / qm_set_nonlocal must have been called for every k used; creation reserves the work spaces
- * (qm_reserve) and may synchronise.  A later qm_set_nonlocal with a different nproj for a k-point in the plan
- * invalidates it.  The plan borrows the handle: destroy it before qm_gspace_destroy. */
+ * (qm_reserve) and may synchronise.  The graph holds the addresses and shapes of the k-points' work spaces, so two
+ * things make a plan STALE: a later call on one of its k-points that needs a larger work space than the plan
+ * reserved (qm_apply_h, qm_reserve, density, Taylor, debug calls with more bands: the block is freed and re-allocated),
+ * and a later qm_set_nonlocal with a different nproj or d_block for one of its k-points.  The library counts both per
+ * k-point; qm_batch_plan_launch on a stale plan launches nothing and returns QM_EINVAL -- destroy the plan and create
+ * it again (or call qm_reserve with the largest band count you will use BEFORE creating plans).  The plan borrows
+ * the handle: destroy it before qm_gspace_destroy. */
 typedef struct qm_batch_plan qm_batch_plan;
 QM_API int qm_batch_plan_create(qm_gspace *g, int nitems, const int *k, const qm_c128 *const *psi_in_dev,
                                 qm_c128 *const *psi_out_dev, const int *nbands, qm_batch_plan **out);
@@ -299,13 +307,6 @@ QM_API const char *qm_kernel_name(int kind);
  * and returns the measured TFLOP/s (HOST output).  Used as the roofline denominator for the
  * projector GEMMs (MEASURED_PEAKS.json has no FP64 entry). Synchronous. */
 QM_API int qm_probe_fp64_tensor_peak(double *tflops_dmma, double *tflops_dfma);
-
-/* Exchange probe (csrc/probe_kernels.cuh): SM time, in ns, of one warp-wide hand-over of a complex128 per lane with 12
- * warps per SM running the same loop -- through shared memory (STS.128 + LDS.128), through warp shuffles (4 x SHFL.32),
- * and the read of a thread-private element from tensor memory (tcgen05.ld).  HOST outputs.  Reported by bench.py beside
- * the plane kernel's figures (why the transposes go through shared memory and the twiddle rows through
- * tensor memory).  Synchronous. */
-QM_API int qm_probe_exchange(double *ns_smem, double *ns_shfl, double *ns_tmem);
 
 QM_API const char *qm_last_error(void);                    /* thread-local text */
 QM_API const char *qm_version(void);

@@ -67,7 +67,6 @@ _SIGS = {
     "qm_debug_r2g": [_vp, _vp, _vp, _i, _i, _vp],
     "qm_get_launch_count": [_vp, ctypes.POINTER(ctypes.c_ulonglong)],
     "qm_probe_fp64_tensor_peak": [ctypes.POINTER(_d), ctypes.POINTER(_d)],
-    "qm_probe_exchange": [ctypes.POINTER(_d), ctypes.POINTER(_d), ctypes.POINTER(_d)],
     "qm_profile_enable": [_vp, _i],
     "qm_profile_reset": [_vp],
     "qm_profile_read": [_vp, _i, ctypes.POINTER(_d), ctypes.POINTER(ctypes.c_ulonglong)],
@@ -435,13 +434,6 @@ def qm_probe_fp64_tensor_peak():
     a, b = _d(), _d()
     _check(load_library().qm_probe_fp64_tensor_peak(ctypes.byref(a), ctypes.byref(b)))
     return a.value, b.value
-
-
-def qm_probe_exchange():
-    """(ns via shared memory, ns via warp shuffles, ns tensor-memory read) per warp-wide complex128 hand-over."""
-    a, b, c = _d(), _d(), _d()
-    _check(load_library().qm_probe_exchange(ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)))
-    return a.value, b.value, c.value
 
 
 def qm_profile_enable(h, on: bool):

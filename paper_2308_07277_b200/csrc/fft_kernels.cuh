@@ -148,15 +148,6 @@ k_zfwd(QmKPlanDev kp, const c128 *__restrict__ tw, const c128 *__restrict__ W,
 #ifndef QM_PLANE_GROUP
 #define QM_PLANE_GROUP 96
 #endif
-#ifndef QM_PLANE_YROWS
-#define QM_PLANE_YROWS 1        /* plane rows a team works on between two group barriers of the y phase (2: spills, 343 vs 300 us) */
-#endif
-#ifndef QM_PLANE_XPREFETCH
-#define QM_PLANE_XPREFETCH 0    /* x phase: fetch a column's step-1 inputs one column ahead (quarter rule) */
-#endif
-#ifndef QM_PLANE_XTW_LATE
-#define QM_PLANE_XTW_LATE 0     /* x phase: forward inter-pass twiddles applied in step 3 (on the way in) instead of step 2: measured +2 % at cfg5 */
-#endif
 #ifndef QM_PLANE_TW_TMEM
 #define QM_PLANE_TW_TMEM 1      /* per-thread twiddle rows live in tensor memory (tmem_rows.cuh) instead of registers */
 #endif
@@ -297,9 +288,9 @@ __device__ __forceinline__ void plane_y_phase(const PlaneCtx cx, c128 *__restric
     const int pc = have_cur ? pl : 0, pp = prev >= 0 ? prev : 0;
     const WView Wcur = qm_wview(W + (size_t)(pc / n3) * cx.wband, pc % n3, n3);
     const WView Wprev = qm_wview(W + (size_t)(pp / n3) * cx.wband, pp % n3, n3);
-    // A team works on NR rows per round (rows r, r + rstride, ...): the same number of row steps with 1/NR of the
-    // group barriers and NR independent load -> transform -> store chains between two barriers.
-    constexpr int NR = QM_PLANE_YROWS;
+    // A team works on NR rows per round (rows r, r + rstride, ...).  NR = 1: two rows per round spill at the register
+    // budget of this kernel and were measured slower; the helpers below take row arrays.
+    constexpr int NR = 1;
     const int rstride = cx.ngroups * TPG;
     for (int r0 = grp * TPG + slot; r0 - slot < X; r0 += NR * rstride) {      // same trip count for a whole group
         int sbase[NR];
@@ -356,7 +347,7 @@ __device__ __forceinline__ void plane_y_phase(const PlaneCtx cx, c128 *__restric
 template <class C, int MODE>
 __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_iv, const double *__restrict__ vt,
                                            c128 *__restrict__ box, const c128 *__restrict__ box2, int npair2, int pl,
-                                           double scale, int stagger_ns,
+                                           double scale,
                                            double *__restrict__ rhot, const TwRow<C::R1> &twa, const TwRow<C::R2> &twb)
 {
     constexpr int G = QM_GROUP, TPG = G / C::TT, RP = C::L | 1;
@@ -374,20 +365,9 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
     const SLine scrA[1] = {id.a2 ? teamscr : sink}, scrB[1] = {id.a1 ? teamscr : sink};
     const double *vplane = vt + (size_t)p * C::N * VLayout<C>::COL;
     VRow<C::R2> vr;
-    // De-phase the groups: they all do identical load -> FP64 -> store bursts, and when they run in
-    // lock step the shared-memory pipe and the FP64 pipe are used alternately instead of together.
-    if (stagger_ns > 0) __nanosleep((unsigned)(grp * stagger_ns));
     const int col0 = grp * TPG + slot;
     auto vcol = [&](int c) { return vplane + (size_t)(c < C::N ? c : C::N - 1) * VLayout<C>::COL; };
     if constexpr (MODE == 0) load_vrow<C>(vr, vcol(col0), id.u1);       // V of the first column: in flight while step 1 runs
-    // Step-1 inputs of a column under the quarter rule: fetched one column ahead (before the barrier in front of the
-    // previous column's step 3), so that their shared-memory latency hides behind that barrier and step 3.  Nobody else
-    // touches a column of the plane array during the x phase: every column is owned by one team.
-    constexpr bool XPRE = (MODE == 0 || MODE == 4) && QM_PLANE_XPREFETCH;
-    c128 xpre[2 * Quarter<C>::Q];
-    if constexpr (XPRE) {
-        if (xq) prefetch_quarter<C>(As + C::pos(col0), C::R2 * RP, (id.a2 && col0 < C::N) ? px : pnone, xpre);
-    }
     for (int col = col0; col - slot < C::N; col += nteams) {      // same trip count for a whole group
         const bool ok = id.team_ok && col < C::N;
         const int colc = col < C::N ? col : C::N - 1;    // a column that exists, for the addresses of lanes without one
@@ -395,16 +375,11 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
         const Pruned pxc = (ok && id.a2) ? px : pnone;   // plane-array accesses of a lane without work are masked off
         if constexpr (MODE != 2) {
             c128 t[1][C::R1];
-            if constexpr (XPRE) {
-                if (xq) prunedA_step1_pre_head<C, false>(xpre, t[0], id.u2);
-                else prunedA_step1_head<C, false>(Acol, C::R2 * RP, pxc, t[0], id.u2);
-            } else {
-                if (xq) {
-                    c128 pre[2 * Quarter<C>::Q];
-                    prefetch_quarter<C>(Acol, C::R2 * RP, pxc, pre);
-                    prunedA_step1_pre_head<C, false>(pre, t[0], id.u2);
-                } else prunedA_step1_head<C, false>(Acol, C::R2 * RP, pxc, t[0], id.u2);
-            }
+            if (xq) {
+                c128 pre[2 * Quarter<C>::Q];
+                prefetch_quarter<C>(Acol, C::R2 * RP, pxc, pre);
+                prunedA_step1_pre_head<C, false>(pre, t[0], id.u2);
+            } else prunedA_step1_head<C, false>(Acol, C::R2 * RP, pxc, t[0], id.u2);
             plane_tail<C, false>(t, scrA, id.u2, twa, cx.tw_a);
             group_barrier<G>(grp);
         }
@@ -425,39 +400,16 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
             if constexpr (MODE == 4) bx2 = box2 + coloff;
             c128 t[1][C::R2];
             xcol_step2_head<C, MODE, false>(scrB[0], id.u1, vr, bx, bx2, scale, t[0], ok && id.a1);
-            if constexpr (MODE != 1) {
-                if constexpr (QM_PLANE_XTW_LATE) stepB1_store<C>(t[0], scrB[0], id.u1);
-                else plane_tail<C, true>(t, scrB, id.u1, twb, cx.tw_b);
-            }
+            if constexpr (MODE != 1) plane_tail<C, true>(t, scrB, id.u1, twb, cx.tw_b);
         }
         if constexpr (MODE == 0)     // prefetch V of this team's next column behind steps 3 and 1
             load_vrow<C>(vr, vcol(col + nteams), id.u1);
-        if constexpr (XPRE) {
-            const int ncol = col + nteams;
-            if (xq) prefetch_quarter<C>(As + C::pos(ncol), C::R2 * RP, (id.a2 && ncol < C::N) ? px : pnone, xpre);
-        }
         group_barrier<G>(grp);
         if constexpr (MODE != 1 && MODE != 3) {
             // no barrier after step 3: the scratch column a thread reads here is exactly the one it
             // overwrites in the next iteration's step 1 (MODE 2 has no step 1 and writes rows: barrier).
-            if constexpr (QM_PLANE_XTW_LATE) {
-                c128 t[C::R1];
-                stepB2_load<C>(scrA[0], id.u2, t);
-                if constexpr (plane_tw_tmem<C>) {
-                    static_for<(C::R1 + QM_TW_CHUNK - 1) / QM_TW_CHUNK>([&](auto I) {
-                        constexpr int j0 = decltype(I)::value * QM_TW_CHUNK, j1 = j0 + QM_TW_CHUNK < C::R1 ? j0 + QM_TW_CHUNK : C::R1;
-                        constexpr int l0 = j0 == 0 ? 1 : j0;
-                        TwChunk<l0, (l0 < j1 ? j1 : l0 + 1)> ch;
-                        if constexpr (l0 < j1) { tmem_load_chunk(ch, cx.tw_a); stepB2_twiddle_range<C, l0, j1>(t, ch); }
-                    });
-                } else {
-                    stepB2_twiddle_range<C, 0, C::R1>(t, twa);
-                }
-                stepB2_finish<C>(t, Acol, C::R2 * RP, pxc, xq);
-            } else {
-                if (xq) prunedB_step2_quarter<C, false>(scrA[0], Acol, C::R2 * RP, pxc, id.u2);
-                else prunedB_step2<C, false>(scrA[0], Acol, C::R2 * RP, pxc, id.u2);
-            }
+            if (xq) prunedB_step2_quarter<C, false>(scrA[0], Acol, C::R2 * RP, pxc, id.u2);
+            else prunedB_step2<C, false>(scrA[0], Acol, C::R2 * RP, pxc, id.u2);
             if constexpr (MODE == 2) group_barrier<G>(grp);
         }
     }
@@ -466,7 +418,7 @@ __device__ __forceinline__ void plane_x_phase(const PlaneCtx cx, const short4 x_
 template <class C, int MODE>
 __global__ void __launch_bounds__(QM_PLANE_MAX_THREADS)
 k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ box, const c128 *__restrict__ box2,
-        int npair2, int ngroups, double scale, int stagger_ns, int nplanes, int quarter, const double *__restrict__ occ,
+        int npair2, int ngroups, double scale, int nplanes, int quarter, const double *__restrict__ occ,
         double *__restrict__ rhot)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -547,7 +499,7 @@ k_plane(QmKPlanDev kp, QmGridDev gd, c128 *__restrict__ W, c128 *__restrict__ bo
         __syncthreads();
         double sc = scale;
         if constexpr (MODE == 3) sc = scale * occ[pl / n3];
-        plane_x_phase<C, MODE>(cx, kp.x_iv, gd.vt, box, box2, npair2, pl, sc, stagger_ns, rhot, twa, twb);
+        plane_x_phase<C, MODE>(cx, kp.x_iv, gd.vt, box, box2, npair2, pl, sc, rhot, twa, twb);
         __syncthreads();
         prev = pl;
     }

@@ -258,48 +258,6 @@ QM_HD void prunedB_step2(const L srcline, const P dst, int estride, const Pruned
         }
     });
 }
-// Forward step 2 in three parts, for callers that apply the inter-pass twiddles HERE (on the way in) instead of at the end
-// of step 1: load the thread's R1 elements, multiply element a by w^(u a) (the same per-thread row the backward first pass
-// uses, conjugated there), finish (butterflies + pruned stores).  The x phase of the plane kernel uses this to move 44
-// FP64 instructions per thread and column out of its FP64-bound step 2 into its shared-memory-bound step 3.
-template <class C, class L> QM_HD void stepB2_load(const L srcline, int u, c128 (&t)[C::R1]) {
-    static_for<C::R1>([&](auto I) { constexpr int a = decltype(I)::value; t[a] = srcline[a * C::R2P + u]; });
-}
-template <class C, int J0, int J1, class TW> QM_HD void stepB2_twiddle_range(c128 (&t)[C::R1], const TW &tw) {
-    static_for<J1 - J0>([&](auto I) {
-        constexpr int a = J0 + decltype(I)::value;
-        if constexpr (a > 0) t[a] = cmul(t[a], tw.template get<a>());
-    });
-}
-template <class C, class P> QM_HD void stepB2_finish(c128 (&t)[C::R1], const P dst, int estride, const Pruned pr, bool quarter) {
-    const P p1 = dst + pr.c1, p2 = dst + pr.c2;
-    if (quarter) {
-        constexpr int Q = Quarter<C>::Q;
-        DftQuarterOut<C::R1, -1>::run(t);
-        static_for<Q>([&](auto I) {
-            constexpr int j = decltype(I)::value;
-            constexpr int c2 = C::R1 - Q + j;
-            st_pred(p1 + j * estride, t[j], (pr.m1 >> j) & 1u);
-            st_pred(p2 + c2 * estride, t[c2], (pr.m2 >> c2) & 1u);
-        });
-    } else {
-        Dft<C::R1, -1>::run(t);
-        const unsigned mm = pr.m1 | pr.m2;
-        static_for<C::R1>([&](auto I) {
-            constexpr int c = decltype(I)::value;
-            if constexpr (2 * (c + 1) * C::R2 <= C::N) st_pred(p1 + c * estride, t[c], (mm & (1u << c)) != 0u);
-            else if constexpr (2 * c * C::R2 >= C::N) st_pred(p2 + c * estride, t[c], (mm & (1u << c)) != 0u);
-            else {
-                const bool in2 = (pr.m2 >> c) & 1u;
-                st_pred((in2 ? p2 : p1) + c * estride, t[c], (mm & (1u << c)) != 0u);
-            }
-        });
-    }
-}
-// first forward pass without its twiddles (see above): plain store of the butterflies' outputs
-template <class C, class L> QM_HD void stepB1_store(const c128 (&t)[C::R2], const L line, int u) {
-    static_for<C::R2>([&](auto I) { constexpr int d = decltype(I)::value; line[u * C::R2P + d] = t[d]; });
-}
 // Quarter-rule form of the pruned forward step 2: only the first Q and last Q outputs of a thread can exist.
 template <class C, bool GUARD = true, class L, class P>
 QM_HD void prunedB_step2_quarter(const L srcline, const P dst, int estride, const Pruned pr, int u) {

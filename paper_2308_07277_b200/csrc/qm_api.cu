@@ -3,7 +3,6 @@
 #include "qm_internal.h"
 #include "proj_kernels.cuh"
 #include "subspace_kernels.cuh"
-#include "probe_kernels.cuh"
 #include <cstdint>
 #include <mutex>
 
@@ -407,7 +406,6 @@ QM_API int qm_gspace_create(const double *lattice_bohr, double ecutwfc_ry, const
     if (const char *e = getenv("QM_PDL")) g->pdl = atoi(e) != 0;
     rc = prepare_kernels(g);
     if (rc != QM_OK) return bail(rc);
-    if (const char *e = getenv("QM_PLANE_STAGGER_NS")) g->plane_stagger_ns = atoi(e);
     if (const char *e = getenv("QM_Z_CTA_PER_SM")) g->z_cta_per_sm = std::max(1, atoi(e));
     if (const char *e = getenv("QM_PLANE_CTAS")) g->plane_ctas_per_sm = std::max(0, atoi(e));
     if (const char *e = getenv("QM_FFT_CHUNK")) g->fft_chunk = std::max(0, atoi(e));
@@ -479,6 +477,7 @@ QM_API int qm_set_nonlocal(qm_gspace *g, int k, const qm_c128 *beta_kG_dev, int 
     int rc = check_handle(g, k); if (rc) return rc;
     KPoint *kp = g->kpts[k];
     if (nproj < 0) return fail(QM_EINVAL, "qm_set_nonlocal: nproj < 0");
+    if (kp->nl_set && (nproj != kp->nproj || (nproj > 0 && d_block != kp->dblock))) kp->ws_gen++;   // batch plans of this k go stale
     if (nproj == 0) { kp->nproj = 0; kp->nl_set = true; return QM_OK; }
     if (!beta_kG_dev || !D_dev || d_block <= 0 || nproj % d_block != 0)
         return fail(QM_EINVAL, "qm_set_nonlocal: bad beta / D / d_block");
@@ -690,6 +689,11 @@ QM_API int qm_batch_plan_create(qm_gspace *g, int nitems, const int *k, const qm
     const cudaError_t e2 = cudaStreamEndCapture(s0, &graph);
     p->launches = g->launches - l0;
     g->launches = l0;                               // capturing launched nothing
+    for (int i = 0; i < nitems; ++i) {
+        bool seen = false;
+        for (const auto &kg : p->gens) seen = seen || kg.first == k[i];
+        if (!seen) p->gens.emplace_back(k[i], g->kpts[k[i]]->ws_gen);
+    }
     if (rc == QM_OK && (e != cudaSuccess || e2 != cudaSuccess)) rc = fail(QM_ECUDA, cudaGetErrorString(e != cudaSuccess ? e : e2));
     if (rc == QM_OK) {
         p->graph = graph;
@@ -704,6 +708,11 @@ QM_API int qm_batch_plan_create(qm_gspace *g, int nitems, const int *k, const qm
 QM_API int qm_batch_plan_launch(qm_batch_plan *p, void *stream) {
     if (!p || !p->exec) return fail(QM_EINVAL, "qm_batch_plan_launch: null plan");
     int rc = check_device(p->g); if (rc) return rc;
+    for (const auto &kg : p->gens)
+        if (p->g->kpts[kg.first]->ws_gen != kg.second)
+            return fail(QM_EINVAL, "qm_batch_plan_launch: stale plan -- a work space of k-point " + std::to_string(kg.first) +
+                                   " was re-allocated by a larger call, or its projector shape changed, after the plan "
+                                   "was created; destroy the plan and create it again");
     CU_TRY(cudaGraphLaunch(p->exec, (cudaStream_t)stream));
     p->g->launches += p->launches;
     return QM_OK;
@@ -713,6 +722,7 @@ QM_API int qm_batch_plan_destroy(qm_batch_plan *p) { delete p; return QM_OK; }
 QM_API int qm_host_synchronize(qm_gspace *g) {
     if (!g) return fail(QM_EINVAL, "null handle");
     if (!g->pipe.init) return QM_OK;
+    int rc = check_device(g); if (rc) return rc;
     CU_TRY(cudaStreamSynchronize(g->pipe.s_in));
     CU_TRY(cudaStreamSynchronize(g->pipe.s_out));
     return QM_OK;
@@ -919,6 +929,7 @@ static size_t qm_rhot_elems(const qm_gspace *g) {
 }
 QM_API int qm_density_reset(qm_gspace *g, void *stream) {
     if (!g) return fail(QM_EINVAL, "null handle");
+    int rc = check_device(g); if (rc) return rc;
     const size_t n = qm_rhot_elems(g);
     CU_TRY(g->d_rhot.resize(n));
     CU_TRY(cudaMemsetAsync(g->d_rhot.p, 0, n * sizeof(double), (cudaStream_t)stream));
@@ -946,6 +957,7 @@ QM_API int qm_density_accumulate(qm_gspace *g, int k, const qm_c128 *psi_dev, in
 QM_API int qm_density_get(qm_gspace *g, double *rho_dev, double scale, void *stream) {
     if (!g || !rho_dev) return fail(QM_EINVAL, "qm_density_get: null argument");
     if (!g->rho_open) return fail(QM_ENOTSET, "qm_density_get before qm_density_reset");
+    int rc = check_device(g); if (rc) return rc;
     k_density_out<<<g->sm_count * 4, 256, 0, (cudaStream_t)stream>>>(g->d_rhot.p, rho_dev, g->ax[0], g->ax[1], g->ax[2], scale);
     g->launches++;
     CU_TRY(cudaGetLastError());
@@ -1064,36 +1076,6 @@ QM_API int qm_probe_fp64_tensor_peak(double *tflops_dmma, double *tflops_dfma) {
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
     if (tflops_dmma) *tflops_dmma = best_mma;
     if (tflops_dfma) *tflops_dfma = best_fma;
-    return QM_OK;
-}
-
-QM_API int qm_probe_exchange(double *ns_smem, double *ns_shfl, double *ns_tmem) {
-    int dev = 0, sms = 0, count = 0;
-    if (cudaGetDeviceCount(&count) != cudaSuccess || count == 0) return fail(QM_ECUDA, "no CUDA device");
-    CU_TRY(cudaGetDevice(&dev));
-    CU_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    double *sink = nullptr;
-    CU_TRY(cudaMalloc(&sink, sizeof(double)));
-    cudaEvent_t e0, e1;
-    CU_TRY(cudaEventCreate(&e0)); CU_TRY(cudaEventCreate(&e1));
-    const int iters = 1 << 14, threads = 384, blocks = sms;       // 12 warps per SM, like the plane kernel
-    double best[3] = {1e30, 1e30, 1e30};
-    for (int rep = 0; rep < 3; ++rep)
-        for (int mode = 0; mode < 3; ++mode) {
-            float ms = 0.f;
-            CU_TRY(cudaEventRecord(e0));
-            if (mode == 0) k_probe_exchange<0><<<blocks, threads>>>(sink, iters);
-            else if (mode == 1) k_probe_exchange<1><<<blocks, threads>>>(sink, iters);
-            else k_probe_exchange<2><<<blocks, threads>>>(sink, iters);
-            CU_TRY(cudaEventRecord(e1)); CU_TRY(cudaEventSynchronize(e1));
-            CU_TRY(cudaEventElapsedTime(&ms, e0, e1));
-            // SM-time per warp-wide exchange of one complex128 per lane: 12 warps share the SM
-            best[mode] = std::min(best[mode], (double)ms * 1e6 / ((double)iters * (threads / 32)));
-        }
-    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
-    if (ns_smem) *ns_smem = best[0];
-    if (ns_shfl) *ns_shfl = best[1];
-    if (ns_tmem) *ns_tmem = best[2];
     return QM_OK;
 }
 

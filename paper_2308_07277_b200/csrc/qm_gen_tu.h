@@ -15,8 +15,11 @@ template <class C, bool BACK> int launch_gen_y(qm_gspace *g, KPoint *kp, c128 *W
     if (items * GG::TPG >= (1LL << 31)) return fail(QM_EINVAL, "unfused y pass: too many rows in one launch");
     // persistent: a CTA walks row chunks gridDim.x apart (twiddle rows loaded once); several CTAs per SM hide latency
     const long long nchunks = (items + GG::TPG - 1) / GG::TPG;
-    int per_sm = 1;
-    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_gen_y<C, BACK>, GEN_GROUP, GG::y_smem()));
+    int &per_sm = kp->gen_y_per_sm[BACK ? 1 : 0];
+    if (per_sm == 0) {
+        CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_gen_y<C, BACK>, GEN_GROUP, GG::y_smem()));
+        per_sm = std::max(1, per_sm);
+    }
     const unsigned grid = (unsigned)std::min<long long>(nchunks, (long long)g->sm_count * std::max(1, per_sm));
     const size_t wband = (size_t)((kp->nsticks + QM_ZT - 1) / QM_ZT) * QM_ZT * g->grid[2];
     g->prof.begin(QM_K_GENY, st);
@@ -37,8 +40,11 @@ template <class C, int MODE> int launch_gen_x(qm_gspace *g, KPoint *kp, c128 *sl
     const int nchunk = (n2 + GG::TC - 1) / GG::TC;
     const long long tiles = (long long)(MODE == 3 ? n3 : nbp) * nchunk;
     // persistent: a CTA walks tiles gridDim.x apart; as many CTAs as are resident
-    int per_sm = 1;
-    CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_gen_x<C, MODE>, GG::XG * GEN_GROUP, smem));
+    int &per_sm = kp->gen_x_per_sm[MODE];
+    if (per_sm == 0) {
+        CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_gen_x<C, MODE>, GG::XG * GEN_GROUP, smem));
+        per_sm = std::max(1, per_sm);
+    }
     const unsigned grid = (unsigned)std::min<long long>(tiles, (long long)g->sm_count * std::max(1, per_sm));
     g->prof.begin(QM_K_GENX, st);
     CU_TRY(qm_launch_pdl(k_gen_x<C, MODE>, dim3(grid), dim3(GG::XG * GEN_GROUP), smem, st, g->pdl, kp->plan(), (const c128 *)g->d_tw[0].p,
@@ -71,6 +77,14 @@ int qm_prepare_gen_y(qm_gspace *g) {
                                     (int)GenGeom<LineCfg<A, B>>::y_smem()));                                           \
         CU_TRY(cudaFuncSetAttribute(k_gen_y<LineCfg<A, B>, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,        \
                                     (int)GenGeom<LineCfg<A, B>>::y_smem()));                                           \
+        for (KPoint *kp : g->kpts) {                                                                                  \
+            CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&kp->gen_y_per_sm[0], k_gen_y<LineCfg<A, B>, false>, \
+                                                                 GEN_GROUP, GenGeom<LineCfg<A, B>>::y_smem()));        \
+            CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&kp->gen_y_per_sm[1], k_gen_y<LineCfg<A, B>, true>,  \
+                                                                 GEN_GROUP, GenGeom<LineCfg<A, B>>::y_smem()));        \
+            kp->gen_y_per_sm[0] = std::max(1, kp->gen_y_per_sm[0]);                                                   \
+            kp->gen_y_per_sm[1] = std::max(1, kp->gen_y_per_sm[1]);                                                   \
+        }                                                                                                             \
         return QM_OK;
         QM_FOR_SIZES_ALL(X)
 #undef X
@@ -91,6 +105,14 @@ int QM_CAT(qm_prepare_gen_x_m, QM_GEN_TU)(qm_gspace *g) {
 #define X(N, A, B)                                                                                                              \
     case N: CU_TRY(cudaFuncSetAttribute(k_gen_x<LineCfg<A, B>, QM_GEN_TU>, cudaFuncAttributeMaxDynamicSharedMemorySize,          \
                                         g->max_smem));                                                                           \
+        for (KPoint *kp : g->kpts) {    /* the x tile must fit, and its occupancy is asked once, here */                         \
+            const size_t smem = GenGeom<LineCfg<A, B>>::x_smem(kp->nx);                                                          \
+            if (smem > (size_t)g->max_smem) return fail(QM_EGRID, "x tile of the unfused path does not fit shared memory");      \
+            int &per_sm = kp->gen_x_per_sm[QM_GEN_TU];                                                                           \
+            CU_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_gen_x<LineCfg<A, B>, QM_GEN_TU>,                     \
+                                                                 GenGeom<LineCfg<A, B>>::XG * GEN_GROUP, smem));                 \
+            per_sm = std::max(1, per_sm);                                                                                        \
+        }                                                                                                                        \
         return QM_OK;
         QM_FOR_SIZES_ALL(X)
 #undef X

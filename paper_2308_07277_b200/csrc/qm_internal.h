@@ -2,7 +2,7 @@
 //   qm_api.cu          the C ABI, host-side set-up, projector / subspace launches
 //   qm_z.cu            launches of the z-stick kernels (k_zinv, k_zfwd), every supported length
 //   qm_plane<M>.cu     launches of the fused xy-plane kernel, one translation unit per MODE (compiled in parallel)
-//   qm_general.cu      the unfused y / x passes for boxes the fused kernel cannot take (n1 != n2, large planes)
+//   qm_geny.cu, qm_genx<M>.cu   the unfused y / x passes for boxes the fused kernel cannot take (n1 != n2, large planes)
 #pragma once
 #include <cuda_runtime.h>
 #include <algorithm>
@@ -12,6 +12,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/qm_hpsi.h"
@@ -32,10 +33,11 @@ inline int fail(int code, const std::string &msg) { qm_g_err = msg; return code;
 
 template <class T> struct DevBuf {
     T *p = nullptr; size_t n = 0;
+    unsigned long long *moved = nullptr;    // counter to bump when a live block is freed and re-allocated (KPoint::ws_gen)
     ~DevBuf() { if (p) cudaFree(p); }
     cudaError_t resize(size_t m) {
         if (m <= n) return cudaSuccess;
-        if (p) { cudaFree(p); p = nullptr; n = 0; }
+        if (p) { cudaFree(p); p = nullptr; n = 0; if (moved) ++*moved; }
         cudaError_t e = cudaMalloc(&p, m * sizeof(T));
         if (e == cudaSuccess) n = m;
         return e;
@@ -65,11 +67,27 @@ struct KPoint : QmKTables {
     DevBuf<c128> d_sophase;                             // split-operator: exp(-i dt |k+G|^2 / 4)
     cudaStream_t side_stream = nullptr;                 // GEMM 1 of an apply runs here, beside the FFT path (qm_api.cu run_apply)
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    // Work-space generation: goes up whenever one of the blocks above is moved by a growing resize, or qm_set_nonlocal
+    // changes the projector shape.  A qm_batch_plan holds these addresses and shapes inside its graph; it records the
+    // generation of every k-point it uses and qm_batch_plan_launch refuses to run a stale graph.
+    unsigned long long ws_gen = 0;
+    KPoint() {
+        d_beta1.moved = d_beta2.moved = d_W.moved = d_Ppart.moved = d_P.moved = d_part.moved = d_slab.moved = &ws_gen;
+        d_D.moved = d_qt.moved = &ws_gen;
+        d_pdesc.moved = &ws_gen;
+    }
+    KPoint(const KPoint &) = delete;
+    KPoint &operator=(const KPoint &) = delete;
     ~KPoint() {
         if (ev_fork) cudaEventDestroy(ev_fork);
         if (ev_join) cudaEventDestroy(ev_join);
         if (side_stream) cudaStreamDestroy(side_stream);
     }
+    // unfused passes: resident CTAs per SM of k_gen_y (forward / backward) and of k_gen_x per MODE for this k-point's x
+    // tile; 0 = not asked yet.  Filled by qm_prepare_gen_* at qm_gspace_create (and at the first launch for the sphere
+    // of a qm_mtxel handle), so that no launch on the hot path or under stream capture queries the occupancy.
+    int gen_y_per_sm[2] = {0, 0};
+    int gen_x_per_sm[5] = {0, 0, 0, 0, 0};
     double ecut_override = 0.0;                         // epsilon spheres (qm_mtxel) carry their own cut-off
     QmKPlanDev plan() const {
         QmKPlanDev p;
@@ -154,7 +172,6 @@ struct qm_gspace {
     size_t l2_bytes = 0;
     int fft_chunk = 0;              // bands per internal pass of the FFT path (0: derived from the L2 size; QM_FFT_CHUNK)
     int z_cta_per_sm = 2;           // resident z-kernel CTAs per SM the grid is sized for (QM_Z_CTA_PER_SM)
-    int plane_stagger_ns = 0;       // de-phasing delay between the plane kernel's groups (QM_PLANE_STAGGER_NS)
     int plane_ctas_per_sm = 0;      // resident plane-kernel CTAs per SM (0: two when two plane arrays fit, else one; QM_PLANE_CTAS)
     ~qm_gspace() { for (auto *k : kpts) delete k; }
 };
@@ -174,6 +191,7 @@ struct qm_batch_plan {
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t exec = nullptr;
     unsigned long long launches = 0;        // kernels per graph launch
+    std::vector<std::pair<int, unsigned long long>> gens;   // (k, KPoint::ws_gen at capture) of every k-point in the graph
     ~qm_batch_plan() {
         if (exec) cudaGraphExecDestroy(exec);
         if (graph) cudaGraphDestroy(graph);

@@ -14,6 +14,10 @@ template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *W,
     int cps = MODE == 3 ? 1 : (g->plane_ctas_per_sm > 0 ? g->plane_ctas_per_sm : 2);
     int ngroups = plane_groups(g, kp, cps);
     // every resident CTA allocates its own tensor-memory columns (512 per SM): one CTA per SM if two do not fit
+    // (one CTA always fits: a build whose thread limit needs more than an SM's 512 columns does not compile)
+    static_assert(!plane_tw_tmem<C> ||
+                      (4 * C::R1 + (C::R1 != C::R2 ? 4 * C::R2 : 0)) * ((QM_PLANE_MAX_THREADS / 32 + 3) / 4) <= 512,
+                  "QM_PLANE_MAX_THREADS: the twiddle rows of this line factorisation do not fit 512 tensor-memory columns");
     if (plane_tw_tmem<C> && cps > 1 && ngroups > 0) {
         const int rowcols = 4 * C::R1 + (C::R1 != C::R2 ? 4 * C::R2 : 0);
         if (cps * qm_tmem_cols_pow2(rowcols * ((ngroups * PLANE_GROUP / 32 + 3) / 4)) > 512) ngroups = 0;
@@ -34,7 +38,7 @@ template <class C, int MODE> int launch_plane(qm_gspace *g, KPoint *kp, c128 *W,
     const int grid = MODE == 3 ? std::min(g->grid[2], g->sm_count) : std::min(nplanes, g->sm_count * cps);
     g->prof.begin(QM_K_PLANE, st);
     CU_TRY(qm_launch_pdl(k_plane<C, MODE>, dim3(grid), dim3(ngroups * PLANE_GROUP), smem, st, g->pdl, kp->plan(), gd, W, a.box, a.box2,
-                         a.npair2, ngroups, a.scale, g->plane_stagger_ns, nplanes,
+                         a.npair2, ngroups, a.scale, nplanes,
                          (kp->y_quarter ? 1 : 0) | (kp->x_quarter ? 2 : 0) | (rowtab ? 4 : 0), a.occ, a.rhot));
     g->prof.end(st);
     g->launches++;

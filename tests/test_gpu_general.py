@@ -150,8 +150,12 @@ def test_hooks_density_splitop_on_a_general_box(qm):
     bra = rng.standard_normal((2, ib.size)) + 1j * rng.standard_normal((2, ib.size))
     ket = rng.standard_normal((3, ikk.size)) + 1j * rng.standard_normal((3, ikk.size))
     me = gs.mtxel(1, 0, 6.0)
+    # the epsilon sphere is the oracle's (strict cut-off at q = k_bra - k_ket, reading A21), not the library's own list
+    m_eps, i_eps, _ = og.gsphere(lat, 6.0, grid, kpts[1] - kpts[0], strict=True)
+    np.testing.assert_array_equal(me.miller(), m_eps)
+    np.testing.assert_array_equal(me.index_map(), i_eps)
     got = me.apply(torch.from_numpy(bra).to(dev), torch.from_numpy(ket).to(dev)).cpu().numpy()
-    ref = om.matrix_elements(bra, mb, ket, mk, me.miller(), grid)
+    ref = om.matrix_elements(bra, mb, ket, mk, m_eps, grid)
     scale = np.linalg.norm(bra, axis=1)[:, None, None] * np.linalg.norm(ket, axis=1)[None, :, None]
     assert np.max(np.abs(got - ref) / scale) <= TOL
     me.close()

@@ -152,8 +152,10 @@ def test_matrix_elements_wrapping_grid(qm):
     gs.close()
 
 
-@pytest.mark.parametrize("name,nbra,nket,ecut_eps", [("cfg4", 4, 6, 8.0), ("cfg5", 3, 4, 6.0)])
+@pytest.mark.parametrize("name,nbra,nket,ecut_eps", [("cfg4", 4, 6, 8.0), ("cfg5", 3, 4, 6.0), ("cfg5", 16, 16, 6.0)])
 def test_matrix_elements_sampled_full_size(qm, name, nbra, nket, ecut_eps):
+    """Sampled G against the plane-wave sum of eq. 56 (oracle/mtxel.py), every element against the FFT route of eq. 57;
+    the last case is the 16 x 16 block bench.py times."""
     torch, dev = _torch()
     cfg, lat, kpts, (mb, ib, bra), (mk, ik, ket) = _mtxel_inputs(name, 0, 0, nbra, nket, 5)
     gs = qm.GSpace(lat, cfg.ecutwfc_ry, cfg.grid, kpts)
@@ -161,7 +163,8 @@ def test_matrix_elements_sampled_full_size(qm, name, nbra, nket, ecut_eps):
     m_eps, i_eps, _ = og.gsphere(lat, ecut_eps, cfg.grid, np.zeros(3), strict=True)
     np.testing.assert_array_equal(me.index_map(), i_eps)
     got = me.apply(torch.from_numpy(bra).to(dev), torch.from_numpy(ket).to(dev)).cpu().numpy()
-    sel = np.unique(np.concatenate([[0, 1, i_eps.size - 1], np.random.default_rng(6).integers(0, i_eps.size, 40)]))
+    nsel = 40 if nbra * nket <= 24 else 16              # the direct sum costs nbra * nket * ng per sampled G
+    sel = np.unique(np.concatenate([[0, 1, i_eps.size - 1], np.random.default_rng(6).integers(0, i_eps.size, nsel)]))
     ref = om.matrix_elements(bra, mb, ket, mk, m_eps[sel], cfg.grid)
     assert _mtxel_err(got[:, :, sel], ref, bra, ket) <= TOL
     # every element against the library-FFT route of eq. 57 (second opinion)

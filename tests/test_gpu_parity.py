@@ -414,10 +414,3 @@ def test_side_stream_projection_is_bitwise_neutral(qm):
         res[mode] = outs[0].clone()
         gs.close()
     assert torch.equal(res["1"], res["0"])
-
-
-def test_exchange_probe_orders_the_three_mechanisms(qm):
-    """qm_probe_exchange: a tensor-memory read is cheaper than a shuffle hand-over, which is cheaper than the shared-memory
-    round trip; all three are positive and of nanosecond order."""
-    smem, shfl, tmem = qm.qm_probe_exchange()
-    assert 0.1 < tmem < shfl < smem < 100.0, (smem, shfl, tmem)

@@ -80,3 +80,20 @@ def test_subspace_full_size_sampled_entries(qm):
     for i, j in zip(ii, jj):
         ref = osub.vdot_matrix(a[i:i + 1], b[j:j + 1])[0, 0]
         assert abs(got[i, j] - ref) <= TOL * scale[i, j]
+
+
+def test_subspace_bench_shape_512_by_512_sampled_entries(qm):
+    """The shape bench.py times (512 x 512 states on the cfg5 sphere): 256 sampled entries, the four corners
+    among them, against oracle/subspace.py; every entry against the library product as a second opinion."""
+    p = problem("cfg5", 0, nbands=512, orthonormalise=False)
+    ng = p["idx"].size
+    rng = np.random.default_rng(21)
+    a, b = p["psi"], _rand(rng, 512, ng)
+    got = _run(qm, p, a, b)
+    scale = np.linalg.norm(a, axis=1)[:, None] * np.linalg.norm(b, axis=1)[None, :]
+    assert np.max(np.abs(got - np.conj(a) @ b.T) / scale) <= TOL
+    ii = np.concatenate([[0, 0, 511, 511], rng.integers(0, 512, size=252)])
+    jj = np.concatenate([[0, 511, 0, 511], rng.integers(0, 512, size=252)])
+    for i, j in zip(ii, jj):
+        ref = osub.vdot_matrix(a[i:i + 1], b[j:j + 1])[0, 0]
+        assert abs(got[i, j] - ref) <= TOL * scale[i, j], (i, j)

@@ -200,3 +200,14 @@ def test_fft_route_agrees_with_direct_sum(name):
     b = of.apply_h_fft(psi, idx, g2, v, cfg.grid, beta, d)
     for n in range(4):
         assert np.max(np.abs(a[n] - b[n])) <= 1e-12 * np.max(np.abs(a[n]))
+
+
+def test_expand_d_is_the_block_diagonal_embedding():
+    """oracle.hpsi.expand_d against scipy.linalg.block_diag (a library routine the oracle does not call): the blocks sit on
+    the diagonal in order, everything else is zero (D couples projectors of one atom only)."""
+    import scipy.linalg
+    from oracle import hpsi as oh
+    rng = np.random.default_rng(3)
+    for nblk, bs in ((1, 4), (3, 2), (5, 18), (7, 1)):
+        b = rng.standard_normal((nblk, bs, bs))
+        np.testing.assert_array_equal(oh.expand_d(b), scipy.linalg.block_diag(*b))
